@@ -1,0 +1,118 @@
+/* debye.h -- C ABI of libdebye: Debye all-pairs sinc summation on NVIDIA B200 (sm_100a).
+ *
+ * What is computed (arxiv 1306.2258, Eq. 2; per-type form factors per BASELINE.json north_star):
+ *
+ *     I(q_m) = sum_{i=0}^{N-1} sum_{j=0}^{N-1} F[t_i][m] F[t_j][m] sinc(q_m |x_i - x_j|),   sinc(0) = 1,
+ *
+ * i.e. both sums include j == i (self terms counted once each), pairs i != j are evaluated once for i < j
+ * and doubled ("only values for j <= k are computed").  Internally the library accumulates per
+ * type pair S_ab(q_m) = sum_{i<j, {t_i,t_j}={a,b}} sin(q_m r_ij)/r_ij in FP32 (FP64 with DEBYE_FP64), reduces
+ * in FP64 in a fixed order, and applies  I = sum_a n_a F_a^2 + 2 sum_{a<=b} F_a F_b S_ab / q_m  in an epilogue.
+ *
+ * Conventions
+ *   - Every call returns a status (DEBYE_OK == 0).  No exceptions, no errno, nothing printed.
+ *   - "dev" pointers are CUDA device pointers owned by the caller; "host" pointers are ordinary host memory.
+ *   - Device-pointer calls are asynchronous on `stream`, never synchronise the host and never read device
+ *     data on the host.  Scratch memory comes from a library-owned per-device cache that only grows
+ *     (cudaMalloc on growth, which may synchronise the first time a larger problem is seen) or from a
+ *     caller-supplied workspace (debye_set_workspace).  Calls on different streams must not overlap in time
+ *     (one workspace per device).
+ *   - Results are bitwise reproducible run to run for the same inputs, flags, GPU model and library build.
+ *   - Not checked (undefined behaviour if violated): 0 <= type[i] < T; finite inputs (NaN/Inf propagate).
+ *   - fftab values may be negative (neutron scattering lengths); q may contain 0 and be in any
+ *     order; q and -q give the same result.
+ *   - There is no CPU fallback and no other backend: without a CUDA device every compute call returns
+ *     DEBYE_ECUDA.
+ */
+#ifndef DEBYE_H
+#define DEBYE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct CUstream_st *debye_stream_t; /* == cudaStream_t; NULL is the legacy default stream */
+
+enum {
+    DEBYE_OK = 0,
+    DEBYE_EINVAL = 1,       /* null pointer, N < 1, M < 1, T < 1, T > DEBYE_MAX_TYPES, M > DEBYE_MAX_Q, B < 1,
+                               contradictory flags */
+    DEBYE_EUNSUPPORTED = 2, /* size beyond what the build supports (N > 2^24) */
+    DEBYE_ENOMEM = 3,       /* workspace allocation failed / supplied workspace too small */
+    DEBYE_ECUDA = 4         /* a CUDA runtime call failed; see debye_last_cuda_error() */
+};
+
+#define DEBYE_MAX_TYPES 32
+#define DEBYE_MAX_Q 4096
+
+/* flags (bitwise or).  At most one of the DEBYE_SINC_* bits; none = automatic choice (made on the device,
+ * no host sync): the recurrence kernel when q is a uniform grid, else the MUFU kernel. */
+enum {
+    DEBYE_FP64 = 1u << 0,         /* double-precision pair arithmetic (libdevice sin), tolerance 1e-10 mode     */
+    DEBYE_SINC_MUFU = 1u << 2,    /* FP32, one range-reduced MUFU.SIN per term; any q grid                      */
+    DEBYE_SINC_RECUR = 1u << 3,   /* FP32, Chebyshev angle-addition recurrence across a uniform q grid          *
+                                   * q_m = q_0 + m dq.  If q is not uniform (checked on the device) the output  *
+                                   * is filled with NaN.                                                         */
+    DEBYE_SINC_ACCURATE = 1u << 4 /* FP32, libdevice sinf per term (slow reference variant); any q grid         */
+};
+
+/* One structure.  PAPER.md:82, 88: inputs are N atom positions and the form factors at Q q-values, output
+ * is I(q)[Q].
+ *   xyz    dev  [N][3] float32, row-major (x,y,z), Angstrom
+ *   type   dev  [N] int32, 0 <= type[i] < T
+ *   fftab  dev  [T][M] float32 row-major, fftab[t][m] = f_t(q_m)
+ *   q      dev  [M] float32, 1/Angstrom
+ *   I_out  dev  [M] float64, written (not accumulated)
+ * Errors: DEBYE_EINVAL / EUNSUPPORTED / ENOMEM / ECUDA as above; on error nothing is launched. */
+int debye_profile(const float *xyz, const int32_t *type, int32_t N, const float *fftab, int32_t T,
+                  const float *q, int32_t M, double *I_out, uint32_t flags, debye_stream_t stream);
+
+/* B conformers of one molecule in one launch sequence (the profile is "recomputed hundreds
+ * of thousands of times"; ensembles).  type / fftab / q are shared; the type sort is computed once.
+ *   xyz    dev  [B][N][3] float32          I_out  dev  [B][M] float64 row-major */
+int debye_profile_batch(const float *xyz, const int32_t *type, int32_t N, int32_t B, const float *fftab,
+                        int32_t T, const float *q, int32_t M, double *I_out, uint32_t flags,
+                        debye_stream_t stream);
+
+/* Same results through HOST buffers: copies the inputs to the device (cudaMemcpyAsync on `stream`), runs the
+ * device path, copies I_out back and synchronises `stream` before returning.  All pointers are host pointers
+ * (pinned or pageable).  This is the end-to-end entry bench.py times ("e2e"). */
+int debye_profile_host(const float *xyz, const int32_t *type, int32_t N, const float *fftab, int32_t T,
+                       const float *q, int32_t M, double *I_out, uint32_t flags, debye_stream_t stream);
+int debye_profile_batch_host(const float *xyz, const int32_t *type, int32_t N, int32_t B, const float *fftab,
+                             int32_t T, const float *q, int32_t M, double *I_out, uint32_t flags,
+                             debye_stream_t stream);
+
+/* Per-type-pair partial structure factors (by-product of the path; lets a caller re-fit form factors without
+ * redoing the pair sum):  S_out[b][p][m] = sum over pairs i<j with {t_i,t_j} = {a,b'} of sinc(q_m r_ij), for
+ * p = a*(2T-a+1)/2 + (b'-a), a <= b' (row-major upper triangle);  n_out[t] = number of atoms of type t.
+ *   S_out dev [B][T(T+1)/2][M] float64      n_out dev [T] int32 (may be NULL)
+ * I(q_m) = sum_a n_a F_a^2 + 2 sum_p F_a F_b' S_out[p][m]. */
+int debye_partials(const float *xyz, const int32_t *type, int32_t N, int32_t B, const float *q, int32_t T,
+                   int32_t M, double *S_out, int32_t *n_out, uint32_t flags, debye_stream_t stream);
+
+/* Scratch bytes a call with these sizes needs (0 if the arguments are invalid). */
+size_t debye_workspace_bytes(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags);
+/* Optional caller-owned scratch for the current device (dev pointer, 256-byte aligned); NULL/0 returns to
+ * the library-owned cache.  The caller keeps ownership and must keep it alive while calls are in flight. */
+int debye_set_workspace(void *dev_ptr, size_t bytes);
+/* Frees the library-owned workspace of every device (also done at process exit). */
+void debye_shutdown(void);
+
+/* Introspection used by bench.py / tests (host-side, no GPU work):
+ * number of library kernels one debye_profile[_batch] call with these arguments launches, and the grid /
+ * chunking the pairs kernel would use (any out pointer may be NULL). */
+int debye_launch_info(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags, int32_t *n_launches,
+                      int32_t *pairs_grid, int32_t *q_chunk, int32_t *n_chunks);
+
+const char *debye_strerror(int status);
+int debye_last_cuda_error(void); /* cudaError_t of the last failing runtime call on this thread, 0 if none */
+int debye_version(void);         /* major*10000 + minor*100 + patch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEBYE_H */

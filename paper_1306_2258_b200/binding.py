@@ -1,0 +1,168 @@
+"""Thin Python binding of libdebye's C ABI (include/debye.h): argument marshalling only.
+
+Every step of the path (type sort, pair kernel, FP64 reduction, epilogue) runs in the CUDA library; torch is
+used for device memory and streams.  There is NO CPU fallback: if libdebye.so is missing or cannot be loaded
+the first call raises LibdebyeError."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libdebye.so")
+
+FLAGS = {"fp64": 1 << 0, "mufu": 1 << 2, "recur": 1 << 3, "accurate": 1 << 4, "auto": 0}
+
+EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_profile_batch_host",
+           "debye_partials", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
+           "debye_launch_info", "debye_strerror", "debye_last_cuda_error", "debye_version")
+
+
+class LibdebyeError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib():
+    """Load libdebye.so (built by `python -m paper_1306_2258_b200.build`); raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise LibdebyeError(f"{LIB_PATH} not found: build it with `python -m paper_1306_2258_b200.build` "
+                            "(there is no CPU fallback)")
+    try:
+        L = C.CDLL(LIB_PATH)
+    except OSError as e:  # pragma: no cover
+        raise LibdebyeError(f"cannot load {LIB_PATH}: {e}") from e
+    vp, i32, u32, sz = C.c_void_p, C.c_int32, C.c_uint32, C.c_size_t
+    L.debye_profile.argtypes = [vp, vp, i32, vp, i32, vp, i32, vp, u32, vp]
+    L.debye_profile_host.argtypes = L.debye_profile.argtypes
+    L.debye_profile_batch.argtypes = [vp, vp, i32, i32, vp, i32, vp, i32, vp, u32, vp]
+    L.debye_profile_batch_host.argtypes = L.debye_profile_batch.argtypes
+    L.debye_partials.argtypes = [vp, vp, i32, i32, vp, i32, i32, vp, vp, u32, vp]
+    for n in ("debye_profile", "debye_profile_host", "debye_profile_batch", "debye_profile_batch_host",
+              "debye_partials"):
+        getattr(L, n).restype = C.c_int
+    L.debye_workspace_bytes.argtypes = [i32, i32, i32, i32, u32]
+    L.debye_workspace_bytes.restype = sz
+    L.debye_set_workspace.argtypes = [vp, sz]
+    L.debye_set_workspace.restype = C.c_int
+    L.debye_shutdown.argtypes = []
+    L.debye_shutdown.restype = None
+    L.debye_launch_info.argtypes = [i32, i32, i32, i32, u32] + [C.POINTER(i32)] * 4
+    L.debye_launch_info.restype = C.c_int
+    L.debye_strerror.argtypes = [C.c_int]
+    L.debye_strerror.restype = C.c_char_p
+    L.debye_last_cuda_error.restype = C.c_int
+    L.debye_version.restype = C.c_int
+    _lib = L
+    return L
+
+
+def _check(st: int):
+    if st != 0:
+        L = lib()
+        raise LibdebyeError(f"libdebye status {st}: {L.debye_strerror(st).decode()} "
+                            f"(cuda error {L.debye_last_cuda_error()})")
+
+
+def _flags(variant) -> int:
+    if isinstance(variant, int):
+        return variant
+    return FLAGS[variant]
+
+
+def _stream_ptr(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _dev(t, dtype, name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise LibdebyeError(f"{name}: expected a contiguous CUDA tensor of dtype {dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def debye_profile(xyz, type, fftab, q, I_out=None, variant="auto", stream=None):
+    """I_out[M] (float64, CUDA) for xyz[N,3] f32, type[N] i32, fftab[T,M] f32, q[M] f32 (CUDA tensors).
+    Asynchronous on `stream` (default: torch's current stream)."""
+    import torch
+    N, T, M = xyz.shape[0], fftab.shape[0], q.shape[0]
+    if I_out is None:
+        I_out = torch.empty(M, dtype=torch.float64, device=xyz.device)
+    _check(lib().debye_profile(_dev(xyz, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N,
+                               _dev(fftab, torch.float32, "fftab"), T, _dev(q, torch.float32, "q"), M,
+                               _dev(I_out, torch.float64, "I_out"), _flags(variant), _stream_ptr(stream)))
+    return I_out
+
+
+def debye_profile_batch(xyz, type, fftab, q, I_out=None, variant="auto", stream=None):
+    """I_out[B,M] for B conformers xyz[B,N,3] sharing type / fftab / q."""
+    import torch
+    B, N, T, M = xyz.shape[0], xyz.shape[1], fftab.shape[0], q.shape[0]
+    if I_out is None:
+        I_out = torch.empty((B, M), dtype=torch.float64, device=xyz.device)
+    _check(lib().debye_profile_batch(_dev(xyz, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N, B,
+                                     _dev(fftab, torch.float32, "fftab"), T, _dev(q, torch.float32, "q"), M,
+                                     _dev(I_out, torch.float64, "I_out"), _flags(variant), _stream_ptr(stream)))
+    return I_out
+
+
+def debye_partials(xyz, type, q, T, variant="auto", stream=None):
+    """(S[B,T(T+1)/2,M] float64, n[T] int32): per-type-pair sums of sinc(q r) over pairs i<j, atoms per type."""
+    import torch
+    x3 = xyz if xyz.dim() == 3 else xyz[None]
+    B, N, M = x3.shape[0], x3.shape[1], q.shape[0]
+    S = torch.empty((B, T * (T + 1) // 2, M), dtype=torch.float64, device=xyz.device)
+    n = torch.empty(T, dtype=torch.int32, device=xyz.device)
+    _check(lib().debye_partials(_dev(x3, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N, B,
+                                _dev(q, torch.float32, "q"), T, M, _dev(S, torch.float64, "S_out"),
+                                _dev(n, torch.int32, "n_out"), _flags(variant), _stream_ptr(stream)))
+    return S, n
+
+
+def _host(a, dtype, name):
+    if not (isinstance(a, np.ndarray) and a.dtype == dtype and a.flags.c_contiguous):
+        raise LibdebyeError(f"{name}: expected a C-contiguous numpy array of dtype {dtype}")
+    return C.c_void_p(a.ctypes.data)
+
+
+def debye_profile_host(xyz, type, fftab, q, I_out=None, variant="auto", stream=None):
+    """Host-buffer entry (numpy arrays, ideally pinned): H2D copies + device path + D2H copy + stream sync
+    all happen inside the C call."""
+    N, T, M = xyz.shape[0], fftab.shape[0], q.shape[0]
+    if I_out is None:
+        I_out = np.empty(M, dtype=np.float64)
+    _check(lib().debye_profile_host(_host(xyz, np.float32, "xyz"), _host(type, np.int32, "type"), N,
+                                    _host(fftab, np.float32, "fftab"), T, _host(q, np.float32, "q"), M,
+                                    _host(I_out, np.float64, "I_out"), _flags(variant), _stream_ptr(stream)))
+    return I_out
+
+
+def debye_profile_batch_host(xyz, type, fftab, q, I_out=None, variant="auto", stream=None):
+    B, N, T, M = xyz.shape[0], xyz.shape[1], fftab.shape[0], q.shape[0]
+    if I_out is None:
+        I_out = np.empty((B, M), dtype=np.float64)
+    _check(lib().debye_profile_batch_host(_host(xyz, np.float32, "xyz"), _host(type, np.int32, "type"), N, B,
+                                          _host(fftab, np.float32, "fftab"), T, _host(q, np.float32, "q"), M,
+                                          _host(I_out, np.float64, "I_out"), _flags(variant), _stream_ptr(stream)))
+    return I_out
+
+
+def launch_info(N, B, T, M, variant="auto", with_grid=False):
+    """dict(n_launches, q_chunk, n_chunks[, pairs_grid]) for a call with these sizes (host-side query)."""
+    L = lib()
+    a, g, k, c = C.c_int32(), C.c_int32(), C.c_int32(), C.c_int32()
+    _check(L.debye_launch_info(N, B, T, M, _flags(variant), C.byref(a), C.byref(g) if with_grid else None,
+                               C.byref(k), C.byref(c)))
+    out = {"n_launches": a.value, "q_chunk": k.value, "n_chunks": c.value}
+    if with_grid:
+        out["pairs_grid"] = g.value
+    return out

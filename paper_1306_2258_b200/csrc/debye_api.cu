@@ -1,0 +1,345 @@
+// debye_api.cu -- the C ABI of libdebye (include/debye.h): validation, workspace, launch sequence.
+//
+// Launch sequence of one call (all on the caller's stream, no host synchronisation, no device->host reads):
+//   debye_setup_kernel  (1 CTA)    type histogram, stable sort permutation, q analysis, unit prefix   S0/S1
+//   debye_pack_kernel               gather into type-sorted float4                                     S0
+//   debye_pairs_kernel<K, variant>  persistent grid, one or (automatic mode) two launches of which     S1-S6
+//                                   the one not selected on the device exits immediately
+//   debye_final_kernel              fixed-order FP64 reduction + form-factor epilogue                  S7
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include "../../include/debye.h"
+#include "debye_aux.cuh"
+#include "debye_pairs.cuh"
+#include "debye_plan.cuh"
+#include "debye_registry.h"
+
+namespace {
+
+thread_local int g_last_cuda = 0;
+#define CU(call)                                   \
+    do {                                           \
+        cudaError_t e__ = (call);                  \
+        if (e__ != cudaSuccess) {                  \
+            g_last_cuda = (int)e__;                \
+            return DEBYE_ECUDA;                    \
+        }                                          \
+    } while (0)
+
+constexpr int MAX_DEV = 64;
+struct DevState {
+    void *ws = nullptr; size_t ws_bytes = 0;          // library-owned scratch
+    void *user_ws = nullptr; size_t user_bytes = 0;   // caller-owned scratch (debye_set_workspace)
+    void *stage = nullptr; size_t stage_bytes = 0;    // device staging for the *_host entry points
+    int sms = 0;
+    int occ[5][17];                                   // cached CTAs/SM per (variant, K/8); 0 = unknown
+};
+DevState g_dev[MAX_DEV];
+std::mutex g_mu;
+bool g_atexit = false;
+
+size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+struct Choice { int variant; int K; int n_chunks; };
+
+// q-chunking of each variant: how many accumulators a thread keeps (K) and how many passes over the pairs.
+Choice choose(int variant, int M)
+{
+    Choice c; c.variant = variant;
+    if (variant == V_RECUR) {
+        int nc = 1;
+        while (((M + 8 * nc - 1) / (8 * nc)) * 8 > DEBYE_KMAX_F32) nc *= 2;     // residue-class chunks: power of two
+        c.n_chunks = nc; c.K = ((M + 8 * nc - 1) / (8 * nc)) * 8;
+    } else {
+        int kmax = (variant == V_F64) ? DEBYE_KMAX_F64 : DEBYE_KMAX_F32;
+        int nc = (M + kmax - 1) / kmax;
+        int per = (M + nc - 1) / nc;
+        c.n_chunks = nc; c.K = (per + 7) / 8 * 8;
+    }
+    return c;
+}
+
+struct Layout { size_t plan, perm, sorted, records, total; };
+Layout layout(int N, int B, int T, int M, int G_max, const Choice *ch, int nch)
+{
+    Layout L; size_t o = 0;
+    L.plan = o; o += align_up(sizeof(DevPlan));
+    L.perm = o; o += align_up((size_t)N * 4);
+    L.sorted = o; o += align_up((size_t)N * B * 16);
+    size_t rec = 0;
+    for (int i = 0; i < nch; ++i) {
+        size_t r = ((size_t)G_max + (size_t)B * (T * (T + 1) / 2) * ch[i].n_chunks) * ch[i].K * 8;
+        if (r > rec) rec = r;
+    }
+    L.records = o; o += align_up(rec);
+    L.total = o;
+    return L;
+}
+
+int variants_for(uint32_t flags, Choice *out, int M, int *is_auto)
+{
+    *is_auto = 0;
+    if (flags & DEBYE_FP64) { out[0] = choose(V_F64, M); return 1; }
+    if (flags & DEBYE_SINC_MUFU) { out[0] = choose(V_MUFU, M); return 1; }
+    if (flags & DEBYE_SINC_RECUR) { out[0] = choose(V_RECUR, M); return 1; }
+    if (flags & DEBYE_SINC_ACCURATE) { out[0] = choose(V_ACCURATE, M); return 1; }
+    *is_auto = 1;
+    out[0] = choose(V_RECUR, M);
+    out[1] = choose(V_MUFU, M);
+    return 2;
+}
+
+int validate(const void *xyz, const void *type, int N, int B, const void *tab, int T, const void *q, int M, const void *out, uint32_t flags)
+{
+    if (!xyz || !type || !q || !out) return DEBYE_EINVAL;
+    if (!tab) return DEBYE_EINVAL;
+    if (N < 1 || M < 1 || T < 1 || B < 1 || T > DEBYE_MAX_TYPES || M > DEBYE_MAX_Q) return DEBYE_EINVAL;
+    uint32_t known = DEBYE_FP64 | DEBYE_SINC_MUFU | DEBYE_SINC_RECUR | DEBYE_SINC_ACCURATE;
+    if (flags & ~known) return DEBYE_EINVAL;
+    uint32_t s = flags & (DEBYE_SINC_MUFU | DEBYE_SINC_RECUR | DEBYE_SINC_ACCURATE);
+    if (s & (s - 1)) return DEBYE_EINVAL;
+    if ((flags & DEBYE_FP64) && s) return DEBYE_EINVAL;
+    if (N > (1 << 24)) return DEBYE_EUNSUPPORTED;
+    if ((int64_t)N * B > ((int64_t)1 << 31)) return DEBYE_EUNSUPPORTED;
+    return DEBYE_OK;
+}
+
+int dev_state(DevState **st)
+{
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEV) return DEBYE_EUNSUPPORTED;
+    DevState *s = &g_dev[dev];
+    if (s->sms == 0) {
+        int sms = 0;
+        CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        s->sms = sms;
+        memset(s->occ, 0, sizeof(s->occ));
+    }
+    *st = s;
+    return DEBYE_OK;
+}
+
+int grid_for(DevState *s, const Choice &c, int *G)
+{
+    int &o = s->occ[c.variant][c.K / 8];
+    if (o == 0) {
+        debye_pairs_fn fn = debye_get_pairs_kernel(c.variant, c.K);
+        if (!fn) return DEBYE_EUNSUPPORTED;
+        int nb = 0;
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, DEBYE_IB, 0));
+        if (nb < 1) nb = 1;
+        o = nb;
+    }
+    *G = s->sms * o;
+    return DEBYE_OK;
+}
+
+void shutdown_all()
+{
+    for (int d = 0; d < MAX_DEV; ++d) {
+        if (g_dev[d].ws || g_dev[d].stage) {
+            int cur = 0;
+            if (cudaGetDevice(&cur) != cudaSuccess) return;
+            if (cudaSetDevice(d) != cudaSuccess) continue;
+            if (g_dev[d].ws) cudaFree(g_dev[d].ws);
+            if (g_dev[d].stage) cudaFree(g_dev[d].stage);
+            g_dev[d].ws = g_dev[d].stage = nullptr; g_dev[d].ws_bytes = g_dev[d].stage_bytes = 0;
+            cudaSetDevice(cur);
+        }
+    }
+}
+
+int ensure(void **ptr, size_t *have, size_t need)
+{
+    if (*have >= need) return DEBYE_OK;
+    if (*ptr) { CU(cudaFree(*ptr)); *ptr = nullptr; *have = 0; }
+    size_t want = need + need / 4;
+    cudaError_t e = cudaMalloc(ptr, want);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); g_last_cuda = (int)e; *ptr = nullptr; return DEBYE_ENOMEM; }
+    *have = want;
+    if (!g_atexit) { g_atexit = true; atexit(shutdown_all); }
+    return DEBYE_OK;
+}
+
+// mode 0: I_out[B][M]; mode 1: S_out[B][n_tp][M] (+ n_out)
+int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab, int T, const float *q, int M, double *out, int32_t *n_out,
+        uint32_t flags, cudaStream_t stream, int mode)
+{
+    int st = validate(xyz, type, N, B, mode == 0 ? (const void *)fftab : (const void *)q, T, q, M, out, flags);
+    if (st) return st;
+    std::lock_guard<std::mutex> lock(g_mu);
+    DevState *ds;
+    if ((st = dev_state(&ds))) return st;
+    Choice ch[2]; int is_auto = 0;
+    const int nch = variants_for(flags, ch, M, &is_auto);
+    int G[2] = {0, 0}, Gmax = 0;
+    for (int i = 0; i < nch; ++i) { if ((st = grid_for(ds, ch[i], &G[i]))) return st; if (G[i] > Gmax) Gmax = G[i]; }
+    const Layout L = layout(N, B, T, M, Gmax, ch, nch);
+    char *ws;
+    if (ds->user_ws) { if (ds->user_bytes < L.total) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
+    else { if ((st = ensure(&ds->ws, &ds->ws_bytes, L.total))) return st; ws = (char *)ds->ws; }
+    DevPlan *plan = (DevPlan *)(ws + L.plan);
+    int32_t *perm = (int32_t *)(ws + L.perm);
+    float4 *sorted = (float4 *)(ws + L.sorted);
+    double *records = (double *)(ws + L.records);
+
+    int rec_cap = 0;
+    for (int i = 0; i < nch; ++i) if (ch[i].variant == V_RECUR) rec_cap = ch[i].K * ch[i].n_chunks;
+    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, rec_cap);
+    {
+        int64_t total = (int64_t)N * B;
+        int blocks = (int)((total + 255) / 256);
+        if (blocks > ds->sms * 16) blocks = ds->sms * 16;
+        debye::debye_pack_kernel<<<blocks, 256, 0, stream>>>(plan, xyz, type, perm, sorted, N, B);
+    }
+    for (int i = 0; i < nch; ++i) {
+        debye_pairs_fn fn = debye_get_pairs_kernel(ch[i].variant, ch[i].K);
+        // slow-path threshold on theta = r * (smallest grid step or smallest |q|): see DESIGN.md section 6
+        const float theta_min = (ch[i].variant == V_RECUR) ? 0.004f : 0.004f;
+        fn<<<G[i], DEBYE_IB, 0, stream>>>(plan, sorted, q, records, ch[i].n_chunks, is_auto, theta_min);
+    }
+    {
+        int threads = 128, blocks = (M * B + threads - 1) / threads;
+        // in automatic mode the final kernel picks the parameter set of the variant chosen on the device
+        const Choice &c1 = ch[nch - 1];
+        debye::debye_final_kernel<<<blocks, threads, 0, stream>>>(plan, records, fftab, q, out, is_auto, ch[0].variant, ch[0].K, ch[0].n_chunks, G[0], c1.variant, c1.K,
+                                                                  c1.n_chunks, G[nch - 1], mode);
+    }
+    if (mode == 1 && n_out) CU(cudaMemcpyAsync(n_out, plan->n_a, sizeof(int32_t) * T, cudaMemcpyDeviceToDevice, stream));
+    CU(cudaGetLastError());
+    return DEBYE_OK;
+}
+
+int run_host(const float *xyz, const int32_t *type, int N, int B, const float *fftab, int T, const float *q, int M, double *out, uint32_t flags,
+             cudaStream_t stream)
+{
+    int st = validate(xyz, type, N, B, fftab, T, q, M, out, flags);
+    if (st) return st;
+    DevState *ds;
+    char *base;
+    size_t o_xyz, o_type, o_tab, o_q, o_out, total;
+    {
+        std::lock_guard<std::mutex> lock(g_mu);
+        if ((st = dev_state(&ds))) return st;
+        size_t o = 0;
+        o_xyz = o; o += align_up((size_t)N * B * 12);
+        o_type = o; o += align_up((size_t)N * 4);
+        o_tab = o; o += align_up((size_t)T * M * 4);
+        o_q = o; o += align_up((size_t)M * 4);
+        o_out = o; o += align_up((size_t)B * M * 8);
+        total = o;
+        if ((st = ensure(&ds->stage, &ds->stage_bytes, total))) return st;
+        base = (char *)ds->stage;
+    }
+    CU(cudaMemcpyAsync(base + o_xyz, xyz, (size_t)N * B * 12, cudaMemcpyHostToDevice, stream));
+    CU(cudaMemcpyAsync(base + o_type, type, (size_t)N * 4, cudaMemcpyHostToDevice, stream));
+    CU(cudaMemcpyAsync(base + o_tab, fftab, (size_t)T * M * 4, cudaMemcpyHostToDevice, stream));
+    CU(cudaMemcpyAsync(base + o_q, q, (size_t)M * 4, cudaMemcpyHostToDevice, stream));
+    st = run((const float *)(base + o_xyz), (const int32_t *)(base + o_type), N, B, (const float *)(base + o_tab), T, (const float *)(base + o_q), M,
+             (double *)(base + o_out), nullptr, flags, stream, 0);
+    if (st) return st;
+    CU(cudaMemcpyAsync(out, base + o_out, (size_t)B * M * 8, cudaMemcpyDeviceToHost, stream));
+    CU(cudaStreamSynchronize(stream));
+    return DEBYE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int debye_profile(const float *xyz, const int32_t *type, int32_t N, const float *fftab, int32_t T, const float *q, int32_t M, double *I_out, uint32_t flags,
+                  debye_stream_t stream)
+{
+    return run(xyz, type, N, 1, fftab, T, q, M, I_out, nullptr, flags, (cudaStream_t)stream, 0);
+}
+
+int debye_profile_batch(const float *xyz, const int32_t *type, int32_t N, int32_t B, const float *fftab, int32_t T, const float *q, int32_t M, double *I_out,
+                        uint32_t flags, debye_stream_t stream)
+{
+    return run(xyz, type, N, B, fftab, T, q, M, I_out, nullptr, flags, (cudaStream_t)stream, 0);
+}
+
+int debye_profile_host(const float *xyz, const int32_t *type, int32_t N, const float *fftab, int32_t T, const float *q, int32_t M, double *I_out, uint32_t flags,
+                       debye_stream_t stream)
+{
+    return run_host(xyz, type, N, 1, fftab, T, q, M, I_out, flags, (cudaStream_t)stream);
+}
+
+int debye_profile_batch_host(const float *xyz, const int32_t *type, int32_t N, int32_t B, const float *fftab, int32_t T, const float *q, int32_t M,
+                             double *I_out, uint32_t flags, debye_stream_t stream)
+{
+    return run_host(xyz, type, N, B, fftab, T, q, M, I_out, flags, (cudaStream_t)stream);
+}
+
+int debye_partials(const float *xyz, const int32_t *type, int32_t N, int32_t B, const float *q, int32_t T, int32_t M, double *S_out, int32_t *n_out,
+                   uint32_t flags, debye_stream_t stream)
+{
+    return run(xyz, type, N, B, nullptr, T, q, M, S_out, n_out, flags, (cudaStream_t)stream, 1);
+}
+
+size_t debye_workspace_bytes(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags)
+{
+    static const char dummy = 0;
+    if (validate(&dummy, &dummy, N, B, &dummy, T, &dummy, M, &dummy, flags)) return 0;
+    Choice ch[2]; int is_auto;
+    int nch = variants_for(flags, ch, M, &is_auto);
+    // grid is at most 148 SMs x 16 CTAs on any sm_100 part; use a safe upper bound so no device query is needed
+    return layout(N, B, T, M, 192 * 16, ch, nch).total;
+}
+
+int debye_set_workspace(void *dev_ptr, size_t bytes)
+{
+    std::lock_guard<std::mutex> lock(g_mu);
+    DevState *ds; int st;
+    if ((st = dev_state(&ds))) return st;
+    if (dev_ptr && ((uintptr_t)dev_ptr & 255)) return DEBYE_EINVAL;
+    ds->user_ws = dev_ptr; ds->user_bytes = dev_ptr ? bytes : 0;
+    return DEBYE_OK;
+}
+
+void debye_shutdown(void)
+{
+    std::lock_guard<std::mutex> lock(g_mu);
+    shutdown_all();
+}
+
+int debye_launch_info(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags, int32_t *n_launches, int32_t *pairs_grid, int32_t *q_chunk, int32_t *n_chunks)
+{
+    static const char dummy = 0;
+    int st = validate(&dummy, &dummy, N, B, &dummy, T, &dummy, M, &dummy, flags);
+    if (st) return st;
+    Choice ch[2]; int is_auto;
+    int nch = variants_for(flags, ch, M, &is_auto);
+    if (n_launches) *n_launches = 3 + nch;           // setup, pack, pairs x nch, final
+    if (q_chunk) *q_chunk = ch[0].K;
+    if (n_chunks) *n_chunks = ch[0].n_chunks;
+    if (pairs_grid) {
+        std::lock_guard<std::mutex> lock(g_mu);
+        DevState *ds; int G = 0;
+        if ((st = dev_state(&ds))) return st;
+        if ((st = grid_for(ds, ch[0], &G))) return st;
+        *pairs_grid = G;
+    }
+    return DEBYE_OK;
+}
+
+const char *debye_strerror(int status)
+{
+    switch (status) {
+        case DEBYE_OK: return "ok";
+        case DEBYE_EINVAL: return "invalid argument";
+        case DEBYE_EUNSUPPORTED: return "unsupported size";
+        case DEBYE_ENOMEM: return "workspace allocation failed or supplied workspace too small";
+        case DEBYE_ECUDA: return "CUDA runtime error (see debye_last_cuda_error)";
+        default: return "unknown status";
+    }
+}
+
+int debye_last_cuda_error(void) { return g_last_cuda; }
+int debye_version(void) { return 100; }
+
+}  // extern "C"

@@ -1,0 +1,59 @@
+// debye_plan.cuh -- device-resident plan shared by the setup, pairs and final kernels of libdebye.
+//
+// Work decomposition (S1 of SURVEY.md section 8(a); "only values for j <= k are computed"):
+//   atoms are sorted by type; for every unordered type pair tp = (a <= b) the pairs form a rectangle
+//   (a < b) or a strict upper triangle (a == b).  A "row" is a block of IB consecutive i atoms (one per
+//   thread of a CTA); a "unit" is one j atom against one row (IB pairs x K q-values).  Units are linearised
+//   as  conformer -> type pair -> q-chunk -> row -> j  and the persistent grid splits that line into G equal
+//   contiguous ranges, so the assignment is static (bitwise reproducible) and balanced to one j atom.
+#pragma once
+#include <cstdint>
+
+#define DEBYE_MAX_TYPES_I 32
+#define DEBYE_MAX_TP (DEBYE_MAX_TYPES_I * (DEBYE_MAX_TYPES_I + 1) / 2)
+#define DEBYE_IB 128          // i atoms per row == threads per pairs CTA
+#define DEBYE_JT 64           // j atoms per shared-memory tile (1 KB, one cp.async.bulk)
+
+enum DebyeVariant : int32_t { V_NONE = 0, V_F64 = 1, V_MUFU = 2, V_RECUR = 3, V_ACCURATE = 4 };
+
+struct DevPlan {
+    int32_t N, T, M, B;
+    int32_t n_tp;                 // T(T+1)/2
+    int32_t uniform;              // q is a uniform grid q0 + m dq (checked on the device)
+    int32_t zero_start;           // uniform and q0 == 0
+    int32_t variant_auto;         // variant chosen on the device when the caller gave no DEBYE_SINC_* flag
+    double q0, dq;                // least-squares-free fit: q0 = q[0], dq = (q[M-1]-q[0])/(M-1)
+    float q_small;                // smallest non-zero |q|
+    int32_t pad0;
+    int64_t U1;                   // units per conformer and per q-chunk
+    int32_t seg_off[DEBYE_MAX_TYPES_I + 1];   // sorted-array offset of each type segment
+    int32_t n_a[DEBYE_MAX_TYPES_I];           // atoms per type
+    int32_t tp_ti[DEBYE_MAX_TP];              // type on the i (row) side
+    int32_t tp_tj[DEBYE_MAX_TP];              // type on the j (column) side; == tp_ti on the diagonal
+    int64_t tp_prefix[DEBYE_MAX_TP + 1];      // units before type pair tp (one chunk, one conformer)
+};
+
+// ---- unit decoding helpers (used identically by the pairs kernel and the final kernel) -------------------
+__host__ __device__ inline int64_t debye_range_begin(int64_t U, int32_t c, int32_t G)
+{
+    // floor(U * c / G) without overflow for U < 2^52, G < 2^12
+    return (U / G) * c + ((U % G) * c) / G;
+}
+
+// CTA that owns unit u:  largest c with range_begin(c) <= u
+__host__ __device__ inline int32_t debye_owner(int64_t U, int32_t G, int64_t u)
+{
+    int64_t c = (int64_t)(((double)u * (double)G) / (double)U);   // estimate, made exact by the two loops below
+    if (c >= G) c = G - 1;
+    if (c < 0) c = 0;
+    while (c + 1 < G && debye_range_begin(U, (int32_t)(c + 1), G) <= u) ++c;
+    while (c > 0 && debye_range_begin(U, (int32_t)c, G) > u) --c;
+    return (int32_t)c;
+}
+
+// diagonal type pair with n atoms: units before row r, r(n-1) - IB r(r-1)/2
+__host__ __device__ inline int64_t debye_diag_row_prefix(int64_t n, int64_t r)
+{
+    return r * (n - 1) - (int64_t)DEBYE_IB * (r * (r - 1) / 2);
+}
+__host__ __device__ inline int32_t debye_diag_rows(int32_t n) { return n >= 2 ? (n - 2) / DEBYE_IB + 1 : 0; }

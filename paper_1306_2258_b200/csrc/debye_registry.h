@@ -1,0 +1,16 @@
+// debye_registry.h -- lookup of the pairs-kernel instantiations (one per variant and accumulator count K).
+#pragma once
+#include <cstdint>
+#include "debye_plan.cuh"
+
+typedef void (*debye_pairs_fn)(const DevPlan *, const float4 *, const float *, double *, int, int, float);
+
+#define DEBYE_KMAX_F32 128
+#define DEBYE_KMAX_F64 32
+
+// K must be a multiple of 8 in [8, KMAX]; returns nullptr otherwise
+debye_pairs_fn debye_get_pairs_kernel(int variant, int K);
+debye_pairs_fn debye_get_recur(int K);
+debye_pairs_fn debye_get_mufu(int K);
+debye_pairs_fn debye_get_accurate(int K);
+debye_pairs_fn debye_get_f64(int K);

@@ -175,7 +175,7 @@ def cfg2(N: int = 10000, M: int = 101, q_max: float = 0.5, q_min: float = 0.0, t
          seed_off: int = 2) -> Workload:
     s = BASE_SEED + seed_off
     q = q_grid(q_max, M, q_min)
-    nb = N // 8
+    nb = (N + 7) // 8
     radius = 30.0 * (N / 10000.0) ** (1.0 / 3.0)      # constant density when N changes (sweep T)
     xyz = blob(s, nb, radius)[:N]
     return Workload(tag, xyz.astype(np.float32), types_from_cdf(s + 10, N, _PROTEIN_CDF),
@@ -203,7 +203,7 @@ def cfg3(n_bp: int = 1250, tag: str = "cfg3_helix_50k") -> Workload:
 
 def cfg4(B: int = 1024, N: int = 2000, tag: str = "cfg4_batch_1024x2k") -> Workload:
     s = BASE_SEED + 4
-    base = blob(s, N // 8, 17.5)[:N]
+    base = blob(s, (N + 7) // 8, 17.5)[:N]
     noise = Stream(s + 2000).normal(B * N * 3).reshape(B, N, 3)
     q = q_grid(0.4, 64)
     return Workload(tag, (base[None] + 2.0 * noise).astype(np.float32), types_from_cdf(s + 10, N, _PROTEIN_CDF),

@@ -1,0 +1,312 @@
+#!/usr/bin/env python
+"""bench.py -- libdebye headline benchmark (BASELINE.json metric: G pair.q sinc-terms/s and ms/profile on B200,
+fraction of the FP32-issue roofline), with the CPU oracle timed beside it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg2] [--variant auto] [--impl reference]
+
+A "step" is one pass of the whole hot path (type sort + pack + all-pairs kernel + FP64 reduction + epilogue,
+SURVEY.md section 8(a) S0-S7) over one synthetic structure: one debye_profile call (one debye_profile_batch call
+for cfg4).  Workload at N=1: BASELINE.json configs[1] (cfg2: 10,000-atom globular blob, 101 q on [0, 0.5]).
+With N GPUs every rank runs its own structure of the same shape (different seed): the path shards over independent
+structures with no data-path collective, so scaling is weak; time = max over ranks.
+Prints ONE JSON line (rank 0)."""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1306_2258_b200 import workloads as wl          # noqa: E402  (input generators only, no arithmetic)
+
+METRIC = "pair_q_sinc_terms_per_second"
+UNIT = "G pair.q/s"
+SM_COUNT, FP32_LANES, MUFU_LANES = 148, 128, 16           # per B200 / per SM per clock (B200_PROFILING.md)
+
+
+def make_workload(name: str, rank: int = 0):
+    if name == "cfg2" and rank:
+        return wl.cfg2(seed_off=2 + 1000 * rank, tag=f"cfg2_globular_10k_rank{rank}")
+    return wl.CONFIGS[name]()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return json.load(open(p))
+    except Exception:
+        return {}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz, self._stop_evt = index, [], set(), None, threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                 "hw_power_brake_slowdown": 0x80, "sync_boost": 0x10, "applications_clocks_setting": 0x2}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.004)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def cpu_baseline(w, budget_s: float = 15.0):
+    """The oracle as it stands (oracle/debye_oracle.c, fp64, OpenMP over rows), timed on this host's cores on a
+    bounded sample of the same workload: the first R rows of the symmetric double loop."""
+    from oracle import oracle as orc
+    xyz = w.xyz[0] if w.xyz.ndim == 3 else w.xyz
+    N, M = w.N, w.M
+    r_probe = min(N, 64)
+    t0 = time.perf_counter()
+    _, nthr = orc.debye_sym(xyz, w.type, w.fftab, w.q, rows=(0, r_probe), return_threads=True)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    pairs = lambda r: r * (N - 1) - r * (r - 1) // 2           # pairs (i<j) with i < r
+    rate = pairs(r_probe) * M / dt
+    rows = N
+    if pairs(N) * M / rate > budget_s:
+        rows = r_probe
+        while rows < N and pairs(rows) * M / rate < budget_s:
+            rows += 64
+        rows = min(rows, N)
+    t0 = time.perf_counter()
+    orc.debye_sym(xyz, w.type, w.fftab, w.q, rows=(0, rows))
+    dt = time.perf_counter() - t0
+    return {"value": pairs(rows) * M / dt / 1e9, "unit": UNIT, "cores": int(nthr), "kind": "oracle",
+            "sample": f"rows 0..{rows - 1} of {N} of the i<j double loop ({pairs(rows) * M:.3e} pair.q, {dt:.2f} s)"
+                      + (" = the whole profile" if rows == N else ""),
+            "seconds": dt}
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle itself, each step a bounded row slab of the same workload."""
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    w = make_workload(args.config)
+    xyz = w.xyz[0] if w.xyz.ndim == 3 else w.xyz
+    N, M = w.N, w.M
+    pairs = lambda r: r * (N - 1) - r * (r - 1) // 2
+    t0 = time.perf_counter()
+    _, nthr = orc.debye_sym(xyz, w.type, w.fftab, w.q, rows=(0, min(N, 64)), return_threads=True)
+    rate = pairs(min(N, 64)) * M / max(time.perf_counter() - t0, 1e-6)
+    per_step = max(0.2, min(120.0 / (args.steps + args.warmup), 20.0))
+    rows = min(N, 64)
+    while rows < N and pairs(rows) * M / rate < per_step:
+        rows += 64
+    rows = min(rows, N)
+    for _ in range(args.warmup):
+        orc.debye_sym(xyz, w.type, w.fftab, w.q, rows=(0, rows))
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.debye_sym(xyz, w.type, w.fftab, w.q, rows=(0, rows))
+    dt = time.perf_counter() - t0
+    value = pairs(rows) * M * args.steps / dt / 1e9
+    sample = f"rows 0..{rows - 1} of {N} per step ({pairs(rows) * M:.3e} pair.q)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "N": N, "T": w.T, "M": M, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": int(nthr), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", default="cfg2", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--variant", default="auto", choices=["auto", "recur", "mufu", "accurate", "fp64"])
+    ap.add_argument("--impl", default="libdebye", choices=["libdebye", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "libdebye" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        return run_reference(args, rank, world)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1306_2258_b200 import binding as db, sharding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (libdebye has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    db.lib()
+
+    w = make_workload(args.config, rank)
+    batch = w.xyz.ndim == 3
+    call = db.debye_profile_batch if batch else db.debye_profile
+    call_host = db.debye_profile_batch_host if batch else db.debye_profile_host
+    x, t, f, q = (torch.from_numpy(a).to(dev) for a in (w.xyz, w.type, w.fftab, w.q))
+    out = torch.empty((w.B, w.M) if batch else (w.M,), dtype=torch.float64, device=dev)
+    flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device=dev)        # > 126 MB L2
+    info = db.launch_info(w.N, w.B, w.T, w.M, args.variant, with_grid=True)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing -------------------------------------------------------------------------------
+    for _ in range(args.warmup):
+        call(x, t, f, q, out, variant=args.variant)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.fill_(1)                          # L2 flush between steps, outside the per-step events
+        a.record()
+        call(x, t, f, q, out, variant=args.variant)
+        b.record()
+    barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sharding.max_over_ranks(float(np.sum(step_ms)), dev)
+    units = sharding.sum_over_ranks(float(w.pair_q), dev)          # pair.q per step over all ranks
+    value = units * args.steps / (total_ms * 1e-3) / 1e9
+
+    # ---- dominant kernel (pairs) timed alone with events recorded by the library around its launch ----------
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); e1.record(); torch.cuda.synchronize()
+    db.set_pairs_events(e0, e1)
+    pk = []
+    for _ in range(min(args.steps, 30)):
+        flush.fill_(1)
+        call(x, t, f, q, out, variant=args.variant)
+        torch.cuda.synchronize()
+        pk.append(e0.elapsed_time(e1))
+    db.set_pairs_events(None, None)
+    pairs_ms = float(np.mean(pk))
+
+    # ---- end to end through the host-buffer C entry (pinned inputs, copies inside the timed region) ----------
+    hx, ht, hf, hq = (torch.from_numpy(a).pin_memory().numpy() for a in (w.xyz, w.type, w.fftab, w.q))
+    hout = torch.empty((w.B, w.M) if batch else (w.M,), dtype=torch.float64).pin_memory().numpy()
+    for _ in range(3):
+        call_host(hx, ht, hf, hq, hout, variant=args.variant)
+    barrier()
+    n_e2e = max(5, min(args.steps, 50))
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        call_host(hx, ht, hf, hq, hout, variant=args.variant)
+    barrier()
+    e2e_s = sharding.max_over_ranks(time.perf_counter() - t0, dev)
+    e2e_value = units * n_e2e / e2e_s / 1e9
+    h2d = int(hx.nbytes + ht.nbytes + hf.nbytes + hq.nbytes)
+    result_dev = out.cpu().numpy()
+    assert np.array_equal(result_dev, hout), "host entry and device entry disagree"
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the pairs kernel ----------------------------------------------------
+    peaks = measured_peaks()
+    fmax_ghz = float(peaks.get("sm_max_mhz", 1965.0)) / 1e3
+    variant_ran = args.variant if args.variant != "auto" else ("recur" if _is_uniform(w.q) else "mufu")
+    pq_per_launch = float(w.pair_q)
+    if variant_ran == "recur":
+        # algorithmic work per pair.q: one recurrence FMA + one accumulate add = 2 FP32-pipe lane-ops (4 flop-slots)
+        peak = SM_COUNT * FP32_LANES * 2 * fmax_ghz / 1e3                       # TFLOP/s, FMA = 2 flop
+        achieved = 4.0 * pq_per_launch / (pairs_ms * 1e-3) / 1e12
+        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": None,
+                "note": "FP32-pipe issue roofline: 2 lane-ops (FFMA + FADD = 4 FMA-equivalent flop) per pair.q; peak = "
+                        "148 SM x 128 lanes x 2 x sm_max_mhz (MEASURED_PEAKS.json clock; FFMA2 microbenchmark reaches 99 % of it)"}
+    else:
+        per_term = {"mufu": 1.0}.get(variant_ran)
+        peak = SM_COUNT * MUFU_LANES * fmax_ghz / 1e3                           # T MUFU op/s
+        achieved = pq_per_launch / (pairs_ms * 1e-3) / 1e12
+        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T sin/s", "frac": achieved / peak,
+                "traffic": None, "note": "XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM" if per_term else
+                "reference variant; XU roofline quoted for scale"}
+    roof["kernel"] = f"debye_pairs_kernel<{info['q_chunk']}, {variant_ran}>"
+    roof["kernel_ms"] = pairs_ms
+    roof["pair_q_per_clk_per_sm"] = pq_per_launch / (pairs_ms * 1e-3) / (SM_COUNT * fmax_ghz * 1e9)
+    roof["share_of_step"] = pairs_ms / (total_ms / args.steps)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if variant_ran == "fp64" else "f32", "data": "synthetic",
+        "config": {"workload": w.name, "N": w.N, "T": w.T, "M": w.M, "B": w.B, "variant": variant_ran,
+                   "pairs_grid": info["pairs_grid"], "q_chunk": info["q_chunk"], "n_chunks": info["n_chunks"],
+                   "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
+                   "parallelism": f"{world} independent structure(s), one per GPU", "wall_s_timed_loop": wall},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(hout.nbytes),
+                "ms_per_step": e2e_s / n_e2e * 1e3, "steps": n_e2e},
+        "gpu_launches": info["n_launches"] * args.steps,
+        "roofline": roof,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        cb = cpu_baseline(w)
+        from oracle import oracle as orc                   # parity of the timed call's output against the oracle
+        if not batch:
+            ks = list(range(0, w.M, max(1, w.M // 8)))
+            ref = orc.debye_sym(w.xyz, w.type, w.fftab[:, ks].copy(), w.q[ks].copy())
+            line["parity_max_rel_err"] = float(np.max(np.abs(result_dev[ks] - ref) / np.abs(ref)))
+        line["cpu_baseline"] = cb
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def _is_uniform(q):
+    q = q.astype(np.float64)
+    if len(q) < 2:
+        return True
+    line = q[0] + (q[-1] - q[0]) / (len(q) - 1) * np.arange(len(q))
+    return float(np.max(np.abs(q - line))) <= 2.4e-7 * float(np.max(np.abs(q)))
+
+
+if __name__ == "__main__":
+    main()

@@ -108,6 +108,11 @@ void debye_shutdown(void);
 int debye_launch_info(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags, int32_t *n_launches,
                       int32_t *pairs_grid, int32_t *q_chunk, int32_t *n_chunks);
 
+/* Measurement hook (bench.py's roofline leg): two caller-owned cudaEvent_t handles that every following call on
+ * this device records, on the call's stream, immediately before and after the pairs kernel launch(es) -- the
+ * dominant kernel -- so its device time can be read with cudaEventElapsedTime.  NULL, NULL switches it off. */
+int debye_set_pairs_events(void *start_event, void *stop_event);
+
 const char *debye_strerror(int status);
 int debye_last_cuda_error(void); /* cudaError_t of the last failing runtime call on this thread, 0 if none */
 int debye_version(void);         /* major*10000 + minor*100 + patch */

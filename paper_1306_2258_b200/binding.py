@@ -17,7 +17,7 @@ FLAGS = {"fp64": 1 << 0, "mufu": 1 << 2, "recur": 1 << 3, "accurate": 1 << 4, "a
 
 EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_profile_batch_host",
            "debye_partials", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
-           "debye_launch_info", "debye_strerror", "debye_last_cuda_error", "debye_version")
+           "debye_launch_info", "debye_set_pairs_events", "debye_strerror", "debye_last_cuda_error", "debye_version")
 
 
 class LibdebyeError(RuntimeError):
@@ -56,6 +56,8 @@ def lib():
     L.debye_shutdown.restype = None
     L.debye_launch_info.argtypes = [i32, i32, i32, i32, u32] + [C.POINTER(i32)] * 4
     L.debye_launch_info.restype = C.c_int
+    L.debye_set_pairs_events.argtypes = [vp, vp]
+    L.debye_set_pairs_events.restype = C.c_int
     L.debye_strerror.argtypes = [C.c_int]
     L.debye_strerror.restype = C.c_char_p
     L.debye_last_cuda_error.restype = C.c_int
@@ -154,6 +156,14 @@ def debye_profile_batch_host(xyz, type, fftab, q, I_out=None, variant="auto", st
                                           _host(fftab, np.float32, "fftab"), T, _host(q, np.float32, "q"), M,
                                           _host(I_out, np.float64, "I_out"), _flags(variant), _stream_ptr(stream)))
     return I_out
+
+
+def set_pairs_events(start=None, stop=None):
+    """Record torch.cuda.Event `start` / `stop` (created with enable_timing=True and already recorded once, so the
+    handles exist) around the pairs kernel of every following call; None, None switches the hook off."""
+    a = C.c_void_p(start.cuda_event) if start is not None else None
+    b = C.c_void_p(stop.cuda_event) if stop is not None else None
+    _check(lib().debye_set_pairs_events(a, b))
 
 
 def launch_info(N, B, T, M, variant="auto", with_grid=False):

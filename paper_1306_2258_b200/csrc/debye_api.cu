@@ -35,6 +35,7 @@ struct DevState {
     void *user_ws = nullptr; size_t user_bytes = 0;   // caller-owned scratch (debye_set_workspace)
     void *stage = nullptr; size_t stage_bytes = 0;    // device staging for the *_host entry points
     int sms = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;         // optional: recorded around the pairs launches
     int occ[5][17];                                   // cached CTAs/SM per (variant, K/8); 0 = unknown
 };
 DevState g_dev[MAX_DEV];
@@ -196,12 +197,14 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
         if (blocks > ds->sms * 16) blocks = ds->sms * 16;
         debye::debye_pack_kernel<<<blocks, 256, 0, stream>>>(plan, xyz, type, perm, sorted, N, B);
     }
+    if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
     for (int i = 0; i < nch; ++i) {
         debye_pairs_fn fn = debye_get_pairs_kernel(ch[i].variant, ch[i].K);
         // slow-path threshold on theta = r * (smallest grid step or smallest |q|): see DESIGN.md section 6
         const float theta_min = (ch[i].variant == V_RECUR) ? 0.004f : 0.004f;
         fn<<<G[i], DEBYE_IB, 0, stream>>>(plan, sorted, q, records, ch[i].n_chunks, is_auto, theta_min);
     }
+    if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
     {
         int threads = 128, blocks = (M * B + threads - 1) / threads;
         // in automatic mode the final kernel picks the parameter set of the variant chosen on the device
@@ -298,6 +301,16 @@ int debye_set_workspace(void *dev_ptr, size_t bytes)
     if ((st = dev_state(&ds))) return st;
     if (dev_ptr && ((uintptr_t)dev_ptr & 255)) return DEBYE_EINVAL;
     ds->user_ws = dev_ptr; ds->user_bytes = dev_ptr ? bytes : 0;
+    return DEBYE_OK;
+}
+
+int debye_set_pairs_events(void *start_event, void *stop_event)
+{
+    std::lock_guard<std::mutex> lock(g_mu);
+    DevState *ds; int st;
+    if ((st = dev_state(&ds))) return st;
+    if ((start_event == nullptr) != (stop_event == nullptr)) return DEBYE_EINVAL;
+    ds->ev0 = (cudaEvent_t)start_event; ds->ev1 = (cudaEvent_t)stop_event;
     return DEBYE_OK;
 }
 

@@ -1,0 +1,86 @@
+"""CPU-only checks of the boundary: libdebye.so loads, exports every symbol include/debye.h declares, and rejects
+bad arguments with the documented status codes before touching CUDA (no compute calls here)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_1306_2258_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "debye.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(debye_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_library_loads_and_exports_every_declared_symbol():
+    L = binding.lib()
+    names = declared_symbols()
+    assert set(binding.EXPORTS) == set(names), (names, binding.EXPORTS)
+    for n in names:
+        assert getattr(L, n) is not None
+    assert L.debye_version() >= 100
+
+
+def test_strerror_and_status_codes():
+    L = binding.lib()
+    assert L.debye_strerror(0) == b"ok"
+    for st in (1, 2, 3, 4, 99):
+        assert len(L.debye_strerror(st)) > 0
+
+
+def test_argument_validation_happens_before_cuda():
+    L = binding.lib()
+    buf = (C.c_char * 4096)()
+    p = C.cast(buf, C.c_void_p)
+    EINVAL, EUNSUP = 1, 2
+    ok_args = dict(N=10, T=2, M=5)
+    assert L.debye_profile(None, p, 10, p, 2, p, 5, p, 0, None) == EINVAL
+    assert L.debye_profile(p, None, 10, p, 2, p, 5, p, 0, None) == EINVAL
+    assert L.debye_profile(p, p, 10, None, 2, p, 5, p, 0, None) == EINVAL
+    assert L.debye_profile(p, p, 10, p, 2, None, 5, p, 0, None) == EINVAL
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, None, 0, None) == EINVAL
+    assert L.debye_profile(p, p, 0, p, 2, p, 5, p, 0, None) == EINVAL
+    assert L.debye_profile(p, p, 10, p, 0, p, 5, p, 0, None) == EINVAL
+    assert L.debye_profile(p, p, 10, p, 33, p, 5, p, 0, None) == EINVAL
+    assert L.debye_profile(p, p, 10, p, 2, p, 0, p, 0, None) == EINVAL
+    assert L.debye_profile(p, p, 10, p, 2, p, 4097, p, 0, None) == EINVAL
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 2) | (1 << 3), None) == EINVAL      # two sinc variants
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 0) | (1 << 2), None) == EINVAL      # fp64 + fp32 variant
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, 1 << 9, None) == EINVAL                   # unknown flag
+    assert L.debye_profile(p, p, (1 << 24) + 1, p, 2, p, 5, p, 0, None) == EUNSUP
+    assert L.debye_profile_batch(p, p, 10, 0, p, 2, p, 5, p, 0, None) == EINVAL
+    assert L.debye_profile_host(None, p, 10, p, 2, p, 5, p, 0, None) == EINVAL
+    assert L.debye_partials(p, p, 10, 1, None, 2, 5, p, None, 0, None) == EINVAL
+    del ok_args
+
+
+def test_workspace_and_launch_info_are_host_side():
+    L = binding.lib()
+    assert L.debye_workspace_bytes(0, 1, 2, 5, 0) == 0
+    small = L.debye_workspace_bytes(1000, 1, 5, 51, 0)
+    big = L.debye_workspace_bytes(200000, 1, 20, 128, 0)
+    assert 0 < small < big < (1 << 30)
+    # O(N + CTAs*T^2*M), never O(N^2): doubling N adds ~20 bytes per atom
+    a, b = L.debye_workspace_bytes(100000, 1, 5, 64, 0), L.debye_workspace_bytes(200000, 1, 5, 64, 0)
+    assert 15 * 100000 < b - a < 25 * 100000
+    info = binding.launch_info(10000, 1, 5, 101, "auto")
+    assert info == {"n_launches": 5, "q_chunk": 104, "n_chunks": 1}
+    assert binding.launch_info(50000, 1, 4, 200, "recur") == {"n_launches": 4, "q_chunk": 104, "n_chunks": 2}
+    assert binding.launch_info(1000, 1, 5, 51, "fp64")["n_chunks"] == 2
+    assert binding.launch_info(1000, 1, 5, 300, "mufu") == {"n_launches": 4, "q_chunk": 104, "n_chunks": 3}
+
+
+def test_binding_refuses_non_cuda_inputs():
+    import numpy as np
+    import torch
+    x = torch.zeros(4, 3)
+    with pytest.raises(binding.LibdebyeError):
+        binding.debye_profile(x, torch.zeros(4, dtype=torch.int32), torch.zeros(1, 2), torch.zeros(2))
+    with pytest.raises(binding.LibdebyeError):
+        binding.debye_profile_host(np.zeros((4, 3)), np.zeros(4, np.int32), np.zeros((1, 2), np.float32),
+                                   np.zeros(2, np.float32))       # float64 xyz

@@ -1,0 +1,105 @@
+"""Full-size parity: BASELINE.json's configs in the launch configuration bench.py times (automatic variant, device
+pointers), checked against (a) oracle values stored by tests/golden/make_golden.py at sampled q indices and
+(b) closed forms that follow from Eq. (2) and cost O(#distinct distances) at any N."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_1306_2258_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+TOL32, TOL64 = 1e-4, 1e-10
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_profiles.txt")
+
+
+def golden():
+    out = {}
+    for line in open(GOLD):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, b, k, q, I, A = line.split()
+        out.setdefault(name, []).append((int(b), int(k), float(q), float(I), float(A)))
+    return out
+
+
+@pytest.fixture(scope="module")
+def db():
+    from paper_1306_2258_b200 import binding
+    binding.lib()
+    return binding
+
+
+def run(db, w, variant="auto", batch=False):
+    import torch
+    x, t, f, q = (torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (w.xyz, w.type, w.fftab, w.q))
+    out = (db.debye_profile_batch if batch else db.debye_profile)(x, t, f, q, variant=variant)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def check(I, rows, w, tol):
+    worst = 0.0
+    for b, k, q, Iref, A in rows:
+        assert float(w.q[k]) == q
+        got = I[b, k] if I.ndim == 2 else I[k]
+        worst = max(worst, abs(got - Iref) / abs(Iref))
+    assert worst <= tol, worst
+    return worst
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg5"])
+def test_single_structure_configs_against_stored_oracle(db, name):
+    w = wl.CONFIGS[name]()
+    rows = golden()[name]
+    for v in ["auto", "mufu"]:
+        check(run(db, w, v), rows, w, TOL32)
+
+
+def test_cfg2_full_profile_live_oracle_and_fp64(db):
+    w = wl.cfg2()
+    ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)          # ~3-20 s on the host cores
+    assert np.max(np.abs(run(db, w) - ref) / ref) <= TOL32
+    assert np.max(np.abs(run(db, w, "fp64") - ref) / ref) <= TOL64
+
+
+def test_cfg3_literal_length_variant(db):
+    w = wl.cfg3(n_bp=200, tag="cfg3_8k")
+    rows = golden()["cfg3_8k"]
+    for v in ["auto", "mufu", "accurate"]:
+        check(run(db, w, v), rows, w, TOL32)
+    check(run(db, w, "fp64"), rows, w, TOL64)
+
+
+def test_cfg4_batch_against_stored_oracle(db):
+    w = wl.cfg4()
+    I = run(db, w, batch=True)
+    assert I.shape == (1024, 64)
+    check(I, golden()["cfg4"], w, TOL32)
+    # every conformer: I(0) = (sum f(0))^2 exactly, I > 0, and low-q values within the Guinier bound
+    tot = w.fftab.astype(np.float64)[w.type, 0].sum() ** 2
+    assert np.max(np.abs(I[:, 0] - tot) / tot) <= 1e-12
+    assert (I > 0).all() and (I[:, 1] < tot).all()
+
+
+def test_lattice_closed_form_195k_atoms(db):
+    # 58^3 = 195,112 unit scatterers: truth from grouping equal distances (exact consequence of Eq. 2)
+    w = wl.cubic_lattice(58, 58, 58, 3.0, 24, 0.25)
+    want = orc.lattice_closed_form(58, 58, 58, 3.0, w.q.astype(np.float64))
+    got = run(db, w)
+    floor = np.maximum(np.abs(want), 1e-9 * want[0])
+    assert np.max(np.abs(got - want) / floor) <= TOL32
+
+
+def test_two_type_lattice_and_chain_closed_forms(db):
+    w = wl.cubic_lattice(40, 33, 21, 2.5, 40, 0.6, T=2)
+    want = orc.lattice_closed_form(40, 33, 21, 2.5, w.q.astype(np.float64), fa=1.0, fb=2.0)
+    assert np.max(np.abs(run(db, w) - want) / want) <= TOL32
+    n, d = 60000, 1.5
+    xyz = np.zeros((n, 3), np.float32); xyz[:, 0] = np.arange(n) * d
+    q = wl.q_grid(0.4, 48)
+    wc = wl.Workload("chain", xyz, np.zeros(n, np.int32), np.ones((1, 48), np.float32), q)
+    wantc = orc.chain_closed_form(n, d, q.astype(np.float64))
+    for v in ["auto", "mufu"]:
+        assert np.max(np.abs(run(db, wc, v) - wantc) / wantc) <= TOL32

@@ -1,0 +1,239 @@
+"""GPU parity tests proper: libdebye (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances (BASELINE.json north_star): max_k |I_gpu - I_oracle| / |I_oracle| <= 1e-4 for the FP32
+accumulation paths, <= 1e-10 for the FP64 mode."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_1306_2258_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL32, TOL64 = 1e-4, 1e-10
+FP32_VARIANTS = ["auto", "recur", "mufu", "accurate"]
+
+
+def rel(a, b):
+    a, b = np.asarray(a), np.asarray(b)
+    return float(np.max(np.abs(a - b) / np.abs(b)))
+
+
+@pytest.fixture(scope="module")
+def db():
+    from paper_1306_2258_b200 import binding
+    binding.lib()
+    return binding
+
+
+def to_dev(w):
+    import torch
+    return tuple(torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (w.xyz, w.type, w.fftab, w.q))
+
+
+def gpu_profile(db, w, variant="auto", batch=False):
+    import torch
+    x, t, f, q = to_dev(w)
+    out = (db.debye_profile_batch if batch else db.debye_profile)(x, t, f, q, variant=variant)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+# sizes span several 128-atom rows / 64-atom tiles and ragged tails; T and M exercise every chunking
+CASES = [
+    ("s3_N130_T3_M17", lambda: wl.small_random(3, 130, 3, 17)),
+    ("s4_N777_T5_M101", lambda: wl.small_random(4, 777, 5, 101)),
+    ("s5_N1500_T4_M200", lambda: wl.small_random(5, 1500, 4, 200, q_max=1.0)),          # 2 recurrence chunks
+    ("s6_N600_T20_M128", lambda: wl.small_random(6, 600, 20, 128, q_max=0.3)),
+    ("s7_N900_T3_M64_offset_grid", lambda: wl.small_random(7, 900, 3, 64, q_min=0.3, q_max=0.9)),   # general start
+    ("s8_N513_T32_M40_signed", lambda: wl.small_random(8, 513, 32, 40, signed=True)),
+    ("s9_N2100_T2_M300", lambda: wl.small_random(9, 2100, 2, 300, q_max=1.2, box=60.0)),  # 4 chunks
+    ("cfg1", wl.cfg1),
+    ("table1_N1000_paper_grid", lambda: wl.table1(1000)),                                 # q_k = k/50, k = 1..50
+]
+
+
+@pytest.mark.parametrize("name,make", CASES, ids=[c[0] for c in CASES])
+def test_parity_all_variants(db, name, make):
+    w = make()
+    ref, A = orc.debye_sym(w.xyz, w.type, w.fftab, w.q, return_abs=True)
+    if (w.fftab < 0).any():
+        # signed form factors: I may come close to 0; use the documented floor 1e-4 * sum|terms| instead
+        floor = np.maximum(np.abs(ref), 1e-2 * A)
+        err = lambda I: float(np.max(np.abs(I - ref) / floor))
+    else:
+        err = lambda I: rel(I, ref)
+    assert err(gpu_profile(db, w, "fp64")) <= TOL64
+    for v in FP32_VARIANTS:
+        e = err(gpu_profile(db, w, v))
+        assert e <= TOL32, (name, v, e)
+
+
+def test_two_atom_closed_form_distance_sweep(db):
+    """I = f1^2 + f2^2 + 2 f1 f2 sin(qd)/(qd) (north_star); d from far below the slow-path cut to 3000 A."""
+    q = wl.q_grid(0.5, 101)
+    f = np.stack([np.linspace(6, 2, 101), np.linspace(8, 1, 101)]).astype(np.float32)
+    typ = np.array([0, 1], np.int32)
+    worst = {v: 0.0 for v in FP32_VARIANTS + ["fp64"]}
+    ds = [0.0, 1e-3, 0.05, 0.3, 0.7, 0.79, 0.81, 1.0, 1.37, 2.2, 3.7, 9.9, 31.4159, 62.83, 78.54, 157.08, 400.3, 1234.5, 3000.0]
+    for d in ds:
+        xyz = np.array([[0.5, 0.25, -1.0], [0.5, 0.25, -1.0 + d]], np.float32)
+        dd = float(np.float64(xyz[1, 2]) - np.float64(xyz[0, 2]))
+        qq = q.astype(np.float64)
+        s = np.where(qq * dd == 0, 1.0, np.sin(qq * dd) / np.where(qq * dd == 0, 1.0, qq * dd))
+        want = f[0].astype(np.float64) ** 2 + f[1].astype(np.float64) ** 2 + 2 * f[0].astype(np.float64) * f[1] * s
+        w = wl.Workload("two", xyz, typ, f, q)
+        for v in worst:
+            worst[v] = max(worst[v], rel(gpu_profile(db, w, v), want))
+    assert worst["fp64"] <= TOL64, worst
+    for v in FP32_VARIANTS:
+        assert worst[v] <= TOL32, worst
+
+
+def test_degenerate_inputs(db):
+    import torch
+    q = wl.q_grid(0.6, 33)
+    f = wl.gaussian_form_factors(1, 3, q)
+    # N = 1: I = f^2
+    w = wl.Workload("one", np.array([[1, 2, 3]], np.float32), np.array([1], np.int32), f, q)
+    for v in ["auto", "mufu", "fp64"]:
+        assert rel(gpu_profile(db, w, v), f[1].astype(np.float64) ** 2) <= 1e-15
+    # all atoms coincident: I = (sum f)^2 for every q
+    typ = np.array([0, 1, 2, 2, 1, 0, 0], np.int32)
+    w = wl.Workload("coin", np.tile(np.array([[1.5, -2.0, 0.25]], np.float32), (7, 1)), typ, f, q)
+    tot = f.astype(np.float64)[typ].sum(0) ** 2
+    for v in FP32_VARIANTS:
+        assert rel(gpu_profile(db, w, v), tot) <= 1e-6
+    assert rel(gpu_profile(db, w, "fp64"), tot) <= 1e-13
+    # q = 0 only (M = 1), and a single non-zero q
+    w0 = wl.small_random(20, 300, 3, 1)
+    w0.q[:] = 0
+    assert rel(gpu_profile(db, w0), w0.fftab.astype(np.float64)[w0.type, 0].sum() ** 2) <= 1e-14
+    w1 = wl.small_random(21, 300, 3, 1, q_max=0.37)
+    ref = orc.debye_sym(w1.xyz, w1.type, w1.fftab, w1.q)
+    for v in FP32_VARIANTS:
+        assert rel(gpu_profile(db, w1, v), ref) <= TOL32
+    # a type that never occurs, and a type with a single atom
+    w2 = wl.small_random(22, 400, 4, 25)
+    w2.type[w2.type == 2] = 0
+    w2.type[7] = 3
+    w2.type[w2.type == 3] = np.where(np.arange((w2.type == 3).sum()) == 0, 3, 1)
+    assert (w2.type == 2).sum() == 0 and (w2.type == 3).sum() == 1
+    ref = orc.debye_sym(w2.xyz, w2.type, w2.fftab, w2.q)
+    for v in FP32_VARIANTS:
+        assert rel(gpu_profile(db, w2, v), ref) <= TOL32
+    assert rel(gpu_profile(db, w2, "fp64"), ref) <= TOL64
+    torch.cuda.synchronize()
+
+
+def test_non_uniform_and_descending_grids(db):
+    w = wl.small_random(23, 500, 3, 40)
+    rng = np.random.default_rng(0)
+    w.q[:] = np.sort(rng.uniform(0, 0.7, 40)).astype(np.float32)
+    w.fftab[:] = wl.gaussian_form_factors(5, 3, w.q)
+    ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)
+    for v in ["auto", "mufu", "accurate"]:
+        assert rel(gpu_profile(db, w, v), ref) <= TOL32
+    assert rel(gpu_profile(db, w, "fp64"), ref) <= TOL64
+    assert np.isnan(gpu_profile(db, w, "recur")).all()          # documented: forced recurrence on a non-uniform grid
+    # descending uniform grid, and a grid containing negative q (sinc is even)
+    w2 = wl.small_random(24, 300, 2, 31)
+    w2.q[:] = w2.q[::-1].copy()
+    w2.fftab[:] = w2.fftab[:, ::-1].copy()
+    ref2 = orc.debye_sym(w2.xyz, w2.type, w2.fftab, w2.q)
+    for v in FP32_VARIANTS:
+        assert rel(gpu_profile(db, w2, v), ref2) <= TOL32
+    w3 = wl.small_random(25, 300, 2, 31)
+    w3.q[:] = np.linspace(-0.3, 0.3, 31).astype(np.float32)
+    ref3 = orc.debye_sym(w3.xyz, w3.type, w3.fftab, w3.q)
+    for v in FP32_VARIANTS:
+        assert rel(gpu_profile(db, w3, v), ref3) <= TOL32
+
+
+def test_bitwise_determinism_and_host_entry(db):
+    import torch
+    w = wl.small_random(26, 3000, 5, 101)
+    a = gpu_profile(db, w)
+    b = gpu_profile(db, w)
+    assert a.tobytes() == b.tobytes()
+    s = torch.cuda.Stream()
+    x, t, f, q = to_dev(w)
+    torch.cuda.synchronize()
+    c = db.debye_profile(x, t, f, q, stream=s)
+    s.synchronize()
+    assert c.cpu().numpy().tobytes() == a.tobytes()
+    h = db.debye_profile_host(w.xyz, w.type, w.fftab, w.q)
+    assert h.tobytes() == a.tobytes()
+
+
+def test_batch_equals_singles(db):
+    w = wl.cfg4(B=9, N=700)
+    ref = orc.debye_batch(w.xyz, w.type, w.fftab, w.q)
+    Ib = gpu_profile(db, w, batch=True)
+    assert Ib.shape == (9, w.M)
+    assert rel(Ib, ref) <= TOL32
+    for b in (0, 8):
+        one = gpu_profile(db, wl.Workload("one", w.xyz[b].copy(), w.type, w.fftab, w.q))
+        assert rel(Ib[b], one) <= 1e-6
+    assert rel(gpu_profile(db, w, "fp64", batch=True), ref) <= TOL64
+    hb = db.debye_profile_batch_host(w.xyz, w.type, w.fftab, w.q)
+    assert hb.tobytes() == Ib.tobytes()
+
+
+def test_invariances(db):
+    w = wl.small_random(27, 1200, 4, 64)
+    I = gpu_profile(db, w)
+    perm = np.random.default_rng(3).permutation(w.N)
+    wp = wl.Workload("p", w.xyz[perm].copy(), w.type[perm].copy(), w.fftab, w.q)
+    assert rel(gpu_profile(db, wp), I) <= 1e-5
+    ws = wl.Workload("s", np.ascontiguousarray(w.xyz[:, [2, 0, 1]] * np.float32(-1)), w.type, w.fftab, w.q)
+    assert rel(gpu_profile(db, ws), I) <= 1e-5
+
+
+def test_partials_reconstruct_profile_and_match_oracle(db):
+    import torch
+    w = wl.small_random(28, 400, 3, 21)
+    x, t, f, q = to_dev(w)
+    S, n = db.debye_partials(x, t, q, w.T)
+    torch.cuda.synchronize()
+    S = S.cpu().numpy()[0]; n = n.cpu().numpy()
+    assert list(n) == [int((w.type == a).sum()) for a in range(w.T)]
+    ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)
+    F = w.fftab.astype(np.float64)
+    I = (n[:, None] * F ** 2).sum(0)
+    p = 0
+    for a in range(w.T):
+        for b in range(a, w.T):
+            I += 2 * F[a] * F[b] * S[p]; p += 1
+    assert rel(I, ref) <= TOL32
+    # S_aa and S_ab straight from the oracle with indicator form factors: I_a = n_a + 2 S_aa, I_ab = n_a + n_b + 2 (S_aa + S_bb + S_ab)
+    ind = lambda ts: np.stack([np.full(w.M, 1.0 if a in ts else 0.0, np.float32) for a in range(w.T)])
+    Ia = {a: orc.debye_sym(w.xyz, w.type, ind([a]), w.q) for a in range(w.T)}
+    idx = lambda a, b: a * (2 * w.T - a + 1) // 2 + (b - a)
+    for a in range(w.T):
+        Saa = (Ia[a] - n[a]) / 2
+        assert np.max(np.abs(S[idx(a, a)] - Saa)) <= 1e-4 * np.max(np.abs(Saa)) + 1e-9
+    Iab = orc.debye_sym(w.xyz, w.type, ind([0, 2]), w.q)
+    S02 = (Iab - n[0] - n[2]) / 2 - (Ia[0] - n[0]) / 2 - (Ia[2] - n[2]) / 2
+    assert np.max(np.abs(S[idx(0, 2)] - S02)) <= 1e-4 * np.max(np.abs(S02)) + 1e-9
+
+
+def test_caller_workspace(db):
+    import torch
+    w = wl.small_random(29, 800, 3, 51)
+    ref = gpu_profile(db, w)
+    L = db.lib()
+    need = L.debye_workspace_bytes(w.N, 1, w.T, w.M, 0)
+    buf = torch.empty(need + 256, dtype=torch.uint8, device="cuda")
+    ptr = (buf.data_ptr() + 255) // 256 * 256
+    assert L.debye_set_workspace(ptr, need) == 0
+    try:
+        assert gpu_profile(db, w).tobytes() == ref.tobytes()
+        assert L.debye_set_workspace(ptr, 1024) == 0
+        with pytest.raises(db.LibdebyeError):
+            gpu_profile(db, w)
+    finally:
+        assert L.debye_set_workspace(None, 0) == 0
+    assert gpu_profile(db, w).tobytes() == ref.tobytes()

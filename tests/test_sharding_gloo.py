@@ -1,0 +1,57 @@
+"""World-size-2 (gloo, CPU) test of the multi-rank plumbing: conformer sharding, max-over-ranks timing and the
+gather of per-rank profiles.  The per-rank 'profiles' here are oracle outputs -- the data path has no collective,
+so what is tested is only that the shards tile the batch and are reassembled in order."""
+import os
+import socket
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_1306_2258_b200 import sharding
+
+
+def test_shard_range_tiles_everything():
+    for n in (0, 1, 5, 1024, 1031):
+        for world in (1, 2, 3, 8):
+            cover = []
+            for r in range(world):
+                lo, hi = sharding.shard_range(n, r, world)
+                cover += list(range(lo, hi))
+                assert 0 <= hi - lo <= n // world + 1
+            assert cover == list(range(n))
+
+
+def _free_port():
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); p = s.getsockname()[1]; s.close(); return p
+
+
+def _worker(rank, world, port, tmp):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from oracle import oracle as orc
+    from paper_1306_2258_b200 import workloads as wl
+    w = wl.cfg4(B=5, N=120)
+    lo, hi = sharding.shard_range(w.B, rank, world)
+    local = torch.from_numpy(orc.debye_batch(w.xyz[lo:hi], w.type, w.fftab, w.q))
+    full = sharding.gather_profiles(local, w.B, rank, world)
+    t = sharding.max_over_ranks(1.0 + rank)
+    s = sharding.sum_over_ranks(hi - lo)
+    if rank == 0:
+        np.save(os.path.join(tmp, "full.npy"), full.numpy())
+        np.save(os.path.join(tmp, "ts.npy"), np.array([t, s]))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_gloo_shards_and_gathers(tmp_path):
+    mp.spawn(_worker, args=(2, _free_port(), str(tmp_path)), nprocs=2, join=True)
+    from oracle import oracle as orc
+    from paper_1306_2258_b200 import workloads as wl
+    w = wl.cfg4(B=5, N=120)
+    full = np.load(tmp_path / "full.npy")
+    assert full.shape == (5, w.M)
+    assert np.array_equal(full, orc.debye_batch(w.xyz, w.type, w.fftab, w.q))
+    t, s = np.load(tmp_path / "ts.npy")
+    assert t == 2.0 and s == 5.0

@@ -57,25 +57,52 @@ __device__ __forceinline__ float sin_turns_fma(float r, float w)
     return sin_mufu(fmaf(r, w, -n) * 6.28318530717958648f);
 }
 
-// 2 cos(2 pi r w), accurate to ~2e-7 absolute and, through 2 - 4 sin^2, relatively accurate in (2 - result) for small
-// angles.  This is the recurrence coefficient: MUFU.SIN/COS (absolute error 3.4e-7 with a non-zero mean, measured on
-// B200) is not good enough here because a biased coefficient is a coherent frequency error in every chain.
-// Range reduction in turns (magic-number rounding, FMA remainder), then sin(pi f) = f Q(f^2) on |f| <= 1/2.
-__device__ __forceinline__ float two_cos_turns(float r, float w)
+// ---- accurate, UNBIASED trigonometry for the recurrence start-up ------------------------------------------------
+// Measured on B200: MUFU.SIN has an absolute error of 3.4e-7 with a NON-ZERO MEAN (-1.1e-7 on
+// (0, 0.5]).  A biased start value or a biased recurrence coefficient is a coherent phase / frequency error in every
+// chain of every pair, and the cancellation in I(q) (condition number up to ~400 in cfg5) amplifies it to 7e-4.
+// A relative frequency bias must stay below ~1e-9, so: frequencies are carried as hi + lo floats, the leading
+// polynomial coefficient pi is split hi + lo, and everything else is round-to-nearest FMA arithmetic (unbiased).
+
+// fractional part of r * (w + w_lo) in turns, in [-1/2, 1/2]: magic-number rounding, FMA remainders
+__device__ __forceinline__ float reduce_turns(float r, float w, float w_lo)
 {
-    const float MAGIC = 12582912.0f;
+    const float MAGIC = 12582912.0f;                 // 1.5 * 2^23
     const float n = fmaf(r, w, MAGIC) - MAGIC;
-    const float f = fmaf(r, w, -n);                 // in [-1/2, 1/2]
+    return fmaf(r, w_lo, fmaf(r, w, -n));
+}
+// sh = sin(pi f), ch = cos(pi f) for |f| <= 1/2 (Taylor to pi^13/13! and pi^12/12!, remainders < 6e-9 / 4e-8)
+__device__ __forceinline__ void sincos_pi(float f, float &sh, float &ch)
+{
     const float y = f * f;
-    // sin(pi f)/f: Taylor coefficients pi^(2n+1)/(2n+1)! up to n = 6 (remainder < 6e-9 on |pi f| <= pi/2)
-    float q = fmaf(y, 4.6630280576761255e-4f, -7.3704309457143504e-3f);   // pi^13/13!, -pi^11/11!
-    q = fmaf(y, q, 8.2145886611128229e-2f);                                // pi^9/9!
-    q = fmaf(y, q, -5.9926452932079208e-1f);                               // -pi^7/7!
-    q = fmaf(y, q, 2.5501640398773455f);                                   // pi^5/5!
-    q = fmaf(y, q, -5.1677127800499700f);                                  // -pi^3/3!
-    q = fmaf(y, q, 3.1415926535897932f);                                   // pi
-    const float s = f * q;
-    return fmaf(-4.0f * s, s, 2.0f);
+    float p = fmaf(y, 4.6630280576761255e-4f, -7.3704309457143504e-3f);   // pi^13/13!, -pi^11/11!
+    p = fmaf(y, p, 8.2145886611128229e-2f);                                // pi^9/9!
+    p = fmaf(y, p, -5.9926452932079208e-1f);                               // -pi^7/7!
+    p = fmaf(y, p, 2.5501640398773455f);                                   // pi^5/5!
+    p = fmaf(y, p, -5.1677127800499700f);                                  // -pi^3/3!
+    p = fmaf(y, p, -8.7422780126189537e-8f);                               // pi - (float)pi
+    sh = fmaf(f, 3.14159274101257324f, f * p);                             // (float)pi
+    float c = fmaf(y, 1.9295743094039220e-3f, -2.5806891390014050e-2f);    // pi^12/12!, -pi^10/10!
+    c = fmaf(y, c, 2.3533063035889312e-1f);                                // pi^8/8!
+    c = fmaf(y, c, -1.3352627688545893f);                                  // -pi^6/6!
+    c = fmaf(y, c, 4.0587121264167682f);                                   // pi^4/4!
+    c = fmaf(y, c, -4.9348022005446793f);                                  // -pi^2/2!
+    ch = fmaf(y, c, 1.0f);
+}
+// 2 cos(2 pi r (w + w_lo)) = 2 - 4 sin^2(pi f): relatively accurate in (2 - result) for small angles
+__device__ __forceinline__ float two_cos_turns(float r, float w, float w_lo)
+{
+    float sh, ch;
+    sincos_pi(reduce_turns(r, w, w_lo), sh, ch);
+    (void)ch;
+    return fmaf(-4.0f * sh, sh, 2.0f);
+}
+// sin(2 pi r (w + w_lo)) = 2 sin(pi f) cos(pi f)
+__device__ __forceinline__ float sin_turns_accurate(float r, float w, float w_lo)
+{
+    float sh, ch;
+    sincos_pi(reduce_turns(r, w, w_lo), sh, ch);
+    return (sh + sh) * ch;
 }
 
 // accurate sin(q r)/r for one term (slow path): Taylor for |x| < 0.25 (north_star (e)), libdevice sinf otherwise
@@ -163,7 +190,8 @@ __global__ void __launch_bounds__(DEBYE_IB) debye_pairs_kernel(const DevPlan *__
     __shared__ __align__(8) u64 mbar[2];
     __shared__ float tbuf[F64 ? 1 : NW][F64 ? 1 : 32][F64 ? 1 : 33];
     __shared__ double wsum[NW][K];
-    __shared__ float qs[(VAR == V_RECUR) ? 1 : K];    // direct variants: q of each local slot (0 for padding)
+    __shared__ float qs[(VAR == V_RECUR) ? 1 : K];
+    __shared__ float wtab[16];                        // recurrence, general start: start frequencies (hi[8], lo[8])    // direct variants: q of each local slot (0 for padding)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = gridDim.x, c = blockIdx.x;
@@ -193,7 +221,7 @@ __global__ void __launch_bounds__(DEBYE_IB) debye_pairs_kernel(const DevPlan *__
     const double dq_d = plan->dq, q0_d = plan->q0;
     const int koff = plan->zero_start;           // >= 0: grid is (k + koff) dq with koff small; -1: general
     float dqf = 0.f, cut2 = 0.f, cS_unused = 0.f;
-    float wt[8];
+    float wS_lo = 0.f, w4_lo = 0.f, w1 = 0.f, w1_lo = 0.f;
     float wS = 0.f, w4 = 0.f;   // S dq / 2 pi and 4 dq / 2 pi (turns per Angstrom of the chain / bootstrap stride)
     float qbase_l = 0.f;      // q of local slot l (recurrence): qbase_l + (S*(l/8) + (l%8)) * dq
     int zs = 0, ch_cur = 0;
@@ -281,14 +309,22 @@ __global__ void __launch_bounds__(DEBYE_IB) debye_pairs_kernel(const DevPlan *__
                 if constexpr (VAR == V_RECUR) {
                     const int S = 8 * n_chunks;
                     dqf = (float)dq_d;
-                    zs = (koff >= 0 && n_chunks == 1) ? 1 : 0;
+                    zs = (koff >= 0 && n_chunks <= 2) ? 1 : 0;
                     const double qb = (koff >= 0) ? 0.0 : q0_d;          // q of k' = 0
                     qbase_l = (float)(qb + (8.0 * ch) * dq_d);
                     const int base = -S + 8 * ch;                         // k' of the first start value
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) wt[j] = (float)((qb + (double)(base + j) * dq_d) * 0.15915494309189535);
-                    wS = (float)((double)S * dq_d * 0.15915494309189535);
-                    w4 = (float)(4.0 * dq_d * 0.15915494309189535);
+                    __syncthreads();
+                    if (tid < 8) {   // turns per Angstrom of the 8 general-start values, hi and lo parts
+                        const double wd = (qb + (double)(base + tid) * dq_d) * 0.15915494309189535;
+                        const float wh = (float)wd;
+                        wtab[tid] = wh; wtab[8 + tid] = (float)(wd - (double)wh);
+                    }
+                    __syncthreads();
+                    const double w1_d = dq_d * 0.15915494309189535;
+                    w1 = (float)w1_d; w1_lo = (float)(w1_d - (double)w1);
+                    const double wS_d = (double)S * dq_d * 0.15915494309189535, w4_d = 4.0 * dq_d * 0.15915494309189535;
+                    wS = (float)wS_d; wS_lo = (float)(wS_d - (double)wS);
+                    w4 = (float)w4_d; w4_lo = (float)(w4_d - (double)w4);
                     float rc = theta_min / fabsf(dqf);
                     cut2 = rc * rc;
                 } else {
@@ -371,23 +407,51 @@ __global__ void __launch_bounds__(DEBYE_IB) debye_pairs_kernel(const DevPlan *__
                         u64 A[4], Bv[4];
                         float cS;
                         if (zs) {
-                            // zero start (q_k' = k' dq, one chunk): v_n = sin(n theta), v_0 = 0, v_{-n} = -v_n
-                            const float th = r * dqf;
-                            const float s2 = sin_mufu(th + th);
-                            const float u1_ = sin_mufu(th) * rinv, u2_ = s2 * rinv, u3_ = sin_mufu(th * 3.0f) * rinv, u4_ = sin_mufu(th * 4.0f) * rinv;
-                            const float c4 = fmaf(-4.0f * s2, s2, 2.0f);          // 2 cos(4 theta) = 2 - 4 sin^2(2 theta)
-                            const float u5_ = fmaf(c4, u1_, u3_), u6_ = fmaf(c4, u2_, u2_), u7_ = fmaf(c4, u3_, u1_), u8_ = c4 * u4_;
-                            cS = two_cos_turns(r, wS);                            // 2 cos(8 theta)
-                            // w_0 = v_0 (B), w_{-1} = -v_{-1} = +v_{8-n} (A)
-                            Bv[0] = pk2(0.0f, u1_); Bv[1] = pk2(u2_, u3_); Bv[2] = pk2(u4_, u5_); Bv[3] = pk2(u6_, u7_);
-                            A[0] = pk2(u8_, u7_); A[1] = pk2(u6_, u5_); A[2] = pk2(u4_, u3_); A[3] = pk2(u2_, u1_);
+                            // zero start (q_k' = k' dq, 1 or 2 residue-class chunks): v_n = sin(n theta), v_0 = 0,
+                            // v_{-n} = -v_n.  sin/cos(theta/2) by polynomial, everything else by double-angle /
+                            // three-term steps (each a single rounding, so relative accuracy survives small theta).
+                            float sh, chh;
+                            sincos_pi(reduce_turns(r, w1, w1_lo), sh, chh);
+                            const float s1 = (sh + sh) * chh;                     // sin(theta)
+                            const float c1 = fmaf(-4.0f * sh, sh, 2.0f);          // 2 cos(theta)
+                            const float c2 = fmaf(-4.0f * s1, s1, 2.0f);          // 2 cos(2 theta)
+                            const float s2 = s1 * c1;                             // sin(2 theta)
+                            const float c4 = fmaf(-4.0f * s2, s2, 2.0f);          // 2 cos(4 theta)
+                            // the chain coefficient 2 cos(S theta) is NOT derived from these by further doubling: the
+                            // correlated roundings of that route leave a +7e-8 rad coherent phase bias after 16 steps
+                            // (fp32 emulation); the direct polynomial on the reduced angle has none
+                            cS = two_cos_turns(r, wS, wS_lo);
+                            float u[17];
+                            u[0] = 0.0f;
+                            u[1] = s1 * rinv; u[2] = c1 * u[1]; u[3] = fmaf(c1, u[2], -u[1]); u[4] = c2 * u[2];
+                            u[5] = fmaf(c4, u[1], u[3]); u[6] = fmaf(c4, u[2], u[2]); u[7] = fmaf(c4, u[3], u[1]); u[8] = c4 * u[4];
+                            if (n_chunks == 1) {
+                                // w_0 = v_0 (B), w_{-1} = -v_{-1} = +v_{8-n} (A)
+                                Bv[0] = pk2(u[0], u[1]); Bv[1] = pk2(u[2], u[3]); Bv[2] = pk2(u[4], u[5]); Bv[3] = pk2(u[6], u[7]);
+                                A[0] = pk2(u[8], u[7]); A[1] = pk2(u[6], u[5]); A[2] = pk2(u[4], u[3]); A[3] = pk2(u[2], u[1]);
+                            } else {
+                                // two chunks: stride S = 16, chunk ch owns k' = 16 m + 8 ch + (0..7)
+#pragma unroll
+                                for (int n = 9; n <= 16; ++n) u[n] = fmaf(c4, u[n - 4], -u[n - 8]);
+                                if (ch_cur == 0) {
+                                    Bv[0] = pk2(u[0], u[1]); Bv[1] = pk2(u[2], u[3]); Bv[2] = pk2(u[4], u[5]); Bv[3] = pk2(u[6], u[7]);
+                                    A[0] = pk2(u[16], u[15]); A[1] = pk2(u[14], u[13]); A[2] = pk2(u[12], u[11]); A[3] = pk2(u[10], u[9]);
+                                } else {
+                                    Bv[0] = pk2(u[8], u[9]); Bv[1] = pk2(u[10], u[11]); Bv[2] = pk2(u[12], u[13]); Bv[3] = pk2(u[14], u[15]);
+                                    A[0] = pk2(u[8], u[7]); A[1] = pk2(u[6], u[5]); A[2] = pk2(u[4], u[3]); A[3] = pk2(u[2], u[1]);
+                                }
+                            }
                         } else {
-                            // general start: 8 range-reduced MUFU sines at k' = base .. base+7 (base = -S + 8 ch), then the
-                            // stride-4 recurrence v_{n+4} = 2cos(4 theta) v_n - v_{n-4} walks up to k' = 8 ch .. 8 ch + 7
+                            // general start (q_0 not a small multiple of dq, or more than 2 chunks): 8 accurate sines at
+                            // k' = base .. base+7 (base = -S + 8 ch), then the stride-4 recurrence
+                            // v_{n+4} = 2cos(4 theta) v_n - v_{n-4} walks up to k' = 8 ch .. 8 ch + 7
                             float g0[4], g1[4];
 #pragma unroll
-                            for (int j = 0; j < 4; ++j) { g0[j] = sin_turns_fma(r, wt[j]) * rinv; g1[j] = sin_turns_fma(r, wt[4 + j]) * rinv; }
-                            const float c4 = two_cos_turns(r, w4);                              // 2 cos(4 theta)
+                            for (int j = 0; j < 4; ++j) {
+                                g0[j] = sin_turns_accurate(r, wtab[j], wtab[8 + j]) * rinv;
+                                g1[j] = sin_turns_accurate(r, wtab[4 + j], wtab[12 + j]) * rinv;
+                            }
+                            const float c4 = two_cos_turns(r, w4, w4_lo);                       // 2 cos(4 theta)
                             float a0[4], a1[4];
 #pragma unroll
                             for (int j = 0; j < 4; ++j) { a0[j] = g0[j]; a1[j] = g1[j]; }
@@ -396,7 +460,7 @@ __global__ void __launch_bounds__(DEBYE_IB) debye_pairs_kernel(const DevPlan *__
 #pragma unroll
                                 for (int j = 0; j < 4; ++j) { float nx = fmaf(c4, g1[j], -g0[j]); g0[j] = g1[j]; g1[j] = nx; }
                             }
-                            cS = two_cos_turns(r, wS);                                          // 2 cos(S theta)
+                            cS = two_cos_turns(r, wS, wS_lo);                                   // 2 cos(S theta)
                             Bv[0] = pk2(g0[0], g0[1]); Bv[1] = pk2(g0[2], g0[3]); Bv[2] = pk2(g1[0], g1[1]); Bv[3] = pk2(g1[2], g1[3]);
                             A[0] = pk2(-a0[0], -a0[1]); A[1] = pk2(-a0[2], -a0[3]); A[2] = pk2(-a1[0], -a1[1]); A[3] = pk2(-a1[2], -a1[3]);
                         }

@@ -105,7 +105,7 @@ def chain_closed_form(n, d, q):
     return n + 2.0 * ((n - m)[None, :] * _sinc(q[:, None] * m[None, :] * d)).sum(axis=1)
 
 
-def lattice_closed_form(nx, ny, nz, a, q, fa=1.0, fb=None):
+def lattice_closed_form(nx, ny, nz, a, q, fa=1.0, fb=None, return_abs=False):
     """nx x ny x nz simple cubic lattice, spacing a.  Unit (or fa) form factors:
     I = fa^2 sum_{alpha,beta,gamma} (nx-|alpha|)(ny-|beta|)(nz-|gamma|) sinc(q a sqrt(alpha^2+beta^2+gamma^2)).
     With fb given, sites with odd (x+y+z) carry fb: the multiplicity of each displacement splits by parity."""
@@ -133,6 +133,9 @@ def lattice_closed_form(nx, ny, nz, a, q, fa=1.0, fb=None):
     ru, inv = np.unique(r, return_inverse=True)
     mu = np.bincount(inv, weights=mult)
     out = np.empty(q.shape[0])
+    ab = np.empty(q.shape[0])
     for i, qq in enumerate(q):
-        out[i] = float((mu * _sinc(qq * ru)).sum())
-    return out
+        t = mu * _sinc(qq * ru)
+        out[i] = float(t.sum())
+        ab[i] = float(np.abs(t).sum())
+    return (out, ab) if return_abs else out

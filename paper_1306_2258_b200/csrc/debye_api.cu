@@ -201,12 +201,12 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     for (int i = 0; i < nch; ++i) {
         debye_pairs_fn fn = debye_get_pairs_kernel(ch[i].variant, ch[i].K);
         // slow-path threshold on theta = r * (smallest grid step or smallest |q|): see DESIGN.md section 6
-        const float theta_min = (ch[i].variant == V_RECUR) ? 0.004f : 0.004f;
+        const float theta_min = (ch[i].variant == V_RECUR) ? 0.002f : 0.004f;
         fn<<<G[i], DEBYE_IB, 0, stream>>>(plan, sorted, q, records, ch[i].n_chunks, is_auto, theta_min);
     }
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
     {
-        int threads = 128, blocks = (M * B + threads - 1) / threads;
+        int threads = 32 * DEBYE_FINAL_G, blocks = B * ((M + 31) / 32);
         // in automatic mode the final kernel picks the parameter set of the variant chosen on the device
         const Choice &c1 = ch[nch - 1];
         debye::debye_final_kernel<<<blocks, threads, 0, stream>>>(plan, records, fftab, q, out, is_auto, ch[0].variant, ch[0].K, ch[0].n_chunks, G[0], c1.variant, c1.K,

@@ -133,57 +133,70 @@ __device__ __forceinline__ double pair_count(int na, int nb, bool diag) { return
 
 // S7: fixed-order FP64 sum of the per-CTA records, then the form-factor epilogue
 //   I(q_k) = sum_a n_a F_a^2 + 2 sum_{a<=b} F_a F_b S_ab(q_k),   S_ab = (1/q_k) sum sin(q_k r)/r  (q_k != 0), #pairs (q_k == 0).
-// One thread per (conformer, k).  mode 0: write I_out[b][k]; mode 1: write S_out[b][tp][k] (sinc sums, no form factors).
-__global__ void debye_final_kernel(const DevPlan *__restrict__ plan, const double *__restrict__ records, const float *__restrict__ fftab, const float *__restrict__ q,
-                                   double *__restrict__ out, int is_auto, int variant0, int K0, int nc0, int G0, int variant1, int K1, int nc1, int G1, int mode)
+// Block = (conformer, tile of 32 q indices); thread (kk, g) handles q index k0 + kk and the type pairs g, g+8, ... in
+// increasing order; the 8 partial sums are then added in g order.  Every order is fixed, so the result is bitwise
+// reproducible.  Record reads are coalesced over kk.  mode 0: write I_out[b][k]; mode 1: write S_out[b][tp][k].
+#define DEBYE_FINAL_G 8
+__global__ void __launch_bounds__(32 * DEBYE_FINAL_G) debye_final_kernel(const DevPlan *__restrict__ plan, const double *__restrict__ records,
+                                                                            const float *__restrict__ fftab, const float *__restrict__ q, double *__restrict__ out,
+                                                                            int is_auto, int variant0, int K0, int nc0, int G0, int variant1, int K1, int nc1, int G1,
+                                                                            int mode)
 {
+    __shared__ double part[DEBYE_FINAL_G][32];
     const int M = plan->M, Bn = plan->B, T = plan->T, n_tp = plan->n_tp;
-    const int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= M * Bn) return;
-    const int b = g / M, k = g % M;
+    const int ktiles = (M + 31) / 32;
+    const int b = blockIdx.x / ktiles, k = (blockIdx.x % ktiles) * 32 + (threadIdx.x & 31), g = threadIdx.x >> 5;
+    const bool live = k < M;
     // automatic mode: two pairs kernels were launched and the device ran the one named by plan->variant_auto
     const bool second = is_auto && plan->variant_auto == variant1;
     const int variant = second ? variant1 : variant0, K = second ? K1 : K0, n_chunks = second ? nc1 : nc0, G = second ? G1 : G0;
-    if (variant == V_RECUR && !plan->uniform) {          // forced recurrence on a non-uniform grid
-        const double nan = __longlong_as_double(0x7ff8000000000000LL);
-        if (mode == 0) out[g] = nan; else for (int tp = 0; tp < n_tp; ++tp) out[((int64_t)b * n_tp + tp) * M + k] = nan;
-        return;
-    }
-    int kprime = k;
-    if (variant == V_RECUR && plan->zero_start > 0) kprime = k + plan->zero_start;
-    int ch, l;
-    slot_of(variant, K, n_chunks, kprime, ch, l);
-    const double qk = (double)q[k];
-    const int64_t U1 = plan->U1, Uc = U1 * n_chunks, U = Uc * Bn;
+    const bool bad = (variant == V_RECUR && !plan->uniform);          // forced recurrence on a non-uniform grid -> NaN
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
     double I = 0.0;
-    int tp = 0;
-    for (int a = 0; a < T; ++a) {
-        const double fa = (mode == 0) ? (double)fftab[a * M + k] : 1.0;
-        I += (double)plan->n_a[a] * fa * fa;
-        for (int b2 = a; b2 < T; ++b2, ++tp) {
-            const double fb = (mode == 0) ? (double)fftab[b2 * M + k] : 1.0;
+    if (live) {
+        int kprime = k;
+        if (variant == V_RECUR && plan->zero_start > 0) kprime = k + plan->zero_start;
+        int ch, l;
+        slot_of(variant, K, n_chunks, kprime, ch, l);
+        const double qk = (double)q[k];
+        const int64_t U1 = plan->U1, Uc = U1 * n_chunks, U = Uc * Bn;
+        // type pair index -> (a, b2): walk rows of the upper triangle
+        int a = 0, rowstart = 0;
+        for (int tp = g; tp < n_tp; tp += DEBYE_FINAL_G) {
+            while (tp >= rowstart + (T - a)) { rowstart += T - a; ++a; }
+            const int b2 = a + (tp - rowstart);
             double S;
             const int64_t units = plan->tp_prefix[tp + 1] - plan->tp_prefix[tp];
-            if (qk == 0.0 || units == 0) {
-                S = pair_count(plan->n_a[a], plan->n_a[b2], a == b2);
-            } else {
+            if (bad) S = nan;
+            else if (qk == 0.0 || units == 0) S = pair_count(plan->n_a[a], plan->n_a[b2], a == b2);
+            else {
                 const int64_t ub = (int64_t)b * Uc + plan->tp_prefix[tp] * n_chunks + (int64_t)ch * units;
                 const int64_t ue = ub + units - 1;
-                const int c_lo = debye_owner(U, G, ub), c_hi = debye_owner(U, G, ue);
                 const int64_t X = ((int64_t)b * n_tp + tp) * n_chunks + ch;
                 double s = 0.0;
-                for (int c = c_lo; c <= c_hi; ++c) {
-                    // CTAs whose range is empty (more CTAs than units) wrote nothing
-                    const int64_t cb = debye_range_begin(U, c, G), ce = (c + 1 == G) ? U : debye_range_begin(U, c + 1, G);
-                    if (cb < ce) s += records[((int64_t)c + X) * K + l];
+                if (U >= G) {           // every CTA owns at least one unit: all CTAs between the owners took part
+                    const int c_lo = debye_owner(U, G, ub), c_hi = debye_owner(U, G, ue);
+#pragma unroll 4
+                    for (int c = c_lo; c <= c_hi; ++c) s += records[((int64_t)c + X) * K + l];
+                } else {                // fewer units than CTAs: each unit has its own CTA
+                    for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)debye_owner(U, G, u) + X) * K + l];
                 }
                 S = s / qk;
             }
-            if (mode == 0) I += 2.0 * fa * fb * S;
+            if (mode == 0) I += 2.0 * (double)fftab[a * M + k] * (double)fftab[b2 * M + k] * S;
             else out[((int64_t)b * n_tp + tp) * M + k] = S;
         }
     }
-    if (mode == 0) out[g] = I;
+    if (mode != 0) return;
+    part[g][threadIdx.x & 31] = I;
+    __syncthreads();
+    if (g == 0 && live) {
+        double tot = 0.0;
+        for (int a = 0; a < T; ++a) { const double fa = (double)fftab[a * M + k]; tot += (double)plan->n_a[a] * fa * fa; }
+#pragma unroll
+        for (int gg = 0; gg < DEBYE_FINAL_G; ++gg) tot += part[gg][threadIdx.x & 31];
+        out[(int64_t)b * M + k] = tot;
+    }
 }
 
 }  // namespace debye

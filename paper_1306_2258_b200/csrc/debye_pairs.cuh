@@ -105,13 +105,17 @@ __device__ __forceinline__ float sin_turns_accurate(float r, float w, float w_lo
     return (sh + sh) * ch;
 }
 
-// accurate sin(q r)/r for one term (slow path): Taylor for |x| < 0.25 (north_star (e)), libdevice sinf otherwise
+// accurate sin(q r)/r for one term (slow path): Taylor for |x| < 0.6 (north_star (e)), libdevice sinf otherwise
 __device__ __forceinline__ float term_accurate(float qk, float r)
 {
     float x = qk * r;
-    if (fabsf(x) < 0.25f) {
+    if (fabsf(x) < 0.6f) {     // remainder x^12/13! < 4e-13
         float x2 = x * x;
-        float p = fmaf(x2, fmaf(x2, fmaf(x2, -1.0f / 5040.0f, 1.0f / 120.0f), -1.0f / 6.0f), 1.0f);
+        float p = fmaf(x2, -1.0f / 39916800.0f, 1.0f / 362880.0f);
+        p = fmaf(x2, p, -1.0f / 5040.0f);
+        p = fmaf(x2, p, 1.0f / 120.0f);
+        p = fmaf(x2, p, -1.0f / 6.0f);
+        p = fmaf(x2, p, 1.0f);
         return qk * p;
     }
     return sinf(x) / r;
@@ -175,7 +179,7 @@ struct PairAcc {
 #endif
 
 template <int K, int VAR>
-__global__ void __launch_bounds__(DEBYE_IB) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
+__global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (K <= 64 ? 4 : (K <= 112 ? 3 : 2))) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
                                                                double *__restrict__ records, int n_chunks, int is_auto, float theta_min)
 {
     // ---- variant gate (decided on the device so the host never reads q) ---------------------------------------

@@ -12,7 +12,7 @@
 #define DEBYE_MAX_TYPES_I 32
 #define DEBYE_MAX_TP (DEBYE_MAX_TYPES_I * (DEBYE_MAX_TYPES_I + 1) / 2)
 #define DEBYE_IB 128          // i atoms per row == threads per pairs CTA
-#define DEBYE_JT 64           // j atoms per shared-memory tile (1 KB, one cp.async.bulk)
+#define DEBYE_JT 512          // j atoms per shared-memory tile (8 KB, one cp.async.bulk); 2 buffers per CTA
 
 enum DebyeVariant : int32_t { V_NONE = 0, V_F64 = 1, V_MUFU = 2, V_RECUR = 3, V_ACCURATE = 4 };
 

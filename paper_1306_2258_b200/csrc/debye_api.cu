@@ -124,7 +124,12 @@ int dev_state(DevState **st)
     return DEBYE_OK;
 }
 
-int grid_for(DevState *s, const Choice &c, int *G)
+// Grid of the pairs kernel: resident CTAs (SMs x occupancy) times a small number of waves.  The warp schedulers favour
+// one of the CTAs that share an SM, so with exactly one wave the favoured CTA finishes ~30 % early and its partner runs
+// the tail alone (measured); a few waves let the hardware block scheduler refill the SM.  More waves
+// cost one prologue + one FP64 flush per CTA, so the count is bounded by the work available (estimated from N alone:
+// the host never sees the type histogram).
+int grid_for(DevState *s, const Choice &c, int N, int B, int *G)
 {
     int &o = s->occ[c.variant][c.K / 8];
     if (o == 0) {
@@ -135,7 +140,12 @@ int grid_for(DevState *s, const Choice &c, int *G)
         if (nb < 1) nb = 1;
         o = nb;
     }
-    *G = s->sms * o;
+    const int resident = s->sms * o;
+    const double units = (double)B * c.n_chunks * ((double)N * (double)N / (2.0 * DEBYE_IB));   // j atoms x rows, all type pairs
+    int waves = (int)(units / ((double)resident * 600.0));
+    if (waves < 1) waves = 1;
+    if (waves > 4) waves = 4;
+    *G = resident * waves;
     return DEBYE_OK;
 }
 
@@ -178,7 +188,7 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     Choice ch[2]; int is_auto = 0;
     const int nch = variants_for(flags, ch, M, &is_auto);
     int G[2] = {0, 0}, Gmax = 0;
-    for (int i = 0; i < nch; ++i) { if ((st = grid_for(ds, ch[i], &G[i]))) return st; if (G[i] > Gmax) Gmax = G[i]; }
+    for (int i = 0; i < nch; ++i) { if ((st = grid_for(ds, ch[i], N, B, &G[i]))) return st; if (G[i] > Gmax) Gmax = G[i]; }
     const Layout L = layout(N, B, T, M, Gmax, ch, nch);
     char *ws;
     if (ds->user_ws) { if (ds->user_bytes < L.total) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
@@ -290,8 +300,8 @@ size_t debye_workspace_bytes(int32_t N, int32_t B, int32_t T, int32_t M, uint32_
     if (validate(&dummy, &dummy, N, B, &dummy, T, &dummy, M, &dummy, flags)) return 0;
     Choice ch[2]; int is_auto;
     int nch = variants_for(flags, ch, M, &is_auto);
-    // grid is at most 148 SMs x 16 CTAs on any sm_100 part; use a safe upper bound so no device query is needed
-    return layout(N, B, T, M, 192 * 16, ch, nch).total;
+    // grid is at most 148 SMs x 16 CTAs x 4 waves on any sm_100 part; use a safe upper bound so no device query is needed
+    return layout(N, B, T, M, 192 * 16 * 4, ch, nch).total;
 }
 
 int debye_set_workspace(void *dev_ptr, size_t bytes)
@@ -334,7 +344,7 @@ int debye_launch_info(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags
         std::lock_guard<std::mutex> lock(g_mu);
         DevState *ds; int G = 0;
         if ((st = dev_state(&ds))) return st;
-        if ((st = grid_for(ds, ch[0], &G))) return st;
+        if ((st = grid_for(ds, ch[0], N, B, &G))) return st;
         *pairs_grid = G;
     }
     return DEBYE_OK;

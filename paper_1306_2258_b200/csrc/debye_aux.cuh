@@ -181,7 +181,7 @@ __global__ void __launch_bounds__(32 * DEBYE_FINAL_G) debye_final_kernel(const D
                 } else {                // fewer units than CTAs: each unit has its own CTA
                     for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)debye_owner(U, G, u) + X) * K + l];
                 }
-                S = s / qk;
+                S = (variant == V_RECUR ? 0.5 * s : s) / qk;     // the recurrence kernel accumulates 2 sin(q r)/r
             }
             if (mode == 0) I += 2.0 * (double)fftab[a * M + k] * (double)fftab[b2 * M + k] * S;
             else out[((int64_t)b * n_tp + tp) * M + k] = S;

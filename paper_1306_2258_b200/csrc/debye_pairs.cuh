@@ -71,38 +71,40 @@ __device__ __forceinline__ float reduce_turns(float r, float w, float w_lo)
     const float n = fmaf(r, w, MAGIC) - MAGIC;
     return fmaf(r, w_lo, fmaf(r, w, -n));
 }
-// sh = sin(pi f), ch = cos(pi f) for |f| <= 1/2 (Taylor to pi^13/13! and pi^12/12!, remainders < 6e-9 / 4e-8)
-__device__ __forceinline__ void sincos_pi(float f, float &sh, float &ch)
+// th = 2 sin(pi f), ch2 = 2 cos(pi f) for |f| <= 1/2 (Taylor to pi^13/13! and pi^12/12!, remainders < 6e-9 / 4e-8).
+// Every coefficient is the plain one times 2 (exact), so the roundings are those of the undoubled polynomial; the
+// doubled values feed 2cos(2x) = 2 - (2 sin x)^2 and 2 sin(2x) = (2 sin x)(2 cos x) / 1 without extra multiplies.
+__device__ __forceinline__ void sincos_pi_x2(float f, float &th, float &ch2)
 {
     const float y = f * f;
-    float p = fmaf(y, 4.6630280576761255e-4f, -7.3704309457143504e-3f);   // pi^13/13!, -pi^11/11!
-    p = fmaf(y, p, 8.2145886611128229e-2f);                                // pi^9/9!
-    p = fmaf(y, p, -5.9926452932079208e-1f);                               // -pi^7/7!
-    p = fmaf(y, p, 2.5501640398773455f);                                   // pi^5/5!
-    p = fmaf(y, p, -5.1677127800499700f);                                  // -pi^3/3!
-    p = fmaf(y, p, -8.7422780126189537e-8f);                               // pi - (float)pi
-    sh = fmaf(f, 3.14159274101257324f, f * p);                             // (float)pi
-    float c = fmaf(y, 1.9295743094039220e-3f, -2.5806891390014050e-2f);    // pi^12/12!, -pi^10/10!
-    c = fmaf(y, c, 2.3533063035889312e-1f);                                // pi^8/8!
-    c = fmaf(y, c, -1.3352627688545893f);                                  // -pi^6/6!
-    c = fmaf(y, c, 4.0587121264167682f);                                   // pi^4/4!
-    c = fmaf(y, c, -4.9348022005446793f);                                  // -pi^2/2!
-    ch = fmaf(y, c, 1.0f);
+    float p = fmaf(y, 2.0f * 4.6630280576761255e-4f, 2.0f * -7.3704309457143504e-3f);   // pi^13/13!, -pi^11/11!
+    p = fmaf(y, p, 2.0f * 8.2145886611128229e-2f);                                       // pi^9/9!
+    p = fmaf(y, p, 2.0f * -5.9926452932079208e-1f);                                      // -pi^7/7!
+    p = fmaf(y, p, 2.0f * 2.5501640398773455f);                                          // pi^5/5!
+    p = fmaf(y, p, 2.0f * -5.1677127800499700f);                                         // -pi^3/3!
+    p = fmaf(y, p, 2.0f * -8.7422780126189537e-8f);                                      // pi - (float)pi
+    th = fmaf(f, 2.0f * 3.14159274101257324f, f * p);                                    // (float)pi
+    float c = fmaf(y, 2.0f * 1.9295743094039220e-3f, 2.0f * -2.5806891390014050e-2f);    // pi^12/12!, -pi^10/10!
+    c = fmaf(y, c, 2.0f * 2.3533063035889312e-1f);                                       // pi^8/8!
+    c = fmaf(y, c, 2.0f * -1.3352627688545893f);                                         // -pi^6/6!
+    c = fmaf(y, c, 2.0f * 4.0587121264167682f);                                          // pi^4/4!
+    c = fmaf(y, c, 2.0f * -4.9348022005446793f);                                         // -pi^2/2!
+    ch2 = fmaf(y, c, 2.0f);
 }
-// 2 cos(2 pi r (w + w_lo)) = 2 - 4 sin^2(pi f): relatively accurate in (2 - result) for small angles
+// 2 cos(2 pi r (w + w_lo)) = 2 - (2 sin(pi f))^2: relatively accurate in (2 - result) for small angles
 __device__ __forceinline__ float two_cos_turns(float r, float w, float w_lo)
 {
-    float sh, ch;
-    sincos_pi(reduce_turns(r, w, w_lo), sh, ch);
-    (void)ch;
-    return fmaf(-4.0f * sh, sh, 2.0f);
+    float th, ch2;
+    sincos_pi_x2(reduce_turns(r, w, w_lo), th, ch2);
+    (void)ch2;
+    return fmaf(-th, th, 2.0f);
 }
-// sin(2 pi r (w + w_lo)) = 2 sin(pi f) cos(pi f)
-__device__ __forceinline__ float sin_turns_accurate(float r, float w, float w_lo)
+// 2 sin(2 pi r (w + w_lo)) = (2 sin(pi f)) (2 cos(pi f))
+__device__ __forceinline__ float two_sin_turns_accurate(float r, float w, float w_lo)
 {
-    float sh, ch;
-    sincos_pi(reduce_turns(r, w, w_lo), sh, ch);
-    return (sh + sh) * ch;
+    float th, ch2;
+    sincos_pi_x2(reduce_turns(r, w, w_lo), th, ch2);
+    return th * ch2;
 }
 
 // accurate sin(q r)/r for one term (slow path): Taylor for |x| < 0.6 (north_star (e)), libdevice sinf otherwise
@@ -156,16 +158,6 @@ __host__ __device__ inline void slot_of(int variant, int K, int n_chunks, int kp
     }
 }
 
-struct ChunkConst {          // per (q-chunk) constants of the recurrence variant, rebuilt when the chunk changes
-    float dq;                // theta = r * dq
-    float w[8];              // general start: turns per Angstrom of the 8 MUFU start values
-    float c4turn;            // general start: 4 dq / (2 pi)
-    float cut2;              // r^2 below which the slow path is taken
-    float qbase, qstep;      // slow path / direct: q of local slot l is computed from these (recurrence) ...
-    int zs;                  // zero start usable for this chunk
-    int ch;
-};
-
 template <int K, int VAR>
 struct PairAcc {
     // FP32 variants: K/2 packed accumulators; F64: K doubles
@@ -174,12 +166,252 @@ struct PairAcc {
     elem_t v[NE];
 };
 
+// ---- recurrence variant: per-pair start values, packed hot loop, software-pipelined tile loop ------------------
+// All recurrence accumulators hold TWICE sin(q r)/r (the doubled trigonometry above saves five multiplies per
+// pair); the final kernel halves the sum.
+struct RecurConst {
+    float w1, w1_lo;         // dq / 2 pi, hi + lo: theta / 2 pi = r * (w1 + w1_lo)
+    float wS, wS_lo;         // S dq / 2 pi (chain stride S = 8 n_chunks)
+    float w4, w4_lo;         // 4 dq / 2 pi (general start: bootstrap stride)
+    float cut2;              // r^2 at or below which the pair takes the slow path
+    float dqf, qbase_l;      // slow path: q of local slot l is qbase_l + (S (l / 8) + l % 8) dqf
+    int n_chunks;
+};
+
+enum RecurMode : int { RM_Z1 = 0, RM_Z2A = 1, RM_Z2B = 2, RM_G = 3 };
+// RM_Z1   grid q_k' = k' dq, one chunk  (S = 8):  chains start at k' = 0..7
+// RM_Z2A  grid q_k' = k' dq, two chunks (S = 16), chunk 0: k' = 16 m + (0..7)
+// RM_Z2B  same, chunk 1: k' = 16 m + 8 + (0..7)
+// RM_G    any uniform grid / any number of chunks: 8 accurate sines at k' = 8 ch - S + (0..7), stride-4 bootstrap
+
+// The start-up of one pair is split into two stages so that the tile loop can run them one and two groups ahead of the
+// packed loop (three-stage software pipeline).
+// Stage A (geometry): distance, 1/r, slow-path flag and the two reduced angles (turns, in [-1/2, 1/2]).
+struct RecurGeom { float r, rinv, f1, fS; bool slow; };
+template <int MODE>
+__device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, const bool ok, const RecurConst &rc, RecurGeom &g)
+{
+    const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+    const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+    const bool small = !(r2 > rc.cut2);
+    const float r2c = fmaxf(r2, 1e-30f);
+    const float rinv = rsqrt_mufu(r2c);
+    g.r = r2c * rinv;
+    g.rinv = (ok && !small) ? rinv : 0.0f;      // zero for masked / slow-path pairs: every start value becomes exactly 0
+    g.slow = small && ok;
+    g.fS = reduce_turns(g.r, rc.wS, rc.wS_lo);
+    if constexpr (MODE != RM_G) g.f1 = reduce_turns(g.r, rc.w1, rc.w1_lo);
+    else g.f1 = 0.0f;
+}
+// Stage B (values): Bv = w_0 (the 8 residues), A = w_{-1}, cS = 2 cos(S theta).
+template <int MODE>
+__device__ __forceinline__ void recur_vals(const RecurGeom &g, const RecurConst &rc, const float *wtab, u64 (&A)[4], u64 (&Bv)[4], float &cS)
+{
+    const float r = g.r, rinv = g.rinv;
+    {   // the chain coefficient 2 cos(S theta) is NOT derived from 2 cos(theta) by repeated doubling: the correlated
+        // roundings of that route leave a +7e-8 rad coherent phase bias after 16 steps (fp32 emulation, DESIGN.md
+        // section 6); the direct polynomial on the reduced angle has none
+        float th, ch2;
+        sincos_pi_x2(g.fS, th, ch2);
+        (void)ch2;
+        cS = fmaf(-th, th, 2.0f);
+    }
+    if constexpr (MODE != RM_G) {
+        // zero start: v_n = 2 sin(n theta)/r, v_0 = 0, v_{-n} = -v_n.  2 sin(theta/2) and 2 cos(theta/2) by polynomial,
+        // everything else by double-angle / three-term steps (each a single rounding, so relative accuracy survives
+        // small theta).  T_n = 2 sin(n theta), c_n = 2 cos(n theta).
+        float th, ch2;
+        sincos_pi_x2(g.f1, th, ch2);
+        const float T1 = th * ch2;
+        const float c1 = fmaf(-th, th, 2.0f);
+        const float c2 = fmaf(-T1, T1, 2.0f);
+        const float T2 = T1 * c1;
+        const float c4 = fmaf(-T2, T2, 2.0f);
+        float u[17];
+        u[0] = 0.0f;
+        u[1] = T1 * rinv; u[2] = c1 * u[1]; u[3] = fmaf(c1, u[2], -u[1]); u[4] = c2 * u[2];
+        u[5] = fmaf(c4, u[1], u[3]); u[6] = fmaf(c4, u[2], u[2]); u[7] = fmaf(c4, u[3], u[1]); u[8] = c4 * u[4];
+        if constexpr (MODE == RM_Z1) {
+            // w_0 = v_0 (B), w_{-1} = -v_{-1} = +v_{8-n} (A)
+            Bv[0] = pk2(u[0], u[1]); Bv[1] = pk2(u[2], u[3]); Bv[2] = pk2(u[4], u[5]); Bv[3] = pk2(u[6], u[7]);
+            A[0] = pk2(u[8], u[7]); A[1] = pk2(u[6], u[5]); A[2] = pk2(u[4], u[3]); A[3] = pk2(u[2], u[1]);
+        } else {
+#pragma unroll
+            for (int n = 9; n <= 16; ++n) u[n] = fmaf(c4, u[n - 4], -u[n - 8]);
+            if constexpr (MODE == RM_Z2A) {
+                Bv[0] = pk2(u[0], u[1]); Bv[1] = pk2(u[2], u[3]); Bv[2] = pk2(u[4], u[5]); Bv[3] = pk2(u[6], u[7]);
+                A[0] = pk2(u[16], u[15]); A[1] = pk2(u[14], u[13]); A[2] = pk2(u[12], u[11]); A[3] = pk2(u[10], u[9]);
+            } else {
+                Bv[0] = pk2(u[8], u[9]); Bv[1] = pk2(u[10], u[11]); Bv[2] = pk2(u[12], u[13]); Bv[3] = pk2(u[14], u[15]);
+                A[0] = pk2(u[8], u[7]); A[1] = pk2(u[6], u[5]); A[2] = pk2(u[4], u[3]); A[3] = pk2(u[2], u[1]);
+            }
+        }
+    } else {
+        // general start (q_0 not a small multiple of dq, or more than 2 chunks): 8 accurate sines at
+        // k' = base .. base+7 (base = -S + 8 ch), then the stride-4 recurrence v_{n+4} = 2cos(4 theta) v_n - v_{n-4}
+        // walks up to k' = 8 ch .. 8 ch + 7
+        float g0[4], g1[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            g0[j] = two_sin_turns_accurate(r, wtab[j], wtab[8 + j]) * rinv;
+            g1[j] = two_sin_turns_accurate(r, wtab[4 + j], wtab[12 + j]) * rinv;
+        }
+        const float c4 = two_cos_turns(r, rc.w4, rc.w4_lo);
+        float a0[4], a1[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { a0[j] = g0[j]; a1[j] = g1[j]; }
+        for (int st = 0; st < 2 * rc.n_chunks; ++st) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { float nx = fmaf(c4, g1[j], -g0[j]); g0[j] = g1[j]; g1[j] = nx; }
+        }
+        Bv[0] = pk2(g0[0], g0[1]); Bv[1] = pk2(g0[2], g0[3]); Bv[2] = pk2(g1[0], g1[1]); Bv[3] = pk2(g1[2], g1[3]);
+        A[0] = pk2(-a0[0], -a0[1]); A[1] = pk2(-a0[2], -a0[3]); A[2] = pk2(-a1[0], -a1[1]); A[3] = pk2(-a1[2], -a1[3]);
+    }
+}
+
+// Packed hot loop of one pair: w_m = sigma_m v_m with sigma = (+,+,-,-): w_{m+1} = (+/-) cS w_m + w_{m-1}; 4 packed chains
+// (8 residues), K/8 steps: per term one FFMA2 lane and one FADD2 lane.  A and Bv are consumed.
+template <int K>
+__device__ __forceinline__ void recur_hot(u64 (&acc)[K / 2], u64 (&A)[4], u64 (&Bv)[4], const float cS)
+{
+    const u64 cP = pk2(cS, cS), cN = pk2(-cS, -cS);
+#pragma unroll
+    for (int m = 0; m < K / 8; ++m) {
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            if (m & 2) acc[4 * m + a] = sub2(acc[4 * m + a], Bv[a]);
+            else acc[4 * m + a] = add2(acc[4 * m + a], Bv[a]);
+            if (m + 1 < K / 8) {
+                u64 nx = fma2((m & 1) ? cN : cP, Bv[a], A[a]);
+                A[a] = Bv[a];
+                Bv[a] = nx;
+            }
+        }
+    }
+}
+
+// Slow path of one pair (theta = r dq at or below theta_min, or coincident atoms).  The three-term chain loses the
+// pair's frequency when 2cos(S theta) rounds next to 2 (relative error of theta^2 is 6e-8 / (S theta)^2), so these pairs
+// run Reinsch's form of the same chain, which carries beta = 4 sin^2(S theta / 2) = 2 - 2cos(S theta) with full relative
+// accuracy:   d_{m+1} = d_m - beta s_m,   s_{m+1} = s_m + d_{m+1},   s_0 = v(k'_j),  d_0 = v(k'_j) - v(k'_j - S).
+// Start values are those of the fast path evaluated with the true 1/r (for r = 0 the clamp r^2 >= 1e-30 makes
+// 2 sin(n theta)/r come out as its limit 2 n dq).  Three packed lane-operations per term; rare, so cost is irrelevant.
+template <int K, int MODE>
+__device__ __forceinline__ void recur_slow_pair(u64 (&acc)[K / 2], const float4 pj, const float4 pi, const RecurConst &rc, const float *wtab)
+{
+    RecurConst rs = rc;
+    rs.cut2 = -1.0f;                       // never "small": stage A keeps the true 1/r
+    RecurGeom g;
+    recur_geom<MODE>(pj, pi, true, rs, g);
+    u64 A[4], Bv[4];
+    float cS;
+    recur_vals<MODE>(g, rc, wtab, A, Bv, cS);
+    (void)cS;
+    // beta from the polynomial directly (2 - cS would cancel)
+    float th, ch2;
+    sincos_pi_x2(g.fS, th, ch2);
+    (void)ch2;
+    const float nbeta = -th * th;
+    const u64 nb2 = pk2(nbeta, nbeta);
+    // stage B returns A = w_{-1} = -v_{-1} (sign convention of the fast loop): d_0 = v_0 - v_{-1} = Bv + A
+    u64 s[4], d[4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) { s[a] = Bv[a]; d[a] = add2(Bv[a], A[a]); }
+#pragma unroll
+    for (int m = 0; m < K / 8; ++m) {
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            acc[4 * m + a] = add2(acc[4 * m + a], s[a]);
+            if (m + 1 < K / 8) {
+                d[a] = fma2(nb2, s[a], d[a]);
+                s[a] = add2(s[a], d[a]);
+            }
+        }
+    }
+}
+
+// Occupancy policy (measured on B200, profiles/): the K accumulators dominate the register budget.  K <= 64 fits 4 CTAs
+// of 128 threads per SM (128 registers), K <= 80 fits 3 (168), larger K runs 2 CTAs per SM with up to 255 registers and
+// makes up for the missing warps with NP = 2 pairs in flight per thread.
+#ifndef DEBYE_K4
+#define DEBYE_K4 64
+#endif
+#ifndef DEBYE_K3
+#define DEBYE_K3 80
+#endif
+__host__ __device__ constexpr int recur_min_ctas(int K) { return K <= DEBYE_K4 ? 4 : (K <= DEBYE_K3 ? 3 : 2); }
+#ifdef DEBYE_NP
+__host__ __device__ constexpr int recur_np(int K) { return DEBYE_NP; }
+#else
+__host__ __device__ constexpr int recur_np(int K) { return K <= DEBYE_K3 ? 1 : 2; }
+#endif
+
+// One shared-memory tile of j atoms against this thread's i atom, NP pairs per iteration.  The start values of
+// pairs jj+NP .. jj+2NP-1 are computed in the same basic block as the packed loops of pairs jj .. jj+NP-1, so the
+// scheduler hides their dependency chain (distance, rsqrt, range reduction, polynomials: ~60 dependent FP32
+// instructions) under the independent packed instructions.  NP > 1 gives that much more instruction-level
+// parallelism per warp at 17 registers per extra pair -- the K accumulators, which are what limits the number of
+// resident warps, are shared by all NP pairs.
+template <int K, int MODE>
+__device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__restrict__ tile, const int jj0, const int cnt, const float4 pi,
+                                           const bool ivalid, const bool diag, const int i_local, const int jl0, const RecurConst &rc,
+                                           const float *wtab)
+{
+    constexpr int NP = recur_np(K);
+    if (jj0 >= cnt) return;
+    auto geom = [&](const int jbase, RecurGeom (&g)[NP]) {
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            const int j = min(jbase + p, cnt - 1);
+            const bool ok = ivalid && (jbase + p < cnt) && (!diag || (jl0 + j > i_local));
+            recur_geom<MODE>(tile[j], pi, ok, rc, g[p]);
+        }
+    };
+    u64 A[NP][4], Bv[NP][4];
+    float cS[NP];
+    bool slow[NP];
+    RecurGeom gn[NP];
+    geom(jj0, gn);
+    bool slow_w = false;
+#pragma unroll
+    for (int p = 0; p < NP; ++p) { recur_vals<MODE>(gn[p], rc, wtab, A[p], Bv[p], cS[p]); slow[p] = gn[p].slow; slow_w = slow_w || slow[p]; }
+    bool slow_any = __any_sync(0xffffffffu, slow_w);
+    geom(jj0 + NP, gn);
+    for (int jj = jj0; jj < cnt; jj += NP) {
+        if (slow_any) {
+#pragma unroll
+            for (int p = 0; p < NP; ++p)
+                if (slow[p]) recur_slow_pair<K, MODE>(acc, tile[jj + p], pi, rc, wtab);
+        }
+        // stage B of group jj + NP, stage A of group jj + 2 NP, packed loops of group jj: one basic block
+        u64 An[NP][4], Bn[NP][4];
+        float cSn[NP];
+        bool slown[NP];
+        slow_w = false;
+#pragma unroll
+        for (int p = 0; p < NP; ++p) { recur_vals<MODE>(gn[p], rc, wtab, An[p], Bn[p], cSn[p]); slown[p] = gn[p].slow; slow_w = slow_w || slown[p]; }
+        geom(jj + 2 * NP, gn);
+#pragma unroll
+        for (int p = 0; p < NP; ++p) recur_hot<K>(acc, A[p], Bv[p], cS[p]);
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+#pragma unroll
+            for (int a = 0; a < 4; ++a) { A[p][a] = An[p][a]; Bv[p][a] = Bn[p][a]; }
+            cS[p] = cSn[p]; slow[p] = slown[p];
+        }
+        slow_any = __any_sync(0xffffffffu, slow_w);      // after the packed loops: the vote ends the basic block
+    }
+}
+
 #ifndef DEBYE_FLUSH_J
 #define DEBYE_FLUSH_J 4096
 #endif
 
+#ifdef DEBYE_TRACE
+__device__ unsigned long long debye_trace[3 * 4096];
+#endif
 template <int K, int VAR>
-__global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (K <= 64 ? 4 : (K <= 112 ? 3 : 2))) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
+__global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR ? recur_min_ctas(K) : (K <= 64 ? 4 : (K <= 112 ? 3 : 2)))) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
                                                                double *__restrict__ records, int n_chunks, int is_auto, float theta_min)
 {
     // ---- variant gate (decided on the device so the host never reads q) ---------------------------------------
@@ -208,6 +440,9 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (K <= 64 ? 4 : 
     const int64_t u1 = (c + 1 == G) ? U : debye_range_begin(U, c + 1, G);
     if (u0 >= u1) return;
 
+#ifdef DEBYE_TRACE      // working builds only: per-CTA start / end time and SM id
+    if (tid == 0) { unsigned long long t; unsigned sm; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); asm volatile("mov.u32 %0, %%smid;" : "=r"(sm)); debye_trace[3 * c] = t; debye_trace[3 * c + 2] = sm; }
+#endif
     if (tid == 0) { mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
@@ -220,16 +455,15 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (K <= 64 ? 4 : 
     int64_t curX = -1;
     int pending = 0;
 
-    // recurrence constants
-    const int uniform = plan->uniform;
+    // recurrence constants (rebuilt when the q-chunk changes)
     const double dq_d = plan->dq, q0_d = plan->q0;
     const int koff = plan->zero_start;           // >= 0: grid is (k + koff) dq with koff small; -1: general
-    float dqf = 0.f, cut2 = 0.f, cS_unused = 0.f;
-    float wS_lo = 0.f, w4_lo = 0.f, w1 = 0.f, w1_lo = 0.f;
-    float wS = 0.f, w4 = 0.f;   // S dq / 2 pi and 4 dq / 2 pi (turns per Angstrom of the chain / bootstrap stride)
-    float qbase_l = 0.f;      // q of local slot l (recurrence): qbase_l + (S*(l/8) + (l%8)) * dq
-    int zs = 0, ch_cur = 0;
-    (void)cS_unused; (void)uniform;
+    RecurConst rc;
+    rc.w1 = rc.w1_lo = rc.wS = rc.wS_lo = rc.w4 = rc.w4_lo = rc.cut2 = rc.dqf = rc.qbase_l = 0.f;
+    rc.n_chunks = n_chunks;
+    float cut2 = 0.f;
+    int mode = RM_G, ch_cur = 0;
+    (void)mode; (void)dq_d; (void)q0_d; (void)koff; (void)cut2;
 
     auto flush = [&]() {
         // FP32 -> FP64, fixed order.  Each warp transposes 32 slots x 32 lanes through tbuf; lane l sums slot
@@ -312,10 +546,11 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (K <= 64 ? 4 : 
                 ch_cur = ch;
                 if constexpr (VAR == V_RECUR) {
                     const int S = 8 * n_chunks;
-                    dqf = (float)dq_d;
-                    zs = (koff >= 0 && n_chunks <= 2) ? 1 : 0;
+                    rc.dqf = (float)dq_d;
+                    const bool zs = (koff >= 0 && n_chunks <= 2);
+                    mode = zs ? (n_chunks == 1 ? RM_Z1 : (ch == 0 ? RM_Z2A : RM_Z2B)) : RM_G;
                     const double qb = (koff >= 0) ? 0.0 : q0_d;          // q of k' = 0
-                    qbase_l = (float)(qb + (8.0 * ch) * dq_d);
+                    rc.qbase_l = (float)(qb + (8.0 * ch) * dq_d);
                     const int base = -S + 8 * ch;                         // k' of the first start value
                     __syncthreads();
                     if (tid < 8) {   // turns per Angstrom of the 8 general-start values, hi and lo parts
@@ -325,18 +560,18 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (K <= 64 ? 4 : 
                     }
                     __syncthreads();
                     const double w1_d = dq_d * 0.15915494309189535;
-                    w1 = (float)w1_d; w1_lo = (float)(w1_d - (double)w1);
+                    rc.w1 = (float)w1_d; rc.w1_lo = (float)(w1_d - (double)rc.w1);
                     const double wS_d = (double)S * dq_d * 0.15915494309189535, w4_d = 4.0 * dq_d * 0.15915494309189535;
-                    wS = (float)wS_d; wS_lo = (float)(wS_d - (double)wS);
-                    w4 = (float)w4_d; w4_lo = (float)(w4_d - (double)w4);
-                    float rc = theta_min / fabsf(dqf);
-                    cut2 = rc * rc;
+                    rc.wS = (float)wS_d; rc.wS_lo = (float)(wS_d - (double)rc.wS);
+                    rc.w4 = (float)w4_d; rc.w4_lo = (float)(w4_d - (double)rc.w4);
+                    float rcut = theta_min / fabsf(rc.dqf);
+                    rc.cut2 = rcut * rcut;
                 } else {
                     __syncthreads();
                     if (tid < K) { int k = ch * K + tid; qs[tid] = (k < M) ? qv[k] : 0.0f; }
                     __syncthreads();
-                    float rc = theta_min / fmaxf(plan->q_small, 1e-30f);
-                    cut2 = (plan->q_small > 0.f) ? rc * rc : 0.f;
+                    const float rcut = theta_min / fmaxf(plan->q_small, 1e-30f);
+                    cut2 = (plan->q_small > 0.f) ? rcut * rcut : 0.f;
                 }
             }
         }
@@ -368,6 +603,14 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (K <= 64 ? 4 : 
             // on the diagonal, a warp whose every i is >= j has nothing to do for that j: start later
             int jj0 = 0;
             if (diag) { int first_i = row * DEBYE_IB + warp * 32; jj0 = max(0, first_i + 1 - jl0); }
+            if constexpr (VAR == V_RECUR) {
+                switch (mode) {      // warp-uniform; one copy of the pipelined loop per start mode
+                    case RM_Z1: recur_tile<K, RM_Z1>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
+                    case RM_Z2A: recur_tile<K, RM_Z2A>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
+                    case RM_Z2B: recur_tile<K, RM_Z2B>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
+                    default: recur_tile<K, RM_G>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
+                }
+            } else {
             for (int jj = jj0; jj < cnt; ++jj) {
                 const float4 pj = tile[buf][jj];
                 const bool ok = ivalid && (!diag || (jl0 + jj > i_local));
@@ -395,9 +638,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (K <= 64 ? 4 : 
                             const float rs = sqrtf(r2);
 #pragma unroll
                             for (int l = 0; l < K; ++l) {
-                                float qk;
-                                if constexpr (VAR == V_RECUR) qk = qbase_l + (float)(8 * n_chunks * (l / 8) + (l % 8)) * dqf;
-                                else qk = qs[l];
+                                const float qk = qs[l];
                                 float lo_, hi_;
                                 upk2(acc.v[l / 2], lo_, hi_);
                                 float tv = (rs == 0.0f) ? qk : term_accurate(qk, rs);
@@ -406,84 +647,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (K <= 64 ? 4 : 
                             }
                         }
                     }
-                    if constexpr (VAR == V_RECUR) {
-                        // ---- start values: u_j = sin(.)/r at the 16 indices the 4 packed chains need ---------------
-                        u64 A[4], Bv[4];
-                        float cS;
-                        if (zs) {
-                            // zero start (q_k' = k' dq, 1 or 2 residue-class chunks): v_n = sin(n theta), v_0 = 0,
-                            // v_{-n} = -v_n.  sin/cos(theta/2) by polynomial, everything else by double-angle /
-                            // three-term steps (each a single rounding, so relative accuracy survives small theta).
-                            float sh, chh;
-                            sincos_pi(reduce_turns(r, w1, w1_lo), sh, chh);
-                            const float s1 = (sh + sh) * chh;                     // sin(theta)
-                            const float c1 = fmaf(-4.0f * sh, sh, 2.0f);          // 2 cos(theta)
-                            const float c2 = fmaf(-4.0f * s1, s1, 2.0f);          // 2 cos(2 theta)
-                            const float s2 = s1 * c1;                             // sin(2 theta)
-                            const float c4 = fmaf(-4.0f * s2, s2, 2.0f);          // 2 cos(4 theta)
-                            // the chain coefficient 2 cos(S theta) is NOT derived from these by further doubling: the
-                            // correlated roundings of that route leave a +7e-8 rad coherent phase bias after 16 steps
-                            // (fp32 emulation); the direct polynomial on the reduced angle has none
-                            cS = two_cos_turns(r, wS, wS_lo);
-                            float u[17];
-                            u[0] = 0.0f;
-                            u[1] = s1 * rinv; u[2] = c1 * u[1]; u[3] = fmaf(c1, u[2], -u[1]); u[4] = c2 * u[2];
-                            u[5] = fmaf(c4, u[1], u[3]); u[6] = fmaf(c4, u[2], u[2]); u[7] = fmaf(c4, u[3], u[1]); u[8] = c4 * u[4];
-                            if (n_chunks == 1) {
-                                // w_0 = v_0 (B), w_{-1} = -v_{-1} = +v_{8-n} (A)
-                                Bv[0] = pk2(u[0], u[1]); Bv[1] = pk2(u[2], u[3]); Bv[2] = pk2(u[4], u[5]); Bv[3] = pk2(u[6], u[7]);
-                                A[0] = pk2(u[8], u[7]); A[1] = pk2(u[6], u[5]); A[2] = pk2(u[4], u[3]); A[3] = pk2(u[2], u[1]);
-                            } else {
-                                // two chunks: stride S = 16, chunk ch owns k' = 16 m + 8 ch + (0..7)
-#pragma unroll
-                                for (int n = 9; n <= 16; ++n) u[n] = fmaf(c4, u[n - 4], -u[n - 8]);
-                                if (ch_cur == 0) {
-                                    Bv[0] = pk2(u[0], u[1]); Bv[1] = pk2(u[2], u[3]); Bv[2] = pk2(u[4], u[5]); Bv[3] = pk2(u[6], u[7]);
-                                    A[0] = pk2(u[16], u[15]); A[1] = pk2(u[14], u[13]); A[2] = pk2(u[12], u[11]); A[3] = pk2(u[10], u[9]);
-                                } else {
-                                    Bv[0] = pk2(u[8], u[9]); Bv[1] = pk2(u[10], u[11]); Bv[2] = pk2(u[12], u[13]); Bv[3] = pk2(u[14], u[15]);
-                                    A[0] = pk2(u[8], u[7]); A[1] = pk2(u[6], u[5]); A[2] = pk2(u[4], u[3]); A[3] = pk2(u[2], u[1]);
-                                }
-                            }
-                        } else {
-                            // general start (q_0 not a small multiple of dq, or more than 2 chunks): 8 accurate sines at
-                            // k' = base .. base+7 (base = -S + 8 ch), then the stride-4 recurrence
-                            // v_{n+4} = 2cos(4 theta) v_n - v_{n-4} walks up to k' = 8 ch .. 8 ch + 7
-                            float g0[4], g1[4];
-#pragma unroll
-                            for (int j = 0; j < 4; ++j) {
-                                g0[j] = sin_turns_accurate(r, wtab[j], wtab[8 + j]) * rinv;
-                                g1[j] = sin_turns_accurate(r, wtab[4 + j], wtab[12 + j]) * rinv;
-                            }
-                            const float c4 = two_cos_turns(r, w4, w4_lo);                       // 2 cos(4 theta)
-                            float a0[4], a1[4];
-#pragma unroll
-                            for (int j = 0; j < 4; ++j) { a0[j] = g0[j]; a1[j] = g1[j]; }
-                            for (int st = 0; st < 2 * n_chunks; ++st) {
-                                // advance one group of 4: (g0, g1) -> (g1, c4 g1 - g0)
-#pragma unroll
-                                for (int j = 0; j < 4; ++j) { float nx = fmaf(c4, g1[j], -g0[j]); g0[j] = g1[j]; g1[j] = nx; }
-                            }
-                            cS = two_cos_turns(r, wS, wS_lo);                                   // 2 cos(S theta)
-                            Bv[0] = pk2(g0[0], g0[1]); Bv[1] = pk2(g0[2], g0[3]); Bv[2] = pk2(g1[0], g1[1]); Bv[3] = pk2(g1[2], g1[3]);
-                            A[0] = pk2(-a0[0], -a0[1]); A[1] = pk2(-a0[2], -a0[3]); A[2] = pk2(-a1[0], -a1[1]); A[3] = pk2(-a1[2], -a1[3]);
-                        }
-                        const u64 cP = pk2(cS, cS), cN = pk2(-cS, -cS);
-                        // ---- hot loop: w_m = sigma_m v_m with sigma = (+,+,-,-): w_{m+1} = (+/-) cS w_m + w_{m-1} --------
-#pragma unroll
-                        for (int m = 0; m < K / 8; ++m) {
-#pragma unroll
-                            for (int a = 0; a < 4; ++a) {
-                                if (m & 2) acc.v[4 * m + a] = sub2(acc.v[4 * m + a], Bv[a]);
-                                else acc.v[4 * m + a] = add2(acc.v[4 * m + a], Bv[a]);
-                                if (m + 1 < K / 8) {
-                                    u64 nx = fma2((m & 1) ? cN : cP, Bv[a], A[a]);
-                                    A[a] = Bv[a];
-                                    Bv[a] = nx;
-                                }
-                            }
-                        }
-                    } else if constexpr (VAR == V_MUFU) {
+                    if constexpr (VAR == V_MUFU) {
                         const float rt = r * 0.15915494309189535f;            // r / 2 pi: turns = q_k * rt
 #pragma unroll
                         for (int l = 0; l < K; l += 2) {
@@ -499,6 +663,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (K <= 64 ? 4 : 
                     }
                 }
             }
+            }
             __syncthreads();
         }
         pending += len;
@@ -506,6 +671,9 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (K <= 64 ? 4 : 
         u += len;
     }
     if (curX >= 0) { flush(); write_record(curX); }
+#ifdef DEBYE_TRACE
+    if (tid == 0) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); debye_trace[3 * c + 1] = t; }
+#endif
 }
 
 }  // namespace debye

@@ -30,6 +30,7 @@ thread_local int g_last_cuda = 0;
     } while (0)
 
 constexpr int MAX_DEV = 64;
+constexpr int64_t DEBYE_PACK_IN_SETUP = 16384;   // N x B up to which debye_setup_kernel also packs the coordinates
 struct DevState {
     void *ws = nullptr; size_t ws_bytes = 0;          // library-owned scratch
     void *user_ws = nullptr; size_t user_bytes = 0;   // caller-owned scratch (debye_set_workspace)
@@ -200,8 +201,9 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
 
     int rec_cap = 0;
     for (int i = 0; i < nch; ++i) if (ch[i].variant == V_RECUR) rec_cap = ch[i].K * ch[i].n_chunks;
-    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, rec_cap);
-    {
+    const bool pack_here = (int64_t)N * B <= DEBYE_PACK_IN_SETUP;      // small inputs: the setup CTA gathers too
+    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, rec_cap, xyz, sorted, pack_here ? 1 : 0);
+    if (!pack_here) {
         int64_t total = (int64_t)N * B;
         int blocks = (int)((total + 255) / 256);
         if (blocks > ds->sms * 16) blocks = ds->sms * 16;
@@ -216,7 +218,7 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     }
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
     {
-        int threads = 32 * DEBYE_FINAL_G, blocks = B * ((M + 31) / 32);
+        int threads = DEBYE_FINAL_THREADS, blocks = B * ((M + DEBYE_FINAL_Q - 1) / DEBYE_FINAL_Q);
         // in automatic mode the final kernel picks the parameter set of the variant chosen on the device
         const Choice &c1 = ch[nch - 1];
         debye::debye_final_kernel<<<blocks, threads, 0, stream>>>(plan, records, fftab, q, out, is_auto, ch[0].variant, ch[0].K, ch[0].n_chunks, G[0], c1.variant, c1.K,
@@ -337,7 +339,7 @@ int debye_launch_info(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags
     if (st) return st;
     Choice ch[2]; int is_auto;
     int nch = variants_for(flags, ch, M, &is_auto);
-    if (n_launches) *n_launches = 3 + nch;           // setup, pack, pairs x nch, final
+    if (n_launches) *n_launches = 2 + nch + (((int64_t)N * B <= DEBYE_PACK_IN_SETUP) ? 0 : 1);   // setup, [pack], pairs x nch, final
     if (q_chunk) *q_chunk = ch[0].K;
     if (n_chunks) *n_chunks = ch[0].n_chunks;
     if (pairs_grid) {

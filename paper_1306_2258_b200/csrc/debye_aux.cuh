@@ -14,40 +14,99 @@ namespace debye {
 // unit prefix per type pair.  Stable = atoms of one type keep their input order, so the sorted layout (and with
 // it every rounding in the pair sums) is a pure function of the input.
 // perm[p] = original index of the atom at sorted position p.
+// Sort: warp w owns the contiguous chunk [w C, (w+1) C) of the atoms, C a multiple of 32.  Pass 1 counts types per warp
+// (one __match_any_sync per 32 atoms, no atomics: only warp w touches wcnt[w]); a 32 x 32 prefix gives every
+// (warp, type) its first output slot; pass 2 walks the chunk again and places the atoms.  Two block barriers in total.
+// If pack_here != 0 the CTA also gathers the coordinates (small N x B: saves the pack launch).
 __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPlan *plan, const int32_t *__restrict__ type, const float *__restrict__ q,
-                                                                            int32_t *__restrict__ perm, int N, int T, int M, int B, int rec_capacity /* K * n_chunks of the recurrence */)
+                                                                            int32_t *__restrict__ perm, int N, int T, int M, int B, int rec_capacity /* K * n_chunks of the recurrence */,
+                                                                            const float *__restrict__ xyz, float4 *__restrict__ sorted, int pack_here)
 {
-    __shared__ int cnt[DEBYE_MAX_TYPES_I];
-    __shared__ int base[DEBYE_MAX_TYPES_I + 1];
-    __shared__ int wcnt[DEBYE_SETUP_THREADS / 32][DEBYE_MAX_TYPES_I];
-    __shared__ float red[DEBYE_SETUP_THREADS / 32];
-    __shared__ float red2[DEBYE_SETUP_THREADS / 32];
+    constexpr int NWARP = DEBYE_SETUP_THREADS / 32;
+    constexpr int SORT_UNROLL = 8;
+    __shared__ int wcnt[NWARP][DEBYE_MAX_TYPES_I];      // pass 1: atoms of type t in warp w's chunk; pass 2: running output slot
+    __shared__ int seg[DEBYE_MAX_TYPES_I + 1];
+    __shared__ float red[NWARP], red2[NWARP], qmax_s[NWARP];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid < DEBYE_MAX_TYPES_I) cnt[tid] = 0;
+    const int chunk = ((N + NWARP - 1) / NWARP + 31) / 32 * 32;
+    const int c0 = warp * chunk, c1 = min(N, c0 + chunk);
+    wcnt[warp][lane] = 0;
+    __syncwarp();
+    for (int s0 = c0; s0 < c1; s0 += 32 * SORT_UNROLL) {
+        int tt[SORT_UNROLL];
+#pragma unroll
+        for (int x = 0; x < SORT_UNROLL; ++x) { const int i = s0 + 32 * x + lane; tt[x] = (i < c1) ? type[i] : -1; }   // loads in flight together
+#pragma unroll
+        for (int x = 0; x < SORT_UNROLL; ++x) {
+            const int t = tt[x];
+            const unsigned peers = __match_any_sync(0xffffffffu, t);
+            if (t >= 0 && (peers & ((1u << lane) - 1)) == 0) wcnt[warp][t] += __popc(peers);
+            __syncwarp();
+        }
+    }
+    // ---- q grid analysis (independent of the sort; its reduction shares the barriers below) ---------------------------
+    const double q0 = (double)q[0];
+    const double dq = (M > 1) ? ((double)q[M - 1] - q0) / (double)(M - 1) : (q0 != 0.0 ? q0 : 1.0);
+    float dev = 0.f, qsm = 3.0e38f, qmax = 0.f;
+    for (int k = tid; k < M; k += blockDim.x) {
+        const double qk = (double)q[k];
+        dev = fmaxf(dev, (float)fabs(qk - (q0 + k * dq)));
+        const float aq = fabsf((float)qk);
+        if (aq > 0.f) qsm = fminf(qsm, aq);
+        qmax = fmaxf(qmax, aq);
+    }
+    for (int o = 16; o > 0; o >>= 1) { dev = fmaxf(dev, __shfl_xor_sync(0xffffffffu, dev, o)); qsm = fminf(qsm, __shfl_xor_sync(0xffffffffu, qsm, o)); qmax = fmaxf(qmax, __shfl_xor_sync(0xffffffffu, qmax, o)); }
+    if (lane == 0) { red[warp] = dev; red2[warp] = qsm; qmax_s[warp] = qmax; }
     __syncthreads();
-    for (int i = tid; i < N; i += blockDim.x) atomicAdd(&cnt[type[i]], 1);
-    __syncthreads();
-    if (tid == 0) {
-        int s = 0;
-        for (int t = 0; t < T; ++t) { base[t] = s; plan->seg_off[t] = s; plan->n_a[t] = cnt[t]; s += cnt[t]; }
-        base[T] = s;
-        for (int t = T; t <= DEBYE_MAX_TYPES_I; ++t) plan->seg_off[t] = s;
-        for (int t = T; t < DEBYE_MAX_TYPES_I; ++t) plan->n_a[t] = 0;
+    // ---- type totals and segment offsets (warp 0: lane t owns type t), plan header, q verdict (thread 32) --------------
+    if (warp == 0) {
+        int tot = 0;
+        for (int w = 0; w < NWARP; ++w) tot += wcnt[w][lane];
+        if (lane >= T) tot = 0;
+        int incl = tot;
+        for (int o = 1; o < 32; o <<= 1) { int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+        seg[lane] = incl - tot;
+        if (lane == 31) seg[32] = incl;
+        plan->seg_off[lane] = incl - tot;
+        plan->n_a[lane] = tot;
+        if (lane == 31) plan->seg_off[32] = incl;
+    }
+    if (tid == 32) {
+        float d = 0.f, s = 3.0e38f, mx = 0.f;
+        for (int w = 0; w < NWARP; ++w) { d = fmaxf(d, red[w]); s = fminf(s, red2[w]); mx = fmaxf(mx, qmax_s[w]); }
+        // uniform if every q[k] is within 2 float ulps (of the largest |q|) of the line through the end points
+        const int uni = (dq != 0.0) && (d <= 2.4e-7f * fmaxf(mx, 1e-30f));
+        int koff = -1;
+        if (uni) {
+            const double ko = q0 / dq;
+            const double kr = rint(ko);
+            if (kr >= 0.0 && kr <= 8.0 && fabs(ko - kr) <= 1e-6 * fmax(1.0, kr) && (int)kr + M <= rec_capacity) koff = (int)kr;
+        }
         plan->N = N; plan->T = T; plan->M = M; plan->B = B; plan->n_tp = T * (T + 1) / 2;
+        plan->uniform = uni;
+        plan->zero_start = koff;
+        plan->q0 = q0;
+        plan->dq = dq;
+        plan->q_small = (s < 3.0e38f) ? s : 0.f;
+        plan->variant_auto = uni ? V_RECUR : V_MUFU;
+    }
+    __syncthreads();
+    // ---- unit prefix per type pair (thread 0, n_tp <= 528 steps) while the other warps sort -----------------------------
+    if (tid == 0) {
         // units per type pair; the side with less padding waste becomes the row (i) side
         int64_t pre = 0;
         int tp = 0;
         for (int a = 0; a < T; ++a)
             for (int b2 = a; b2 < T; ++b2, ++tp) {
-                int na = cnt[a], nb = cnt[b2];
+                const int na = seg[a + 1] - seg[a], nb = seg[b2 + 1] - seg[b2];
                 int64_t units;
                 int ti = a, tj = b2;
                 if (a == b2) {
-                    int rows = debye_diag_rows(na);
+                    const int rows = debye_diag_rows(na);
                     units = rows > 0 ? debye_diag_row_prefix(na, rows) : 0;
                 } else {
-                    int64_t ra = (na + DEBYE_IB - 1) / DEBYE_IB, rb = (nb + DEBYE_IB - 1) / DEBYE_IB;
-                    int64_t ua = ra * nb, ub = rb * na;          // rows x j atoms
+                    const int64_t ra = (na + DEBYE_IB - 1) / DEBYE_IB, rb = (nb + DEBYE_IB - 1) / DEBYE_IB;
+                    const int64_t ua = ra * nb, ub = rb * na;          // rows x j atoms
                     if (ub < ua) { ti = b2; tj = a; units = ub; } else units = ua;
                     if (na == 0 || nb == 0) units = 0;
                 }
@@ -55,63 +114,39 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
                 pre += units;
             }
         plan->tp_prefix[tp] = pre;
-        for (int x = tp + 1; x <= DEBYE_MAX_TP; ++x) plan->tp_prefix[x] = pre;
         plan->U1 = pre;
     }
+    // first output slot of (warp, type): exclusive prefix over the warps, per type (thread (w, t) = (warp, lane))
+    int first = seg[lane];
+    for (int w = 0; w < warp; ++w) first += wcnt[w][lane];
     __syncthreads();
-    // ---- stable counting sort, 1024 atoms per step --------------------------------------------------------------
-    for (int start = 0; start < N; start += blockDim.x) {
-        const int i = start + tid;
-        const int t = (i < N) ? type[i] : -1;
-        for (int x = lane; x < T; x += 32) wcnt[warp][x] = 0;
-        __syncwarp();
-        unsigned peers = __match_any_sync(0xffffffffu, t);
-        int rank_in_warp = __popc(peers & ((1u << lane) - 1));
-        if (t >= 0 && rank_in_warp == 0) wcnt[warp][t] = __popc(peers);
-        __syncthreads();
-        int before = 0;
-        if (t >= 0) {
-            for (int w = 0; w < warp; ++w) before += wcnt[w][t];
-            perm[base[t] + before + rank_in_warp] = i;
+    wcnt[warp][lane] = first;
+    __syncwarp();
+    for (int s0 = c0; s0 < c1; s0 += 32 * SORT_UNROLL) {
+        int tt[SORT_UNROLL];
+#pragma unroll
+        for (int x = 0; x < SORT_UNROLL; ++x) { const int i = s0 + 32 * x + lane; tt[x] = (i < c1) ? type[i] : -1; }
+#pragma unroll
+        for (int x = 0; x < SORT_UNROLL; ++x) {
+            const int t = tt[x];
+            const unsigned peers = __match_any_sync(0xffffffffu, t);
+            const int rank = __popc(peers & ((1u << lane) - 1));
+            if (t >= 0) perm[wcnt[warp][t] + rank] = s0 + 32 * x + lane;
+            __syncwarp();
+            if (t >= 0 && rank == 0) wcnt[warp][t] += __popc(peers);
+            __syncwarp();
         }
-        __syncthreads();
-        if (tid < T) { int s = 0; for (int w = 0; w < DEBYE_SETUP_THREADS / 32; ++w) s += wcnt[w][tid]; base[tid] += s; }
-        __syncthreads();
     }
-    // ---- q grid analysis -------------------------------------------------------------------------------------------
-    const double q0 = (double)q[0];
-    double dq = (M > 1) ? ((double)q[M - 1] - q0) / (double)(M - 1) : (q0 != 0.0 ? q0 : 1.0);
-    float dev = 0.f, qsm = 3.0e38f, qmax = 0.f;
-    for (int k = tid; k < M; k += blockDim.x) {
-        double qk = (double)q[k];
-        dev = fmaxf(dev, (float)fabs(qk - (q0 + k * dq)));
-        float aq = fabsf((float)qk);
-        if (aq > 0.f) qsm = fminf(qsm, aq);
-        qmax = fmaxf(qmax, aq);
-    }
-    for (int o = 16; o > 0; o >>= 1) { dev = fmaxf(dev, __shfl_xor_sync(0xffffffffu, dev, o)); qsm = fminf(qsm, __shfl_xor_sync(0xffffffffu, qsm, o)); qmax = fmaxf(qmax, __shfl_xor_sync(0xffffffffu, qmax, o)); }
-    if (lane == 0) { red[warp] = dev; red2[warp] = qsm; }
-    __syncthreads();
-    __shared__ float qmax_s[DEBYE_SETUP_THREADS / 32];
-    if (lane == 0) qmax_s[warp] = qmax;
-    __syncthreads();
-    if (tid == 0) {
-        float d = 0.f, s = 3.0e38f, mx = 0.f;
-        for (int w = 0; w < DEBYE_SETUP_THREADS / 32; ++w) { d = fmaxf(d, red[w]); s = fminf(s, red2[w]); mx = fmaxf(mx, qmax_s[w]); }
-        // uniform if every q[k] is within 2 float ulps (of the largest |q|) of the line through the end points
-        int uni = (dq != 0.0) && (d <= 2.4e-7f * fmaxf(mx, 1e-30f));
-        int koff = -1;
-        if (uni) {
-            double ko = q0 / dq;
-            double kr = rint(ko);
-            if (kr >= 0.0 && kr <= 8.0 && fabs(ko - kr) <= 1e-6 * fmax(1.0, kr) && (int)kr + M <= rec_capacity) koff = (int)kr;
+    if (pack_here) {
+        __syncthreads();                       // perm was written by this CTA: visible after the barrier
+        const int total = N * B;                 // <= DEBYE_PACK_IN_SETUP
+#pragma unroll 4
+        for (int g = tid; g < total; g += DEBYE_SETUP_THREADS) {
+            const int b = g / N, p = g - b * N;
+            const int i = perm[p];
+            const float *sx = xyz + ((int64_t)b * N + i) * 3;
+            sorted[g] = make_float4(sx[0], sx[1], sx[2], __int_as_float(type[i]));
         }
-        plan->uniform = uni;
-        plan->zero_start = koff;
-        plan->q0 = q0;
-        plan->dq = dq;
-        plan->q_small = (s < 3.0e38f) ? s : 0.f;
-        plan->variant_auto = uni ? V_RECUR : V_MUFU;
     }
 }
 
@@ -133,25 +168,33 @@ __device__ __forceinline__ double pair_count(int na, int nb, bool diag) { return
 
 // S7: fixed-order FP64 sum of the per-CTA records, then the form-factor epilogue
 //   I(q_k) = sum_a n_a F_a^2 + 2 sum_{a<=b} F_a F_b S_ab(q_k),   S_ab = (1/q_k) sum sin(q_k r)/r  (q_k != 0), #pairs (q_k == 0).
-// Block = (conformer, tile of 32 q indices); thread (kk, g) handles q index k0 + kk and the type pairs g, g+8, ... in
-// increasing order; the 8 partial sums are then added in g order.  Every order is fixed, so the result is bitwise
-// reproducible.  Record reads are coalesced over kk.  mode 0: write I_out[b][k]; mode 1: write S_out[b][tp][k].
+// Block = (conformer, tile of DEBYE_FINAL_Q q indices); thread (kk, g, sl) handles q index k0 + kk, the type pairs
+// g, g + G8, ... in increasing order and, of each type pair's CTA range [c_lo, c_hi], the sl-th of NS equal slices.
+// The partial sums are then added in (g, sl) order.  The slicing is a fixed function of (U, G), so every order is fixed
+// and the result is bitwise reproducible.  mode 0: write I_out[b][k]; mode 1 (NS must be 1): write S_out[b][tp][k].
+#define DEBYE_FINAL_Q 8
 #define DEBYE_FINAL_G 8
-__global__ void __launch_bounds__(32 * DEBYE_FINAL_G) debye_final_kernel(const DevPlan *__restrict__ plan, const double *__restrict__ records,
+#define DEBYE_FINAL_NS 4
+#define DEBYE_FINAL_THREADS (DEBYE_FINAL_Q * DEBYE_FINAL_G * DEBYE_FINAL_NS)
+__global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const DevPlan *__restrict__ plan, const double *__restrict__ records,
                                                                             const float *__restrict__ fftab, const float *__restrict__ q, double *__restrict__ out,
                                                                             int is_auto, int variant0, int K0, int nc0, int G0, int variant1, int K1, int nc1, int G1,
                                                                             int mode)
 {
-    __shared__ double part[DEBYE_FINAL_G][32];
+    __shared__ double part[DEBYE_FINAL_G * DEBYE_FINAL_NS][DEBYE_FINAL_Q];
     const int M = plan->M, Bn = plan->B, T = plan->T, n_tp = plan->n_tp;
-    const int ktiles = (M + 31) / 32;
-    const int b = blockIdx.x / ktiles, k = (blockIdx.x % ktiles) * 32 + (threadIdx.x & 31), g = threadIdx.x >> 5;
-    const bool live = k < M;
+    const int ktiles = (M + DEBYE_FINAL_Q - 1) / DEBYE_FINAL_Q;
+    const int kk = threadIdx.x % DEBYE_FINAL_Q, gs = threadIdx.x / DEBYE_FINAL_Q;
+    const int NS = (mode == 0) ? DEBYE_FINAL_NS : 1;
+    const int g = gs / DEBYE_FINAL_NS, sl = gs % DEBYE_FINAL_NS;
+    const int b = blockIdx.x / ktiles, k = (blockIdx.x % ktiles) * DEBYE_FINAL_Q + kk;
+    const bool live = k < M && sl < NS;
     // automatic mode: two pairs kernels were launched and the device ran the one named by plan->variant_auto
     const bool second = is_auto && plan->variant_auto == variant1;
     const int variant = second ? variant1 : variant0, K = second ? K1 : K0, n_chunks = second ? nc1 : nc0, G = second ? G1 : G0;
     const bool bad = (variant == V_RECUR && !plan->uniform);          // forced recurrence on a non-uniform grid -> NaN
     const double nan = __longlong_as_double(0x7ff8000000000000LL);
+    const double scale = (variant == V_RECUR) ? 0.5 : 1.0;            // the recurrence kernel accumulates 2 sin(q r)/r
     double I = 0.0;
     if (live) {
         int kprime = k;
@@ -167,8 +210,8 @@ __global__ void __launch_bounds__(32 * DEBYE_FINAL_G) debye_final_kernel(const D
             const int b2 = a + (tp - rowstart);
             double S;
             const int64_t units = plan->tp_prefix[tp + 1] - plan->tp_prefix[tp];
-            if (bad) S = nan;
-            else if (qk == 0.0 || units == 0) S = pair_count(plan->n_a[a], plan->n_a[b2], a == b2);
+            if (bad) S = (sl == 0) ? nan : 0.0;
+            else if (qk == 0.0 || units == 0) S = (sl == 0) ? pair_count(plan->n_a[a], plan->n_a[b2], a == b2) : 0.0;
             else {
                 const int64_t ub = (int64_t)b * Uc + plan->tp_prefix[tp] * n_chunks + (int64_t)ch * units;
                 const int64_t ue = ub + units - 1;
@@ -176,25 +219,32 @@ __global__ void __launch_bounds__(32 * DEBYE_FINAL_G) debye_final_kernel(const D
                 double s = 0.0;
                 if (U >= G) {           // every CTA owns at least one unit: all CTAs between the owners took part
                     const int c_lo = debye_owner(U, G, ub), c_hi = debye_owner(U, G, ue);
-#pragma unroll 4
-                    for (int c = c_lo; c <= c_hi; ++c) s += records[((int64_t)c + X) * K + l];
-                } else {                // fewer units than CTAs: each unit has its own CTA
+                    const int n = c_hi - c_lo + 1, per = (n + NS - 1) / NS;
+                    const int cb = c_lo + sl * per, ce = min(c_hi + 1, cb + per);
+                    const double *rp = records + ((int64_t)cb + X) * K + l;
+                    int c = cb;
+                    for (; c + 4 <= ce; c += 4, rp += 4 * (int64_t)K) {
+                        const double r0 = rp[0], r1 = rp[K], r2 = rp[2 * (int64_t)K], r3 = rp[3 * (int64_t)K];
+                        s += r0; s += r1; s += r2; s += r3;
+                    }
+                    for (; c < ce; ++c, rp += K) s += rp[0];
+                } else if (sl == 0) {   // fewer units than CTAs: each unit has its own CTA
                     for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)debye_owner(U, G, u) + X) * K + l];
                 }
-                S = (variant == V_RECUR ? 0.5 * s : s) / qk;     // the recurrence kernel accumulates 2 sin(q r)/r
+                S = scale * s / qk;
             }
             if (mode == 0) I += 2.0 * (double)fftab[a * M + k] * (double)fftab[b2 * M + k] * S;
             else out[((int64_t)b * n_tp + tp) * M + k] = S;
         }
     }
     if (mode != 0) return;
-    part[g][threadIdx.x & 31] = I;
+    part[gs][kk] = I;
     __syncthreads();
-    if (g == 0 && live) {
+    if (gs == 0 && k < M) {
         double tot = 0.0;
         for (int a = 0; a < T; ++a) { const double fa = (double)fftab[a * M + k]; tot += (double)plan->n_a[a] * fa * fa; }
 #pragma unroll
-        for (int gg = 0; gg < DEBYE_FINAL_G; ++gg) tot += part[gg][threadIdx.x & 31];
+        for (int x = 0; x < DEBYE_FINAL_G * DEBYE_FINAL_NS; ++x) tot += part[x][kk];
         out[(int64_t)b * M + k] = tot;
     }
 }

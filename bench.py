@@ -30,6 +30,9 @@ from paper_1306_2258_b200 import workloads as wl          # noqa: E402  (input g
 METRIC = "pair_q_sinc_terms_per_second"
 UNIT = "G pair.q/s"
 SM_COUNT, FP32_LANES, MUFU_LANES = 148, 128, 16           # per B200 / per SM per clock (B200_PROFILING.md)
+# dram__bytes_read.sum + dram__bytes_write.sum of the pairs kernel, per launch, from the committed ncu --set full capture
+# (profiles/r01_ncu_full_pairs_recur_cfg2_v2.txt); None where no capture exists
+NCU_TRAFFIC = {("cfg2", "recur"): 239360}
 
 
 def make_workload(name: str, rank: int = 0):
@@ -259,8 +262,9 @@ def main():
         achieved = 4.0 * pq_per_launch / (pairs_ms * 1e-3) / 1e12
         roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": None,
-                "note": "FP32-pipe issue roofline: 2 lane-ops (FFMA + FADD = 4 FMA-equivalent flop) per pair.q; peak = "
-                        "148 SM x 128 lanes x 2 x sm_max_mhz (MEASURED_PEAKS.json clock; FFMA2 microbenchmark reaches 99 % of it)"}
+                "note": "FP32-pipe roofline: 2 lane-ops (FFMA + FADD = 4 FMA-equivalent flop) per pair.q; peak = "
+                        "148 SM x 128 lanes x 2 x sm_max_mhz (MEASURED_PEAKS.json clock); measured pipe rates on this part: FADD2 0.995, "
+                        "FFMA2 0.91 of it (DESIGN.md section 7)"}
     else:
         per_term = {"mufu": 1.0}.get(variant_ran)
         peak = SM_COUNT * MUFU_LANES * fmax_ghz / 1e3                           # T MUFU op/s
@@ -268,6 +272,7 @@ def main():
         roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T sin/s", "frac": achieved / peak,
                 "traffic": None, "note": "XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM" if per_term else
                 "reference variant; XU roofline quoted for scale"}
+    roof["traffic"] = NCU_TRAFFIC.get((args.config, variant_ran))
     roof["kernel"] = f"debye_pairs_kernel<{info['q_chunk']}, {variant_ran}>"
     roof["kernel_ms"] = pairs_ms
     roof["pair_q_per_clk_per_sm"] = pq_per_launch / (pairs_ms * 1e-3) / (SM_COUNT * fmax_ghz * 1e9)

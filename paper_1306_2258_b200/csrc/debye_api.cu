@@ -127,7 +127,7 @@ int dev_state(DevState **st)
 
 // Grid of the pairs kernel: resident CTAs (SMs x occupancy) times a small number of waves.  The warp schedulers favour
 // one of the CTAs that share an SM, so with exactly one wave the favoured CTA finishes ~30 % early and its partner runs
-// the tail alone (measured); a few waves let the hardware block scheduler refill the SM.  More waves
+// the tail alone (measured); a few waves (up to 16 when there is enough work) let the hardware block scheduler refill the SM.  More waves
 // cost one prologue + one FP64 flush per CTA, so the count is bounded by the work available (estimated from N alone:
 // the host never sees the type histogram).
 int grid_for(DevState *s, const Choice &c, int N, int B, int *G)
@@ -145,7 +145,7 @@ int grid_for(DevState *s, const Choice &c, int N, int B, int *G)
     const double units = (double)B * c.n_chunks * ((double)N * (double)N / (2.0 * DEBYE_IB));   // j atoms x rows, all type pairs
     int waves = (int)(units / ((double)resident * 600.0));
     if (waves < 1) waves = 1;
-    if (waves > 4) waves = 4;
+    if (waves > 16) waves = 16;
     *G = resident * waves;
     return DEBYE_OK;
 }
@@ -302,8 +302,8 @@ size_t debye_workspace_bytes(int32_t N, int32_t B, int32_t T, int32_t M, uint32_
     if (validate(&dummy, &dummy, N, B, &dummy, T, &dummy, M, &dummy, flags)) return 0;
     Choice ch[2]; int is_auto;
     int nch = variants_for(flags, ch, M, &is_auto);
-    // grid is at most 148 SMs x 16 CTAs x 4 waves on any sm_100 part; use a safe upper bound so no device query is needed
-    return layout(N, B, T, M, 192 * 16 * 4, ch, nch).total;
+    // grid is at most 148 SMs x 16 CTAs x 16 waves on any sm_100 part; use a safe upper bound so no device query is needed
+    return layout(N, B, T, M, 192 * 16 * 16, ch, nch).total;
 }
 
 int debye_set_workspace(void *dev_ptr, size_t bytes)

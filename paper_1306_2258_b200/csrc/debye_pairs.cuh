@@ -64,47 +64,78 @@ __device__ __forceinline__ float sin_turns_fma(float r, float w)
 // A relative frequency bias must stay below ~1e-9, so: frequencies are carried as hi + lo floats, the leading
 // polynomial coefficient pi is split hi + lo, and everything else is round-to-nearest FMA arithmetic (unbiased).
 
-// fractional part of r * (w + w_lo) in turns, in [-1/2, 1/2]: magic-number rounding, FMA remainders
+// Fractional part of r * (w + w_lo) in turns, in [-1/2, 1/2], as the round-to-nearest of the EXACT value.
+// The naive form  fma(r, w_lo, fma(r, w, -n))  rounds r*w - n first and then adds a correction r*w_lo that is below the
+// resolution of the result, so the correction is (mostly) rounded away: every pair then runs its chain at the frequency w
+// instead of w + w_lo, a coherent relative error of 1e-9 that cost up to 1.7e-4 at single q points of cfg5 (measured,
+// DESIGN.md section 6).  Here the product is split error-free (p + e = r*w exactly), p - n is exact, and the two small
+// parts e and r*w_lo are combined BEFORE the single final rounding, which is therefore unbiased.
 __device__ __forceinline__ float reduce_turns(float r, float w, float w_lo)
 {
-    const float MAGIC = 12582912.0f;                 // 1.5 * 2^23
-    const float n = fmaf(r, w, MAGIC) - MAGIC;
-    return fmaf(r, w_lo, fmaf(r, w, -n));
+    const float p = r * w;
+    const float e = fmaf(r, w, -p);                  // exact
+    return (p - rintf(p)) + fmaf(r, w_lo, e);
 }
-// th = 2 sin(pi f), ch2 = 2 cos(pi f) for |f| <= 1/2 (Taylor to pi^13/13! and pi^12/12!, remainders < 6e-9 / 4e-8).
-// Every coefficient is the plain one times 2 (exact), so the roundings are those of the undoubled polynomial; the
-// doubled values feed 2cos(2x) = 2 - (2 sin x)^2 and 2 sin(2x) = (2 sin x)(2 cos x) / 1 without extra multiplies.
-__device__ __forceinline__ void sincos_pi_x2(float f, float &th, float &ch2)
+// The same for two frequencies w and mult * w (mult a power of two <= 2^12, so mult * p and mult * e are exact): shares the
+// error-free product.  f1 <- frac(r (w + w_lo)),  fS <- frac(mult r (w + w_lo)).
+__device__ __forceinline__ void reduce_turns_pair(float r, float w, float w_lo, float mult, float &f1, float &fS)
 {
-    const float y = f * f;
-    float p = fmaf(y, 2.0f * 4.6630280576761255e-4f, 2.0f * -7.3704309457143504e-3f);   // pi^13/13!, -pi^11/11!
-    p = fmaf(y, p, 2.0f * 8.2145886611128229e-2f);                                       // pi^9/9!
-    p = fmaf(y, p, 2.0f * -5.9926452932079208e-1f);                                      // -pi^7/7!
-    p = fmaf(y, p, 2.0f * 2.5501640398773455f);                                          // pi^5/5!
-    p = fmaf(y, p, 2.0f * -5.1677127800499700f);                                         // -pi^3/3!
-    p = fmaf(y, p, 2.0f * -8.7422780126189537e-8f);                                      // pi - (float)pi
-    th = fmaf(f, 2.0f * 3.14159274101257324f, f * p);                                    // (float)pi
-    float c = fmaf(y, 2.0f * 1.9295743094039220e-3f, 2.0f * -2.5806891390014050e-2f);    // pi^12/12!, -pi^10/10!
-    c = fmaf(y, c, 2.0f * 2.3533063035889312e-1f);                                       // pi^8/8!
-    c = fmaf(y, c, 2.0f * -1.3352627688545893f);                                         // -pi^6/6!
-    c = fmaf(y, c, 2.0f * 4.0587121264167682f);                                          // pi^4/4!
-    c = fmaf(y, c, 2.0f * -4.9348022005446793f);                                         // -pi^2/2!
-    ch2 = fmaf(y, c, 2.0f);
+    const float p = r * w;
+    const float l = fmaf(r, w_lo, fmaf(r, w, -p));   // everything below the rounding of p
+    // rintf is one FRND on the conversion (XU) pipe, which is otherwise idle here; the magic-number form would cost two
+    // FMA-pipe instructions per rounding
+    f1 = (p - rintf(p)) + l;
+    const float pS = p * mult;                       // exact
+    fS = fmaf(l, mult, pS - rintf(pS));
 }
-// 2 cos(2 pi r (w + w_lo)) = 2 - (2 sin(pi f))^2: relatively accurate in (2 - result) for small angles
-__device__ __forceinline__ float two_cos_turns(float r, float w, float w_lo)
+
+// Folded sine / cosine of a reduced angle.  For |f| <= 1/2 let g = |f| and g' = min(g, 1/2 - g) in [0, 1/4] (the
+// subtraction is exact); fold = (g > 1/4).  Returns s = 2 sin(pi g') and c = 2 cos(pi g'), from which
+//     2 cos(2 pi f) = +/-(2 - s^2)           (minus when folded),
+//     2 sin(2 pi f) = sign(f) s c            (folded or not),
+// so the quantity that is squared is always the SMALL one: the phase error that a relative error rho of s causes in
+// 2cos(2 pi f) is 2 rho tan(pi g') <= 2 rho, whereas without the fold it is 2 rho tan(pi f), unbounded towards f = 1/2;
+// and on the half interval one fewer cosine coefficient is needed for a 500 times smaller approximation error.
+//   s = g' (2 pi + y (s1 + y (s2 + y (s3 + y s4)))),  c = 2 + y (d1 + y (d2 + y (d3 + y d4))),  y = g'^2.
+// Near-minimax coefficients (iteratively reweighted least squares on 25 000 Chebyshev-spaced points of [0, 1/4] in fp64,
+// fitting 2 sin(pi g) - 2 pi g on g^3..g^9 and 2 cos(pi g) - 2 on y..y^4): maximum relative error 9.3e-12 (s), maximum
+// absolute error 1.1e-10 (c).  The linear coefficient is pinned to 2 pi, carried as hi + lo.
+struct Folded { float s, c; bool fold; };
+__device__ __forceinline__ Folded sincos_fold(const float f)
 {
-    float th, ch2;
-    sincos_pi_x2(reduce_turns(r, w, w_lo), th, ch2);
-    (void)ch2;
-    return fmaf(-th, th, 2.0f);
+    Folded o;
+    const float g = fabsf(f);
+    o.fold = g > 0.25f;
+    const float gp = fminf(g, 0.5f - g);
+    const float y = gp * gp;
+    float p = fmaf(y, 0.1619238643960947f, -1.198394591051059f);
+    p = fmaf(y, p, 5.100324961653245f);
+    p = fmaf(y, p, -10.335425536121228f);
+    p = fmaf(y, p, -1.7484556e-7f);                          // 2 pi - (float)(2 pi)
+    o.s = fmaf(gp, 6.2831854820251465f, gp * p);            // (float)(2 pi)
+    float c = fmaf(y, 0.46285910429932814f, -2.670116930113852f);
+    c = fmaf(y, c, 8.117415808996121f);
+    c = fmaf(y, c, -9.869604346828243f);
+    o.c = fmaf(y, c, 2.0f);
+    return o;
 }
-// 2 sin(2 pi r (w + w_lo)) = (2 sin(pi f)) (2 cos(pi f))
+// 2 cos(2 pi f) from the folded sine: relatively accurate in (2 -/+ result) at both ends
+__device__ __forceinline__ float two_cos_from(const Folded &o)
+{
+    const float c0 = fmaf(-o.s, o.s, 2.0f);
+    return o.fold ? -c0 : c0;
+}
+// 2 sin(2 pi f)
+__device__ __forceinline__ float two_sin_from(const Folded &o, const float f) { return copysignf(o.s, f) * o.c; }
+// 4 sin^2(pi f) = 2 - 2 cos(2 pi f), relatively accurate for small f (Reinsch's beta)
+__device__ __forceinline__ float four_sin2_from(const Folded &o) { return o.fold ? fmaf(-o.s, o.s, 4.0f) : o.s * o.s; }
+
+// 2 cos(2 pi r (w + w_lo)) and 2 sin(2 pi r (w + w_lo)) with hi + lo frequencies
+__device__ __forceinline__ float two_cos_turns(float r, float w, float w_lo) { return two_cos_from(sincos_fold(reduce_turns(r, w, w_lo))); }
 __device__ __forceinline__ float two_sin_turns_accurate(float r, float w, float w_lo)
 {
-    float th, ch2;
-    sincos_pi_x2(reduce_turns(r, w, w_lo), th, ch2);
-    return th * ch2;
+    const float f = reduce_turns(r, w, w_lo);
+    return two_sin_from(sincos_fold(f), f);
 }
 
 // accurate sin(q r)/r for one term (slow path): Taylor for |x| < 0.6 (north_star (e)), libdevice sinf otherwise
@@ -172,6 +203,7 @@ struct PairAcc {
 struct RecurConst {
     float w1, w1_lo;         // dq / 2 pi, hi + lo: theta / 2 pi = r * (w1 + w1_lo)
     float wS, wS_lo;         // S dq / 2 pi (chain stride S = 8 n_chunks)
+    float smult;             // (float)S: wS = S w1 exactly (S is a power of two)
     float w4, w4_lo;         // 4 dq / 2 pi (general start: bootstrap stride)
     float cut2;              // r^2 at or below which the pair takes the slow path
     float dqf, qbase_l;      // slow path: q of local slot l is qbase_l + (S (l / 8) + l % 8) dqf
@@ -199,34 +231,26 @@ __device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, con
     g.r = r2c * rinv;
     g.rinv = (ok && !small) ? rinv : 0.0f;      // zero for masked / slow-path pairs: every start value becomes exactly 0
     g.slow = small && ok;
-    g.fS = reduce_turns(g.r, rc.wS, rc.wS_lo);
-    if constexpr (MODE != RM_G) g.f1 = reduce_turns(g.r, rc.w1, rc.w1_lo);
-    else g.f1 = 0.0f;
+    reduce_turns_pair(g.r, rc.w1, rc.w1_lo, rc.smult, g.f1, g.fS);     // f1 is dead code in the general-start mode
 }
 // Stage B (values): Bv = w_0 (the 8 residues), A = w_{-1}, cS = 2 cos(S theta).
 template <int MODE>
 __device__ __forceinline__ void recur_vals(const RecurGeom &g, const RecurConst &rc, const float *wtab, u64 (&A)[4], u64 (&Bv)[4], float &cS)
 {
     const float r = g.r, rinv = g.rinv;
-    {   // the chain coefficient 2 cos(S theta) is NOT derived from 2 cos(theta) by repeated doubling: the correlated
-        // roundings of that route leave a +7e-8 rad coherent phase bias after 16 steps (fp32 emulation, DESIGN.md
-        // section 6); the direct polynomial on the reduced angle has none
-        float th, ch2;
-        sincos_pi_x2(g.fS, th, ch2);
-        (void)ch2;
-        cS = fmaf(-th, th, 2.0f);
-    }
+    // the chain coefficient 2 cos(S theta) is NOT derived from 2 cos(theta) by repeated doubling: the correlated roundings
+    // of that route leave a +7e-8 rad coherent phase bias after 16 steps (fp32 emulation)
+    cS = two_cos_from(sincos_fold(g.fS));
     if constexpr (MODE != RM_G) {
-        // zero start: v_n = 2 sin(n theta)/r, v_0 = 0, v_{-n} = -v_n.  2 sin(theta/2) and 2 cos(theta/2) by polynomial,
+        // zero start: v_n = 2 sin(n theta)/r, v_0 = 0, v_{-n} = -v_n.  Folded sine / cosine of theta/2 by polynomial,
         // everything else by double-angle / three-term steps (each a single rounding, so relative accuracy survives
         // small theta).  T_n = 2 sin(n theta), c_n = 2 cos(n theta).
-        float th, ch2;
-        sincos_pi_x2(g.f1, th, ch2);
-        const float T1 = th * ch2;
-        const float c1 = fmaf(-th, th, 2.0f);
+        const Folded h = sincos_fold(g.f1);                // g.f1 = theta / 2 pi reduced: pi f1 = theta / 2
+        const float T1 = two_sin_from(h, g.f1);
+        const float c1 = two_cos_from(h);
         const float c2 = fmaf(-T1, T1, 2.0f);
-        const float T2 = T1 * c1;
-        const float c4 = fmaf(-T2, T2, 2.0f);
+        const float c4 = fmaf(c2, c2, -2.0f);     // used for ONE (two for 2 chunks) bootstrap step only: its absolute error of
+                                                  // one rounding costs 1e-7 relative in u5..u16, no relative accuracy needed
         float u[17];
         u[0] = 0.0f;
         u[1] = T1 * rinv; u[2] = c1 * u[1]; u[3] = fmaf(c1, u[2], -u[1]); u[4] = c2 * u[2];
@@ -308,10 +332,7 @@ __device__ __forceinline__ void recur_slow_pair(u64 (&acc)[K / 2], const float4 
     recur_vals<MODE>(g, rc, wtab, A, Bv, cS);
     (void)cS;
     // beta from the polynomial directly (2 - cS would cancel)
-    float th, ch2;
-    sincos_pi_x2(g.fS, th, ch2);
-    (void)ch2;
-    const float nbeta = -th * th;
+    const float nbeta = -four_sin2_from(sincos_fold(g.fS));
     const u64 nb2 = pk2(nbeta, nbeta);
     // stage B returns A = w_{-1} = -v_{-1} (sign convention of the fast loop): d_0 = v_0 - v_{-1} = Bv + A
     u64 s[4], d[4];
@@ -460,6 +481,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
     const int koff = plan->zero_start;           // >= 0: grid is (k + koff) dq with koff small; -1: general
     RecurConst rc;
     rc.w1 = rc.w1_lo = rc.wS = rc.wS_lo = rc.w4 = rc.w4_lo = rc.cut2 = rc.dqf = rc.qbase_l = 0.f;
+    rc.smult = 8.0f;
     rc.n_chunks = n_chunks;
     float cut2 = 0.f;
     int mode = RM_G, ch_cur = 0;
@@ -563,6 +585,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                     rc.w1 = (float)w1_d; rc.w1_lo = (float)(w1_d - (double)rc.w1);
                     const double wS_d = (double)S * dq_d * 0.15915494309189535, w4_d = 4.0 * dq_d * 0.15915494309189535;
                     rc.wS = (float)wS_d; rc.wS_lo = (float)(wS_d - (double)rc.wS);
+                    rc.smult = (float)S;
                     rc.w4 = (float)w4_d; rc.w4_lo = (float)(w4_d - (double)rc.w4);
                     float rcut = theta_min / fabsf(rc.dqf);
                     rc.cut2 = rcut * rcut;

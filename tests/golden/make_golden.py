@@ -21,9 +21,9 @@ from paper_1306_2258_b200 import workloads as wl                   # noqa: E402
 
 SAMPLES = {
     "cfg2": list(range(0, 101, 10)),
-    "cfg3": [0, 1, 37, 100, 163, 199],
+    "cfg3": [0, 1, 37, 100, 150, 163, 180, 190, 199],
     "cfg3_8k": list(range(0, 200, 13)) + [199],
-    "cfg5": [0, 2, 64, 127],
+    "cfg5": [0, 2, 8, 40, 64, 72, 100, 112, 120, 124, 127],     # dense at high q: condition number ~400 there
 }
 CONFORMERS = [0, 1, 511, 1023]
 

@@ -54,7 +54,11 @@ def test_single_structure_configs_against_stored_oracle(db, name):
     w = wl.CONFIGS[name]()
     rows = golden()[name]
     for v in ["auto", "mufu"]:
-        check(run(db, w, v), rows, w, TOL32)
+        worst = check(run(db, w, v), rows, w, TOL32)
+        # regression guard, tighter than the tolerance: a biased reduced angle once cost 1.7e-4 at single q points of cfg5
+        # while four sparse samples stayed below 1e-4; with the unbiased reduction every stored
+        # sample is below 1e-5
+        assert worst <= 3e-5, (name, v, worst)
 
 
 def test_cfg2_full_profile_live_oracle_and_fp64(db):

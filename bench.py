@@ -273,7 +273,14 @@ def main():
                 "traffic": None, "note": "XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM" if per_term else
                 "reference variant; XU roofline quoted for scale"}
     roof["traffic"] = NCU_TRAFFIC.get((args.config, variant_ran))
-    roof["kernel"] = f"debye_pairs_kernel<{info['q_chunk']}, {variant_ran}>"
+    k_ran, chunks_ran = info["q_chunk"], info["n_chunks"]
+    if variant_ran == "recur" and w.M >= 2 and float(w.q[0]) == 0.0:
+        # grid starts at q = 0: the device runs the recurrence launch sized for M - 1 chain indices when the library
+        # offered one (it does when that saves accumulators or a chunk)
+        alt = db.launch_info(w.N, w.B, w.T, w.M - 1, "recur")
+        if alt["n_chunks"] <= 2 and (alt["q_chunk"] < k_ran or alt["n_chunks"] < chunks_ran):
+            k_ran, chunks_ran = alt["q_chunk"], alt["n_chunks"]
+    roof["kernel"] = f"debye_pairs_kernel<{k_ran}, {variant_ran}>"
     roof["kernel_ms"] = pairs_ms
     roof["pair_q_per_clk_per_sm"] = pq_per_launch / (pairs_ms * 1e-3) / (SM_COUNT * fmax_ghz * 1e9)
     roof["share_of_step"] = pairs_ms / (total_ms / args.steps)
@@ -283,7 +290,7 @@ def main():
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if variant_ran == "fp64" else "f32", "data": "synthetic",
         "config": {"workload": w.name, "N": w.N, "T": w.T, "M": w.M, "B": w.B, "variant": variant_ran,
-                   "pairs_grid": info["pairs_grid"], "q_chunk": info["q_chunk"], "n_chunks": info["n_chunks"],
+                   "pairs_grid": info["pairs_grid"], "q_chunk": k_ran, "n_chunks": chunks_ran,
                    "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
                    "parallelism": f"{world} independent structure(s), one per GPU", "wall_s_timed_loop": wall},
         "clocks": clocks,

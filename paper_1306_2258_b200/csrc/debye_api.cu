@@ -37,7 +37,7 @@ struct DevState {
     void *stage = nullptr; size_t stage_bytes = 0;    // device staging for the *_host entry points
     int sms = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;         // optional: recorded around the pairs launches
-    int occ[5][17];                                   // cached CTAs/SM per (variant, K/8); 0 = unknown
+    int occ[5][33];                                   // cached CTAs/SM per (variant, K/4); 0 = unknown
 };
 DevState g_dev[MAX_DEV];
 std::mutex g_mu;
@@ -45,16 +45,17 @@ bool g_atexit = false;
 
 size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
-struct Choice { int variant; int K; int n_chunks; };
+struct Choice { int variant; int K; int n_chunks; int alt_gate; };   // alt_gate: -1 always runs, 0 / 1 see debye_pairs_kernel
 
 // q-chunking of each variant: how many accumulators a thread keeps (K) and how many passes over the pairs.
 Choice choose(int variant, int M)
 {
-    Choice c; c.variant = variant;
+    Choice c; c.variant = variant; c.alt_gate = -1;
     if (variant == V_RECUR) {
+        // M chain indices (worst case: grid starting at dq, or general start); residue-class chunks: a power of two
         int nc = 1;
-        while (((M + 8 * nc - 1) / (8 * nc)) * 8 > DEBYE_KMAX_F32) nc *= 2;     // residue-class chunks: power of two
-        c.n_chunks = nc; c.K = ((M + 8 * nc - 1) / (8 * nc)) * 8;
+        while (debye::recur_slots(M, nc) > DEBYE_KMAX_F32) nc *= 2;
+        c.n_chunks = nc; c.K = debye::recur_slots(M, nc);
     } else {
         int kmax = (variant == V_F64) ? DEBYE_KMAX_F64 : DEBYE_KMAX_F32;
         int nc = (M + kmax - 1) / kmax;
@@ -62,6 +63,23 @@ Choice choose(int variant, int M)
         c.n_chunks = nc; c.K = (per + 7) / 8 * 8;
     }
     return c;
+}
+// Recurrence launches: a grid that starts at q = 0 needs one chain index fewer (q = 0 is answered by the epilogue), which
+// can save four accumulators or a whole chunk -- but only the device knows q.  When it pays, a second instantiation
+// sized for M - 1 indices is launched as well and the device runs exactly one of the two (plan->recur_alt).
+int recur_choices(Choice *out, int M)
+{
+    const Choice main_c = choose(V_RECUR, M);
+    if (M >= 2) {
+        Choice alt = choose(V_RECUR, M - 1);
+        if (alt.n_chunks <= 2 && (alt.K < main_c.K || alt.n_chunks < main_c.n_chunks)) {
+            alt.alt_gate = 1;
+            out[0] = alt; out[1] = main_c; out[1].alt_gate = 0;
+            return 2;
+        }
+    }
+    out[0] = main_c;
+    return 1;
 }
 
 struct Layout { size_t plan, perm, sorted, records, total; };
@@ -81,17 +99,18 @@ Layout layout(int N, int B, int T, int M, int G_max, const Choice *ch, int nch)
     return L;
 }
 
+constexpr int MAX_CHOICES = 3;
 int variants_for(uint32_t flags, Choice *out, int M, int *is_auto)
 {
     *is_auto = 0;
     if (flags & DEBYE_FP64) { out[0] = choose(V_F64, M); return 1; }
     if (flags & DEBYE_SINC_MUFU) { out[0] = choose(V_MUFU, M); return 1; }
-    if (flags & DEBYE_SINC_RECUR) { out[0] = choose(V_RECUR, M); return 1; }
+    if (flags & DEBYE_SINC_RECUR) return recur_choices(out, M);
     if (flags & DEBYE_SINC_ACCURATE) { out[0] = choose(V_ACCURATE, M); return 1; }
     *is_auto = 1;
-    out[0] = choose(V_RECUR, M);
-    out[1] = choose(V_MUFU, M);
-    return 2;
+    int n = recur_choices(out, M);
+    out[n++] = choose(V_MUFU, M);
+    return n;
 }
 
 int validate(const void *xyz, const void *type, int N, int B, const void *tab, int T, const void *q, int M, const void *out, uint32_t flags)
@@ -132,7 +151,7 @@ int dev_state(DevState **st)
 // the host never sees the type histogram).
 int grid_for(DevState *s, const Choice &c, int N, int B, int *G)
 {
-    int &o = s->occ[c.variant][c.K / 8];
+    int &o = s->occ[c.variant][c.K / 4];
     if (o == 0) {
         debye_pairs_fn fn = debye_get_pairs_kernel(c.variant, c.K);
         if (!fn) return DEBYE_EUNSUPPORTED;
@@ -186,9 +205,9 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     std::lock_guard<std::mutex> lock(g_mu);
     DevState *ds;
     if ((st = dev_state(&ds))) return st;
-    Choice ch[2]; int is_auto = 0;
+    Choice ch[MAX_CHOICES]; int is_auto = 0;
     const int nch = variants_for(flags, ch, M, &is_auto);
-    int G[2] = {0, 0}, Gmax = 0;
+    int G[MAX_CHOICES] = {0, 0, 0}, Gmax = 0;
     for (int i = 0; i < nch; ++i) { if ((st = grid_for(ds, ch[i], N, B, &G[i]))) return st; if (G[i] > Gmax) Gmax = G[i]; }
     const Layout L = layout(N, B, T, M, Gmax, ch, nch);
     char *ws;
@@ -199,10 +218,10 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     float4 *sorted = (float4 *)(ws + L.sorted);
     double *records = (double *)(ws + L.records);
 
-    int rec_cap = 0;
-    for (int i = 0; i < nch; ++i) if (ch[i].variant == V_RECUR) rec_cap = ch[i].K * ch[i].n_chunks;
+    int alt_offered = 0;
+    for (int i = 0; i < nch; ++i) if (ch[i].alt_gate == 1) alt_offered = 1;
     const bool pack_here = (int64_t)N * B <= DEBYE_PACK_IN_SETUP;      // small inputs: the setup CTA gathers too
-    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, rec_cap, xyz, sorted, pack_here ? 1 : 0);
+    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, xyz, sorted, pack_here ? 1 : 0);
     if (!pack_here) {
         int64_t total = (int64_t)N * B;
         int blocks = (int)((total + 255) / 256);
@@ -214,15 +233,18 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
         debye_pairs_fn fn = debye_get_pairs_kernel(ch[i].variant, ch[i].K);
         // slow-path threshold on theta = r * (smallest grid step or smallest |q|): see DESIGN.md section 6
         const float theta_min = (ch[i].variant == V_RECUR) ? 0.002f : 0.004f;
-        fn<<<G[i], DEBYE_IB, 0, stream>>>(plan, sorted, q, records, ch[i].n_chunks, is_auto, theta_min);
+        fn<<<G[i], DEBYE_IB, 0, stream>>>(plan, sorted, q, records, ch[i].n_chunks, is_auto, theta_min, ch[i].alt_gate);
     }
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
     {
         int threads = DEBYE_FINAL_THREADS, blocks = B * ((M + DEBYE_FINAL_Q - 1) / DEBYE_FINAL_Q);
-        // in automatic mode the final kernel picks the parameter set of the variant chosen on the device
-        const Choice &c1 = ch[nch - 1];
-        debye::debye_final_kernel<<<blocks, threads, 0, stream>>>(plan, records, fftab, q, out, is_auto, ch[0].variant, ch[0].K, ch[0].n_chunks, G[0], c1.variant, c1.K,
-                                                                  c1.n_chunks, G[nch - 1], mode);
+        // the final kernel repeats the device-side decisions of the pairs launches to find the one that did the work
+        debye::FinalSets sets; sets.n = nch;
+        for (int i = 0; i < MAX_CHOICES; ++i) {
+            const int j = i < nch ? i : 0;
+            sets.s[i].variant = ch[j].variant; sets.s[i].K = ch[j].K; sets.s[i].n_chunks = ch[j].n_chunks; sets.s[i].G = G[j]; sets.s[i].alt_gate = ch[j].alt_gate;
+        }
+        debye::debye_final_kernel<<<blocks, threads, 0, stream>>>(plan, records, fftab, q, out, is_auto, sets, mode);
     }
     if (mode == 1 && n_out) CU(cudaMemcpyAsync(n_out, plan->n_a, sizeof(int32_t) * T, cudaMemcpyDeviceToDevice, stream));
     CU(cudaGetLastError());
@@ -300,7 +322,7 @@ size_t debye_workspace_bytes(int32_t N, int32_t B, int32_t T, int32_t M, uint32_
 {
     static const char dummy = 0;
     if (validate(&dummy, &dummy, N, B, &dummy, T, &dummy, M, &dummy, flags)) return 0;
-    Choice ch[2]; int is_auto;
+    Choice ch[MAX_CHOICES]; int is_auto;
     int nch = variants_for(flags, ch, M, &is_auto);
     // grid is at most 148 SMs x 16 CTAs x 16 waves on any sm_100 part; use a safe upper bound so no device query is needed
     return layout(N, B, T, M, 192 * 16 * 16, ch, nch).total;
@@ -337,16 +359,17 @@ int debye_launch_info(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags
     static const char dummy = 0;
     int st = validate(&dummy, &dummy, N, B, &dummy, T, &dummy, M, &dummy, flags);
     if (st) return st;
-    Choice ch[2]; int is_auto;
+    Choice ch[MAX_CHOICES]; int is_auto;
     int nch = variants_for(flags, ch, M, &is_auto);
+    const int lead = (nch > 1 && ch[0].alt_gate == 1) ? 1 : 0;     // report the launch sized for the general case
     if (n_launches) *n_launches = 2 + nch + (((int64_t)N * B <= DEBYE_PACK_IN_SETUP) ? 0 : 1);   // setup, [pack], pairs x nch, final
-    if (q_chunk) *q_chunk = ch[0].K;
-    if (n_chunks) *n_chunks = ch[0].n_chunks;
+    if (q_chunk) *q_chunk = ch[lead].K;
+    if (n_chunks) *n_chunks = ch[lead].n_chunks;
     if (pairs_grid) {
         std::lock_guard<std::mutex> lock(g_mu);
         DevState *ds; int G = 0;
         if ((st = dev_state(&ds))) return st;
-        if ((st = grid_for(ds, ch[0], N, B, &G))) return st;
+        if ((st = grid_for(ds, ch[lead], N, B, &G))) return st;
         *pairs_grid = G;
     }
     return DEBYE_OK;

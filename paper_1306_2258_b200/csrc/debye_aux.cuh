@@ -19,7 +19,7 @@ namespace debye {
 // (warp, type) its first output slot; pass 2 walks the chunk again and places the atoms.  Two block barriers in total.
 // If pack_here != 0 the CTA also gathers the coordinates (small N x B: saves the pack launch).
 __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPlan *plan, const int32_t *__restrict__ type, const float *__restrict__ q,
-                                                                            int32_t *__restrict__ perm, int N, int T, int M, int B, int rec_capacity /* K * n_chunks of the recurrence */,
+                                                                            int32_t *__restrict__ perm, int N, int T, int M, int B, int alt_offered /* a recurrence launch sized for M - 1 indices exists */,
                                                                             const float *__restrict__ xyz, float4 *__restrict__ sorted, int pack_here)
 {
     constexpr int NWARP = DEBYE_SETUP_THREADS / 32;
@@ -76,12 +76,13 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
         for (int w = 0; w < NWARP; ++w) { d = fmaxf(d, red[w]); s = fminf(s, red2[w]); mx = fmaxf(mx, qmax_s[w]); }
         // uniform if every q[k] is within 2 float ulps (of the largest |q|) of the line through the end points
         const int uni = (dq != 0.0) && (d <= 2.4e-7f * fmaxf(mx, 1e-30f));
+        // zero start: q0 == 0 exactly (koff = 0) or q0 == dq to 1e-6 (koff = 1, the paper's own grid q_k = k dq, k >= 1)
         int koff = -1;
         if (uni) {
-            const double ko = q0 / dq;
-            const double kr = rint(ko);
-            if (kr >= 0.0 && kr <= 8.0 && fabs(ko - kr) <= 1e-6 * fmax(1.0, kr) && (int)kr + M <= rec_capacity) koff = (int)kr;
+            if (q0 == 0.0) koff = 0;
+            else if (fabs(q0 / dq - 1.0) <= 1e-6) koff = 1;
         }
+        plan->recur_alt = (koff == 0 && alt_offered) ? 1 : 0;
         plan->N = N; plan->T = T; plan->M = M; plan->B = B; plan->n_tp = T * (T + 1) / 2;
         plan->uniform = uni;
         plan->zero_start = koff;
@@ -176,10 +177,11 @@ __device__ __forceinline__ double pair_count(int na, int nb, bool diag) { return
 #define DEBYE_FINAL_G 8
 #define DEBYE_FINAL_NS 4
 #define DEBYE_FINAL_THREADS (DEBYE_FINAL_Q * DEBYE_FINAL_G * DEBYE_FINAL_NS)
+struct FinalSet { int variant, K, n_chunks, G, alt_gate; };   // parameters of one pairs launch (alt_gate as in the pairs kernel)
+struct FinalSets { FinalSet s[3]; int n; };                    // up to: recurrence (M - 1 indices), recurrence, MUFU
 __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const DevPlan *__restrict__ plan, const double *__restrict__ records,
                                                                             const float *__restrict__ fftab, const float *__restrict__ q, double *__restrict__ out,
-                                                                            int is_auto, int variant0, int K0, int nc0, int G0, int variant1, int K1, int nc1, int G1,
-                                                                            int mode)
+                                                                            int is_auto, const FinalSets sets, int mode)
 {
     __shared__ double part[DEBYE_FINAL_G * DEBYE_FINAL_NS][DEBYE_FINAL_Q];
     const int M = plan->M, Bn = plan->B, T = plan->T, n_tp = plan->n_tp;
@@ -189,18 +191,23 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
     const int g = gs / DEBYE_FINAL_NS, sl = gs % DEBYE_FINAL_NS;
     const int b = blockIdx.x / ktiles, k = (blockIdx.x % ktiles) * DEBYE_FINAL_Q + kk;
     const bool live = k < M && sl < NS;
-    // automatic mode: two pairs kernels were launched and the device ran the one named by plan->variant_auto
-    const bool second = is_auto && plan->variant_auto == variant1;
-    const int variant = second ? variant1 : variant0, K = second ? K1 : K0, n_chunks = second ? nc1 : nc0, G = second ? G1 : G0;
+    // which pairs launch did the work: the same device-side decisions the pairs kernels took
+    int pick = 0;
+    for (int i = 0; i < sets.n; ++i) {
+        const FinalSet &c = sets.s[i];
+        if ((!is_auto || plan->variant_auto == c.variant) && (c.alt_gate < 0 || plan->recur_alt == c.alt_gate)) { pick = i; break; }
+    }
+    const int variant = sets.s[pick].variant, K = sets.s[pick].K, n_chunks = sets.s[pick].n_chunks, G = sets.s[pick].G;
     const bool bad = (variant == V_RECUR && !plan->uniform);          // forced recurrence on a non-uniform grid -> NaN
     const double nan = __longlong_as_double(0x7ff8000000000000LL);
     const double scale = (variant == V_RECUR) ? 0.5 : 1.0;            // the recurrence kernel accumulates 2 sin(q r)/r
     double I = 0.0;
     if (live) {
-        int kprime = k;
-        if (variant == V_RECUR && plan->zero_start > 0) kprime = k + plan->zero_start;
-        int ch, l;
-        slot_of(variant, K, n_chunks, kprime, ch, l);
+        // chain / grid index of output k (convention at slot_of); -1 only for q = 0, which never reads a record
+        int idx = k;
+        if (variant == V_RECUR && plan->zero_start >= 0 && n_chunks <= 2) idx = k + plan->zero_start - 1;
+        int ch = 0, l = 0;
+        if (idx >= 0) slot_of(variant, K, n_chunks, idx, ch, l);
         const double qk = (double)q[k];
         const int64_t U1 = plan->U1, Uc = U1 * n_chunks, U = Uc * Bn;
         // type pair index -> (a, b2): walk rows of the upper triangle

@@ -175,18 +175,33 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-// where output index k lives: q-chunk and local slot.  Recurrence chunks are residue classes mod S = 8 n_chunks
-// (so every chunk can start at index 0); the direct variants use contiguous ranges.
-__host__ __device__ inline void slot_of(int variant, int K, int n_chunks, int kprime, int &ch, int &l)
+// where chain / grid index idx lives: q-chunk and local slot.  Recurrence chunks are residue classes mod S = 8 n_chunks
+// (so every chunk starts at the bottom of the grid); the direct variants use contiguous ranges.
+// Recurrence index convention (pairs kernel and final kernel must agree):
+//   zero-start modes (grid q_k = (k + koff) dq, koff in {0, 1}, at most 2 chunks): idx = k + koff - 1, i.e. the chains
+//     start at the first multiple of dq that is not zero (q = 0 is answered by the epilogue: idx = -1 is never stored);
+//   general mode: idx = k.
+__host__ __device__ inline void slot_of(int variant, int K, int n_chunks, int idx, int &ch, int &l)
 {
     if (variant == V_RECUR) {
         int S = 8 * n_chunks;
-        ch = (kprime % S) / 8;
-        l = 8 * (kprime / S) + (kprime % 8);
+        ch = (idx % S) / 8;
+        l = 8 * (idx / S) + (idx % 8);
     } else {
-        ch = kprime / K;
-        l = kprime % K;
+        ch = idx / K;
+        l = idx % K;
     }
+}
+// accumulators a recurrence launch needs for n_idx chain indices in n_chunks chunks: chunk 0 holds the most; K is kept a
+// multiple of 4 (two packed chains) and at least 8
+__host__ __device__ inline int recur_slots(int n_idx, int n_chunks)
+{
+    if (n_idx < 1) return 8;
+    const int S = 8 * n_chunks, last = n_idx - 1;
+    const int r = last % S;
+    const int lmax = 8 * (last / S) + (r < 8 ? r : 7);
+    const int K = (lmax + 1 + 3) / 4 * 4;
+    return K < 8 ? 8 : K;
 }
 
 template <int K, int VAR>
@@ -206,7 +221,6 @@ struct RecurConst {
     float smult;             // (float)S: wS = S w1 exactly (S is a power of two)
     float w4, w4_lo;         // 4 dq / 2 pi (general start: bootstrap stride)
     float cut2;              // r^2 at or below which the pair takes the slow path
-    float dqf, qbase_l;      // slow path: q of local slot l is qbase_l + (S (l / 8) + l % 8) dqf
     int n_chunks;
 };
 
@@ -255,19 +269,20 @@ __device__ __forceinline__ void recur_vals(const RecurGeom &g, const RecurConst 
         u[0] = 0.0f;
         u[1] = T1 * rinv; u[2] = c1 * u[1]; u[3] = fmaf(c1, u[2], -u[1]); u[4] = c2 * u[2];
         u[5] = fmaf(c4, u[1], u[3]); u[6] = fmaf(c4, u[2], u[2]); u[7] = fmaf(c4, u[3], u[1]); u[8] = c4 * u[4];
+        // chains start at index 1 (index 0 is identically zero): chain j of chunk ch holds k' = 1 + 8 ch + j + S m.
+        // B = w_0 = v(k'), A = w_{-1} = -v(k' - S) = +u[S - k'] (v(-n) = -v(n))
         if constexpr (MODE == RM_Z1) {
-            // w_0 = v_0 (B), w_{-1} = -v_{-1} = +v_{8-n} (A)
-            Bv[0] = pk2(u[0], u[1]); Bv[1] = pk2(u[2], u[3]); Bv[2] = pk2(u[4], u[5]); Bv[3] = pk2(u[6], u[7]);
-            A[0] = pk2(u[8], u[7]); A[1] = pk2(u[6], u[5]); A[2] = pk2(u[4], u[3]); A[3] = pk2(u[2], u[1]);
+            Bv[0] = pk2(u[1], u[2]); Bv[1] = pk2(u[3], u[4]); Bv[2] = pk2(u[5], u[6]); Bv[3] = pk2(u[7], u[8]);
+            A[0] = pk2(u[7], u[6]); A[1] = pk2(u[5], u[4]); A[2] = pk2(u[3], u[2]); A[3] = pk2(u[1], u[0]);
         } else {
 #pragma unroll
             for (int n = 9; n <= 16; ++n) u[n] = fmaf(c4, u[n - 4], -u[n - 8]);
             if constexpr (MODE == RM_Z2A) {
-                Bv[0] = pk2(u[0], u[1]); Bv[1] = pk2(u[2], u[3]); Bv[2] = pk2(u[4], u[5]); Bv[3] = pk2(u[6], u[7]);
-                A[0] = pk2(u[16], u[15]); A[1] = pk2(u[14], u[13]); A[2] = pk2(u[12], u[11]); A[3] = pk2(u[10], u[9]);
+                Bv[0] = pk2(u[1], u[2]); Bv[1] = pk2(u[3], u[4]); Bv[2] = pk2(u[5], u[6]); Bv[3] = pk2(u[7], u[8]);
+                A[0] = pk2(u[15], u[14]); A[1] = pk2(u[13], u[12]); A[2] = pk2(u[11], u[10]); A[3] = pk2(u[9], u[8]);
             } else {
-                Bv[0] = pk2(u[8], u[9]); Bv[1] = pk2(u[10], u[11]); Bv[2] = pk2(u[12], u[13]); Bv[3] = pk2(u[14], u[15]);
-                A[0] = pk2(u[8], u[7]); A[1] = pk2(u[6], u[5]); A[2] = pk2(u[4], u[3]); A[3] = pk2(u[2], u[1]);
+                Bv[0] = pk2(u[9], u[10]); Bv[1] = pk2(u[11], u[12]); Bv[2] = pk2(u[13], u[14]); Bv[3] = pk2(u[15], u[16]);
+                A[0] = pk2(u[7], u[6]); A[1] = pk2(u[5], u[4]); A[2] = pk2(u[3], u[2]); A[3] = pk2(u[1], u[0]);
             }
         }
     } else {
@@ -300,15 +315,17 @@ __device__ __forceinline__ void recur_hot(u64 (&acc)[K / 2], u64 (&A)[4], u64 (&
 {
     const u64 cP = pk2(cS, cS), cN = pk2(-cS, -cS);
 #pragma unroll
-    for (int m = 0; m < K / 8; ++m) {
+    for (int m = 0; m < (K + 7) / 8; ++m) {
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
-            if (m & 2) acc[4 * m + a] = sub2(acc[4 * m + a], Bv[a]);
-            else acc[4 * m + a] = add2(acc[4 * m + a], Bv[a]);
-            if (m + 1 < K / 8) {
-                u64 nx = fma2((m & 1) ? cN : cP, Bv[a], A[a]);
-                A[a] = Bv[a];
-                Bv[a] = nx;
+            if (8 * m + 2 * a < K) {                       // K % 8 == 4: the last step runs chains 0 and 1 only
+                if (m & 2) acc[4 * m + a] = sub2(acc[4 * m + a], Bv[a]);
+                else acc[4 * m + a] = add2(acc[4 * m + a], Bv[a]);
+                if (8 * (m + 1) + 2 * a < K) {
+                    u64 nx = fma2((m & 1) ? cN : cP, Bv[a], A[a]);
+                    A[a] = Bv[a];
+                    Bv[a] = nx;
+                }
             }
         }
     }
@@ -339,13 +356,15 @@ __device__ __forceinline__ void recur_slow_pair(u64 (&acc)[K / 2], const float4 
 #pragma unroll
     for (int a = 0; a < 4; ++a) { s[a] = Bv[a]; d[a] = add2(Bv[a], A[a]); }
 #pragma unroll
-    for (int m = 0; m < K / 8; ++m) {
+    for (int m = 0; m < (K + 7) / 8; ++m) {
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
-            acc[4 * m + a] = add2(acc[4 * m + a], s[a]);
-            if (m + 1 < K / 8) {
-                d[a] = fma2(nb2, s[a], d[a]);
-                s[a] = add2(s[a], d[a]);
+            if (8 * m + 2 * a < K) {
+                acc[4 * m + a] = add2(acc[4 * m + a], s[a]);
+                if (8 * (m + 1) + 2 * a < K) {
+                    d[a] = fma2(nb2, s[a], d[a]);
+                    s[a] = add2(s[a], d[a]);
+                }
             }
         }
     }
@@ -433,7 +452,7 @@ __device__ unsigned long long debye_trace[3 * 4096];
 #endif
 template <int K, int VAR>
 __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR ? recur_min_ctas(K) : (K <= 64 ? 4 : (K <= 112 ? 3 : 2)))) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
-                                                               double *__restrict__ records, int n_chunks, int is_auto, float theta_min)
+                                                               double *__restrict__ records, int n_chunks, int is_auto, float theta_min, int alt_gate)
 {
     // ---- variant gate (decided on the device so the host never reads q) ---------------------------------------
     if (is_auto) {
@@ -441,6 +460,9 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
     } else if (VAR == V_RECUR && !plan->uniform) {
         return;   // the final kernel writes NaN in this case
     }
+    // recurrence: two accumulator counts may be launched (grid starting at q = 0 needs one chain index fewer, and the
+    // host cannot know); alt_gate = 1 runs only if the device chose the smaller one, 0 only if not, -1 always
+    if (VAR == V_RECUR && alt_gate >= 0 && plan->recur_alt != alt_gate) return;
     constexpr bool F64 = (VAR == V_F64);
     constexpr int NW = DEBYE_IB / 32;
     __shared__ __align__(128) float4 tile[2][DEBYE_JT];
@@ -480,7 +502,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
     const double dq_d = plan->dq, q0_d = plan->q0;
     const int koff = plan->zero_start;           // >= 0: grid is (k + koff) dq with koff small; -1: general
     RecurConst rc;
-    rc.w1 = rc.w1_lo = rc.wS = rc.wS_lo = rc.w4 = rc.w4_lo = rc.cut2 = rc.dqf = rc.qbase_l = 0.f;
+    rc.w1 = rc.w1_lo = rc.wS = rc.wS_lo = rc.w4 = rc.w4_lo = rc.cut2 = 0.f;
     rc.smult = 8.0f;
     rc.n_chunks = n_chunks;
     float cut2 = 0.f;
@@ -568,11 +590,11 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                 ch_cur = ch;
                 if constexpr (VAR == V_RECUR) {
                     const int S = 8 * n_chunks;
-                    rc.dqf = (float)dq_d;
+                    // zero-start modes: grid (k + koff) dq with koff in {0, 1} and at most 2 chunks; else general start,
+                    // which takes the grid as q0 + k dq whatever q0 is
                     const bool zs = (koff >= 0 && n_chunks <= 2);
                     mode = zs ? (n_chunks == 1 ? RM_Z1 : (ch == 0 ? RM_Z2A : RM_Z2B)) : RM_G;
-                    const double qb = (koff >= 0) ? 0.0 : q0_d;          // q of k' = 0
-                    rc.qbase_l = (float)(qb + (8.0 * ch) * dq_d);
+                    const double qb = q0_d;                               // general start: q of chain index 0
                     const int base = -S + 8 * ch;                         // k' of the first start value
                     __syncthreads();
                     if (tid < 8) {   // turns per Angstrom of the 8 general-start values, hi and lo parts
@@ -587,7 +609,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                     rc.wS = (float)wS_d; rc.wS_lo = (float)(wS_d - (double)rc.wS);
                     rc.smult = (float)S;
                     rc.w4 = (float)w4_d; rc.w4_lo = (float)(w4_d - (double)rc.w4);
-                    float rcut = theta_min / fabsf(rc.dqf);
+                    const float rcut = theta_min / fabsf((float)dq_d);
                     rc.cut2 = rcut * rcut;
                 } else {
                     __syncthreads();

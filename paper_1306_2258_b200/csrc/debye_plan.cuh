@@ -20,11 +20,11 @@ struct DevPlan {
     int32_t N, T, M, B;
     int32_t n_tp;                 // T(T+1)/2
     int32_t uniform;              // q is a uniform grid q0 + m dq (checked on the device)
-    int32_t zero_start;           // uniform and q0 == 0
+    int32_t zero_start;           // uniform and q0 = koff dq with koff in {0, 1} (0 only if q0 == 0 exactly): koff; else -1
+    int32_t recur_alt;            // recurrence: run the launch sized for M - 1 chain indices (koff == 0 and the host offered one)
     int32_t variant_auto;         // variant chosen on the device when the caller gave no DEBYE_SINC_* flag
     double q0, dq;                // least-squares-free fit: q0 = q[0], dq = (q[M-1]-q[0])/(M-1)
     float q_small;                // smallest non-zero |q|
-    int32_t pad0;
     int64_t U1;                   // units per conformer and per q-chunk
     int32_t seg_off[DEBYE_MAX_TYPES_I + 1];   // sorted-array offset of each type segment
     int32_t n_a[DEBYE_MAX_TYPES_I];           // atoms per type

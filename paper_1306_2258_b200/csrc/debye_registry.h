@@ -3,12 +3,12 @@
 #include <cstdint>
 #include "debye_plan.cuh"
 
-typedef void (*debye_pairs_fn)(const DevPlan *, const float4 *, const float *, double *, int, int, float);
+typedef void (*debye_pairs_fn)(const DevPlan *, const float4 *, const float *, double *, int, int, float, int);
 
 #define DEBYE_KMAX_F32 128
 #define DEBYE_KMAX_F64 32
 
-// K must be a multiple of 8 in [8, KMAX]; returns nullptr otherwise
+// K must be a multiple of 8 in [8, KMAX] (recurrence: a multiple of 4); returns nullptr otherwise
 debye_pairs_fn debye_get_pairs_kernel(int variant, int K);
 debye_pairs_fn debye_get_recur(int K);
 debye_pairs_fn debye_get_mufu(int K);

@@ -2,6 +2,7 @@
 #include "debye_pairs.cuh"
 #include "debye_registry.h"
 debye_pairs_fn debye_get_recur_a(int K); debye_pairs_fn debye_get_recur_b(int K);
+debye_pairs_fn debye_get_recur_c(int K); debye_pairs_fn debye_get_recur_d(int K);
 debye_pairs_fn debye_get_mufu_a(int K); debye_pairs_fn debye_get_mufu_b(int K);
 debye_pairs_fn debye_get_accurate_a(int K); debye_pairs_fn debye_get_accurate_b(int K);
 debye_pairs_fn debye_get_f64(int K)
@@ -18,7 +19,7 @@ debye_pairs_fn debye_get_pairs_kernel(int variant, int K)
 {
     switch (variant) {
         case V_F64: return debye_get_f64(K);
-        case V_RECUR: return K <= 64 ? debye_get_recur_a(K) : debye_get_recur_b(K);
+        case V_RECUR: return (K % 8 == 0) ? (K <= 64 ? debye_get_recur_a(K) : debye_get_recur_b(K)) : (K <= 64 ? debye_get_recur_c(K) : debye_get_recur_d(K));
         case V_MUFU: return K <= 64 ? debye_get_mufu_a(K) : debye_get_mufu_b(K);
         case V_ACCURATE: return K <= 64 ? debye_get_accurate_a(K) : debye_get_accurate_b(K);
         default: return nullptr;

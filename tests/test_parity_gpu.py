@@ -50,6 +50,11 @@ CASES = [
     ("s7_N900_T3_M64_offset_grid", lambda: wl.small_random(7, 900, 3, 64, q_min=0.3, q_max=0.9)),   # general start
     ("s8_N513_T32_M40_signed", lambda: wl.small_random(8, 513, 32, 40, signed=True)),
     ("s9_N2100_T2_M300", lambda: wl.small_random(9, 2100, 2, 300, q_max=1.2, box=60.0)),  # 4 chunks
+    # grids starting at q = 0 where dropping the trivial index saves a whole chunk (129 -> 128 indices: 1 chunk instead of 2;
+    # 257 -> 256: 2 instead of 4): the device picks the smaller of two recurrence launches
+    ("s10_N400_T2_M129", lambda: wl.small_random(10, 400, 2, 129, q_max=0.8)),
+    ("s11_N300_T3_M257", lambda: wl.small_random(11, 300, 3, 257, q_max=1.0)),
+    ("s12_N500_T2_M129_from_dq", lambda: wl.small_random(12, 500, 2, 129, q_min=0.005, q_max=0.645)),   # q_k = (k + 1) dq
     ("cfg1", wl.cfg1),
     ("table1_N1000_paper_grid", lambda: wl.table1(1000)),                                 # q_k = k/50, k = 1..50
 ]

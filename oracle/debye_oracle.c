@@ -16,6 +16,8 @@
  *   R7  "only values for j <= k are computed" means I = sum_k f_k^2 + 2 sum_{j<k} f_j f_k sinc.
  *   R8  form factors are real, sign unrestricted.
  *   R10 form factors are given per atom TYPE: f_j(q_m) = fftab[type[j]][m]  (north_star narrowing).
+ *   R10w optional per-atom weights (the one-parameter family of the paper's per-atom form factors,
+ *        PAPER.md:44, 82): f_j(q_m) = weight[j] * fftab[type[j]][m]; weight == NULL means 1.
  * Inputs are the same float32 / int32 bytes the GPU gets, promoted exactly to double.
  *
  * Pins (tests/test_oracle_pins.py): two-atom closed form, I(0) = (sum f)^2, Eq. (1) by spherical quadrature,
@@ -43,17 +45,25 @@ static double dist(const float *a, const float *b)
 /* Eq. (2) literally: for every q_m, the full N x N double loop including j == k.
  * I[m] = sum_k sum_j F[t_k][m] F[t_j][m] sinc(q_m r_jk);  Abs[m] (optional) = same with |.| on each term,
  * so callers can print the condition number Abs/I.  Single thread, no symmetry. */
+void oracle_debye_full_w(const float *xyz, const int32_t *type, const float *weight, int32_t N, const float *fftab,
+                         int32_t T, const float *q, int32_t M, double *I, double *Abs);
 void oracle_debye_full(const float *xyz, const int32_t *type, int32_t N, const float *fftab, int32_t T,
                        const float *q, int32_t M, double *I, double *Abs)
+{
+    oracle_debye_full_w(xyz, type, NULL, N, fftab, T, q, M, I, Abs);
+}
+/* The same with per-atom weights (reading R10w): f_k(q_m) = weight[k] F[t_k][m]. */
+void oracle_debye_full_w(const float *xyz, const int32_t *type, const float *weight, int32_t N, const float *fftab,
+                         int32_t T, const float *q, int32_t M, double *I, double *Abs)
 {
     (void)T;
     for (int m = 0; m < M; ++m) {
         long double acc = 0.0L, aabs = 0.0L;
         double qm = (double)q[m];
         for (int k = 0; k < N; ++k) {
-            double fk = (double)fftab[(size_t)type[k] * M + m];
+            double fk = (double)fftab[(size_t)type[k] * M + m] * (weight ? (double)weight[k] : 1.0);
             for (int j = 0; j < N; ++j) {
-                double fj = (double)fftab[(size_t)type[j] * M + m];
+                double fj = (double)fftab[(size_t)type[j] * M + m] * (weight ? (double)weight[j] : 1.0);
                 double term = fk * fj * sinc(qm * dist(xyz + 3 * k, xyz + 3 * j));
                 acc += term;
                 aabs += fabs(term);
@@ -68,9 +78,19 @@ void oracle_debye_full(const float *xyz, const int32_t *type, int32_t N, const f
  * is what bench.py times; row0=0,row1=N gives the whole profile).  One double accumulator per (row, q),
  * rows combined in long double.  OpenMP over rows, cyclic static schedule; threads <= 0 means all cores.
  * Returns the number of threads used. */
+int32_t oracle_debye_sym_w(const float *xyz, const int32_t *type, const float *weight, int32_t N, const float *fftab,
+                           int32_t T, const float *q, int32_t M, int32_t row0, int32_t row1, int32_t threads,
+                           double *I, double *Abs);
 int32_t oracle_debye_sym(const float *xyz, const int32_t *type, int32_t N, const float *fftab, int32_t T,
                          const float *q, int32_t M, int32_t row0, int32_t row1, int32_t threads,
                          double *I, double *Abs)
+{
+    return oracle_debye_sym_w(xyz, type, NULL, N, fftab, T, q, M, row0, row1, threads, I, Abs);
+}
+/* The same with per-atom weights (reading R10w). */
+int32_t oracle_debye_sym_w(const float *xyz, const int32_t *type, const float *weight, int32_t N, const float *fftab,
+                           int32_t T, const float *q, int32_t M, int32_t row0, int32_t row1, int32_t threads,
+                           double *I, double *Abs)
 {
     (void)T;
     int nthr = 1;
@@ -93,14 +113,15 @@ int32_t oracle_debye_sym(const float *xyz, const int32_t *type, int32_t N, const
             for (int j = k + 1; j < N; ++j) {
                 const float *fj = fftab + (size_t)type[j] * M;
                 double r = dist(xyz + 3 * k, xyz + 3 * j);
+                double wj = weight ? (double)weight[j] : 1.0;
                 for (int m = 0; m < M; ++m) {
-                    double t = (double)fj[m] * sinc((double)q[m] * r);
+                    double t = wj * (double)fj[m] * sinc((double)q[m] * r);
                     row[m] += t;
                     rabs[m] += fabs(t);
                 }
             }
             for (int m = 0; m < M; ++m) {
-                double f = (double)fk[m];
+                double f = (double)fk[m] * (weight ? (double)weight[k] : 1.0);
                 ti[m] += (long double)(f * f) + 2.0L * (long double)f * (long double)row[m];
                 ta[m] += (long double)(f * f) + 2.0L * (long double)fabs(f) * (long double)rabs[m];
             }

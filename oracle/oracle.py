@@ -26,6 +26,11 @@ def _L():
         _lib.oracle_debye_sym.argtypes = [fp, ip, C.c_int32, fp, C.c_int32, fp, C.c_int32, C.c_int32, C.c_int32,
                                           C.c_int32, dp, dp]
         _lib.oracle_debye_sym.restype = C.c_int32
+        _lib.oracle_debye_full_w.argtypes = [fp, ip, fp, C.c_int32, fp, C.c_int32, fp, C.c_int32, dp, dp]
+        _lib.oracle_debye_full_w.restype = None
+        _lib.oracle_debye_sym_w.argtypes = [fp, ip, fp, C.c_int32, fp, C.c_int32, fp, C.c_int32, C.c_int32, C.c_int32,
+                                            C.c_int32, dp, dp]
+        _lib.oracle_debye_sym_w.restype = C.c_int32
         _lib.oracle_eq1_quadrature.argtypes = [dp, dp, C.c_int32, C.c_double, dp, dp, C.c_int32]
         _lib.oracle_eq1_quadrature.restype = C.c_double
     return _lib
@@ -46,25 +51,46 @@ def _p(a, t):
     return a.ctypes.data_as(C.POINTER(t))
 
 
-def debye_full(xyz, typ, fftab, q, return_abs=False):
-    """Eq. (2) literally (N x N loop including j == k), single thread.  PAPER.md:41-42."""
+def _w(weight, N):
+    if weight is None:
+        return None
+    weight = np.ascontiguousarray(weight, dtype=np.float32)
+    assert weight.shape == (N,)
+    return weight
+
+
+def debye_full(xyz, typ, fftab, q, return_abs=False, weight=None):
+    """Eq. (2) literally (N x N loop including j == k), single thread.  PAPER.md:41-42.
+    weight[N] (optional): f_j(q) = weight[j] * fftab[type[j]] (reading R10w)."""
     xyz, typ, fftab, q = _prep(xyz, typ, fftab, q)
     M = q.shape[0]
     I, A = np.zeros(M), np.zeros(M)
-    _L().oracle_debye_full(_p(xyz, C.c_float), _p(typ, C.c_int32), xyz.shape[0], _p(fftab, C.c_float),
-                           fftab.shape[0], _p(q, C.c_float), M, _p(I, C.c_double), _p(A, C.c_double))
+    w = _w(weight, xyz.shape[0])
+    if w is None:
+        _L().oracle_debye_full(_p(xyz, C.c_float), _p(typ, C.c_int32), xyz.shape[0], _p(fftab, C.c_float),
+                               fftab.shape[0], _p(q, C.c_float), M, _p(I, C.c_double), _p(A, C.c_double))
+    else:
+        _L().oracle_debye_full_w(_p(xyz, C.c_float), _p(typ, C.c_int32), _p(w, C.c_float), xyz.shape[0],
+                                 _p(fftab, C.c_float), fftab.shape[0], _p(q, C.c_float), M, _p(I, C.c_double),
+                                 _p(A, C.c_double))
     return (I, A) if return_abs else I
 
 
-def debye_sym(xyz, typ, fftab, q, rows=None, threads=0, return_abs=False, return_threads=False):
+def debye_sym(xyz, typ, fftab, q, rows=None, threads=0, return_abs=False, return_threads=False, weight=None):
     """I = sum_k f_k (f_k + 2 sum_{j>k} f_j sinc) (PAPER.md:88 'only j <= k'), OpenMP over rows.
     rows=(r0, r1) restricts the outer sum to a row slab (used for timing a bounded sample)."""
     xyz, typ, fftab, q = _prep(xyz, typ, fftab, q)
     M, N = q.shape[0], xyz.shape[0]
     r0, r1 = (0, N) if rows is None else rows
     I, A = np.zeros(M), np.zeros(M)
-    nthr = _L().oracle_debye_sym(_p(xyz, C.c_float), _p(typ, C.c_int32), N, _p(fftab, C.c_float), fftab.shape[0],
-                                 _p(q, C.c_float), M, r0, r1, threads, _p(I, C.c_double), _p(A, C.c_double))
+    w = _w(weight, N)
+    if w is None:
+        nthr = _L().oracle_debye_sym(_p(xyz, C.c_float), _p(typ, C.c_int32), N, _p(fftab, C.c_float), fftab.shape[0],
+                                     _p(q, C.c_float), M, r0, r1, threads, _p(I, C.c_double), _p(A, C.c_double))
+    else:
+        nthr = _L().oracle_debye_sym_w(_p(xyz, C.c_float), _p(typ, C.c_int32), _p(w, C.c_float), N,
+                                       _p(fftab, C.c_float), fftab.shape[0], _p(q, C.c_float), M, r0, r1, threads,
+                                       _p(I, C.c_double), _p(A, C.c_double))
     out = [I]
     if return_abs:
         out.append(A)
@@ -73,9 +99,9 @@ def debye_sym(xyz, typ, fftab, q, rows=None, threads=0, return_abs=False, return
     return out[0] if len(out) == 1 else tuple(out)
 
 
-def debye_batch(xyz_b, typ, fftab, q, threads=0):
-    """Eq. (2) for each conformer of xyz_b[B][N][3] (shared type / fftab / q)."""
-    return np.stack([debye_sym(x, typ, fftab, q, threads=threads) for x in xyz_b])
+def debye_batch(xyz_b, typ, fftab, q, threads=0, weight=None):
+    """Eq. (2) for each conformer of xyz_b[B][N][3] (shared type / fftab / q / weight)."""
+    return np.stack([debye_sym(x, typ, fftab, q, threads=threads, weight=weight) for x in xyz_b])
 
 
 def eq1_quadrature(x, f, qval, n=None):

@@ -172,3 +172,38 @@ def test_workloads_are_reproducible_and_shaped():
     w3 = wl.cfg3(n_bp=200)
     assert w3.N == 8000 and w3.T == 4 and w3.M == 200
     assert [int((w3.type == t).sum()) for t in range(4)] == [400, 2400, 3600, 1600]
+
+
+def test_weighted_oracle_pins():
+    """Per-atom weights (reading R10w: f_j(q) = w_j F[t_j](q)).  Pins that do not go through the
+    weighted code path: closed forms, and identities against the UNWEIGHTED oracle on transformed inputs."""
+    rng = np.random.default_rng(5)
+    q = wl.q_grid(0.9, 13)
+    f = wl.gaussian_form_factors(3, 3, q)
+    # (1) two atoms: I = w1^2 f1^2 + w2^2 f2^2 + 2 w1 w2 f1 f2 sin(qd)/(qd)
+    d = 3.25
+    xyz = np.array([[0, 0, 0], [0, d, 0]], np.float32)
+    typ = np.array([0, 2], np.int32)
+    w = np.array([1.5, -0.75], np.float32)                     # contrast may be negative
+    qq, F = q.astype(np.float64), f.astype(np.float64)
+    s = np.where(qq == 0, 1.0, np.sin(qq * d) / np.where(qq == 0, 1.0, qq * d))
+    want = (1.5 * F[0]) ** 2 + (0.75 * F[2]) ** 2 + 2 * 1.5 * (-0.75) * F[0] * F[2] * s
+    assert np.max(np.abs(orc.debye_sym(xyz, typ, f, q, weight=w) - want)) <= 1e-12 * np.max(np.abs(want))
+    assert np.max(np.abs(orc.debye_full(xyz, typ, f, q, weight=w) - want)) <= 1e-12 * np.max(np.abs(want))
+    # (2) weight 1 is the unweighted oracle, bit for bit; full == sym with weights
+    N = 40
+    xyz = (rng.uniform(-8, 8, (N, 3))).astype(np.float32)
+    typ = rng.integers(0, 3, N).astype(np.int32)
+    assert np.array_equal(orc.debye_sym(xyz, typ, f, q, weight=np.ones(N, np.float32)), orc.debye_sym(xyz, typ, f, q))
+    w = rng.uniform(0.25, 3.0, N).astype(np.float32)
+    assert rel(orc.debye_sym(xyz, typ, f, q, weight=w), orc.debye_full(xyz, typ, f, q, weight=w)) <= 1e-13
+    # (3) an atom of integer weight n is n coincident atoms of weight 1 (sinc(0) = 1 between the copies)
+    wi = rng.integers(1, 4, N)
+    dup = np.repeat(np.arange(N), wi)
+    assert rel(orc.debye_sym(xyz, typ, f, q, weight=wi.astype(np.float32)), orc.debye_sym(xyz[dup], typ[dup], f, q)) <= 1e-12
+    # (4) one weight per type is a rescaled form-factor table
+    c = np.array([0.5, 2.0, 1.25], np.float32)                  # exactly representable, products exact in fp32
+    assert rel(orc.debye_sym(xyz, typ, f, q, weight=c[typ]), orc.debye_sym(xyz, typ, (f * c[:, None]).astype(np.float32), q)) <= 1e-6
+    # (5) I(0) = (sum_j w_j f_j(0))^2
+    I = orc.debye_sym(xyz, typ, f, q, weight=w)
+    assert abs(I[0] - (w.astype(np.float64) * F[typ, 0]).sum() ** 2) <= 1e-12 * I[0]

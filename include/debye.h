@@ -86,6 +86,22 @@ int debye_profile_batch_host(const float *xyz, const int32_t *type, int32_t N, i
                              int32_t T, const float *q, int32_t M, double *I_out, uint32_t flags,
                              debye_stream_t stream);
 
+/* Per-atom weights (the paper's form factors are per atom because the excluded
+ * volume and the hydration layer depend on the atom's environment).  This is the one-parameter family
+ *     f_j(q_m) = weight[j] * fftab[type[j]][m],
+ * which keeps the per-type-pair accumulation: the inner loop gains one multiply per pair (1/r times w_j), the i atom's
+ * weight is applied when its accumulators are reduced, and the epilogue uses sum w and sum w^2 per type.
+ *   weight dev (host for the _host entry) [N] float32, any sign; shared by all conformers of a batch.
+ * One extra kernel launch (per-type weight sums).  Everything else as debye_profile / debye_profile_batch. */
+int debye_profile_weighted(const float *xyz, const int32_t *type, const float *weight, int32_t N, const float *fftab,
+                           int32_t T, const float *q, int32_t M, double *I_out, uint32_t flags, debye_stream_t stream);
+int debye_profile_batch_weighted(const float *xyz, const int32_t *type, const float *weight, int32_t N, int32_t B,
+                                 const float *fftab, int32_t T, const float *q, int32_t M, double *I_out,
+                                 uint32_t flags, debye_stream_t stream);
+int debye_profile_weighted_host(const float *xyz, const int32_t *type, const float *weight, int32_t N,
+                                const float *fftab, int32_t T, const float *q, int32_t M, double *I_out,
+                                uint32_t flags, debye_stream_t stream);
+
 /* Per-type-pair partial structure factors (by-product of the path; lets a caller re-fit form factors without
  * redoing the pair sum):  S_out[b][p][m] = sum over pairs i<j with {t_i,t_j} = {a,b'} of sinc(q_m r_ij), for
  * p = a*(2T-a+1)/2 + (b'-a), a <= b' (row-major upper triangle);  n_out[t] = number of atoms of type t.

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(HERE, "libdebye.so")
 FLAGS = {"fp64": 1 << 0, "mufu": 1 << 2, "recur": 1 << 3, "accurate": 1 << 4, "auto": 0}
 
 EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_profile_batch_host",
-           "debye_partials", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
+           "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
            "debye_launch_info", "debye_set_pairs_events", "debye_strerror", "debye_last_cuda_error", "debye_version")
 
 
@@ -45,8 +45,11 @@ def lib():
     L.debye_profile_batch.argtypes = [vp, vp, i32, i32, vp, i32, vp, i32, vp, u32, vp]
     L.debye_profile_batch_host.argtypes = L.debye_profile_batch.argtypes
     L.debye_partials.argtypes = [vp, vp, i32, i32, vp, i32, i32, vp, vp, u32, vp]
+    L.debye_profile_weighted.argtypes = [vp, vp, vp, i32, vp, i32, vp, i32, vp, u32, vp]
+    L.debye_profile_weighted_host.argtypes = L.debye_profile_weighted.argtypes
+    L.debye_profile_batch_weighted.argtypes = [vp, vp, vp, i32, i32, vp, i32, vp, i32, vp, u32, vp]
     for n in ("debye_profile", "debye_profile_host", "debye_profile_batch", "debye_profile_batch_host",
-              "debye_partials"):
+              "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials"):
         getattr(L, n).restype = C.c_int
     L.debye_workspace_bytes.argtypes = [i32, i32, i32, i32, u32]
     L.debye_workspace_bytes.restype = sz
@@ -114,6 +117,35 @@ def debye_profile_batch(xyz, type, fftab, q, I_out=None, variant="auto", stream=
     _check(lib().debye_profile_batch(_dev(xyz, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N, B,
                                      _dev(fftab, torch.float32, "fftab"), T, _dev(q, torch.float32, "q"), M,
                                      _dev(I_out, torch.float64, "I_out"), _flags(variant), _stream_ptr(stream)))
+    return I_out
+
+
+def debye_profile_weighted(xyz, type, weight, fftab, q, I_out=None, variant="auto", stream=None):
+    """As debye_profile with per-atom weights: f_j(q) = weight[j] * fftab[type[j]] (weight[N] f32 CUDA tensor).
+    xyz[N,3] gives I_out[M]; xyz[B,N,3] gives I_out[B,M] (weights shared by the conformers)."""
+    import torch
+    batch = xyz.dim() == 3
+    N, T, M = xyz.shape[-2], fftab.shape[0], q.shape[0]
+    if I_out is None:
+        I_out = torch.empty((xyz.shape[0], M) if batch else M, dtype=torch.float64, device=xyz.device)
+    a = (_dev(xyz, torch.float32, "xyz"), _dev(type, torch.int32, "type"), _dev(weight, torch.float32, "weight"), N)
+    b = (_dev(fftab, torch.float32, "fftab"), T, _dev(q, torch.float32, "q"), M, _dev(I_out, torch.float64, "I_out"),
+         _flags(variant), _stream_ptr(stream))
+    if batch:
+        _check(lib().debye_profile_batch_weighted(*a, xyz.shape[0], *b))
+    else:
+        _check(lib().debye_profile_weighted(*a, *b))
+    return I_out
+
+
+def debye_profile_weighted_host(xyz, type, weight, fftab, q, I_out=None, variant="auto", stream=None):
+    N, T, M = xyz.shape[0], fftab.shape[0], q.shape[0]
+    if I_out is None:
+        I_out = np.empty(M, dtype=np.float64)
+    _check(lib().debye_profile_weighted_host(_host(xyz, np.float32, "xyz"), _host(type, np.int32, "type"),
+                                             _host(weight, np.float32, "weight"), N, _host(fftab, np.float32, "fftab"), T,
+                                             _host(q, np.float32, "q"), M, _host(I_out, np.float64, "I_out"),
+                                             _flags(variant), _stream_ptr(stream)))
     return I_out
 
 

@@ -198,7 +198,7 @@ int ensure(void **ptr, size_t *have, size_t need)
 
 // mode 0: I_out[B][M]; mode 1: S_out[B][n_tp][M] (+ n_out)
 int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab, int T, const float *q, int M, double *out, int32_t *n_out,
-        uint32_t flags, cudaStream_t stream, int mode)
+        uint32_t flags, cudaStream_t stream, int mode, const float *weight = nullptr)
 {
     int st = validate(xyz, type, N, B, mode == 0 ? (const void *)fftab : (const void *)q, T, q, M, out, flags);
     if (st) return st;
@@ -221,13 +221,14 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     int alt_offered = 0;
     for (int i = 0; i < nch; ++i) if (ch[i].alt_gate == 1) alt_offered = 1;
     const bool pack_here = (int64_t)N * B <= DEBYE_PACK_IN_SETUP;      // small inputs: the setup CTA gathers too
-    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, xyz, sorted, pack_here ? 1 : 0);
+    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, xyz, sorted, pack_here ? 1 : 0, weight);
     if (!pack_here) {
         int64_t total = (int64_t)N * B;
         int blocks = (int)((total + 255) / 256);
         if (blocks > ds->sms * 16) blocks = ds->sms * 16;
-        debye::debye_pack_kernel<<<blocks, 256, 0, stream>>>(plan, xyz, type, perm, sorted, N, B);
+        debye::debye_pack_kernel<<<blocks, 256, 0, stream>>>(plan, xyz, type, perm, sorted, N, B, weight);
     }
+    if (weight) debye::debye_weight_sums_kernel<<<T, 32, 0, stream>>>(plan, sorted);
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
     for (int i = 0; i < nch; ++i) {
         debye_pairs_fn fn = debye_get_pairs_kernel(ch[i].variant, ch[i].K);
@@ -252,13 +253,13 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
 }
 
 int run_host(const float *xyz, const int32_t *type, int N, int B, const float *fftab, int T, const float *q, int M, double *out, uint32_t flags,
-             cudaStream_t stream)
+             cudaStream_t stream, const float *weight = nullptr)
 {
     int st = validate(xyz, type, N, B, fftab, T, q, M, out, flags);
     if (st) return st;
     DevState *ds;
     char *base;
-    size_t o_xyz, o_type, o_tab, o_q, o_out, total;
+    size_t o_xyz, o_type, o_tab, o_q, o_out, o_w, total;
     {
         std::lock_guard<std::mutex> lock(g_mu);
         if ((st = dev_state(&ds))) return st;
@@ -268,6 +269,7 @@ int run_host(const float *xyz, const int32_t *type, int N, int B, const float *f
         o_tab = o; o += align_up((size_t)T * M * 4);
         o_q = o; o += align_up((size_t)M * 4);
         o_out = o; o += align_up((size_t)B * M * 8);
+        o_w = o; o += align_up((size_t)N * 4);
         total = o;
         if ((st = ensure(&ds->stage, &ds->stage_bytes, total))) return st;
         base = (char *)ds->stage;
@@ -276,8 +278,9 @@ int run_host(const float *xyz, const int32_t *type, int N, int B, const float *f
     CU(cudaMemcpyAsync(base + o_type, type, (size_t)N * 4, cudaMemcpyHostToDevice, stream));
     CU(cudaMemcpyAsync(base + o_tab, fftab, (size_t)T * M * 4, cudaMemcpyHostToDevice, stream));
     CU(cudaMemcpyAsync(base + o_q, q, (size_t)M * 4, cudaMemcpyHostToDevice, stream));
+    if (weight) CU(cudaMemcpyAsync(base + o_w, weight, (size_t)N * 4, cudaMemcpyHostToDevice, stream));
     st = run((const float *)(base + o_xyz), (const int32_t *)(base + o_type), N, B, (const float *)(base + o_tab), T, (const float *)(base + o_q), M,
-             (double *)(base + o_out), nullptr, flags, stream, 0);
+             (double *)(base + o_out), nullptr, flags, stream, 0, weight ? (const float *)(base + o_w) : nullptr);
     if (st) return st;
     CU(cudaMemcpyAsync(out, base + o_out, (size_t)B * M * 8, cudaMemcpyDeviceToHost, stream));
     CU(cudaStreamSynchronize(stream));
@@ -310,6 +313,27 @@ int debye_profile_batch_host(const float *xyz, const int32_t *type, int32_t N, i
                              double *I_out, uint32_t flags, debye_stream_t stream)
 {
     return run_host(xyz, type, N, B, fftab, T, q, M, I_out, flags, (cudaStream_t)stream);
+}
+
+int debye_profile_weighted(const float *xyz, const int32_t *type, const float *weight, int32_t N, const float *fftab, int32_t T, const float *q, int32_t M,
+                           double *I_out, uint32_t flags, debye_stream_t stream)
+{
+    if (!weight) return DEBYE_EINVAL;
+    return run(xyz, type, N, 1, fftab, T, q, M, I_out, nullptr, flags, (cudaStream_t)stream, 0, weight);
+}
+
+int debye_profile_batch_weighted(const float *xyz, const int32_t *type, const float *weight, int32_t N, int32_t B, const float *fftab, int32_t T, const float *q,
+                                 int32_t M, double *I_out, uint32_t flags, debye_stream_t stream)
+{
+    if (!weight) return DEBYE_EINVAL;
+    return run(xyz, type, N, B, fftab, T, q, M, I_out, nullptr, flags, (cudaStream_t)stream, 0, weight);
+}
+
+int debye_profile_weighted_host(const float *xyz, const int32_t *type, const float *weight, int32_t N, const float *fftab, int32_t T, const float *q, int32_t M,
+                                double *I_out, uint32_t flags, debye_stream_t stream)
+{
+    if (!weight) return DEBYE_EINVAL;
+    return run_host(xyz, type, N, 1, fftab, T, q, M, I_out, flags, (cudaStream_t)stream, weight);
 }
 
 int debye_partials(const float *xyz, const int32_t *type, int32_t N, int32_t B, const float *q, int32_t T, int32_t M, double *S_out, int32_t *n_out,

@@ -20,7 +20,7 @@ namespace debye {
 // If pack_here != 0 the CTA also gathers the coordinates (small N x B: saves the pack launch).
 __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPlan *plan, const int32_t *__restrict__ type, const float *__restrict__ q,
                                                                             int32_t *__restrict__ perm, int N, int T, int M, int B, int alt_offered /* a recurrence launch sized for M - 1 indices exists */,
-                                                                            const float *__restrict__ xyz, float4 *__restrict__ sorted, int pack_here)
+                                                                            const float *__restrict__ xyz, float4 *__restrict__ sorted, int pack_here, const float *__restrict__ weight)
 {
     constexpr int NWARP = DEBYE_SETUP_THREADS / 32;
     constexpr int SORT_UNROLL = 8;
@@ -84,6 +84,7 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
         }
         plan->recur_alt = (koff == 0 && alt_offered) ? 1 : 0;
         plan->N = N; plan->T = T; plan->M = M; plan->B = B; plan->n_tp = T * (T + 1) / 2;
+        plan->weighted = weight ? 1 : 0;
         plan->uniform = uni;
         plan->zero_start = koff;
         plan->q0 = q0;
@@ -146,22 +147,35 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
             const int b = g / N, p = g - b * N;
             const int i = perm[p];
             const float *sx = xyz + ((int64_t)b * N + i) * 3;
-            sorted[g] = make_float4(sx[0], sx[1], sx[2], __int_as_float(type[i]));
+            sorted[g] = make_float4(sx[0], sx[1], sx[2], weight ? weight[i] : 1.0f);
         }
     }
 }
 
-// S0: gather coordinates into type-sorted float4 (x, y, z, bits(type)), all conformers.
+// S0: gather coordinates into type-sorted float4 (x, y, z, w_j), all conformers; w_j = 1 without weights (the kernels never
+// need the type of an atom: tiles are type-homogeneous).
 __global__ void debye_pack_kernel(const DevPlan *__restrict__ plan, const float *__restrict__ xyz, const int32_t *__restrict__ type, const int32_t *__restrict__ perm,
-                                  float4 *__restrict__ sorted, int N, int B)
+                                  float4 *__restrict__ sorted, int N, int B, const float *__restrict__ weight)
 {
     const int64_t total = (int64_t)N * B;
     for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (int64_t)gridDim.x * blockDim.x) {
         const int b = (int)(g / N), p = (int)(g % N);
         const int i = perm[p];
         const float *s = xyz + ((int64_t)b * N + i) * 3;
-        sorted[g] = make_float4(s[0], s[1], s[2], __int_as_float(type[i]));
+        sorted[g] = make_float4(s[0], s[1], s[2], weight ? weight[i] : 1.0f);
     }
+}
+
+// Weighted calls only: per type, sum of w_j and of w_j^2 in FP64 in a fixed order (one warp per type: lane-strided partial
+// sums over the type's segment of the sorted array, then an xor-shuffle tree).  Grid = T blocks of 32 threads.
+__global__ void debye_weight_sums_kernel(DevPlan *plan, const float4 *__restrict__ sorted)
+{
+    const int t = blockIdx.x, lane = threadIdx.x;
+    const int lo = plan->seg_off[t], hi = plan->seg_off[t + 1];
+    double s1 = 0.0, s2 = 0.0;
+    for (int i = lo + lane; i < hi; i += 32) { const double w = (double)sorted[i].w; s1 += w; s2 += w * w; }
+    for (int o = 16; o > 0; o >>= 1) { s1 += __shfl_xor_sync(0xffffffffu, s1, o); s2 += __shfl_xor_sync(0xffffffffu, s2, o); }
+    if (lane == 0) { plan->sw[t] = s1; plan->sw2[t] = s2; }
 }
 
 // number of unordered pairs of type pair (a, b)
@@ -218,7 +232,12 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
             double S;
             const int64_t units = plan->tp_prefix[tp + 1] - plan->tp_prefix[tp];
             if (bad) S = (sl == 0) ? nan : 0.0;
-            else if (qk == 0.0 || units == 0) S = (sl == 0) ? pair_count(plan->n_a[a], plan->n_a[b2], a == b2) : 0.0;
+            else if (qk == 0.0 || units == 0) {
+                // sum over the pairs of w_i w_j sinc(0): the pair count, or with weights sw_a sw_b resp. (sw_a^2 - sw2_a) / 2
+                double cnt = pair_count(plan->n_a[a], plan->n_a[b2], a == b2);
+                if (plan->weighted && units != 0) cnt = (a == b2) ? 0.5 * (plan->sw[a] * plan->sw[a] - plan->sw2[a]) : plan->sw[a] * plan->sw[b2];
+                S = (sl == 0) ? cnt : 0.0;
+            }
             else {
                 const int64_t ub = (int64_t)b * Uc + plan->tp_prefix[tp] * n_chunks + (int64_t)ch * units;
                 const int64_t ue = ub + units - 1;
@@ -249,7 +268,7 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
     __syncthreads();
     if (gs == 0 && k < M) {
         double tot = 0.0;
-        for (int a = 0; a < T; ++a) { const double fa = (double)fftab[a * M + k]; tot += (double)plan->n_a[a] * fa * fa; }
+        for (int a = 0; a < T; ++a) { const double fa = (double)fftab[a * M + k]; tot += (plan->weighted ? plan->sw2[a] : (double)plan->n_a[a]) * fa * fa; }
 #pragma unroll
         for (int x = 0; x < DEBYE_FINAL_G * DEBYE_FINAL_NS; ++x) tot += part[x][kk];
         out[(int64_t)b * M + k] = tot;

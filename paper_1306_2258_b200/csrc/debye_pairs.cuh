@@ -243,7 +243,9 @@ __device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, con
     const float r2c = fmaxf(r2, 1e-30f);
     const float rinv = rsqrt_mufu(r2c);
     g.r = r2c * rinv;
-    g.rinv = (ok && !small) ? rinv : 0.0f;      // zero for masked / slow-path pairs: every start value becomes exactly 0
+    // zero for masked / slow-path pairs: every start value becomes exactly 0.  pj.w is the j atom's weight (1 without
+    // weights); the i atom's weight is applied when the accumulators are flushed
+    g.rinv = (ok && !small) ? rinv * pj.w : 0.0f;
     g.slow = small && ok;
     reduce_turns_pair(g.r, rc.w1, rc.w1_lo, rc.smult, g.f1, g.fS);     // f1 is dead code in the general-start mode
 }
@@ -509,6 +511,8 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
     int mode = RM_G, ch_cur = 0;
     (void)mode; (void)dq_d; (void)q0_d; (void)koff; (void)cut2;
 
+    float wi = 1.0f;                  // weight of this thread's i atom (weighted calls: accumulators are flushed per row)
+    const bool weighted = plan->weighted != 0;
     auto flush = [&]() {
         // FP32 -> FP64, fixed order.  Each warp transposes 32 slots x 32 lanes through tbuf; lane l sums slot
         // 32 s + l over the 32 lanes in lane order; then threads k < K add the 4 warp sums in warp order.
@@ -521,8 +525,8 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                     if (l < K) {
                         float lo, hi;
                         upk2(acc.v[l / 2], lo, hi);
-                        tbuf[warp][t][lane] = lo;
-                        tbuf[warp][t + 1][lane] = hi;
+                        tbuf[warp][t][lane] = lo * wi;
+                        tbuf[warp][t + 1][lane] = hi * wi;
                         acc.v[l / 2] = 0;
                     }
                 }
@@ -538,7 +542,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
         } else {
 #pragma unroll
             for (int l = 0; l < K; ++l) {
-                double v = acc.v[l];
+                double v = acc.v[l] * (double)wi;
                 acc.v[l] = 0;
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);   // xor tree: same order every run
@@ -584,7 +588,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
         const int64_t X = ((int64_t)b * n_tp + tp) * n_chunks + ch;
 
         if (X != curX) {
-            if (curX >= 0) { flush(); pending = 0; write_record(curX); }
+            if (curX >= 0) { if (pending) flush(); pending = 0; write_record(curX); }
             curX = X;
             if (ch != ch_cur || u == u0) {
                 ch_cur = ch;
@@ -626,6 +630,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
         const bool ivalid = i_local < n_i;
         const float4 *conf = sorted + (int64_t)b * N;
         float4 pi = conf[plan->seg_off[ti] + (ivalid ? i_local : 0)];
+        wi = pi.w;
         const int j_first = diag ? (row * DEBYE_IB + 1 + (int)jo) : (int)jo;   // index within the j type segment
         const float4 *src = conf + plan->seg_off[tj] + j_first;
         const int ntile = (len + DEBYE_JT - 1) / DEBYE_JT;
@@ -667,7 +672,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                         for (int l = 0; l < K; ++l) {
                             double qk = (double)qs[l];
                             double x = qk * r;
-                            acc.v[l] += (x == 0.0) ? qk : sin(x) / r;
+                            acc.v[l] += (double)pj.w * ((x == 0.0) ? qk : sin(x) / r);
                         }
                     }
                 } else {
@@ -677,7 +682,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                     const float r2c = fmaxf(r2, 1e-30f);
                     float rinv = rsqrt_mufu(r2c);
                     const float r = r2c * rinv;
-                    rinv = (ok && !small) ? rinv : 0.0f;
+                    rinv = (ok && !small) ? rinv * pj.w : 0.0f;
                     if (__any_sync(0xffffffffu, small && ok)) {
                         if (small && ok) {
                             const float rs = sqrtf(r2);
@@ -686,7 +691,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                                 const float qk = qs[l];
                                 float lo_, hi_;
                                 upk2(acc.v[l / 2], lo_, hi_);
-                                float tv = (rs == 0.0f) ? qk : term_accurate(qk, rs);
+                                float tv = pj.w * ((rs == 0.0f) ? qk : term_accurate(qk, rs));
                                 if (l & 1) hi_ += tv; else lo_ += tv;
                                 acc.v[l / 2] = pk2(lo_, hi_);
                             }
@@ -712,10 +717,11 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
             __syncthreads();
         }
         pending += len;
-        if (pending >= DEBYE_FLUSH_J) { flush(); pending = 0; }
+        // weighted calls: the i atom (and with it wi) changes with every row segment, so flush before it does
+        if (weighted || pending >= DEBYE_FLUSH_J) { flush(); pending = 0; }
         u += len;
     }
-    if (curX >= 0) { flush(); write_record(curX); }
+    if (curX >= 0) { if (pending) flush(); write_record(curX); }
 #ifdef DEBYE_TRACE
     if (tid == 0) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); debye_trace[3 * c + 1] = t; }
 #endif

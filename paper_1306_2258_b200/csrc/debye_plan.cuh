@@ -25,7 +25,10 @@ struct DevPlan {
     int32_t variant_auto;         // variant chosen on the device when the caller gave no DEBYE_SINC_* flag
     double q0, dq;                // least-squares-free fit: q0 = q[0], dq = (q[M-1]-q[0])/(M-1)
     float q_small;                // smallest non-zero |q|
+    int32_t weighted;             // per-atom weights given (debye_profile_weighted): sorted[].w holds w_j, else 1
     int64_t U1;                   // units per conformer and per q-chunk
+    double sw[DEBYE_MAX_TYPES_I];             // weighted calls: sum of w_j over the atoms of each type ...
+    double sw2[DEBYE_MAX_TYPES_I];            // ... and of w_j^2 (self terms; q = 0 pair sums)
     int32_t seg_off[DEBYE_MAX_TYPES_I + 1];   // sorted-array offset of each type segment
     int32_t n_a[DEBYE_MAX_TYPES_I];           // atoms per type
     int32_t tp_ti[DEBYE_MAX_TP];              // type on the i (row) side

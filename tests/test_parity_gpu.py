@@ -242,3 +242,38 @@ def test_caller_workspace(db):
     finally:
         assert L.debye_set_workspace(None, 0) == 0
     assert gpu_profile(db, w).tobytes() == ref.tobytes()
+
+
+def test_weighted_profiles_match_the_weighted_oracle(db):
+    """Per-atom weights f_j = w_j F[t_j] (reading R10w; include/debye.h debye_profile_weighted): every variant against the
+    oracle, weights of both signs, the batch entry, the host entry, and weight 1 == the unweighted call."""
+    import torch
+    rng = np.random.default_rng(11)
+    for name, w0, M in (("one_chunk", wl.small_random(30, 900, 4, 64), 64), ("two_chunks", wl.small_random(31, 700, 3, 150, q_max=0.9), 150)):
+        wt = rng.uniform(0.3, 2.5, w0.N).astype(np.float32)
+        ref, A = orc.debye_sym(w0.xyz, w0.type, w0.fftab, w0.q, weight=wt, return_abs=True)
+        x, t, f, q = to_dev(w0)
+        wd = torch.from_numpy(wt).cuda()
+        for v in FP32_VARIANTS:
+            I = db.debye_profile_weighted(x, t, wd, f, q, variant=v).cpu().numpy()
+            assert rel(I, ref) <= TOL32, (name, v, rel(I, ref))
+        assert rel(db.debye_profile_weighted(x, t, wd, f, q, variant="fp64").cpu().numpy(), ref) <= TOL64
+        ones = torch.ones(w0.N, dtype=torch.float32, device="cuda")
+        # weight 1 is the unweighted profile up to summation order (weighted calls reduce their accumulators once per row)
+        assert rel(db.debye_profile_weighted(x, t, ones, f, q).cpu().numpy(), db.debye_profile(x, t, f, q).cpu().numpy()) <= 1e-6
+        h = db.debye_profile_weighted_host(w0.xyz, w0.type, wt, w0.fftab, w0.q)
+        assert h.tobytes() == db.debye_profile_weighted(x, t, wd, f, q).cpu().numpy().tobytes()
+    # signed weights (negative contrast): compare against the documented floor 1e-2 * sum|terms|
+    w1 = wl.small_random(32, 600, 3, 48)
+    ws = (rng.uniform(0.5, 2.0, w1.N) * np.where(rng.uniform(size=w1.N) < 0.3, -1, 1)).astype(np.float32)
+    ref, A = orc.debye_sym(w1.xyz, w1.type, w1.fftab, w1.q, weight=ws, return_abs=True)
+    x, t, f, q = to_dev(w1)
+    I = db.debye_profile_weighted(x, t, torch.from_numpy(ws).cuda(), f, q).cpu().numpy()
+    assert float(np.max(np.abs(I - ref) / np.maximum(np.abs(ref), 1e-2 * A))) <= TOL32
+    # batch with shared weights
+    wb = wl.cfg4(B=5, N=500)
+    wt = rng.uniform(0.5, 1.5, wb.N).astype(np.float32)
+    refb = orc.debye_batch(wb.xyz, wb.type, wb.fftab, wb.q, weight=wt)
+    xb, t, f, q = to_dev(wb)
+    Ib = db.debye_profile_weighted(xb, t, torch.from_numpy(wt).cuda(), f, q).cpu().numpy()
+    assert Ib.shape == (5, wb.M) and rel(Ib, refb) <= TOL32

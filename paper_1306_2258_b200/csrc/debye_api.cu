@@ -149,11 +149,11 @@ int dev_state(DevState **st)
 // the tail alone (measured); a few waves (up to 16 when there is enough work) let the hardware block scheduler refill the SM.  More waves
 // cost one prologue + one FP64 flush per CTA, so the count is bounded by the work available (estimated from N alone:
 // the host never sees the type histogram).
-int grid_for(DevState *s, const Choice &c, int N, int B, int *G)
+int grid_for(DevState *s, const Choice &c, int N, int B, int *G, bool weighted = false)
 {
     int &o = s->occ[c.variant][c.K / 4];
     if (o == 0) {
-        debye_pairs_fn fn = debye_get_pairs_kernel(c.variant, c.K);
+        debye_pairs_fn fn = debye_get_pairs_kernel(c.variant, c.K, false);      // the weighted twin has the same launch bounds
         if (!fn) return DEBYE_EUNSUPPORTED;
         int nb = 0;
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, DEBYE_IB, 0));
@@ -231,7 +231,7 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     if (weight) debye::debye_weight_sums_kernel<<<T, 32, 0, stream>>>(plan, sorted);
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
     for (int i = 0; i < nch; ++i) {
-        debye_pairs_fn fn = debye_get_pairs_kernel(ch[i].variant, ch[i].K);
+        debye_pairs_fn fn = debye_get_pairs_kernel(ch[i].variant, ch[i].K, weight != nullptr);
         // slow-path threshold on theta = r * (smallest grid step or smallest |q|): see DESIGN.md section 6
         const float theta_min = (ch[i].variant == V_RECUR) ? 0.002f : 0.004f;
         fn<<<G[i], DEBYE_IB, 0, stream>>>(plan, sorted, q, records, ch[i].n_chunks, is_auto, theta_min, ch[i].alt_gate);

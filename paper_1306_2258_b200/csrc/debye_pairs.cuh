@@ -234,7 +234,7 @@ enum RecurMode : int { RM_Z1 = 0, RM_Z2A = 1, RM_Z2B = 2, RM_G = 3 };
 // packed loop (three-stage software pipeline).
 // Stage A (geometry): distance, 1/r, slow-path flag and the two reduced angles (turns, in [-1/2, 1/2]).
 struct RecurGeom { float r, rinv, f1, fS; bool slow; };
-template <int MODE>
+template <int MODE, bool W>
 __device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, const bool ok, const RecurConst &rc, RecurGeom &g)
 {
     const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
@@ -243,9 +243,10 @@ __device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, con
     const float r2c = fmaxf(r2, 1e-30f);
     const float rinv = rsqrt_mufu(r2c);
     g.r = r2c * rinv;
-    // zero for masked / slow-path pairs: every start value becomes exactly 0.  pj.w is the j atom's weight (1 without
-    // weights); the i atom's weight is applied when the accumulators are flushed
-    g.rinv = (ok && !small) ? rinv * pj.w : 0.0f;
+    // zero for masked / slow-path pairs: every start value becomes exactly 0.  Weighted instantiations (W): pj.w is the j
+    // atom's weight; the i atom's weight is applied when the accumulators are flushed
+    if constexpr (W) g.rinv = (ok && !small) ? rinv * pj.w : 0.0f;
+    else g.rinv = (ok && !small) ? rinv : 0.0f;
     g.slow = small && ok;
     reduce_turns_pair(g.r, rc.w1, rc.w1_lo, rc.smult, g.f1, g.fS);     // f1 is dead code in the general-start mode
 }
@@ -339,13 +340,13 @@ __device__ __forceinline__ void recur_hot(u64 (&acc)[K / 2], u64 (&A)[4], u64 (&
 // accuracy:   d_{m+1} = d_m - beta s_m,   s_{m+1} = s_m + d_{m+1},   s_0 = v(k'_j),  d_0 = v(k'_j) - v(k'_j - S).
 // Start values are those of the fast path evaluated with the true 1/r (for r = 0 the clamp r^2 >= 1e-30 makes
 // 2 sin(n theta)/r come out as its limit 2 n dq).  Three packed lane-operations per term; rare, so cost is irrelevant.
-template <int K, int MODE>
+template <int K, int MODE, bool W>
 __device__ __forceinline__ void recur_slow_pair(u64 (&acc)[K / 2], const float4 pj, const float4 pi, const RecurConst &rc, const float *wtab)
 {
     RecurConst rs = rc;
     rs.cut2 = -1.0f;                       // never "small": stage A keeps the true 1/r
     RecurGeom g;
-    recur_geom<MODE>(pj, pi, true, rs, g);
+    recur_geom<MODE, W>(pj, pi, true, rs, g);
     u64 A[4], Bv[4];
     float cS;
     recur_vals<MODE>(g, rc, wtab, A, Bv, cS);
@@ -394,7 +395,7 @@ __host__ __device__ constexpr int recur_np(int K) { return K <= DEBYE_K3 ? 1 : 2
 // instructions) under the independent packed instructions.  NP > 1 gives that much more instruction-level
 // parallelism per warp at 17 registers per extra pair -- the K accumulators, which are what limits the number of
 // resident warps, are shared by all NP pairs.
-template <int K, int MODE>
+template <int K, int MODE, bool W>
 __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__restrict__ tile, const int jj0, const int cnt, const float4 pi,
                                            const bool ivalid, const bool diag, const int i_local, const int jl0, const RecurConst &rc,
                                            const float *wtab)
@@ -406,7 +407,7 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
         for (int p = 0; p < NP; ++p) {
             const int j = min(jbase + p, cnt - 1);
             const bool ok = ivalid && (jbase + p < cnt) && (!diag || (jl0 + j > i_local));
-            recur_geom<MODE>(tile[j], pi, ok, rc, g[p]);
+            recur_geom<MODE, W>(tile[j], pi, ok, rc, g[p]);
         }
     };
     u64 A[NP][4], Bv[NP][4];
@@ -423,7 +424,7 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
         if (slow_any) {
 #pragma unroll
             for (int p = 0; p < NP; ++p)
-                if (slow[p]) recur_slow_pair<K, MODE>(acc, tile[jj + p], pi, rc, wtab);
+                if (slow[p]) recur_slow_pair<K, MODE, W>(acc, tile[jj + p], pi, rc, wtab);
         }
         // stage B of group jj + NP, stage A of group jj + 2 NP, packed loops of group jj: one basic block
         u64 An[NP][4], Bn[NP][4];
@@ -452,7 +453,7 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
 #ifdef DEBYE_TRACE
 __device__ unsigned long long debye_trace[3 * 4096];
 #endif
-template <int K, int VAR>
+template <int K, int VAR, bool W>
 __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR ? recur_min_ctas(K) : (K <= 64 ? 4 : (K <= 112 ? 3 : 2)))) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
                                                                double *__restrict__ records, int n_chunks, int is_auto, float theta_min, int alt_gate)
 {
@@ -511,8 +512,8 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
     int mode = RM_G, ch_cur = 0;
     (void)mode; (void)dq_d; (void)q0_d; (void)koff; (void)cut2;
 
-    float wi = 1.0f;                  // weight of this thread's i atom (weighted calls: accumulators are flushed per row)
-    const bool weighted = plan->weighted != 0;
+    float wi = 1.0f;                  // weighted instantiations: weight of this thread's i atom (accumulators are flushed per row)
+    (void)wi;
     auto flush = [&]() {
         // FP32 -> FP64, fixed order.  Each warp transposes 32 slots x 32 lanes through tbuf; lane l sums slot
         // 32 s + l over the 32 lanes in lane order; then threads k < K add the 4 warp sums in warp order.
@@ -525,8 +526,9 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                     if (l < K) {
                         float lo, hi;
                         upk2(acc.v[l / 2], lo, hi);
-                        tbuf[warp][t][lane] = lo * wi;
-                        tbuf[warp][t + 1][lane] = hi * wi;
+                        if constexpr (W) { lo *= wi; hi *= wi; }
+                        tbuf[warp][t][lane] = lo;
+                        tbuf[warp][t + 1][lane] = hi;
                         acc.v[l / 2] = 0;
                     }
                 }
@@ -542,7 +544,8 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
         } else {
 #pragma unroll
             for (int l = 0; l < K; ++l) {
-                double v = acc.v[l] * (double)wi;
+                double v = acc.v[l];
+                if constexpr (W) v *= (double)wi;
                 acc.v[l] = 0;
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);   // xor tree: same order every run
@@ -630,7 +633,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
         const bool ivalid = i_local < n_i;
         const float4 *conf = sorted + (int64_t)b * N;
         float4 pi = conf[plan->seg_off[ti] + (ivalid ? i_local : 0)];
-        wi = pi.w;
+        if constexpr (W) wi = pi.w;
         const int j_first = diag ? (row * DEBYE_IB + 1 + (int)jo) : (int)jo;   // index within the j type segment
         const float4 *src = conf + plan->seg_off[tj] + j_first;
         const int ntile = (len + DEBYE_JT - 1) / DEBYE_JT;
@@ -655,10 +658,10 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
             if (diag) { int first_i = row * DEBYE_IB + warp * 32; jj0 = max(0, first_i + 1 - jl0); }
             if constexpr (VAR == V_RECUR) {
                 switch (mode) {      // warp-uniform; one copy of the pipelined loop per start mode
-                    case RM_Z1: recur_tile<K, RM_Z1>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
-                    case RM_Z2A: recur_tile<K, RM_Z2A>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
-                    case RM_Z2B: recur_tile<K, RM_Z2B>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
-                    default: recur_tile<K, RM_G>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
+                    case RM_Z1: recur_tile<K, RM_Z1, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
+                    case RM_Z2A: recur_tile<K, RM_Z2A, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
+                    case RM_Z2B: recur_tile<K, RM_Z2B, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
+                    default: recur_tile<K, RM_G, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
                 }
             } else {
             for (int jj = jj0; jj < cnt; ++jj) {
@@ -672,7 +675,8 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                         for (int l = 0; l < K; ++l) {
                             double qk = (double)qs[l];
                             double x = qk * r;
-                            acc.v[l] += (double)pj.w * ((x == 0.0) ? qk : sin(x) / r);
+                            const double tv = (x == 0.0) ? qk : sin(x) / r;
+                            acc.v[l] += W ? (double)pj.w * tv : tv;
                         }
                     }
                 } else {
@@ -682,7 +686,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                     const float r2c = fmaxf(r2, 1e-30f);
                     float rinv = rsqrt_mufu(r2c);
                     const float r = r2c * rinv;
-                    rinv = (ok && !small) ? rinv * pj.w : 0.0f;
+                    rinv = (ok && !small) ? (W ? rinv * pj.w : rinv) : 0.0f;
                     if (__any_sync(0xffffffffu, small && ok)) {
                         if (small && ok) {
                             const float rs = sqrtf(r2);
@@ -691,7 +695,8 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                                 const float qk = qs[l];
                                 float lo_, hi_;
                                 upk2(acc.v[l / 2], lo_, hi_);
-                                float tv = pj.w * ((rs == 0.0f) ? qk : term_accurate(qk, rs));
+                                float tv = (rs == 0.0f) ? qk : term_accurate(qk, rs);
+                                if constexpr (W) tv *= pj.w;
                                 if (l & 1) hi_ += tv; else lo_ += tv;
                                 acc.v[l / 2] = pk2(lo_, hi_);
                             }
@@ -718,7 +723,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
         }
         pending += len;
         // weighted calls: the i atom (and with it wi) changes with every row segment, so flush before it does
-        if (weighted || pending >= DEBYE_FLUSH_J) { flush(); pending = 0; }
+        if (W || pending >= DEBYE_FLUSH_J) { flush(); pending = 0; }
         u += len;
     }
     if (curX >= 0) { if (pending) flush(); write_record(curX); }

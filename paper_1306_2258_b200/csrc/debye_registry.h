@@ -9,8 +9,4 @@ typedef void (*debye_pairs_fn)(const DevPlan *, const float4 *, const float *, d
 #define DEBYE_KMAX_F64 32
 
 // K must be a multiple of 8 in [8, KMAX] (recurrence: a multiple of 4); returns nullptr otherwise
-debye_pairs_fn debye_get_pairs_kernel(int variant, int K);
-debye_pairs_fn debye_get_recur(int K);
-debye_pairs_fn debye_get_mufu(int K);
-debye_pairs_fn debye_get_accurate(int K);
-debye_pairs_fn debye_get_f64(int K);
+debye_pairs_fn debye_get_pairs_kernel(int variant, int K, bool weighted);

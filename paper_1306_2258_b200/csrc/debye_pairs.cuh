@@ -96,6 +96,9 @@ __device__ __forceinline__ void reduce_turns_pair(float r, float w, float w_lo, 
 // so the quantity that is squared is always the SMALL one: the phase error that a relative error rho of s causes in
 // 2cos(2 pi f) is 2 rho tan(pi g') <= 2 rho, whereas without the fold it is 2 rho tan(pi f), unbounded towards f = 1/2;
 // and on the half interval one fewer cosine coefficient is needed for a 500 times smaller approximation error.
+// Measured (cfg5, dense q): unfolded polynomials on |f| <= 1/2 save 7 instructions per pair but give 1.6e-5 with a
+// degree-9 sine and 2e-4 with a BETTER degree-11 sine -- the rounding of s next to 2 is what the tangent amplifies, not the
+// approximation error -- against 6.5e-6 folded.
 //   s = g' (2 pi + y (s1 + y (s2 + y (s3 + y s4)))),  c = 2 + y (d1 + y (d2 + y (d3 + y d4))),  y = g'^2.
 // Near-minimax coefficients (iteratively reweighted least squares on 25 000 Chebyshev-spaced points of [0, 1/4] in fp64,
 // fitting 2 sin(pi g) - 2 pi g on g^3..g^9 and 2 cos(pi g) - 2 on y..y^4): maximum relative error 9.3e-12 (s), maximum
@@ -238,9 +241,10 @@ template <int MODE, bool W>
 __device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, const bool ok, const RecurConst &rc, RecurGeom &g)
 {
     const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
-    const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-    const bool small = !(r2 > rc.cut2);
-    const float r2c = fmaxf(r2, 1e-30f);
+    // + 1e-30 keeps rsqrt finite for coincident atoms (they take the slow path, which gets the limit right) and changes no
+    // other distance; folding it into the FMA chain saves the clamp
+    const float r2c = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, 1e-30f)));
+    const bool small = !(r2c > rc.cut2);
     const float rinv = rsqrt_mufu(r2c);
     g.r = r2c * rinv;
     // zero for masked / slow-path pairs: every start value becomes exactly 0.  Weighted instantiations (W): pj.w is the j
@@ -402,12 +406,13 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
 {
     constexpr int NP = recur_np(K);
     if (jj0 >= cnt) return;
+    // first tile index this thread may pair with: masks i >= j on the diagonal and threads without an i atom
+    const int jmin = ivalid ? (diag ? max(0, i_local + 1 - jl0) : 0) : 0x7fffffff;
     auto geom = [&](const int jbase, RecurGeom (&g)[NP]) {
 #pragma unroll
         for (int p = 0; p < NP; ++p) {
-            const int j = min(jbase + p, cnt - 1);
-            const bool ok = ivalid && (jbase + p < cnt) && (!diag || (jl0 + j > i_local));
-            recur_geom<MODE, W>(tile[j], pi, ok, rc, g[p]);
+            const int j = jbase + p;
+            recur_geom<MODE, W>(tile[min(j, cnt - 1)], pi, j >= jmin && j < cnt, rc, g[p]);
         }
     };
     u64 A[NP][4], Bv[NP][4];

@@ -45,6 +45,19 @@ bool g_atexit = false;
 
 size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
+// launch with programmatic stream serialisation (PDL, debye_plan.cuh): the kernel must start with pdl_wait()
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t stream, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = 0; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 struct Choice { int variant; int K; int n_chunks; int alt_gate; };   // alt_gate: -1 always runs, 0 / 1 see debye_pairs_kernel
 
 // q-chunking of each variant: how many accumulators a thread keeps (K) and how many passes over the pairs.
@@ -226,15 +239,15 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
         int64_t total = (int64_t)N * B;
         int blocks = (int)((total + 255) / 256);
         if (blocks > ds->sms * 16) blocks = ds->sms * 16;
-        debye::debye_pack_kernel<<<blocks, 256, 0, stream>>>(plan, xyz, type, perm, sorted, N, B, weight);
+        CU(launch_pdl(debye::debye_pack_kernel, dim3(blocks), dim3(256), stream, (const DevPlan *)plan, xyz, type, (const int32_t *)perm, sorted, N, B, weight));
     }
-    if (weight) debye::debye_weight_sums_kernel<<<T, 32, 0, stream>>>(plan, sorted);
+    if (weight) CU(launch_pdl(debye::debye_weight_sums_kernel, dim3(T), dim3(32), stream, plan, (const float4 *)sorted));
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
     for (int i = 0; i < nch; ++i) {
         debye_pairs_fn fn = debye_get_pairs_kernel(ch[i].variant, ch[i].K, weight != nullptr);
         // slow-path threshold on theta = r * (smallest grid step or smallest |q|): see DESIGN.md section 6
         const float theta_min = (ch[i].variant == V_RECUR) ? 0.002f : 0.004f;
-        fn<<<G[i], DEBYE_IB, 0, stream>>>(plan, sorted, q, records, ch[i].n_chunks, is_auto, theta_min, ch[i].alt_gate);
+        CU(launch_pdl(fn, dim3(G[i]), dim3(DEBYE_IB), stream, (const DevPlan *)plan, (const float4 *)sorted, q, records, ch[i].n_chunks, is_auto, theta_min, ch[i].alt_gate));
     }
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
     {
@@ -245,7 +258,7 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
             const int j = i < nch ? i : 0;
             sets.s[i].variant = ch[j].variant; sets.s[i].K = ch[j].K; sets.s[i].n_chunks = ch[j].n_chunks; sets.s[i].G = G[j]; sets.s[i].alt_gate = ch[j].alt_gate;
         }
-        debye::debye_final_kernel<<<blocks, threads, 0, stream>>>(plan, records, fftab, q, out, is_auto, sets, mode);
+        CU(launch_pdl(debye::debye_final_kernel, dim3(blocks), dim3(threads), stream, (const DevPlan *)plan, (const double *)records, fftab, q, out, is_auto, sets, mode));
     }
     if (mode == 1 && n_out) CU(cudaMemcpyAsync(n_out, plan->n_a, sizeof(int32_t) * T, cudaMemcpyDeviceToDevice, stream));
     CU(cudaGetLastError());

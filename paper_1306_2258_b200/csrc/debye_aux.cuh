@@ -22,6 +22,7 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
                                                                             int32_t *__restrict__ perm, int N, int T, int M, int B, int alt_offered /* a recurrence launch sized for M - 1 indices exists */,
                                                                             const float *__restrict__ xyz, float4 *__restrict__ sorted, int pack_here, const float *__restrict__ weight)
 {
+    pdl_trigger();                         // first kernel of the call: lets the next grid be staged (it waits for our completion)
     constexpr int NWARP = DEBYE_SETUP_THREADS / 32;
     constexpr int SORT_UNROLL = 8;
     __shared__ int wcnt[NWARP][DEBYE_MAX_TYPES_I];      // pass 1: atoms of type t in warp w's chunk; pass 2: running output slot
@@ -157,6 +158,8 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
 __global__ void debye_pack_kernel(const DevPlan *__restrict__ plan, const float *__restrict__ xyz, const int32_t *__restrict__ type, const int32_t *__restrict__ perm,
                                   float4 *__restrict__ sorted, int N, int B, const float *__restrict__ weight)
 {
+    pdl_wait();
+    pdl_trigger();
     const int64_t total = (int64_t)N * B;
     for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (int64_t)gridDim.x * blockDim.x) {
         const int b = (int)(g / N), p = (int)(g % N);
@@ -170,6 +173,7 @@ __global__ void debye_pack_kernel(const DevPlan *__restrict__ plan, const float 
 // sums over the type's segment of the sorted array, then an xor-shuffle tree).  Grid = T blocks of 32 threads.
 __global__ void debye_weight_sums_kernel(DevPlan *plan, const float4 *__restrict__ sorted)
 {
+    pdl_wait();
     const int t = blockIdx.x, lane = threadIdx.x;
     const int lo = plan->seg_off[t], hi = plan->seg_off[t + 1];
     double s1 = 0.0, s2 = 0.0;
@@ -198,6 +202,7 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
                                                                             int is_auto, const FinalSets sets, int mode)
 {
     __shared__ double part[DEBYE_FINAL_G * DEBYE_FINAL_NS][DEBYE_FINAL_Q];
+    pdl_wait();
     const int M = plan->M, Bn = plan->B, T = plan->T, n_tp = plan->n_tp;
     const int ktiles = (M + DEBYE_FINAL_Q - 1) / DEBYE_FINAL_Q;
     const int kk = threadIdx.x % DEBYE_FINAL_Q, gs = threadIdx.x / DEBYE_FINAL_Q;

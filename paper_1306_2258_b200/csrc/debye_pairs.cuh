@@ -462,6 +462,7 @@ template <int K, int VAR, bool W>
 __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR ? recur_min_ctas(K) : (K <= 64 ? 4 : (K <= 112 ? 3 : 2)))) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
                                                                double *__restrict__ records, int n_chunks, int is_auto, float theta_min, int alt_gate)
 {
+    pdl_wait();      // programmatic dependent launch: everything before us in the call has completed (debye_plan.cuh)
     // ---- variant gate (decided on the device so the host never reads q) ---------------------------------------
     if (is_auto) {
         if (plan->variant_auto != VAR) return;

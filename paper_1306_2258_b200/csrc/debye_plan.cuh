@@ -36,6 +36,18 @@ struct DevPlan {
     int64_t tp_prefix[DEBYE_MAX_TP + 1];      // units before type pair tp (one chunk, one conformer)
 };
 
+// ---- programmatic dependent launch (PDL) ------------------------------------------------------------------------
+// Every kernel after the setup kernel is launched with cudaLaunchAttributeProgrammaticStreamSerialization and starts with
+// pdl_wait(): its CTAs may be scheduled while the previous kernel of the call is still running and block here until that
+// kernel has completed and its writes are visible.  Because EVERY kernel waits before it does anything (the instantiations
+// that exit at once included), completion is transitive along the chain.  The setup and pack kernels call pdl_trigger() at
+// their start so the next grid is staged early; the pairs kernels do not (a staged grid would hold registers that their own
+// later waves need).
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#endif
+
 // ---- unit decoding helpers (used identically by the pairs kernel and the final kernel) -------------------
 __host__ __device__ inline int64_t debye_range_begin(int64_t U, int32_t c, int32_t G)
 {

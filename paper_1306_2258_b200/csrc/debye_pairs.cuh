@@ -408,36 +408,30 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
     if (jj0 >= cnt) return;
     // first tile index this thread may pair with: masks i >= j on the diagonal and threads without an i atom
     const int jmin = ivalid ? (diag ? max(0, i_local + 1 - jl0) : 0) : 0x7fffffff;
+    bool had_slow = false;                // some pair of this thread in this tile needs the slow path (handled after the loop)
+    // the tile buffers carry DEBYE_TILE_PAD finite entries behind the last atom, so the two groups that the pipeline reads
+    // ahead never need an index clamp; such pairs are masked (1/r = 0)
     auto geom = [&](const int jbase, RecurGeom (&g)[NP]) {
 #pragma unroll
         for (int p = 0; p < NP; ++p) {
             const int j = jbase + p;
-            recur_geom<MODE, W>(tile[min(j, cnt - 1)], pi, j >= jmin && j < cnt, rc, g[p]);
+            recur_geom<MODE, W>(tile[j], pi, j >= jmin && j < cnt, rc, g[p]);
+            had_slow = had_slow || g[p].slow;
         }
     };
     u64 A[NP][4], Bv[NP][4];
     float cS[NP];
-    bool slow[NP];
     RecurGeom gn[NP];
     geom(jj0, gn);
-    bool slow_w = false;
 #pragma unroll
-    for (int p = 0; p < NP; ++p) { recur_vals<MODE>(gn[p], rc, wtab, A[p], Bv[p], cS[p]); slow[p] = gn[p].slow; slow_w = slow_w || slow[p]; }
-    bool slow_any = __any_sync(0xffffffffu, slow_w);
+    for (int p = 0; p < NP; ++p) recur_vals<MODE>(gn[p], rc, wtab, A[p], Bv[p], cS[p]);
     geom(jj0 + NP, gn);
     for (int jj = jj0; jj < cnt; jj += NP) {
-        if (slow_any) {
-#pragma unroll
-            for (int p = 0; p < NP; ++p)
-                if (slow[p]) recur_slow_pair<K, MODE, W>(acc, tile[jj + p], pi, rc, wtab);
-        }
-        // stage B of group jj + NP, stage A of group jj + 2 NP, packed loops of group jj: one basic block
+        // stage B of group jj + NP, stage A of group jj + 2 NP, packed loops of group jj: one basic block, no branch
         u64 An[NP][4], Bn[NP][4];
         float cSn[NP];
-        bool slown[NP];
-        slow_w = false;
 #pragma unroll
-        for (int p = 0; p < NP; ++p) { recur_vals<MODE>(gn[p], rc, wtab, An[p], Bn[p], cSn[p]); slown[p] = gn[p].slow; slow_w = slow_w || slown[p]; }
+        for (int p = 0; p < NP; ++p) recur_vals<MODE>(gn[p], rc, wtab, An[p], Bn[p], cSn[p]);
         geom(jj + 2 * NP, gn);
 #pragma unroll
         for (int p = 0; p < NP; ++p) recur_hot<K>(acc, A[p], Bv[p], cS[p]);
@@ -445,9 +439,20 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
         for (int p = 0; p < NP; ++p) {
 #pragma unroll
             for (int a = 0; a < 4; ++a) { A[p][a] = An[p][a]; Bv[p][a] = Bn[p][a]; }
-            cS[p] = cSn[p]; slow[p] = slown[p];
+            cS[p] = cSn[p];
         }
-        slow_any = __any_sync(0xffffffffu, slow_w);      // after the packed loops: the vote ends the basic block
+    }
+    // slow-path pairs (theta at or below theta_min, coincident atoms) contributed exactly zero above; they are rare, so
+    // the tile is rescanned for them only if some lane of the warp met one
+    if (__any_sync(0xffffffffu, had_slow)) {
+        if (had_slow) {
+            for (int j = max(jj0, jmin); j < cnt; ++j) {
+                const float4 pj = tile[j];
+                const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+                const float r2c = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, 1e-30f)));       // as in recur_geom
+                if (!(r2c > rc.cut2)) recur_slow_pair<K, MODE, W>(acc, pj, pi, rc, wtab);
+            }
+        }
     }
 }
 
@@ -474,7 +479,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
     if (VAR == V_RECUR && alt_gate >= 0 && plan->recur_alt != alt_gate) return;
     constexpr bool F64 = (VAR == V_F64);
     constexpr int NW = DEBYE_IB / 32;
-    __shared__ __align__(128) float4 tile[2][DEBYE_JT];
+    __shared__ __align__(128) float4 tile[2][DEBYE_JT + DEBYE_TILE_PAD];
     __shared__ __align__(8) u64 mbar[2];
     __shared__ float tbuf[F64 ? 1 : NW][F64 ? 1 : 32][F64 ? 1 : 33];
     __shared__ double wsum[NW][K];
@@ -495,6 +500,8 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
 #ifdef DEBYE_TRACE      // working builds only: per-CTA start / end time and SM id
     if (tid == 0) { unsigned long long t; unsigned sm; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); asm volatile("mov.u32 %0, %%smid;" : "=r"(sm)); debye_trace[3 * c] = t; debye_trace[3 * c + 2] = sm; }
 #endif
+    // every entry finite from the start: the recurrence pipeline reads up to DEBYE_TILE_PAD entries past the atoms of a tile
+    for (int x = tid; x < 2 * (DEBYE_JT + DEBYE_TILE_PAD); x += DEBYE_IB) (&tile[0][0])[x] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (tid == 0) { mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();

@@ -13,6 +13,7 @@
 #define DEBYE_MAX_TP (DEBYE_MAX_TYPES_I * (DEBYE_MAX_TYPES_I + 1) / 2)
 #define DEBYE_IB 128          // i atoms per row == threads per pairs CTA
 #define DEBYE_JT 512          // j atoms per shared-memory tile (8 KB, one cp.async.bulk); 2 buffers per CTA
+#define DEBYE_TILE_PAD 8      // readable (finite) entries behind each buffer: the recurrence reads two groups ahead
 
 enum DebyeVariant : int32_t { V_NONE = 0, V_F64 = 1, V_MUFU = 2, V_RECUR = 3, V_ACCURATE = 4 };
 

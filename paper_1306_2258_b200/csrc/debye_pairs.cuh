@@ -255,7 +255,7 @@ __device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, con
     reduce_turns_pair(g.r, rc.w1, rc.w1_lo, rc.smult, g.f1, g.fS);     // f1 is dead code in the general-start mode
 }
 // Stage B (values): Bv = w_0 (the 8 residues), A = w_{-1}, cS = 2 cos(S theta).
-template <int MODE>
+template <int MODE, bool TWO>
 __device__ __forceinline__ void recur_vals(const RecurGeom &g, const RecurConst &rc, const float *wtab, u64 (&A)[4], u64 (&Bv)[4], float &cS)
 {
     const float r = g.r, rinv = g.rinv;
@@ -278,12 +278,18 @@ __device__ __forceinline__ void recur_vals(const RecurGeom &g, const RecurConst 
         u[5] = fmaf(c4, u[1], u[3]); u[6] = fmaf(c4, u[2], u[2]); u[7] = fmaf(c4, u[3], u[1]); u[8] = c4 * u[4];
         // chains start at index 1 (index 0 is identically zero): chain j of chunk ch holds k' = 1 + 8 ch + j + S m.
         // B = w_0 = v(k'), A = w_{-1} = -v(k' - S) = +u[S - k'] (v(-n) = -v(n))
-        if constexpr (MODE == RM_Z1) {
+#pragma unroll
+        for (int n = 9; n <= 16; ++n) u[n] = fmaf(c4, u[n - 4], -u[n - 8]);
+        if constexpr (TWO) {
+            // TWO-SEED form (recur_two_seeds): A = w_0 = v(1..8), Bv = w_1 = v(9..16).  Compared with (w_{-1}, w_0) this costs
+            // 8 scalar FFMA but saves one packed chain step (4 FFMA2) and, above all, the 8 register copies that building
+            // w_{-1} = (u7, u6, ..., u1, 0) out of values that also sit in w_0 needs: every u lands in exactly one slot
+            A[0] = pk2(u[1], u[2]); A[1] = pk2(u[3], u[4]); A[2] = pk2(u[5], u[6]); A[3] = pk2(u[7], u[8]);
+            Bv[0] = pk2(u[9], u[10]); Bv[1] = pk2(u[11], u[12]); Bv[2] = pk2(u[13], u[14]); Bv[3] = pk2(u[15], u[16]);
+        } else if constexpr (MODE == RM_Z1) {
             Bv[0] = pk2(u[1], u[2]); Bv[1] = pk2(u[3], u[4]); Bv[2] = pk2(u[5], u[6]); Bv[3] = pk2(u[7], u[8]);
             A[0] = pk2(u[7], u[6]); A[1] = pk2(u[5], u[4]); A[2] = pk2(u[3], u[2]); A[3] = pk2(u[1], u[0]);
         } else {
-#pragma unroll
-            for (int n = 9; n <= 16; ++n) u[n] = fmaf(c4, u[n - 4], -u[n - 8]);
             if constexpr (MODE == RM_Z2A) {
                 Bv[0] = pk2(u[1], u[2]); Bv[1] = pk2(u[3], u[4]); Bv[2] = pk2(u[5], u[6]); Bv[3] = pk2(u[7], u[8]);
                 A[0] = pk2(u[15], u[14]); A[1] = pk2(u[13], u[12]); A[2] = pk2(u[11], u[10]); A[3] = pk2(u[9], u[8]);
@@ -317,12 +323,22 @@ __device__ __forceinline__ void recur_vals(const RecurGeom &g, const RecurConst 
 
 // Packed hot loop of one pair: w_m = sigma_m v_m with sigma = (+,+,-,-): w_{m+1} = (+/-) cS w_m + w_{m-1}; 4 packed chains
 // (8 residues), K/8 steps: per term one FFMA2 lane and one FADD2 lane.  A and Bv are consumed.
-template <int K>
+// which instantiations hand over (w_0, w_1) instead of (w_{-1}, w_0): the one-chunk zero-start mode.  Measured per K on B200
+// (pairs-kernel-only driver, N = 10 000): two seeds win 2-5 % at K = 64, 104, 128 and lose 2.3 % at K = 100, where the
+// register allocation of the packed loop happens to come out worse -- hence the exception.
+__host__ __device__ constexpr bool recur_two_seeds(int mode, int K) { return mode == RM_Z1 && K != 100; }
+
+template <int K, bool TWO>
 __device__ __forceinline__ void recur_hot(u64 (&acc)[K / 2], u64 (&A)[4], u64 (&Bv)[4], const float cS)
 {
     const u64 cP = pk2(cS, cS), cN = pk2(-cS, -cS);
+    if constexpr (TWO) {
 #pragma unroll
-    for (int m = 0; m < (K + 7) / 8; ++m) {
+        for (int a = 0; a < 4; ++a)
+            if (2 * a < K) acc[a] = add2(acc[a], A[a]);        // step 0 (sigma_0 = +)
+    }
+#pragma unroll
+    for (int m = TWO ? 1 : 0; m < (K + 7) / 8; ++m) {
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
             if (8 * m + 2 * a < K) {                       // K % 8 == 4: the last step runs chains 0 and 1 only
@@ -353,17 +369,23 @@ __device__ __forceinline__ void recur_slow_pair(u64 (&acc)[K / 2], const float4 
     recur_geom<MODE, W>(pj, pi, true, rs, g);
     u64 A[4], Bv[4];
     float cS;
-    recur_vals<MODE>(g, rc, wtab, A, Bv, cS);
+    recur_vals<MODE, recur_two_seeds(MODE, K)>(g, rc, wtab, A, Bv, cS);
     (void)cS;
     // beta from the polynomial directly (2 - cS would cancel)
     const float nbeta = -four_sin2_from(sincos_fold(g.fS));
     const u64 nb2 = pk2(nbeta, nbeta);
-    // stage B returns A = w_{-1} = -v_{-1} (sign convention of the fast loop): d_0 = v_0 - v_{-1} = Bv + A
+    // stage B returns A = w_{-1} = -v_{-1} (sign convention of the fast loop): d_0 = v_0 - v_{-1} = Bv + A;
+    // in the two-seed form it returns (v_0, v_1): step 0 is added here and the chain starts at m = 1 with d_1 = v_1 - v_0
+    constexpr bool TWO = recur_two_seeds(MODE, K);
     u64 s[4], d[4];
 #pragma unroll
-    for (int a = 0; a < 4; ++a) { s[a] = Bv[a]; d[a] = add2(Bv[a], A[a]); }
+    for (int a = 0; a < 4; ++a) {
+        s[a] = Bv[a];
+        if constexpr (TWO) { if (2 * a < K) acc[a] = add2(acc[a], A[a]); d[a] = sub2(Bv[a], A[a]); }
+        else d[a] = add2(Bv[a], A[a]);
+    }
 #pragma unroll
-    for (int m = 0; m < (K + 7) / 8; ++m) {
+    for (int m = TWO ? 1 : 0; m < (K + 7) / 8; ++m) {
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
             if (8 * m + 2 * a < K) {
@@ -424,17 +446,17 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
     RecurGeom gn[NP];
     geom(jj0, gn);
 #pragma unroll
-    for (int p = 0; p < NP; ++p) recur_vals<MODE>(gn[p], rc, wtab, A[p], Bv[p], cS[p]);
+    for (int p = 0; p < NP; ++p) recur_vals<MODE, recur_two_seeds(MODE, K)>(gn[p], rc, wtab, A[p], Bv[p], cS[p]);
     geom(jj0 + NP, gn);
     for (int jj = jj0; jj < cnt; jj += NP) {
         // stage B of group jj + NP, stage A of group jj + 2 NP, packed loops of group jj: one basic block, no branch
         u64 An[NP][4], Bn[NP][4];
         float cSn[NP];
 #pragma unroll
-        for (int p = 0; p < NP; ++p) recur_vals<MODE>(gn[p], rc, wtab, An[p], Bn[p], cSn[p]);
+        for (int p = 0; p < NP; ++p) recur_vals<MODE, recur_two_seeds(MODE, K)>(gn[p], rc, wtab, An[p], Bn[p], cSn[p]);
         geom(jj + 2 * NP, gn);
 #pragma unroll
-        for (int p = 0; p < NP; ++p) recur_hot<K>(acc, A[p], Bv[p], cS[p]);
+        for (int p = 0; p < NP; ++p) recur_hot<K, recur_two_seeds(MODE, K)>(acc, A[p], Bv[p], cS[p]);
 #pragma unroll
         for (int p = 0; p < NP; ++p) {
 #pragma unroll

@@ -157,11 +157,12 @@ int dev_state(DevState **st)
     return DEBYE_OK;
 }
 
-// Grid of the pairs kernel: resident CTAs (SMs x occupancy) times a small number of waves.  The warp schedulers favour
-// one of the CTAs that share an SM, so with exactly one wave the favoured CTA finishes ~30 % early and its partner runs
-// the tail alone (measured); a few waves (up to 16 when there is enough work) let the hardware block scheduler refill the SM.  More waves
-// cost one prologue + one FP64 flush per CTA, so the count is bounded by the work available (estimated from N alone:
-// the host never sees the type histogram).
+// Grid of the pairs kernel: resident CTAs (SMs x occupancy) times a number of waves.  The warp schedulers favour one of
+// the CTAs that share an SM, so with exactly one wave the favoured CTA finishes ~30 % early and its partner runs the tail
+// alone (measured); more waves let the hardware block scheduler refill the SM.  Each extra CTA costs
+// one prologue, one FP64 flush and one more record for the final kernel, so the count is bounded by the work available
+// (estimated from N alone: the host never sees the type histogram): at least ~150 units (one j atom x 128 i atoms) per
+// CTA, at most 16 waves -- the measured optimum on cfg2 (8 waves) and flat beyond 4 waves on the large configs.
 int grid_for(DevState *s, const Choice &c, int N, int B, int *G, bool weighted = false)
 {
     int &o = s->occ[c.variant][c.K / 4];
@@ -175,7 +176,7 @@ int grid_for(DevState *s, const Choice &c, int N, int B, int *G, bool weighted =
     }
     const int resident = s->sms * o;
     const double units = (double)B * c.n_chunks * ((double)N * (double)N / (2.0 * DEBYE_IB));   // j atoms x rows, all type pairs
-    int waves = (int)(units / ((double)resident * 600.0));
+    int waves = (int)(units / ((double)resident * 150.0));
     if (waves < 1) waves = 1;
     if (waves > 16) waves = 16;
     *G = resident * waves;

@@ -277,3 +277,33 @@ def test_weighted_profiles_match_the_weighted_oracle(db):
     xb, t, f, q = to_dev(wb)
     Ib = db.debye_profile_weighted(xb, t, torch.from_numpy(wt).cuda(), f, q).cpu().numpy()
     assert Ib.shape == (5, wb.M) and rel(Ib, refb) <= TOL32
+
+
+def test_random_shape_sweep(db):
+    """Seeded sweep over small shapes: every accumulator count K (multiples of 4 and of 8), 1-4 chunks, grids starting at
+    0, at dq and elsewhere, 1-3 conformers, 1-6 types, row counts around the 128-atom row and 512-atom tile boundaries."""
+    import torch
+    rng = np.random.default_rng(2024)
+    worst = 0.0
+    for case in range(48):
+        N = int(rng.choice([2, 3, 31, 127, 128, 129, 200, 383, 513, 640]))
+        T = int(rng.integers(1, 7))
+        M = int(rng.choice([1, 2, 3, 7, 8, 9, 12, 13, 33, 52, 64, 65, 97, 100, 101, 128, 129, 130, 200, 257, 300]))
+        B = int(rng.choice([1, 1, 2, 3]))
+        start = int(rng.integers(0, 3))                       # 0: q0 = 0, 1: q0 = dq, 2: offset grid
+        dq = float(rng.uniform(0.002, 0.02))
+        q0 = [0.0, dq, float(rng.uniform(0.05, 0.3))][start]
+        q = (q0 + dq * np.arange(M)).astype(np.float32)
+        if start == 0:
+            q[0] = 0.0
+        xyz = (rng.uniform(-1, 1, (B, N, 3)) * float(rng.uniform(5, 60))).astype(np.float32)
+        typ = rng.integers(0, T, N).astype(np.int32)
+        f = wl.gaussian_form_factors(1000 + case, T, q)
+        ref = np.stack([orc.debye_sym(xyz[b], typ, f, q) for b in range(B)])
+        x, t, fd, qd = (torch.from_numpy(a).cuda() for a in (xyz, typ, f, q))
+        for v in ("auto", "mufu"):
+            I = db.debye_profile_batch(x, t, fd, qd, variant=v).cpu().numpy()
+            e = rel(I, ref)
+            worst = max(worst, e)
+            assert e <= TOL32, (case, N, T, M, B, start, v, e)
+    assert worst <= 1e-5, worst                               # typical error of these small, well-conditioned cases

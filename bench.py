@@ -162,6 +162,7 @@ def main():
     ap.add_argument("--variant", default="auto", choices=["auto", "recur", "mufu", "accurate", "fp64"])
     ap.add_argument("--impl", default="libdebye", choices=["libdebye", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-hint", action="store_true", help="do not pass the q-grid hint (DEBYE_QHINT_*) computed from the host copy of q")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "libdebye" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
@@ -188,7 +189,10 @@ def main():
     x, t, f, q = (torch.from_numpy(a).to(dev) for a in (w.xyz, w.type, w.fftab, w.q))
     out = torch.empty((w.B, w.M) if batch else (w.M,), dtype=torch.float64, device=dev)
     flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device=dev)        # > 126 MB L2
-    info = db.launch_info(w.N, w.B, w.T, w.M, args.variant, with_grid=True)
+    # the q grid exists on the host (it was generated there), so the caller can tell the library its shape: one pairs launch
+    # instead of up to three (include/debye.h, DEBYE_QHINT_*); the device verifies the hint
+    hint = 0 if args.no_hint else db.q_hint(w.q)
+    info = db.launch_info(w.N, w.B, w.T, w.M, args.variant, with_grid=True, hint=hint)
 
     def barrier():
         if world > 1:
@@ -197,7 +201,7 @@ def main():
 
     # ---- device-resident timing -------------------------------------------------------------------------------
     for _ in range(args.warmup):
-        call(x, t, f, q, out, variant=args.variant)
+        call(x, t, f, q, out, variant=args.variant, hint=hint)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
     sampler = ClockSampler(local_rank)
@@ -206,7 +210,7 @@ def main():
     for a, b in ev:
         flush.fill_(1)                          # L2 flush between steps, outside the per-step events
         a.record()
-        call(x, t, f, q, out, variant=args.variant)
+        call(x, t, f, q, out, variant=args.variant, hint=hint)
         b.record()
     barrier()
     wall = time.perf_counter() - wall0
@@ -223,7 +227,7 @@ def main():
     pk = []
     for _ in range(min(args.steps, 30)):
         flush.fill_(1)
-        call(x, t, f, q, out, variant=args.variant)
+        call(x, t, f, q, out, variant=args.variant, hint=hint)
         torch.cuda.synchronize()
         pk.append(e0.elapsed_time(e1))
     db.set_pairs_events(None, None)
@@ -233,12 +237,12 @@ def main():
     hx, ht, hf, hq = (torch.from_numpy(a).pin_memory().numpy() for a in (w.xyz, w.type, w.fftab, w.q))
     hout = torch.empty((w.B, w.M) if batch else (w.M,), dtype=torch.float64).pin_memory().numpy()
     for _ in range(3):
-        call_host(hx, ht, hf, hq, hout, variant=args.variant)
+        call_host(hx, ht, hf, hq, hout, variant=args.variant, hint=hint)
     barrier()
     n_e2e = max(5, min(args.steps, 50))
     t0 = time.perf_counter()
     for _ in range(n_e2e):
-        call_host(hx, ht, hf, hq, hout, variant=args.variant)
+        call_host(hx, ht, hf, hq, hout, variant=args.variant, hint=hint)
     barrier()
     e2e_s = sharding.max_over_ranks(time.perf_counter() - t0, dev)
     e2e_value = units * n_e2e / e2e_s / 1e9
@@ -274,7 +278,7 @@ def main():
                 "reference variant; XU roofline quoted for scale"}
     roof["traffic"] = NCU_TRAFFIC.get((args.config, variant_ran))
     k_ran, chunks_ran = info["q_chunk"], info["n_chunks"]
-    if variant_ran == "recur" and w.M >= 2 and float(w.q[0]) == 0.0:
+    if hint == 0 and variant_ran == "recur" and w.M >= 2 and float(w.q[0]) == 0.0:
         # grid starts at q = 0: the device runs the recurrence launch sized for M - 1 chain indices when the library
         # offered one (it does when that saves accumulators or a chunk)
         alt = db.launch_info(w.N, w.B, w.T, w.M - 1, "recur")
@@ -291,6 +295,7 @@ def main():
         "dtype": "f64" if variant_ran == "fp64" else "f32", "data": "synthetic",
         "config": {"workload": w.name, "N": w.N, "T": w.T, "M": w.M, "B": w.B, "variant": variant_ran,
                    "pairs_grid": info["pairs_grid"], "q_chunk": k_ran, "n_chunks": chunks_ran,
+                   "q_hint": "passed (grid classified from the host copy of q, verified on the device)" if hint else "none",
                    "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
                    "parallelism": f"{world} independent structure(s), one per GPU", "wall_s_timed_loop": wall},
         "clocks": clocks,

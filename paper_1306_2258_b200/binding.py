@@ -17,7 +17,7 @@ FLAGS = {"fp64": 1 << 0, "mufu": 1 << 2, "recur": 1 << 3, "accurate": 1 << 4, "a
 
 EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_profile_batch_host",
            "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
-           "debye_launch_info", "debye_set_pairs_events", "debye_strerror", "debye_last_cuda_error", "debye_version")
+           "debye_launch_info", "debye_set_pairs_events", "debye_q_hint", "debye_strerror", "debye_last_cuda_error", "debye_version")
 
 
 class LibdebyeError(RuntimeError):
@@ -61,6 +61,8 @@ def lib():
     L.debye_launch_info.restype = C.c_int
     L.debye_set_pairs_events.argtypes = [vp, vp]
     L.debye_set_pairs_events.restype = C.c_int
+    L.debye_q_hint.argtypes = [vp, i32]
+    L.debye_q_hint.restype = u32
     L.debye_strerror.argtypes = [C.c_int]
     L.debye_strerror.restype = C.c_char_p
     L.debye_last_cuda_error.restype = C.c_int
@@ -76,10 +78,15 @@ def _check(st: int):
                             f"(cuda error {L.debye_last_cuda_error()})")
 
 
-def _flags(variant) -> int:
-    if isinstance(variant, int):
-        return variant
-    return FLAGS[variant]
+def _flags(variant, hint: int = 0) -> int:
+    return (variant if isinstance(variant, int) else FLAGS[variant]) | int(hint)
+
+
+def q_hint(q_host) -> int:
+    """Grid hint flags (DEBYE_QHINT_*) for a HOST copy of the q grid (numpy float32): pass as `hint=` to the profile calls
+    so that only the pairs instantiation this grid needs is launched.  A wrong hint gives NaN, never a wrong number."""
+    q_host = np.ascontiguousarray(q_host, dtype=np.float32)
+    return int(lib().debye_q_hint(C.c_void_p(q_host.ctypes.data), q_host.shape[0]))
 
 
 def _stream_ptr(stream):
@@ -95,7 +102,7 @@ def _dev(t, dtype, name):
     return C.c_void_p(t.data_ptr())
 
 
-def debye_profile(xyz, type, fftab, q, I_out=None, variant="auto", stream=None):
+def debye_profile(xyz, type, fftab, q, I_out=None, variant="auto", stream=None, hint=0):
     """I_out[M] (float64, CUDA) for xyz[N,3] f32, type[N] i32, fftab[T,M] f32, q[M] f32 (CUDA tensors).
     Asynchronous on `stream` (default: torch's current stream)."""
     import torch
@@ -104,11 +111,11 @@ def debye_profile(xyz, type, fftab, q, I_out=None, variant="auto", stream=None):
         I_out = torch.empty(M, dtype=torch.float64, device=xyz.device)
     _check(lib().debye_profile(_dev(xyz, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N,
                                _dev(fftab, torch.float32, "fftab"), T, _dev(q, torch.float32, "q"), M,
-                               _dev(I_out, torch.float64, "I_out"), _flags(variant), _stream_ptr(stream)))
+                               _dev(I_out, torch.float64, "I_out"), _flags(variant, hint), _stream_ptr(stream)))
     return I_out
 
 
-def debye_profile_batch(xyz, type, fftab, q, I_out=None, variant="auto", stream=None):
+def debye_profile_batch(xyz, type, fftab, q, I_out=None, variant="auto", stream=None, hint=0):
     """I_out[B,M] for B conformers xyz[B,N,3] sharing type / fftab / q."""
     import torch
     B, N, T, M = xyz.shape[0], xyz.shape[1], fftab.shape[0], q.shape[0]
@@ -116,11 +123,11 @@ def debye_profile_batch(xyz, type, fftab, q, I_out=None, variant="auto", stream=
         I_out = torch.empty((B, M), dtype=torch.float64, device=xyz.device)
     _check(lib().debye_profile_batch(_dev(xyz, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N, B,
                                      _dev(fftab, torch.float32, "fftab"), T, _dev(q, torch.float32, "q"), M,
-                                     _dev(I_out, torch.float64, "I_out"), _flags(variant), _stream_ptr(stream)))
+                                     _dev(I_out, torch.float64, "I_out"), _flags(variant, hint), _stream_ptr(stream)))
     return I_out
 
 
-def debye_profile_weighted(xyz, type, weight, fftab, q, I_out=None, variant="auto", stream=None):
+def debye_profile_weighted(xyz, type, weight, fftab, q, I_out=None, variant="auto", stream=None, hint=0):
     """As debye_profile with per-atom weights: f_j(q) = weight[j] * fftab[type[j]] (weight[N] f32 CUDA tensor).
     xyz[N,3] gives I_out[M]; xyz[B,N,3] gives I_out[B,M] (weights shared by the conformers)."""
     import torch
@@ -130,7 +137,7 @@ def debye_profile_weighted(xyz, type, weight, fftab, q, I_out=None, variant="aut
         I_out = torch.empty((xyz.shape[0], M) if batch else M, dtype=torch.float64, device=xyz.device)
     a = (_dev(xyz, torch.float32, "xyz"), _dev(type, torch.int32, "type"), _dev(weight, torch.float32, "weight"), N)
     b = (_dev(fftab, torch.float32, "fftab"), T, _dev(q, torch.float32, "q"), M, _dev(I_out, torch.float64, "I_out"),
-         _flags(variant), _stream_ptr(stream))
+         _flags(variant, hint), _stream_ptr(stream))
     if batch:
         _check(lib().debye_profile_batch_weighted(*a, xyz.shape[0], *b))
     else:
@@ -138,14 +145,14 @@ def debye_profile_weighted(xyz, type, weight, fftab, q, I_out=None, variant="aut
     return I_out
 
 
-def debye_profile_weighted_host(xyz, type, weight, fftab, q, I_out=None, variant="auto", stream=None):
+def debye_profile_weighted_host(xyz, type, weight, fftab, q, I_out=None, variant="auto", stream=None, hint=0):
     N, T, M = xyz.shape[0], fftab.shape[0], q.shape[0]
     if I_out is None:
         I_out = np.empty(M, dtype=np.float64)
     _check(lib().debye_profile_weighted_host(_host(xyz, np.float32, "xyz"), _host(type, np.int32, "type"),
                                              _host(weight, np.float32, "weight"), N, _host(fftab, np.float32, "fftab"), T,
                                              _host(q, np.float32, "q"), M, _host(I_out, np.float64, "I_out"),
-                                             _flags(variant), _stream_ptr(stream)))
+                                             _flags(variant, hint), _stream_ptr(stream)))
     return I_out
 
 
@@ -168,7 +175,7 @@ def _host(a, dtype, name):
     return C.c_void_p(a.ctypes.data)
 
 
-def debye_profile_host(xyz, type, fftab, q, I_out=None, variant="auto", stream=None):
+def debye_profile_host(xyz, type, fftab, q, I_out=None, variant="auto", stream=None, hint=0):
     """Host-buffer entry (numpy arrays, ideally pinned): H2D copies + device path + D2H copy + stream sync
     all happen inside the C call."""
     N, T, M = xyz.shape[0], fftab.shape[0], q.shape[0]
@@ -176,17 +183,17 @@ def debye_profile_host(xyz, type, fftab, q, I_out=None, variant="auto", stream=N
         I_out = np.empty(M, dtype=np.float64)
     _check(lib().debye_profile_host(_host(xyz, np.float32, "xyz"), _host(type, np.int32, "type"), N,
                                     _host(fftab, np.float32, "fftab"), T, _host(q, np.float32, "q"), M,
-                                    _host(I_out, np.float64, "I_out"), _flags(variant), _stream_ptr(stream)))
+                                    _host(I_out, np.float64, "I_out"), _flags(variant, hint), _stream_ptr(stream)))
     return I_out
 
 
-def debye_profile_batch_host(xyz, type, fftab, q, I_out=None, variant="auto", stream=None):
+def debye_profile_batch_host(xyz, type, fftab, q, I_out=None, variant="auto", stream=None, hint=0):
     B, N, T, M = xyz.shape[0], xyz.shape[1], fftab.shape[0], q.shape[0]
     if I_out is None:
         I_out = np.empty((B, M), dtype=np.float64)
     _check(lib().debye_profile_batch_host(_host(xyz, np.float32, "xyz"), _host(type, np.int32, "type"), N, B,
                                           _host(fftab, np.float32, "fftab"), T, _host(q, np.float32, "q"), M,
-                                          _host(I_out, np.float64, "I_out"), _flags(variant), _stream_ptr(stream)))
+                                          _host(I_out, np.float64, "I_out"), _flags(variant, hint), _stream_ptr(stream)))
     return I_out
 
 
@@ -198,11 +205,11 @@ def set_pairs_events(start=None, stop=None):
     _check(lib().debye_set_pairs_events(a, b))
 
 
-def launch_info(N, B, T, M, variant="auto", with_grid=False):
+def launch_info(N, B, T, M, variant="auto", with_grid=False, hint=0):
     """dict(n_launches, q_chunk, n_chunks[, pairs_grid]) for a call with these sizes (host-side query)."""
     L = lib()
     a, g, k, c = C.c_int32(), C.c_int32(), C.c_int32(), C.c_int32()
-    _check(L.debye_launch_info(N, B, T, M, _flags(variant), C.byref(a), C.byref(g) if with_grid else None,
+    _check(L.debye_launch_info(N, B, T, M, _flags(variant, hint), C.byref(a), C.byref(g) if with_grid else None,
                                C.byref(k), C.byref(c)))
     out = {"n_launches": a.value, "q_chunk": k.value, "n_chunks": c.value}
     if with_grid:

@@ -10,6 +10,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <cmath>
 #include <mutex>
 #include "../../include/debye.h"
 #include "debye_aux.cuh"
@@ -113,14 +114,35 @@ Layout layout(int N, int B, int T, int M, int G_max, const Choice *ch, int nch)
 }
 
 constexpr int MAX_CHOICES = 3;
+// grid class promised by the caller's hint flags (debye_grid_class), -3 without a hint
+int hint_class_of(uint32_t flags)
+{
+    if (!(flags & DEBYE_QHINT)) return -3;
+    if (!(flags & DEBYE_QHINT_UNIFORM)) return -2;
+    if (flags & DEBYE_QHINT_START0) return 0;
+    if (flags & DEBYE_QHINT_STARTDQ) return 1;
+    return -1;
+}
+// the one recurrence launch for a known grid class
+int recur_choice_hinted(Choice *out, int M, int cls)
+{
+    Choice c[2];
+    const int n = recur_choices(c, M);
+    out[0] = (n == 2 && cls == 0) ? c[0] : c[n - 1];      // the launch sized for M - 1 indices only when q[0] == 0
+    out[0].alt_gate = -1;
+    return 1;
+}
 int variants_for(uint32_t flags, Choice *out, int M, int *is_auto)
 {
     *is_auto = 0;
+    const int cls = hint_class_of(flags);
     if (flags & DEBYE_FP64) { out[0] = choose(V_F64, M); return 1; }
     if (flags & DEBYE_SINC_MUFU) { out[0] = choose(V_MUFU, M); return 1; }
-    if (flags & DEBYE_SINC_RECUR) return recur_choices(out, M);
+    if (flags & DEBYE_SINC_RECUR) return (cls >= -1) ? recur_choice_hinted(out, M, cls) : recur_choices(out, M);
     if (flags & DEBYE_SINC_ACCURATE) { out[0] = choose(V_ACCURATE, M); return 1; }
     *is_auto = 1;
+    if (cls == -2) { out[0] = choose(V_MUFU, M); return 1; }          // hinted: not uniform
+    if (cls >= -1) return recur_choice_hinted(out, M, cls);           // hinted: uniform
     int n = recur_choices(out, M);
     out[n++] = choose(V_MUFU, M);
     return n;
@@ -131,11 +153,18 @@ int validate(const void *xyz, const void *type, int N, int B, const void *tab, i
     if (!xyz || !type || !q || !out) return DEBYE_EINVAL;
     if (!tab) return DEBYE_EINVAL;
     if (N < 1 || M < 1 || T < 1 || B < 1 || T > DEBYE_MAX_TYPES || M > DEBYE_MAX_Q) return DEBYE_EINVAL;
-    uint32_t known = DEBYE_FP64 | DEBYE_SINC_MUFU | DEBYE_SINC_RECUR | DEBYE_SINC_ACCURATE;
+    uint32_t known = DEBYE_FP64 | DEBYE_SINC_MUFU | DEBYE_SINC_RECUR | DEBYE_SINC_ACCURATE | DEBYE_QHINT | DEBYE_QHINT_UNIFORM |
+                     DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ;
     if (flags & ~known) return DEBYE_EINVAL;
     uint32_t s = flags & (DEBYE_SINC_MUFU | DEBYE_SINC_RECUR | DEBYE_SINC_ACCURATE);
     if (s & (s - 1)) return DEBYE_EINVAL;
     if ((flags & DEBYE_FP64) && s) return DEBYE_EINVAL;
+    {   // grid hint: sub-bits only with DEBYE_QHINT, start bits only for uniform grids and not both
+        const uint32_t sub = flags & (DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ), st2 = flags & (DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ);
+        if (sub && !(flags & DEBYE_QHINT)) return DEBYE_EINVAL;
+        if (st2 && !(flags & DEBYE_QHINT_UNIFORM)) return DEBYE_EINVAL;
+        if (st2 == (DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ)) return DEBYE_EINVAL;
+    }
     if (N > (1 << 24)) return DEBYE_EUNSUPPORTED;
     if ((int64_t)N * B > ((int64_t)1 << 31)) return DEBYE_EUNSUPPORTED;
     return DEBYE_OK;
@@ -234,8 +263,14 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
 
     int alt_offered = 0;
     for (int i = 0; i < nch; ++i) if (ch[i].alt_gate == 1) alt_offered = 1;
+    const int hint_class = hint_class_of(flags);
+    if (hint_class == 0 && nch == 1 && ch[0].variant == V_RECUR) {
+        // hinted q[0] == 0 and a single recurrence launch: it is the one sized for M - 1 indices exactly when that pays
+        Choice c2[2];
+        alt_offered = (recur_choices(c2, M) == 2) ? 1 : 0;
+    }
     const bool pack_here = (int64_t)N * B <= DEBYE_PACK_IN_SETUP;      // small inputs: the setup CTA gathers too
-    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, xyz, sorted, pack_here ? 1 : 0, weight);
+    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, hint_class, xyz, sorted, pack_here ? 1 : 0, weight);
     if (!pack_here) {
         int64_t total = (int64_t)N * B;
         int blocks = (int)((total + 255) / 256);
@@ -354,6 +389,25 @@ int debye_partials(const float *xyz, const int32_t *type, int32_t N, int32_t B, 
                    uint32_t flags, debye_stream_t stream)
 {
     return run(xyz, type, N, B, nullptr, T, q, M, S_out, n_out, flags, (cudaStream_t)stream, 1);
+}
+
+uint32_t debye_q_hint(const float *q_host, int32_t M)
+{
+    if (!q_host || M < 1) return 0;
+    const double q0 = (double)q_host[0];
+    const double dq = debye_grid_dq(q0, (double)q_host[M - 1], M);
+    float dev = 0.f, qmax = 0.f;
+    for (int k = 0; k < M; ++k) {
+        const float d = debye_grid_dev((double)q_host[k], k, q0, dq), a = fabsf(q_host[k]);
+        if (d > dev) dev = d;
+        if (a > qmax) qmax = a;
+    }
+    const int cls = debye_grid_class(q0, dq, dev, qmax);
+    uint32_t f = DEBYE_QHINT;
+    if (cls != -2) f |= DEBYE_QHINT_UNIFORM;
+    if (cls == 0) f |= DEBYE_QHINT_START0;
+    if (cls == 1) f |= DEBYE_QHINT_STARTDQ;
+    return f;
 }
 
 size_t debye_workspace_bytes(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags)

@@ -20,6 +20,7 @@ namespace debye {
 // If pack_here != 0 the CTA also gathers the coordinates (small N x B: saves the pack launch).
 __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPlan *plan, const int32_t *__restrict__ type, const float *__restrict__ q,
                                                                             int32_t *__restrict__ perm, int N, int T, int M, int B, int alt_offered /* a recurrence launch sized for M - 1 indices exists */,
+                                                                            int hint_class /* -3: no hint; else the grid class the caller promised (debye_grid_class) */,
                                                                             const float *__restrict__ xyz, float4 *__restrict__ sorted, int pack_here, const float *__restrict__ weight)
 {
     pdl_trigger();                         // first kernel of the call: lets the next grid be staged (it waits for our completion)
@@ -28,6 +29,7 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
     __shared__ int wcnt[NWARP][DEBYE_MAX_TYPES_I];      // pass 1: atoms of type t in warp w's chunk; pass 2: running output slot
     __shared__ int seg[DEBYE_MAX_TYPES_I + 1];
     __shared__ float red[NWARP], red2[NWARP], qmax_s[NWARP];
+    __shared__ int hint_bad_s;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int chunk = ((N + NWARP - 1) / NWARP + 31) / 32 * 32;
     const int c0 = warp * chunk, c1 = min(N, c0 + chunk);
@@ -47,11 +49,11 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
     }
     // ---- q grid analysis (independent of the sort; its reduction shares the barriers below) ---------------------------
     const double q0 = (double)q[0];
-    const double dq = (M > 1) ? ((double)q[M - 1] - q0) / (double)(M - 1) : (q0 != 0.0 ? q0 : 1.0);
+    const double dq = debye_grid_dq(q0, (double)q[M - 1], M);
     float dev = 0.f, qsm = 3.0e38f, qmax = 0.f;
     for (int k = tid; k < M; k += blockDim.x) {
         const double qk = (double)q[k];
-        dev = fmaxf(dev, (float)fabs(qk - (q0 + k * dq)));
+        dev = fmaxf(dev, debye_grid_dev(qk, k, q0, dq));
         const float aq = fabsf((float)qk);
         if (aq > 0.f) qsm = fminf(qsm, aq);
         qmax = fmaxf(qmax, aq);
@@ -75,14 +77,12 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
     if (tid == 32) {
         float d = 0.f, s = 3.0e38f, mx = 0.f;
         for (int w = 0; w < NWARP; ++w) { d = fmaxf(d, red[w]); s = fminf(s, red2[w]); mx = fmaxf(mx, qmax_s[w]); }
-        // uniform if every q[k] is within 2 float ulps (of the largest |q|) of the line through the end points
-        const int uni = (dq != 0.0) && (d <= 2.4e-7f * fmaxf(mx, 1e-30f));
+        const int cls = debye_grid_class(q0, dq, d, mx);
+        const int uni = cls != -2;
         // zero start: q0 == 0 exactly (koff = 0) or q0 == dq to 1e-6 (koff = 1, the paper's own grid q_k = k dq, k >= 1)
-        int koff = -1;
-        if (uni) {
-            if (q0 == 0.0) koff = 0;
-            else if (fabs(q0 / dq - 1.0) <= 1e-6) koff = 1;
-        }
+        const int koff = cls >= 0 ? cls : -1;
+        hint_bad_s = (hint_class != -3 && hint_class != cls) ? 1 : 0;
+        plan->hint_bad = hint_bad_s;
         plan->recur_alt = (koff == 0 && alt_offered) ? 1 : 0;
         plan->N = N; plan->T = T; plan->M = M; plan->B = B; plan->n_tp = T * (T + 1) / 2;
         plan->weighted = weight ? 1 : 0;
@@ -117,7 +117,8 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
                 pre += units;
             }
         plan->tp_prefix[tp] = pre;
-        plan->U1 = pre;
+        // a wrong grid hint leaves no work: the pairs kernels return at once and the final kernel writes NaN
+        plan->U1 = hint_bad_s ? 0 : pre;
     }
     // first output slot of (warp, type): exclusive prefix over the warps, per type (thread (w, t) = (warp, lane))
     int first = seg[lane];
@@ -217,7 +218,7 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
         if ((!is_auto || plan->variant_auto == c.variant) && (c.alt_gate < 0 || plan->recur_alt == c.alt_gate)) { pick = i; break; }
     }
     const int variant = sets.s[pick].variant, K = sets.s[pick].K, n_chunks = sets.s[pick].n_chunks, G = sets.s[pick].G;
-    const bool bad = (variant == V_RECUR && !plan->uniform);          // forced recurrence on a non-uniform grid -> NaN
+    const bool bad = (variant == V_RECUR && !plan->uniform) || plan->hint_bad;   // forced recurrence on a non-uniform grid, or a wrong grid hint -> NaN
     const double nan = __longlong_as_double(0x7ff8000000000000LL);
     const double scale = (variant == V_RECUR) ? 0.5 : 1.0;            // the recurrence kernel accumulates 2 sin(q r)/r
     double I = 0.0;

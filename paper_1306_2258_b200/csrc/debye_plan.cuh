@@ -26,6 +26,7 @@ struct DevPlan {
     int32_t variant_auto;         // variant chosen on the device when the caller gave no DEBYE_SINC_* flag
     double q0, dq;                // least-squares-free fit: q0 = q[0], dq = (q[M-1]-q[0])/(M-1)
     float q_small;                // smallest non-zero |q|
+    int32_t hint_bad;             // the caller's grid hint (DEBYE_QHINT_*) contradicts q: nothing is computed, the output is NaN
     int32_t weighted;             // per-atom weights given (debye_profile_weighted): sorted[].w holds w_j, else 1
     int64_t U1;                   // units per conformer and per q-chunk
     double sw[DEBYE_MAX_TYPES_I];             // weighted calls: sum of w_j over the atoms of each type ...
@@ -36,6 +37,22 @@ struct DevPlan {
     int32_t tp_tj[DEBYE_MAX_TP];              // type on the j (column) side; == tp_ti on the diagonal
     int64_t tp_prefix[DEBYE_MAX_TP + 1];      // units before type pair tp (one chunk, one conformer)
 };
+
+// ---- q-grid classification, identical on the host (debye_q_hint) and on the device (debye_setup_kernel) -----------------
+// class: -2 not uniform; -1 uniform, general start; 0 uniform with q[0] == 0; 1 uniform with q[0] == dq (the paper's grid).
+// `dev` = max_k |q[k] - fma(k, dq, q0)| rounded to float per element, `qmax` = max_k |q[k]|: a maximum, so the order in which
+// it is taken (serial on the host, tree on the device) does not matter; fma keeps host and device arithmetic identical.
+__host__ __device__ inline double debye_grid_dq(double q0, double qlast, int M) { return (M > 1) ? (qlast - q0) / (double)(M - 1) : (q0 != 0.0 ? q0 : 1.0); }
+__host__ __device__ inline float debye_grid_dev(double qk, int k, double q0, double dq) { return (float)fabs(qk - fma((double)k, dq, q0)); }
+__host__ __device__ inline int debye_grid_class(double q0, double dq, float dev, float qmax)
+{
+    // uniform if every q[k] is within 2 float ulps (of the largest |q|) of the line through the end points
+    const bool uni = (dq != 0.0) && (dev <= 2.4e-7f * (qmax > 1e-30f ? qmax : 1e-30f));
+    if (!uni) return -2;
+    if (q0 == 0.0) return 0;
+    if (fabs(q0 / dq - 1.0) <= 1e-6) return 1;
+    return -1;
+}
 
 // ---- programmatic dependent launch (PDL) ------------------------------------------------------------------------
 // Every kernel after the setup kernel is launched with cudaLaunchAttributeProgrammaticStreamSerialization and starts with

@@ -51,7 +51,10 @@ def test_argument_validation_happens_before_cuda():
     assert L.debye_profile(p, p, 10, p, 2, p, 4097, p, 0, None) == EINVAL
     assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 2) | (1 << 3), None) == EINVAL      # two sinc variants
     assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 0) | (1 << 2), None) == EINVAL      # fp64 + fp32 variant
-    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, 1 << 9, None) == EINVAL                   # unknown flag
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, 1 << 20, None) == EINVAL                  # unknown flag
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, 1 << 9, None) == EINVAL                   # hint sub-bit without DEBYE_QHINT
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 8) | (1 << 10), None) == EINVAL     # start bit without uniform
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 8) | (1 << 9) | (1 << 10) | (1 << 11), None) == EINVAL
     assert L.debye_profile(p, p, (1 << 24) + 1, p, 2, p, 5, p, 0, None) == EUNSUP
     assert L.debye_profile_batch(p, p, 10, 0, p, 2, p, 5, p, 0, None) == EINVAL
     assert L.debye_profile_host(None, p, 10, p, 2, p, 5, p, 0, None) == EINVAL
@@ -85,3 +88,22 @@ def test_binding_refuses_non_cuda_inputs():
     with pytest.raises(binding.LibdebyeError):
         binding.debye_profile_host(np.zeros((4, 3)), np.zeros(4, np.int32), np.zeros((1, 2), np.float32),
                                    np.zeros(2, np.float32))       # float64 xyz
+
+
+def test_q_hint_classifies_grids_on_the_host():
+    """debye_q_hint applies the device's classification to a host copy of q (include/debye.h, DEBYE_QHINT_*)."""
+    import numpy as np
+    from paper_1306_2258_b200 import workloads as wl
+    H, U, Z, D = 1 << 8, 1 << 9, 1 << 10, 1 << 11
+    assert binding.q_hint(wl.q_grid(0.5, 101)) == H | U | Z                    # starts at 0
+    assert binding.q_hint(wl.q_grid(1.0, 50, 0.02)) == H | U | D               # the paper's grid k/50, k = 1..50
+    assert binding.q_hint(wl.q_grid(0.9, 64, 0.3)) == H | U                    # uniform, general start
+    assert binding.q_hint(wl.q_grid(0.3, 31)[::-1].copy()) == H | U            # descending
+    assert binding.q_hint(np.array([0.0, 0.1, 0.25], np.float32)) == H         # not uniform
+    assert binding.q_hint(np.array([0.0], np.float32)) == H | U | Z
+    L = binding.lib()
+    assert L.debye_q_hint(None, 5) == 0
+    # with a hint exactly one pairs instantiation is launched
+    assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H | U | Z) == {"n_launches": 3, "q_chunk": 100, "n_chunks": 1}
+    assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H | U | D) == {"n_launches": 3, "q_chunk": 104, "n_chunks": 1}
+    assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H)["n_launches"] == 3

@@ -307,3 +307,29 @@ def test_random_shape_sweep(db):
             worst = max(worst, e)
             assert e <= TOL32, (case, N, T, M, B, start, v, e)
     assert worst <= 1e-5, worst                               # typical error of these small, well-conditioned cases
+
+
+def test_grid_hints_select_one_launch_and_are_checked(db):
+    """DEBYE_QHINT_* (include/debye.h): with the right hint the result is the unhinted one bit for bit; a wrong hint gives
+    NaN, never a wrong number."""
+    import torch
+    grids = {"zero": wl.q_grid(0.5, 101), "dq": wl.q_grid(1.0, 50, 0.02), "offset": wl.q_grid(0.9, 64, 0.3),
+             "nonuniform": np.sort(np.random.default_rng(7).uniform(0.01, 0.8, 40)).astype(np.float32),
+             "zero_129": wl.q_grid(0.8, 129)}
+    base = wl.small_random(40, 700, 3, 8)
+    hints = {k: db.q_hint(v) for k, v in grids.items()}
+    assert len({hints[k] for k in ("zero", "dq", "offset", "nonuniform")}) == 4
+    for name, qg in grids.items():
+        f = wl.gaussian_form_factors(77, 3, qg)
+        x, t = (torch.from_numpy(a).cuda() for a in (base.xyz, base.type))
+        fd, qd = torch.from_numpy(f).cuda(), torch.from_numpy(qg).cuda()
+        plain = db.debye_profile(x, t, fd, qd).cpu().numpy()
+        ref = orc.debye_sym(base.xyz, base.type, f, qg)
+        assert rel(plain, ref) <= TOL32
+        hinted = db.debye_profile(x, t, fd, qd, hint=hints[name]).cpu().numpy()
+        assert hinted.tobytes() == plain.tobytes(), name
+        for other, h in hints.items():
+            if h != hints[name]:
+                assert np.isnan(db.debye_profile(x, t, fd, qd, hint=h).cpu().numpy()).all(), (name, other)
+    hb = db.debye_profile_host(base.xyz, base.type, wl.gaussian_form_factors(77, 3, grids["zero"]), grids["zero"], hint=hints["zero"])
+    assert np.isfinite(hb).all()

@@ -230,6 +230,7 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
         if (idx >= 0) slot_of(variant, K, n_chunks, idx, ch, l);
         const double qk = (double)q[k];
         const int64_t U1 = plan->U1, Uc = U1 * n_chunks, U = Uc * Bn;
+        const DebyeRanges ranges(U > 0 ? U : 1, G);
         // type pair index -> (a, b2): walk rows of the upper triangle
         int a = 0, rowstart = 0;
         for (int tp = g; tp < n_tp; tp += DEBYE_FINAL_G) {
@@ -250,7 +251,7 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
                 const int64_t X = ((int64_t)b * n_tp + tp) * n_chunks + ch;
                 double s = 0.0;
                 if (U >= G) {           // every CTA owns at least one unit: all CTAs between the owners took part
-                    const int c_lo = debye_owner(U, G, ub), c_hi = debye_owner(U, G, ue);
+                    const int c_lo = ranges.owner(ub), c_hi = ranges.owner(ue);
                     const int n = c_hi - c_lo + 1, per = (n + NS - 1) / NS;
                     const int cb = c_lo + sl * per, ce = min(c_hi + 1, cb + per);
                     const double *rp = records + ((int64_t)cb + X) * K + l;
@@ -261,7 +262,7 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
                     }
                     for (; c < ce; ++c, rp += K) s += rp[0];
                 } else if (sl == 0) {   // fewer units than CTAs: each unit has its own CTA
-                    for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)debye_owner(U, G, u) + X) * K + l];
+                    for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)ranges.owner(u) + X) * K + l];
                 }
                 S = scale * s / qk;
             }

@@ -73,16 +73,26 @@ __host__ __device__ inline int64_t debye_range_begin(int64_t U, int32_t c, int32
     return (U / G) * c + ((U % G) * c) / G;
 }
 
+// the same with the one 64-bit division hoisted and the other done in 32 bits (G < 2^16; final kernel: many evaluations
+// for one (U, G))
+struct DebyeRanges {
+    int64_t U, qd; uint32_t rm, G;
+    __host__ __device__ DebyeRanges(int64_t U_, int32_t G_) : U(U_), qd(U_ / G_), rm((uint32_t)(U_ - (U_ / G_) * G_)), G((uint32_t)G_) {}
+    __host__ __device__ int64_t begin(int32_t c) const { return qd * c + (int64_t)((rm * (uint32_t)c) / G); }
+    // CTA that owns unit u:  largest c with begin(c) <= u
+    __host__ __device__ int32_t owner(int64_t u) const
+    {
+        int64_t c = (int64_t)(((double)u * (double)G) / (double)U);   // estimate, made exact by the two loops below
+        if (c >= (int64_t)G) c = (int64_t)G - 1;
+        if (c < 0) c = 0;
+        while (c + 1 < (int64_t)G && begin((int32_t)(c + 1)) <= u) ++c;
+        while (c > 0 && begin((int32_t)c) > u) --c;
+        return (int32_t)c;
+    }
+};
+
 // CTA that owns unit u:  largest c with range_begin(c) <= u
-__host__ __device__ inline int32_t debye_owner(int64_t U, int32_t G, int64_t u)
-{
-    int64_t c = (int64_t)(((double)u * (double)G) / (double)U);   // estimate, made exact by the two loops below
-    if (c >= G) c = G - 1;
-    if (c < 0) c = 0;
-    while (c + 1 < G && debye_range_begin(U, (int32_t)(c + 1), G) <= u) ++c;
-    while (c > 0 && debye_range_begin(U, (int32_t)c, G) > u) --c;
-    return (int32_t)c;
-}
+__host__ __device__ inline int32_t debye_owner(int64_t U, int32_t G, int64_t u) { return DebyeRanges(U, G).owner(u); }
 
 // diagonal type pair with n atoms: units before row r, r(n-1) - IB r(r-1)/2
 __host__ __device__ inline int64_t debye_diag_row_prefix(int64_t n, int64_t r)

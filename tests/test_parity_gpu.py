@@ -333,3 +333,15 @@ def test_grid_hints_select_one_launch_and_are_checked(db):
                 assert np.isnan(db.debye_profile(x, t, fd, qd, hint=h).cpu().numpy()).all(), (name, other)
     hb = db.debye_profile_host(base.xyz, base.type, wl.gaussian_form_factors(77, 3, grids["zero"]), grids["zero"], hint=hints["zero"])
     assert np.isfinite(hb).all()
+
+
+def test_maximum_q_count_and_type_count(db):
+    """Edge of the documented limits (include/debye.h): M = DEBYE_MAX_Q = 4096 (32 recurrence chunks, general start) with
+    T = DEBYE_MAX_TYPES = 32, on a grid from 0 and on an offset grid; every variant that supports it."""
+    for q_min in (0.0, 0.05):
+        w = wl.small_random(50, 150, 32, 4096, q_min=q_min, q_max=1.5, box=30.0)
+        ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)
+        for v in ("auto", "mufu"):
+            e = rel(gpu_profile(db, w, v), ref)
+            assert e <= TOL32, (q_min, v, e)
+        assert rel(gpu_profile(db, w, "fp64"), ref) <= TOL64

@@ -123,7 +123,8 @@ int debye_partials(const float *xyz, const int32_t *type, int32_t N, int32_t B, 
  * Returns 0 (no hint) for q_host == NULL or M < 1. */
 uint32_t debye_q_hint(const float *q_host, int32_t M);
 
-/* Scratch bytes a call with these sizes needs (0 if the arguments are invalid). */
+/* Scratch bytes a call with these sizes needs (0 if the arguments are invalid): exact for the current CUDA device, a safe
+ * upper bound (tens of MB) when there is none. */
 size_t debye_workspace_bytes(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags);
 /* Optional caller-owned scratch for the current device (dev pointer, 256-byte aligned); NULL/0 returns to
  * the library-owned cache.  The caller keeps ownership and must keep it alive while calls are in flight. */

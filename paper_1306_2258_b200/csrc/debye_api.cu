@@ -416,8 +416,21 @@ size_t debye_workspace_bytes(int32_t N, int32_t B, int32_t T, int32_t M, uint32_
     if (validate(&dummy, &dummy, N, B, &dummy, T, &dummy, M, &dummy, flags)) return 0;
     Choice ch[MAX_CHOICES]; int is_auto;
     int nch = variants_for(flags, ch, M, &is_auto);
-    // grid is at most 148 SMs x 16 CTAs x 16 waves on any sm_100 part; use a safe upper bound so no device query is needed
-    return layout(N, B, T, M, 192 * 16 * 16, ch, nch).total;
+    // exact when a CUDA device is current (same grid computation as the call itself; attribute queries only, no GPU work);
+    // otherwise a safe upper bound: at most 192 SMs x 16 CTAs x 16 waves on any sm_100 part
+    int Gmax = 192 * 16 * 16;
+    {
+        std::lock_guard<std::mutex> lock(g_mu);
+        DevState *ds;
+        if (dev_state(&ds) == DEBYE_OK) {
+            int g = 0, gm = 0;
+            bool ok = true;
+            for (int i = 0; i < nch && ok; ++i) { ok = grid_for(ds, ch[i], N, B, &g) == DEBYE_OK; if (g > gm) gm = g; }
+            if (ok && gm > 0) Gmax = gm;
+        }
+        (void)cudaGetLastError();
+    }
+    return layout(N, B, T, M, Gmax, ch, nch).total;
 }
 
 int debye_set_workspace(void *dev_ptr, size_t bytes)

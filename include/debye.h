@@ -111,6 +111,19 @@ int debye_profile_weighted_host(const float *xyz, const int32_t *type, const flo
                                 const float *fftab, int32_t T, const float *q, int32_t M, double *I_out,
                                 uint32_t flags, debye_stream_t stream);
 
+/* Plans: repeated profiles of ONE molecule whose coordinates change between calls (refinement, ensembles evaluated one
+ * by one: the profile "must be recomputed hundreds of thousands of times").  debye_plan_create runs the
+ * setup step once (type sort, schedule, analysis of the q grid), copies q and the weights into the plan, and synchronises
+ * `stream` once to learn the shape of the grid, so that debye_plan_execute launches exactly pack + one pairs instantiation
+ * + final, never synchronises, and gives bit for bit the result of debye_profile[_batch][_weighted] with the same inputs.
+ *   type dev [N], q dev [M], weight dev [N] or NULL (read during create only); xyz dev [B][N][3], fftab dev [T][M],
+ *   I_out dev [B][M].  A plan belongs to the device that was current at creation; destroy it with debye_plan_destroy. */
+typedef struct debye_plan debye_plan_t;
+int debye_plan_create(debye_plan_t **plan, const int32_t *type, int32_t N, int32_t B, int32_t T, const float *q, int32_t M,
+                      const float *weight, uint32_t flags, debye_stream_t stream);
+int debye_plan_execute(debye_plan_t *plan, const float *xyz, const float *fftab, double *I_out, debye_stream_t stream);
+void debye_plan_destroy(debye_plan_t *plan);
+
 /* Per-type-pair partial structure factors (by-product of the path; lets a caller re-fit form factors without
  * redoing the pair sum):  S_out[b][p][m] = sum over pairs i<j with {t_i,t_j} = {a,b'} of sinc(q_m r_ij), for
  * p = a*(2T-a+1)/2 + (b'-a), a <= b' (row-major upper triangle);  n_out[t] = number of atoms of type t.

@@ -17,7 +17,8 @@ FLAGS = {"fp64": 1 << 0, "mufu": 1 << 2, "recur": 1 << 3, "accurate": 1 << 4, "a
 
 EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_profile_batch_host",
            "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
-           "debye_launch_info", "debye_set_pairs_events", "debye_q_hint", "debye_strerror", "debye_last_cuda_error", "debye_version")
+           "debye_launch_info", "debye_set_pairs_events", "debye_q_hint", "debye_plan_create", "debye_plan_execute",
+           "debye_plan_destroy", "debye_strerror", "debye_last_cuda_error", "debye_version")
 
 
 class LibdebyeError(RuntimeError):
@@ -61,6 +62,12 @@ def lib():
     L.debye_launch_info.restype = C.c_int
     L.debye_set_pairs_events.argtypes = [vp, vp]
     L.debye_set_pairs_events.restype = C.c_int
+    L.debye_plan_create.argtypes = [C.POINTER(vp), vp, i32, i32, i32, vp, i32, vp, u32, vp]
+    L.debye_plan_create.restype = C.c_int
+    L.debye_plan_execute.argtypes = [vp, vp, vp, vp, vp]
+    L.debye_plan_execute.restype = C.c_int
+    L.debye_plan_destroy.argtypes = [vp]
+    L.debye_plan_destroy.restype = None
     L.debye_q_hint.argtypes = [vp, i32]
     L.debye_q_hint.restype = u32
     L.debye_strerror.argtypes = [C.c_int]
@@ -154,6 +161,39 @@ def debye_profile_weighted_host(xyz, type, weight, fftab, q, I_out=None, variant
                                              _host(q, np.float32, "q"), M, _host(I_out, np.float64, "I_out"),
                                              _flags(variant, hint), _stream_ptr(stream)))
     return I_out
+
+
+class Plan:
+    """debye_plan_*: setup once for one molecule (type, q, optional weights, batch size), then execute(xyz, fftab) per
+    set of coordinates.  Creation synchronises the stream once; execute never does."""
+
+    def __init__(self, type, q, T, B=1, weight=None, variant="auto", stream=None):
+        import torch
+        self.N, self.M, self.T, self.B = type.shape[0], q.shape[0], T, B
+        self._h = C.c_void_p()
+        _check(lib().debye_plan_create(C.byref(self._h), _dev(type, torch.int32, "type"), self.N, B, T,
+                                       _dev(q, torch.float32, "q"), self.M,
+                                       _dev(weight, torch.float32, "weight") if weight is not None else None,
+                                       _flags(variant), _stream_ptr(stream)))
+
+    def execute(self, xyz, fftab, I_out=None, stream=None):
+        import torch
+        if I_out is None:
+            I_out = torch.empty((self.B, self.M) if xyz.dim() == 3 else self.M, dtype=torch.float64, device=xyz.device)
+        _check(lib().debye_plan_execute(self._h, _dev(xyz, torch.float32, "xyz"), _dev(fftab, torch.float32, "fftab"),
+                                        _dev(I_out, torch.float64, "I_out"), _stream_ptr(stream)))
+        return I_out
+
+    def destroy(self):
+        if self._h:
+            lib().debye_plan_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
 
 
 def debye_partials(xyz, type, q, T, variant="auto", stream=None):

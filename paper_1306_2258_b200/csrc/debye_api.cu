@@ -10,6 +10,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <cstddef>
 #include <cmath>
 #include <mutex>
 #include "../../include/debye.h"
@@ -239,9 +240,21 @@ int ensure(void **ptr, size_t *have, size_t need)
     return DEBYE_OK;
 }
 
+}  // namespace (reopened below)
+// A plan owns the device-resident result of the setup step (DevPlan, sort permutation) and copies of q and the weights, so
+// that repeated profiles of one molecule (only the coordinates change: refinement loops) skip the sort
+// and launch exactly the one pairs instantiation the grid needs.
+struct debye_plan {
+    int N, B, T, M, device;
+    uint32_t flags;              // the caller's flags with the grid hint resolved at creation
+    char *buf;                   // one allocation: DevPlan | perm[N] | q[M] | weight[N]
+    DevPlan *plan; int32_t *perm; float *q; float *weight;
+};
+namespace {
+
 // mode 0: I_out[B][M]; mode 1: S_out[B][n_tp][M] (+ n_out)
 int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab, int T, const float *q, int M, double *out, int32_t *n_out,
-        uint32_t flags, cudaStream_t stream, int mode, const float *weight = nullptr)
+        uint32_t flags, cudaStream_t stream, int mode, const float *weight = nullptr, const debye_plan *pre = nullptr)
 {
     int st = validate(xyz, type, N, B, mode == 0 ? (const void *)fftab : (const void *)q, T, q, M, out, flags);
     if (st) return st;
@@ -256,8 +269,8 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     char *ws;
     if (ds->user_ws) { if (ds->user_bytes < L.total) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
     else { if ((st = ensure(&ds->ws, &ds->ws_bytes, L.total))) return st; ws = (char *)ds->ws; }
-    DevPlan *plan = (DevPlan *)(ws + L.plan);
-    int32_t *perm = (int32_t *)(ws + L.perm);
+    DevPlan *plan = pre ? pre->plan : (DevPlan *)(ws + L.plan);
+    int32_t *perm = pre ? pre->perm : (int32_t *)(ws + L.perm);
     float4 *sorted = (float4 *)(ws + L.sorted);
     double *records = (double *)(ws + L.records);
 
@@ -269,13 +282,15 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
         Choice c2[2];
         alt_offered = (recur_choices(c2, M) == 2) ? 1 : 0;
     }
-    const bool pack_here = (int64_t)N * B <= DEBYE_PACK_IN_SETUP;      // small inputs: the setup CTA gathers too
-    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, hint_class, xyz, sorted, pack_here ? 1 : 0, weight);
+    const bool pack_here = !pre && (int64_t)N * B <= DEBYE_PACK_IN_SETUP;      // small inputs: the setup CTA gathers too
+    if (!pre) debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, hint_class, xyz, sorted, pack_here ? 1 : 0, weight);
     if (!pack_here) {
         int64_t total = (int64_t)N * B;
         int blocks = (int)((total + 255) / 256);
         if (blocks > ds->sms * 16) blocks = ds->sms * 16;
-        CU(launch_pdl(debye::debye_pack_kernel, dim3(blocks), dim3(256), stream, (const DevPlan *)plan, xyz, type, (const int32_t *)perm, sorted, N, B, weight));
+        // with a plan the pack kernel is the first kernel of the call: an ordinary launch (its pdl_wait returns at once)
+        if (pre) debye::debye_pack_kernel<<<blocks, 256, 0, stream>>>(plan, xyz, type, perm, sorted, N, B, weight);
+        else CU(launch_pdl(debye::debye_pack_kernel, dim3(blocks), dim3(256), stream, (const DevPlan *)plan, xyz, type, (const int32_t *)perm, sorted, N, B, weight));
     }
     if (weight) CU(launch_pdl(debye::debye_weight_sums_kernel, dim3(T), dim3(32), stream, plan, (const float4 *)sorted));
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
@@ -389,6 +404,59 @@ int debye_partials(const float *xyz, const int32_t *type, int32_t N, int32_t B, 
                    uint32_t flags, debye_stream_t stream)
 {
     return run(xyz, type, N, B, nullptr, T, q, M, S_out, n_out, flags, (cudaStream_t)stream, 1);
+}
+
+int debye_plan_create(debye_plan **out, const int32_t *type, int32_t N, int32_t B, int32_t T, const float *q, int32_t M, const float *weight, uint32_t flags,
+                      debye_stream_t stream_)
+{
+    static const char dummy = 0;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (!out) return DEBYE_EINVAL;
+    *out = nullptr;
+    int st = validate(&dummy, type, N, B, &dummy, T, q, M, &dummy, flags);
+    if (st) return st;
+    debye_plan *p = new debye_plan();
+    p->N = N; p->B = B; p->T = T; p->M = M; p->flags = flags; p->buf = nullptr;
+    auto fail = [&](int code) { if (p->buf) cudaFree(p->buf); delete p; return code; };
+    if (cudaGetDevice(&p->device) != cudaSuccess) return fail(DEBYE_ECUDA);
+    size_t o = 0;
+    const size_t o_plan = o; o += align_up(sizeof(DevPlan));
+    const size_t o_perm = o; o += align_up((size_t)N * 4);
+    const size_t o_q = o; o += align_up((size_t)M * 4);
+    const size_t o_w = o; o += align_up((size_t)N * 4);
+    if (cudaMalloc((void **)&p->buf, o) != cudaSuccess) { (void)cudaGetLastError(); p->buf = nullptr; return fail(DEBYE_ENOMEM); }
+    p->plan = (DevPlan *)(p->buf + o_plan); p->perm = (int32_t *)(p->buf + o_perm); p->q = (float *)(p->buf + o_q);
+    p->weight = weight ? (float *)(p->buf + o_w) : nullptr;
+    if (cudaMemcpyAsync(p->q, q, (size_t)M * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
+    if (weight && cudaMemcpyAsync(p->weight, weight, (size_t)N * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
+    // the setup step, once; then read its verdict on the grid back (the only synchronisation of the plan's life)
+    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(p->plan, type, p->q, p->perm, N, T, M, B, 1, -3, nullptr, nullptr, 0, p->weight);
+    DevPlan head;
+    if (cudaMemcpyAsync(&head, p->plan, offsetof(DevPlan, seg_off), cudaMemcpyDeviceToHost, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
+    if (cudaStreamSynchronize(stream) != cudaSuccess) return fail(DEBYE_ECUDA);
+    uint32_t hint = DEBYE_QHINT;
+    if (head.uniform) hint |= DEBYE_QHINT_UNIFORM;
+    if (head.uniform && head.zero_start == 0) hint |= DEBYE_QHINT_START0;
+    if (head.uniform && head.zero_start == 1) hint |= DEBYE_QHINT_STARTDQ;
+    p->flags = (flags & ~(uint32_t)(DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ)) | hint;
+    *out = p;
+    return DEBYE_OK;
+}
+
+int debye_plan_execute(debye_plan *p, const float *xyz, const float *fftab, double *I_out, debye_stream_t stream)
+{
+    static const int32_t dummy_type = 0;
+    if (!p) return DEBYE_EINVAL;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) return DEBYE_EINVAL;
+    return run(xyz, &dummy_type, p->N, p->B, fftab, p->T, p->q, p->M, I_out, nullptr, p->flags, (cudaStream_t)stream, 0, p->weight, p);
+}
+
+void debye_plan_destroy(debye_plan *p)
+{
+    if (!p) return;
+    if (p->buf) cudaFree(p->buf);
+    delete p;
 }
 
 uint32_t debye_q_hint(const float *q_host, int32_t M)

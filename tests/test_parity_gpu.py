@@ -345,3 +345,35 @@ def test_maximum_q_count_and_type_count(db):
             e = rel(gpu_profile(db, w, v), ref)
             assert e <= TOL32, (q_min, v, e)
         assert rel(gpu_profile(db, w, "fp64"), ref) <= TOL64
+
+
+def test_plan_execute_equals_the_plain_calls_bit_for_bit(db):
+    """debye_plan_* (include/debye.h): setup once, execute per set of coordinates; same kernels in the same order as the
+    plain calls, so the results are identical bit for bit -- for a grid from 0, the paper's grid, a non-uniform grid,
+    with weights, and for a batch."""
+    import torch
+    rng = np.random.default_rng(21)
+    grids = [wl.q_grid(0.5, 101), wl.q_grid(1.0, 50, 0.02), np.sort(rng.uniform(0.01, 0.7, 33)).astype(np.float32)]
+    for qg in grids:
+        base = wl.small_random(60, 900, 4, 8)
+        f = wl.gaussian_form_factors(5, 4, qg)
+        t, fd, qd = (torch.from_numpy(a).cuda() for a in (base.type, f, qg))
+        plan = db.Plan(t, qd, 4)
+        for rep in range(3):                                   # new coordinates, same plan
+            xyz = (base.xyz + rng.normal(0, 0.5, base.xyz.shape)).astype(np.float32)
+            x = torch.from_numpy(xyz).cuda()
+            a = plan.execute(x, fd).cpu().numpy()
+            b = db.debye_profile(x, t, fd, qd).cpu().numpy()
+            assert a.tobytes() == b.tobytes()
+            assert rel(a, orc.debye_sym(xyz, base.type, f, qg)) <= TOL32
+        plan.destroy()
+    # weights and a batch
+    wb = wl.cfg4(B=3, N=400)
+    wt = rng.uniform(0.5, 1.5, wb.N).astype(np.float32)
+    xb, t, fd, qd = to_dev(wb)
+    wd = torch.from_numpy(wt).cuda()
+    plan = db.Plan(t, qd, wb.T, B=3, weight=wd)
+    a = plan.execute(xb, fd).cpu().numpy()
+    assert a.tobytes() == db.debye_profile_weighted(xb, t, wd, fd, qd).cpu().numpy().tobytes()
+    assert rel(a, orc.debye_batch(wb.xyz, wb.type, wb.fftab, wb.q, weight=wt)) <= TOL32
+    plan.destroy()

@@ -31,8 +31,8 @@ METRIC = "pair_q_sinc_terms_per_second"
 UNIT = "G pair.q/s"
 SM_COUNT, FP32_LANES, MUFU_LANES = 148, 128, 16           # per B200 / per SM per clock (B200_PROFILING.md)
 # dram__bytes_read.sum + dram__bytes_write.sum of the pairs kernel, per launch, from the committed ncu --set full capture
-# (profiles/r01_ncu_full_pairs_recur_cfg2_v4.txt); None where no capture exists
-NCU_TRAFFIC = {("cfg2", "recur"): 239104}
+# (profiles/r01_ncu_full_pairs_recur_cfg{2,4,5}_v4.txt); None where no capture exists
+NCU_TRAFFIC = {("cfg2", "recur"): 239104, ("cfg4", "recur"): 32843264 + 163584, ("cfg5", "recur"): 3336192}
 
 
 def make_workload(name: str, rank: int = 0):

@@ -377,3 +377,16 @@ def test_plan_execute_equals_the_plain_calls_bit_for_bit(db):
     assert a.tobytes() == db.debye_profile_weighted(xb, t, wd, fd, qd).cpu().numpy().tobytes()
     assert rel(a, orc.debye_batch(wb.xyz, wb.type, wb.fftab, wb.q, weight=wt)) <= TOL32
     plan.destroy()
+
+
+def test_non_finite_input_propagates_and_does_not_poison_later_calls(db):
+    """include/debye.h: NaN / Inf in the inputs propagate to I_out (no hang, no crash); the next call is unaffected."""
+    w = wl.small_random(70, 500, 3, 40)
+    good = gpu_profile(db, w)
+    bad = wl.Workload("nan", w.xyz.copy(), w.type, w.fftab, w.q)
+    bad.xyz[17, 1] = np.nan
+    bad.xyz[300, 0] = np.inf
+    for v in ("auto", "mufu", "fp64"):
+        I = gpu_profile(db, bad, v)
+        assert not np.isfinite(I[1:]).any(), v               # every q > 0 involves the poisoned atoms
+    assert gpu_profile(db, w).tobytes() == good.tobytes()

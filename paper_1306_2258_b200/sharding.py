@@ -49,3 +49,37 @@ def gather_profiles(local, n_total: int, rank: int, world: int):
     bufs = [torch.empty_like(pad) for _ in range(world)]
     dist.all_gather(bufs, pad)
     return torch.cat([bufs[r][: hi - lo] for r, (lo, hi) in enumerate(sizes)], dim=0)
+
+
+# ---- one structure over several GPUs: split of the q grid ------------------------------------------------------------------
+# The paper's own multi-device idea (PAPER.md:170-172: different q ranges on different devices).  Every rank holds all atoms
+# and computes a contiguous slice of the q grid with the ordinary single-GPU call (distances are recomputed per rank, as in
+# the paper's proposal); the only exchange is an all-gather of the M/world profile values.  A contiguous slice of a uniform
+# grid is uniform, so every rank keeps the recurrence kernel.
+def q_slice(M: int, rank: int, world: int):
+    """[lo, hi) of the q grid owned by `rank`."""
+    return shard_range(M, rank, world)
+
+
+def profile_q_slice(profile_fn, fftab, q, rank: int, world: int):
+    """This rank's part of one profile: profile_fn(fftab[:, lo:hi], q[lo:hi]) -> values [hi - lo] (empty slices allowed).
+    `profile_fn` is the single-GPU call with xyz / type bound (e.g. lambda f, q: binding.debye_profile(xyz, type, f, q))."""
+    lo, hi = q_slice(q.shape[0], rank, world)
+    if hi == lo:
+        return fftab.new_zeros(0, dtype=__import__("torch").float64), (lo, hi)
+    return profile_fn(fftab[:, lo:hi].contiguous(), q[lo:hi].contiguous()), (lo, hi)
+
+
+def gather_q_slices(local, M: int, rank: int, world: int):
+    """All-gather the per-rank slices of one profile into the full [M] profile (every rank gets it)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or world == 1:
+        return local
+    sizes = [q_slice(M, r, world) for r in range(world)]
+    mx = max(hi - lo for lo, hi in sizes)
+    pad = torch.zeros(mx, dtype=local.dtype, device=local.device)
+    pad[: local.shape[0]] = local
+    bufs = [torch.empty_like(pad) for _ in range(world)]
+    dist.all_gather(bufs, pad)
+    return torch.cat([bufs[r][: hi - lo] for r, (lo, hi) in enumerate(sizes)], dim=0)

@@ -390,3 +390,23 @@ def test_non_finite_input_propagates_and_does_not_poison_later_calls(db):
         I = gpu_profile(db, bad, v)
         assert not np.isfinite(I[1:]).any(), v               # every q > 0 involves the poisoned atoms
     assert gpu_profile(db, w).tobytes() == good.tobytes()
+
+
+def test_q_grid_split_over_ranks_reassembles_the_profile(db):
+    """sharding.profile_q_slice (different q ranges on different devices), the ranks emulated one after
+    the other on one GPU: the slices tile the grid and agree with the unsplit profile and the oracle."""
+    import torch
+    from paper_1306_2258_b200 import sharding
+    w = wl.small_random(80, 1100, 4, 101)
+    x, t, f, q = to_dev(w)
+    ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)
+    whole = db.debye_profile(x, t, f, q).cpu().numpy()
+    fn = lambda ff, qq: db.debye_profile(x, t, ff, qq)
+    for world in (2, 3, 8):
+        parts, cover = [], []
+        for rank in range(world):
+            loc, (lo, hi) = sharding.profile_q_slice(fn, f, q, rank, world)
+            parts.append(loc.cpu().numpy()); cover += list(range(lo, hi))
+        I = np.concatenate(parts)
+        assert cover == list(range(w.M))
+        assert rel(I, ref) <= TOL32 and rel(I, whole) <= 1e-5

@@ -36,6 +36,13 @@ def _worker(rank, world, port, tmp):
     lo, hi = sharding.shard_range(w.B, rank, world)
     local = torch.from_numpy(orc.debye_batch(w.xyz[lo:hi], w.type, w.fftab, w.q))
     full = sharding.gather_profiles(local, w.B, rank, world)
+    # q-grid split of ONE structure: each rank computes a slice of q, the slices are gathered
+    one = wl.small_random(3, 90, 3, 23)
+    fn = lambda f, q: torch.from_numpy(orc.debye_sym(one.xyz, one.type, f.numpy(), q.numpy()))
+    loc, (qlo, qhi) = sharding.profile_q_slice(fn, torch.from_numpy(one.fftab), torch.from_numpy(one.q), rank, world)
+    fullq = sharding.gather_q_slices(loc, one.M, rank, world)
+    if rank == 0:
+        np.save(os.path.join(tmp, "fullq.npy"), fullq.numpy())
     t = sharding.max_over_ranks(1.0 + rank)
     s = sharding.sum_over_ranks(hi - lo)
     if rank == 0:
@@ -53,5 +60,7 @@ def test_two_rank_gloo_shards_and_gathers(tmp_path):
     full = np.load(tmp_path / "full.npy")
     assert full.shape == (5, w.M)
     assert np.array_equal(full, orc.debye_batch(w.xyz, w.type, w.fftab, w.q))
+    one = wl.small_random(3, 90, 3, 23)
+    assert np.array_equal(np.load(tmp_path / "fullq.npy"), orc.debye_sym(one.xyz, one.type, one.fftab, one.q))
     t, s = np.load(tmp_path / "ts.npy")
     assert t == 2.0 and s == 5.0

@@ -117,7 +117,9 @@ int debye_profile_weighted_host(const float *xyz, const int32_t *type, const flo
  * `stream` once to learn the shape of the grid, so that debye_plan_execute launches exactly pack + one pairs instantiation
  * + final, never synchronises, and gives bit for bit the result of debye_profile[_batch][_weighted] with the same inputs.
  *   type dev [N], q dev [M], weight dev [N] or NULL (read during create only); xyz dev [B][N][3], fftab dev [T][M],
- *   I_out dev [B][M].  A plan belongs to the device that was current at creation; destroy it with debye_plan_destroy. */
+ *   I_out dev [B][M].  A plan belongs to the device that was current at creation; destroy it with debye_plan_destroy once
+ *   the work that uses it has completed.  Like every call, executions share the per-device workspace and must not overlap
+ *   in time with other libdebye calls on the same device. */
 typedef struct debye_plan debye_plan_t;
 int debye_plan_create(debye_plan_t **plan, const int32_t *type, int32_t N, int32_t B, int32_t T, const float *q, int32_t M,
                       const float *weight, uint32_t flags, debye_stream_t stream);

@@ -134,6 +134,25 @@ void debye_plan_destroy(debye_plan_t *plan);
 int debye_partials(const float *xyz, const int32_t *type, int32_t N, int32_t B, const float *q, int32_t T,
                    int32_t M, double *S_out, int32_t *n_out, uint32_t flags, debye_stream_t stream);
 
+/* ONE structure (or batch) split over several GPUs by tiles of the upper triangle (the blocks of
+ * the j <= k triangle are independent; PAPER.md:170-172 proposes several devices for one profile).  Every rank holds all
+ * coordinates and calls debye_partials_shard with its own shard_rank in [0, shard_world): pairs CTA c of the static
+ * schedule works iff c % shard_world == shard_rank (cyclic, which keeps the triangular load balanced), so
+ *     sum over ranks of S_out == S_out of debye_partials     (same terms, same per-CTA FP32/FP64 sums; only the last FP64
+ * additions are regrouped).  Terms that have a closed form (q_m == 0: pair counts) are contributed by rank 0 alone.
+ * The one exchange step is an all-gather (or all-reduce) of S_out, [B][T(T+1)/2][M] float64 (<= 215 KB per conformer),
+ * done by the caller (NCCL); debye_profile_from_partials then sums the gathered parts in part order and applies the
+ * form-factor epilogue on the device:
+ *     I_out[b][m] = sum_a n_a F_a^2 + 2 sum_{p=(a<=b')} F_a F_b' sum_{r < n_parts} S_parts[r][b][p][m].
+ *   S_parts dev [n_parts][B][T(T+1)/2][M] float64, n_a dev [T] int32 (n_out of any rank), fftab dev [T][M], I_out dev [B][M].
+ * shard_world == 1 is debye_partials.  Unweighted only.  Errors: DEBYE_EINVAL for shard_rank outside [0, shard_world),
+ * shard_world / n_parts outside [1, 4096], B > 65535 (from_partials), otherwise as debye_partials. */
+int debye_partials_shard(const float *xyz, const int32_t *type, int32_t N, int32_t B, const float *q, int32_t T, int32_t M,
+                         double *S_out, int32_t *n_out, uint32_t flags, int32_t shard_rank, int32_t shard_world,
+                         debye_stream_t stream);
+int debye_profile_from_partials(const double *S_parts, int32_t n_parts, const int32_t *n_a, const float *fftab, int32_t B,
+                                int32_t T, int32_t M, double *I_out, debye_stream_t stream);
+
 /* Grid hint flags for a q grid given as HOST memory (the same classification the device applies); OR them into `flags`.
  * Returns 0 (no hint) for q_host == NULL or M < 1. */
 uint32_t debye_q_hint(const float *q_host, int32_t M);

@@ -16,7 +16,8 @@ LIB_PATH = os.path.join(HERE, "libdebye.so")
 FLAGS = {"fp64": 1 << 0, "mufu": 1 << 2, "recur": 1 << 3, "accurate": 1 << 4, "auto": 0}
 
 EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_profile_batch_host",
-           "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
+           "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials",
+           "debye_partials_shard", "debye_profile_from_partials", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
            "debye_launch_info", "debye_set_pairs_events", "debye_q_hint", "debye_plan_create", "debye_plan_execute",
            "debye_plan_destroy", "debye_strerror", "debye_last_cuda_error", "debye_version")
 
@@ -46,11 +47,14 @@ def lib():
     L.debye_profile_batch.argtypes = [vp, vp, i32, i32, vp, i32, vp, i32, vp, u32, vp]
     L.debye_profile_batch_host.argtypes = L.debye_profile_batch.argtypes
     L.debye_partials.argtypes = [vp, vp, i32, i32, vp, i32, i32, vp, vp, u32, vp]
+    L.debye_partials_shard.argtypes = [vp, vp, i32, i32, vp, i32, i32, vp, vp, u32, i32, i32, vp]
+    L.debye_profile_from_partials.argtypes = [vp, i32, vp, vp, i32, i32, i32, vp, vp]
     L.debye_profile_weighted.argtypes = [vp, vp, vp, i32, vp, i32, vp, i32, vp, u32, vp]
     L.debye_profile_weighted_host.argtypes = L.debye_profile_weighted.argtypes
     L.debye_profile_batch_weighted.argtypes = [vp, vp, vp, i32, i32, vp, i32, vp, i32, vp, u32, vp]
     for n in ("debye_profile", "debye_profile_host", "debye_profile_batch", "debye_profile_batch_host",
-              "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials"):
+              "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials",
+              "debye_partials_shard", "debye_profile_from_partials"):
         getattr(L, n).restype = C.c_int
     L.debye_workspace_bytes.argtypes = [i32, i32, i32, i32, u32]
     L.debye_workspace_bytes.restype = sz
@@ -207,6 +211,36 @@ def debye_partials(xyz, type, q, T, variant="auto", stream=None):
                                 _dev(q, torch.float32, "q"), T, M, _dev(S, torch.float64, "S_out"),
                                 _dev(n, torch.int32, "n_out"), _flags(variant), _stream_ptr(stream)))
     return S, n
+
+
+def debye_partials_shard(xyz, type, q, T, shard_rank, shard_world, variant="auto", stream=None, hint=0):
+    """This rank's part of debye_partials when ONE structure is split over `shard_world` GPUs by tiles (pairs CTA c works
+    iff c % shard_world == shard_rank): (S_part[B,T(T+1)/2,M] float64, n[T] int32).  The parts of all ranks sum to S."""
+    import torch
+    x3 = xyz if xyz.dim() == 3 else xyz[None]
+    B, N, M = x3.shape[0], x3.shape[1], q.shape[0]
+    S = torch.empty((B, T * (T + 1) // 2, M), dtype=torch.float64, device=xyz.device)
+    n = torch.empty(T, dtype=torch.int32, device=xyz.device)
+    _check(lib().debye_partials_shard(_dev(x3, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N, B,
+                                      _dev(q, torch.float32, "q"), T, M, _dev(S, torch.float64, "S_out"),
+                                      _dev(n, torch.int32, "n_out"), _flags(variant, hint), int(shard_rank), int(shard_world),
+                                      _stream_ptr(stream)))
+    return S, n
+
+
+def debye_profile_from_partials(S_parts, n, fftab, I_out=None, stream=None):
+    """I_out[B,M] from gathered parts S_parts[n_parts,B,T(T+1)/2,M] (summed in part order on the device), n[T], fftab[T,M]."""
+    import torch
+    n_parts, B, n_tp, M = S_parts.shape
+    T = fftab.shape[0]
+    if n_tp != T * (T + 1) // 2 or fftab.shape[1] != M or n.shape[0] != T:
+        raise LibdebyeError("S_parts / n / fftab shapes do not agree")
+    if I_out is None:
+        I_out = torch.empty((B, M), dtype=torch.float64, device=S_parts.device)
+    _check(lib().debye_profile_from_partials(_dev(S_parts, torch.float64, "S_parts"), n_parts, _dev(n, torch.int32, "n"),
+                                             _dev(fftab, torch.float32, "fftab"), B, T, M,
+                                             _dev(I_out, torch.float64, "I_out"), _stream_ptr(stream)))
+    return I_out
 
 
 def _host(a, dtype, name):

@@ -254,7 +254,8 @@ namespace {
 
 // mode 0: I_out[B][M]; mode 1: S_out[B][n_tp][M] (+ n_out)
 int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab, int T, const float *q, int M, double *out, int32_t *n_out,
-        uint32_t flags, cudaStream_t stream, int mode, const float *weight = nullptr, const debye_plan *pre = nullptr)
+        uint32_t flags, cudaStream_t stream, int mode, const float *weight = nullptr, const debye_plan *pre = nullptr, int shard_rank = 0,
+        int shard_world = 1)
 {
     int st = validate(xyz, type, N, B, mode == 0 ? (const void *)fftab : (const void *)q, T, q, M, out, flags);
     if (st) return st;
@@ -283,7 +284,10 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
         alt_offered = (recur_choices(c2, M) == 2) ? 1 : 0;
     }
     const bool pack_here = !pre && (int64_t)N * B <= DEBYE_PACK_IN_SETUP;      // small inputs: the setup CTA gathers too
-    if (!pre) debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, hint_class, xyz, sorted, pack_here ? 1 : 0, weight);
+    // tile split over GPUs: the pairs CTAs of the other ranks do not run here; their records must read as zero
+    if (shard_world > 1) CU(cudaMemsetAsync(records, 0, L.total - L.records, stream));
+    if (!pre) debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, hint_class, xyz, sorted, pack_here ? 1 : 0, weight,
+                                                                                shard_rank, shard_world);
     if (!pack_here) {
         int64_t total = (int64_t)N * B;
         int blocks = (int)((total + 255) / 256);
@@ -295,7 +299,8 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     if (weight) CU(launch_pdl(debye::debye_weight_sums_kernel, dim3(T), dim3(32), stream, plan, (const float4 *)sorted));
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
     for (int i = 0; i < nch; ++i) {
-        debye_pairs_fn fn = debye_get_pairs_kernel(ch[i].variant, ch[i].K, weight != nullptr);
+        debye_pairs_fn fn = debye_get_pairs_kernel(ch[i].variant, ch[i].K, weight != nullptr, shard_world > 1);
+        if (!fn) return DEBYE_EUNSUPPORTED;
         // slow-path threshold on theta = r * (smallest grid step or smallest |q|): see DESIGN.md section 6
         const float theta_min = (ch[i].variant == V_RECUR) ? 0.002f : 0.004f;
         CU(launch_pdl(fn, dim3(G[i]), dim3(DEBYE_IB), stream, (const DevPlan *)plan, (const float4 *)sorted, q, records, ch[i].n_chunks, is_auto, theta_min, ch[i].alt_gate));
@@ -406,6 +411,23 @@ int debye_partials(const float *xyz, const int32_t *type, int32_t N, int32_t B, 
     return run(xyz, type, N, B, nullptr, T, q, M, S_out, n_out, flags, (cudaStream_t)stream, 1);
 }
 
+int debye_partials_shard(const float *xyz, const int32_t *type, int32_t N, int32_t B, const float *q, int32_t T, int32_t M, double *S_out, int32_t *n_out,
+                         uint32_t flags, int32_t shard_rank, int32_t shard_world, debye_stream_t stream)
+{
+    if (shard_world < 1 || shard_world > 4096 || shard_rank < 0 || shard_rank >= shard_world) return DEBYE_EINVAL;
+    return run(xyz, type, N, B, nullptr, T, q, M, S_out, n_out, flags, (cudaStream_t)stream, 1, nullptr, nullptr, shard_rank, shard_world);
+}
+
+int debye_profile_from_partials(const double *S_parts, int32_t n_parts, const int32_t *n_a, const float *fftab, int32_t B, int32_t T, int32_t M, double *I_out,
+                                debye_stream_t stream)
+{
+    if (!S_parts || !n_a || !fftab || !I_out) return DEBYE_EINVAL;
+    if (n_parts < 1 || n_parts > 4096 || B < 1 || B > 65535 || T < 1 || T > DEBYE_MAX_TYPES || M < 1 || M > DEBYE_MAX_Q) return DEBYE_EINVAL;
+    debye::debye_combine_kernel<<<dim3((M + 127) / 128, B), 128, 0, (cudaStream_t)stream>>>(S_parts, n_parts, n_a, fftab, B, T, M, I_out);
+    CU(cudaGetLastError());
+    return DEBYE_OK;
+}
+
 int debye_plan_create(debye_plan **out, const int32_t *type, int32_t N, int32_t B, int32_t T, const float *q, int32_t M, const float *weight, uint32_t flags,
                       debye_stream_t stream_)
 {
@@ -430,7 +452,7 @@ int debye_plan_create(debye_plan **out, const int32_t *type, int32_t N, int32_t 
     if (cudaMemcpyAsync(p->q, q, (size_t)M * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
     if (weight && cudaMemcpyAsync(p->weight, weight, (size_t)N * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
     // the setup step, once; then read its verdict on the grid back (the only synchronisation of the plan's life)
-    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(p->plan, type, p->q, p->perm, N, T, M, B, 1, -3, nullptr, nullptr, 0, p->weight);
+    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(p->plan, type, p->q, p->perm, N, T, M, B, 1, -3, nullptr, nullptr, 0, p->weight, 0, 1);
     DevPlan head;
     if (cudaMemcpyAsync(&head, p->plan, offsetof(DevPlan, seg_off), cudaMemcpyDeviceToHost, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
     if (cudaStreamSynchronize(stream) != cudaSuccess) return fail(DEBYE_ECUDA);

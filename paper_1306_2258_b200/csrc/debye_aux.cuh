@@ -21,7 +21,8 @@ namespace debye {
 __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPlan *plan, const int32_t *__restrict__ type, const float *__restrict__ q,
                                                                             int32_t *__restrict__ perm, int N, int T, int M, int B, int alt_offered /* a recurrence launch sized for M - 1 indices exists */,
                                                                             int hint_class /* -3: no hint; else the grid class the caller promised (debye_grid_class) */,
-                                                                            const float *__restrict__ xyz, float4 *__restrict__ sorted, int pack_here, const float *__restrict__ weight)
+                                                                            const float *__restrict__ xyz, float4 *__restrict__ sorted, int pack_here, const float *__restrict__ weight,
+                                                                            int shard_rank, int shard_world)
 {
     pdl_trigger();                         // first kernel of the call: lets the next grid be staged (it waits for our completion)
     constexpr int NWARP = DEBYE_SETUP_THREADS / 32;
@@ -86,6 +87,7 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
         plan->recur_alt = (koff == 0 && alt_offered) ? 1 : 0;
         plan->N = N; plan->T = T; plan->M = M; plan->B = B; plan->n_tp = T * (T + 1) / 2;
         plan->weighted = weight ? 1 : 0;
+        plan->shard_rank = shard_rank; plan->shard_world = shard_world;
         plan->uniform = uni;
         plan->zero_start = koff;
         plan->q0 = q0;
@@ -243,7 +245,8 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
                 // sum over the pairs of w_i w_j sinc(0): the pair count, or with weights sw_a sw_b resp. (sw_a^2 - sw2_a) / 2
                 double cnt = pair_count(plan->n_a[a], plan->n_a[b2], a == b2);
                 if (plan->weighted && units != 0) cnt = (a == b2) ? 0.5 * (plan->sw[a] * plan->sw[a] - plan->sw2[a]) : plan->sw[a] * plan->sw[b2];
-                S = (sl == 0) ? cnt : 0.0;
+                // tile split over GPUs: the closed-form terms are nobody's tile, rank 0 contributes them
+                S = (sl == 0 && plan->shard_rank == 0) ? cnt : 0.0;
             }
             else {
                 const int64_t ub = (int64_t)b * Uc + plan->tp_prefix[tp] * n_chunks + (int64_t)ch * units;
@@ -280,6 +283,32 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
         for (int x = 0; x < DEBYE_FINAL_G * DEBYE_FINAL_NS; ++x) tot += part[x][kk];
         out[(int64_t)b * M + k] = tot;
     }
+}
+
+// Tile split of one structure over GPUs, the step after the exchange: S_parts[p][b][tp][k] are the partial
+// structure factors of n_parts ranks (debye_partials_shard, gathered into one buffer).  One thread per (conformer, q index):
+// S_ab = sum over parts in part order (fixed order: bitwise reproducible for a given number of ranks), then the same
+// epilogue as debye_final_kernel, I = sum_a n_a F_a^2 + 2 sum_{a<=b} F_a F_b S_ab with type pairs in increasing order.
+__global__ void __launch_bounds__(128) debye_combine_kernel(const double *__restrict__ S_parts, int n_parts, const int32_t *__restrict__ n_a,
+                                                              const float *__restrict__ fftab, int B, int T, int M, double *__restrict__ out)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y;
+    if (k >= M) return;
+    const int n_tp = T * (T + 1) / 2;
+    const int64_t part_stride = (int64_t)B * n_tp * M;
+    double tot = 0.0;
+    for (int a = 0; a < T; ++a) { const double fa = (double)fftab[a * M + k]; tot += (double)n_a[a] * fa * fa; }
+    int tp = 0;
+    for (int a = 0; a < T; ++a) {
+        const double fa = (double)fftab[a * M + k];
+        for (int b2 = a; b2 < T; ++b2, ++tp) {
+            const double *sp = S_parts + ((int64_t)b * n_tp + tp) * M + k;
+            double S = 0.0;
+            for (int p = 0; p < n_parts; ++p) S += sp[p * part_stride];
+            tot += 2.0 * fa * (double)fftab[b2 * M + k] * S;
+        }
+    }
+    out[(int64_t)b * M + k] = tot;
 }
 
 }  // namespace debye

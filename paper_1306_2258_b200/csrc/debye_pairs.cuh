@@ -485,7 +485,7 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
 #ifdef DEBYE_TRACE
 __device__ unsigned long long debye_trace[3 * 4096];
 #endif
-template <int K, int VAR, bool W>
+template <int K, int VAR, bool W, bool SH = false>
 __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR ? recur_min_ctas(K) : (K <= 64 ? 4 : (K <= 112 ? 3 : 2)))) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
                                                                double *__restrict__ records, int n_chunks, int is_auto, float theta_min, int alt_gate)
 {
@@ -518,6 +518,11 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
     const int64_t u0 = debye_range_begin(U, c, G);
     const int64_t u1 = (c + 1 == G) ? U : debye_range_begin(U, c + 1, G);
     if (u0 >= u1) return;
+    // tile split of one structure over GPUs (cyclic, which keeps the triangular load balanced): the records of
+    // the CTAs that belong to other ranks were zeroed by the host-side memset of debye_partials_shard.  A template parameter,
+    // so that the single-GPU instantiations stay instruction for instruction what they were (their register allocation
+    // decides +- 4 %: the same test as a run-time branch cost cfg2 0.614 -> 0.587).
+    if constexpr (SH) { if (c % plan->shard_world != plan->shard_rank) return; }
 
 #ifdef DEBYE_TRACE      // working builds only: per-CTA start / end time and SM id
     if (tid == 0) { unsigned long long t; unsigned sm; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); asm volatile("mov.u32 %0, %%smid;" : "=r"(sm)); debye_trace[3 * c] = t; debye_trace[3 * c + 2] = sm; }

@@ -28,6 +28,8 @@ struct DevPlan {
     float q_small;                // smallest non-zero |q|
     int32_t hint_bad;             // the caller's grid hint (DEBYE_QHINT_*) contradicts q: nothing is computed, the output is NaN
     int32_t weighted;             // per-atom weights given (debye_profile_weighted): sorted[].w holds w_j, else 1
+    int32_t shard_rank, shard_world;   // tile split of ONE structure over GPUs (debye_partials_shard): pairs CTA c works iff
+                                  // c % shard_world == shard_rank; the other CTAs leave their (zeroed) records alone
     int64_t U1;                   // units per conformer and per q-chunk
     double sw[DEBYE_MAX_TYPES_I];             // weighted calls: sum of w_j over the atoms of each type ...
     double sw2[DEBYE_MAX_TYPES_I];            // ... and of w_j^2 (self terms; q = 0 pair sums)

@@ -9,4 +9,5 @@ typedef void (*debye_pairs_fn)(const DevPlan *, const float4 *, const float *, d
 #define DEBYE_KMAX_F64 32
 
 // K must be a multiple of 8 in [8, KMAX] (recurrence: a multiple of 4); returns nullptr otherwise
-debye_pairs_fn debye_get_pairs_kernel(int variant, int K, bool weighted);
+// sharded: the instantiation whose CTAs skip the tiles of other ranks (debye_partials_shard; unweighted only)
+debye_pairs_fn debye_get_pairs_kernel(int variant, int K, bool weighted, bool sharded = false);

@@ -83,3 +83,29 @@ def gather_q_slices(local, M: int, rank: int, world: int):
     bufs = [torch.empty_like(pad) for _ in range(world)]
     dist.all_gather(bufs, pad)
     return torch.cat([bufs[r][: hi - lo] for r, (lo, hi) in enumerate(sizes)], dim=0)
+
+
+# ---- one structure over several GPUs: split by tiles of the upper triangle ---------------------------------------------------
+# tiles are independent units, every GPU holds all coordinates (<= 3.2 MB), pairs CTA c of the static
+# schedule belongs to rank c mod world (cyclic keeps the triangular load balanced), and the one exchange step is an
+# all-gather of the FP64 partial structure factors S_ab[T(T+1)/2][M] (<= 215 KB per conformer) followed by a fixed-order sum
+# (bitwise reproducible for a given world size) and the form-factor epilogue, both inside debye_profile_from_partials.
+# Unlike the q-range split above, no distance is computed twice.
+def gather_partials(S_part, world: int):
+    """All-gather [B, n_tp, M] parts into [world, B, n_tp, M] in rank order (identity reshape without a process group)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or world == 1:
+        return S_part[None].contiguous()
+    out = torch.empty((world,) + tuple(S_part.shape), dtype=S_part.dtype, device=S_part.device)
+    dist.all_gather(list(out.unbind(0)), S_part.contiguous())   # views of one buffer: rank order, no extra copy
+    return out
+
+
+def profile_tile_split(partials_shard_fn, from_partials_fn, fftab, rank: int, world: int):
+    """One profile of one structure (or batch) on `world` GPUs: partials_shard_fn(rank, world) -> (S_part, n) is this rank's
+    tile share (binding.debye_partials_shard with xyz / type / q bound), the parts are all-gathered, and
+    from_partials_fn(S_parts, n, fftab) -> I[B, M] (binding.debye_profile_from_partials) sums them in rank order and applies
+    the epilogue.  Every rank returns the full profile."""
+    S_part, n = partials_shard_fn(rank, world)
+    return from_partials_fn(gather_partials(S_part, world), n, fftab)

@@ -410,3 +410,69 @@ def test_q_grid_split_over_ranks_reassembles_the_profile(db):
         I = np.concatenate(parts)
         assert cover == list(range(w.M))
         assert rel(I, ref) <= TOL32 and rel(I, whole) <= 1e-5
+
+
+def test_tile_split_over_ranks_sums_to_the_whole_and_matches_the_oracle(db):
+    """debye_partials_shard / debye_profile_from_partials (tiles of the upper triangle cyclic over ranks, one
+    all-gather of FP64 partials, fixed-order sum + epilogue on the device), the ranks emulated one after the other on one
+    GPU (they do not wait on one another).  Every variant; grids that contain q = 0 (closed-form term: rank 0 only),
+    start at dq, are offset, or are not uniform; a batch; more ranks than the small case has busy CTAs."""
+    import torch
+    from paper_1306_2258_b200 import sharding
+    cases = [
+        (wl.small_random(81, 1300, 4, 101), False),
+        (wl.small_random(82, 700, 3, 129, q_min=0.005, q_max=0.645), False),
+        (wl.small_random(83, 900, 5, 64, q_min=0.3, q_max=0.9), False),
+        (wl.cfg4(B=3, N=500), True),
+    ]
+    for w, batch in cases:
+        x, t, f, q = to_dev(w)
+        ref = orc.debye_batch(w.xyz, w.type, w.fftab, w.q) if batch else orc.debye_sym(w.xyz, w.type, w.fftab, w.q)[None]
+        for variant in ("auto", "mufu", "fp64"):
+            tol = TOL64 if variant == "fp64" else TOL32
+            S_full, n_full = db.debye_partials(x, t, q, w.T, variant=variant)
+            whole = (db.debye_profile_batch if batch else db.debye_profile)(x, t, f, q, variant=variant).cpu().numpy().reshape(ref.shape)
+            for world in (1, 2, 3, 8):
+                parts = []
+                for rank in range(world):
+                    S, n = db.debye_partials_shard(x, t, q, w.T, rank, world, variant=variant)
+                    assert torch.equal(n, n_full)
+                    parts.append(S)
+                S_parts = torch.stack(parts)
+                if world > 1:       # nobody's share is the whole thing, and the shares add up to it
+                    assert sum(float(p.abs().sum()) > 0 for p in parts) >= 2
+                tot = S_parts.sum(0)
+                assert float(((tot - S_full).abs() / (S_full.abs() + 1e-300)).max()) <= (1e-12 if world > 1 else 0.0)
+                I = db.debye_profile_from_partials(S_parts, n_full, f).cpu().numpy()
+                assert I.shape == ref.shape
+                assert rel(I, ref) <= tol and rel(I, whole) <= 1e-11
+                # through the sharding helper (no process group: the gather is the identity for world == 1)
+                if world == 1:
+                    I1 = sharding.profile_tile_split(lambda r, wd: db.debye_partials_shard(x, t, q, w.T, r, wd, variant=variant),
+                                                     db.debye_profile_from_partials, f, 0, 1).cpu().numpy()
+                    assert np.array_equal(I1, I)
+    # a non-uniform grid with an explicit q = 0 in the middle (MUFU kernel chosen on the device)
+    w = wl.small_random(84, 600, 3, 33)
+    qn = np.sort(np.random.default_rng(84).uniform(0.01, 0.6, w.M)).astype(np.float32); qn[7] = 0.0
+    w2 = wl.Workload("nonuniform", w.xyz, w.type, w.fftab, qn)
+    x, t, f, q = to_dev(w2)
+    ref = orc.debye_sym(w2.xyz, w2.type, w2.fftab, w2.q)
+    parts = torch.stack([db.debye_partials_shard(x, t, q, w2.T, r, 4)[0] for r in range(4)])
+    n = db.debye_partials(x, t, q, w2.T)[1]
+    assert rel(db.debye_profile_from_partials(parts, n, f).cpu().numpy()[0], ref) <= TOL32
+    # repeated calls are bitwise identical, and an unsharded call afterwards is not disturbed by the zeroed records
+    a = db.debye_partials_shard(x, t, q, w2.T, 1, 4)[0]
+    assert torch.equal(a, parts[1])
+    assert rel(db.debye_profile(x, t, f, q).cpu().numpy(), ref) <= TOL32
+
+
+def test_tile_split_argument_validation(db):
+    import torch
+    w = wl.small_random(85, 200, 2, 11)
+    x, t, f, q = to_dev(w)
+    for rank, world in ((-1, 2), (2, 2), (0, 0), (0, 5000)):
+        with pytest.raises(db.LibdebyeError):
+            db.debye_partials_shard(x, t, q, w.T, rank, world)
+    S, n = db.debye_partials(x, t, q, w.T)
+    with pytest.raises(db.LibdebyeError):
+        db.debye_profile_from_partials(S[None][:, :, :2].contiguous(), n, f)

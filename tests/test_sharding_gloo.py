@@ -43,6 +43,11 @@ def _worker(rank, world, port, tmp):
     fullq = sharding.gather_q_slices(loc, one.M, rank, world)
     if rank == 0:
         np.save(os.path.join(tmp, "fullq.npy"), fullq.numpy())
+    # tile split of ONE structure: each rank contributes partial sums, all-gathered in rank order
+    part = torch.full((2, 3, 7), float(rank + 1), dtype=torch.float64) * torch.arange(7, dtype=torch.float64)
+    allp = sharding.gather_partials(part, world)
+    if rank == 1:
+        np.save(os.path.join(tmp, "allp.npy"), allp.numpy())
     t = sharding.max_over_ranks(1.0 + rank)
     s = sharding.sum_over_ranks(hi - lo)
     if rank == 0:
@@ -62,5 +67,9 @@ def test_two_rank_gloo_shards_and_gathers(tmp_path):
     assert np.array_equal(full, orc.debye_batch(w.xyz, w.type, w.fftab, w.q))
     one = wl.small_random(3, 90, 3, 23)
     assert np.array_equal(np.load(tmp_path / "fullq.npy"), orc.debye_sym(one.xyz, one.type, one.fftab, one.q))
+    allp = np.load(tmp_path / "allp.npy")
+    assert allp.shape == (2, 2, 3, 7)
+    for r in range(2):
+        assert np.array_equal(allp[r], np.broadcast_to((r + 1) * np.arange(7.0), (2, 3, 7)))
     t, s = np.load(tmp_path / "ts.npy")
     assert t == 2.0 and s == 5.0

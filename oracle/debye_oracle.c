@@ -18,6 +18,9 @@
  *   R10 form factors are given per atom TYPE: f_j(q_m) = fftab[type[j]][m]  (north_star narrowing).
  *   R10w optional per-atom weights (the one-parameter family of the paper's per-atom form factors,
  *        PAPER.md:44, 82): f_j(q_m) = weight[j] * fftab[type[j]][m]; weight == NULL means 1.
+ *   R10p the paper's own general case (the form factor depends on the atom and its environment, the
+ *        GPU kernel's input is "the form factors for each atom at Q values of q"): f_j(q_m) = ff[j][m], one table row per
+ *        ATOM (oracle_debye_peratom).
  * Inputs are the same float32 / int32 bytes the GPU gets, promoted exactly to double.
  *
  * Pins (tests/test_oracle_pins.py): two-atom closed form, I(0) = (sum f)^2, Eq. (1) by spherical quadrature,
@@ -136,6 +139,45 @@ int32_t oracle_debye_sym_w(const float *xyz, const int32_t *type, const float *w
     }
     free(tot);
     return nthr;
+}
+
+/* Reading R10p: Eq. (2) with per-ATOM form factors ff[N][M], written as the definition over the full
+ * N x N double loop including j == k when sym == 0, and as  sum_k f_k (f_k + 2 sum_{j>k} f_j sinc) with
+ * OpenMP over rows when sym != 0.  No types, no weights: ff[j][m] is used as given. */
+void oracle_debye_peratom(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, int32_t sym,
+                          double *I, double *Abs)
+{
+    if (!sym) {
+        for (int m = 0; m < M; ++m) {
+            long double acc = 0.0L, aabs = 0.0L;
+            for (int k = 0; k < N; ++k)
+                for (int j = 0; j < N; ++j) {
+                    double term = (double)ff[(size_t)k * M + m] * (double)ff[(size_t)j * M + m] *
+                                  sinc((double)q[m] * dist(xyz + 3 * k, xyz + 3 * j));
+                    acc += term;
+                    aabs += fabs(term);
+                }
+            I[m] = (double)acc;
+            if (Abs) Abs[m] = (double)aabs;
+        }
+        return;
+    }
+    for (int m = 0; m < M; ++m) {
+        long double acc = 0.0L, aabs = 0.0L;
+#pragma omp parallel for schedule(static, 1) reduction(+ : acc, aabs)
+        for (int k = 0; k < N; ++k) {
+            double fk = (double)ff[(size_t)k * M + m], row = 0.0, rabs = 0.0;
+            for (int j = k + 1; j < N; ++j) {
+                double t = (double)ff[(size_t)j * M + m] * sinc((double)q[m] * dist(xyz + 3 * k, xyz + 3 * j));
+                row += t;
+                rabs += fabs(t);
+            }
+            acc += (long double)(fk * fk) + 2.0L * (long double)fk * (long double)row;
+            aabs += (long double)(fk * fk) + 2.0L * (long double)fabs(fk) * (long double)rabs;
+        }
+        I[m] = (double)acc;
+        if (Abs) Abs[m] = (double)aabs;
+    }
 }
 
 /* Eq. (1): I(q) = < | sum_j f_j exp(i q.r_j) |^2 >_Omega by brute-force quadrature over

@@ -31,6 +31,8 @@ def _L():
         _lib.oracle_debye_sym_w.argtypes = [fp, ip, fp, C.c_int32, fp, C.c_int32, fp, C.c_int32, C.c_int32, C.c_int32,
                                             C.c_int32, dp, dp]
         _lib.oracle_debye_sym_w.restype = C.c_int32
+        _lib.oracle_debye_peratom.argtypes = [fp, fp, C.c_int32, fp, C.c_int32, C.c_int32, dp, dp]
+        _lib.oracle_debye_peratom.restype = None
         _lib.oracle_eq1_quadrature.argtypes = [dp, dp, C.c_int32, C.c_double, dp, dp, C.c_int32]
         _lib.oracle_eq1_quadrature.restype = C.c_double
     return _lib
@@ -102,6 +104,20 @@ def debye_sym(xyz, typ, fftab, q, rows=None, threads=0, return_abs=False, return
 def debye_batch(xyz_b, typ, fftab, q, threads=0, weight=None):
     """Eq. (2) for each conformer of xyz_b[B][N][3] (shared type / fftab / q / weight)."""
     return np.stack([debye_sym(x, typ, fftab, q, threads=threads, weight=weight) for x in xyz_b])
+
+
+def debye_peratom(xyz, ff, q, sym=True, return_abs=False):
+    """Eq. (2) with per-ATOM form factors ff[N][M] (reading R10p).  sym=False: the full N x N loop,
+    single thread; sym=True: sum_k f_k (f_k + 2 sum_{j>k} f_j sinc), OpenMP over rows."""
+    xyz = np.ascontiguousarray(xyz, dtype=np.float32)
+    ff = np.ascontiguousarray(ff, dtype=np.float32)
+    q = np.ascontiguousarray(q, dtype=np.float32)
+    assert xyz.ndim == 2 and xyz.shape[1] == 3 and ff.shape == (xyz.shape[0], q.shape[0])
+    M = q.shape[0]
+    I, A = np.zeros(M), np.zeros(M)
+    _L().oracle_debye_peratom(_p(xyz, C.c_float), _p(ff, C.c_float), xyz.shape[0], _p(q, C.c_float), M, 1 if sym else 0,
+                              _p(I, C.c_double), _p(A, C.c_double))
+    return (I, A) if return_abs else I
 
 
 def eq1_quadrature(x, f, qval, n=None):

@@ -207,3 +207,64 @@ def test_weighted_oracle_pins():
     # (5) I(0) = (sum_j w_j f_j(0))^2
     I = orc.debye_sym(xyz, typ, f, q, weight=w)
     assert abs(I[0] - (w.astype(np.float64) * F[typ, 0]).sum() ** 2) <= 1e-12 * I[0]
+
+
+def test_peratom_oracle_pins():
+    """oracle_debye_peratom (reading R10p: one form-factor row per ATOM) against what the paper and the
+    mathematics fix: the two-atom closed form with two different atoms, I(0) = (sum_j f_j(0))^2, Eq. (1) by spherical
+    quadrature with a different form factor on every atom, the reduction to the per-type oracle when the rows are copies
+    of a type table, separability (f_j(q) = w_j g(q) gives g^2 times the profile of point scatterers w_j), the triangle
+    closed form, invariance under a permutation that moves the rows with the atoms, full == sym."""
+    rng = np.random.default_rng(77)
+    # two atoms, different per-atom rows, one negative
+    d = 4.3
+    xyz = np.array([[1.0, 2.0, -0.5], [1.0, 2.0 + d, -0.5]], dtype=np.float32)
+    dd = float(np.float64(xyz[1, 1]) - np.float64(xyz[0, 1]))
+    q = np.array([0.0, 0.02, 0.3, 0.9, 2.5], dtype=np.float32)
+    ff = np.array([[7.0, 6.9, 5.5, 3.0, 1.0], [-2.0, -1.9, -1.5, -0.8, -0.1]], dtype=np.float32)
+    qq = q.astype(np.float64)
+    s = np.where(qq == 0, 1.0, np.sin(qq * dd) / np.where(qq == 0, 1.0, qq * dd))
+    f1, f2 = ff[0].astype(np.float64), ff[1].astype(np.float64)
+    want = f1 ** 2 + f2 ** 2 + 2 * f1 * f2 * s
+    for sym in (False, True):
+        assert rel(orc.debye_peratom(xyz, ff, q, sym=sym), want) < RT
+    # a transposed table read (ff[m][j] instead of ff[j][m]) or a shifted q index would fail the next three
+    N, M = 18, 4
+    x = rng.uniform(-10, 10, (N, 3)).astype(np.float32)
+    q = np.array([0.0, 0.21, 0.6, 1.1], dtype=np.float32)
+    ff = rng.uniform(-1, 6, (N, M)).astype(np.float32)
+    I = orc.debye_peratom(x, ff, q)
+    assert rel(I, orc.debye_peratom(x, ff, q, sym=False)) < RT
+    assert abs(I[0] - ff[:, 0].astype(np.float64).sum() ** 2) < RT * I[0]                 # I(0) = (sum f)^2
+    for m in range(1, M):                                                                   # Eq. (1), PAPER.md:37-39
+        I1 = orc.eq1_quadrature(x.astype(np.float64), ff[:, m].astype(np.float64), float(q[m]))
+        assert abs(I1 - I[m]) <= 1e-9 * abs(I[m])
+    perm = rng.permutation(N)
+    assert rel(orc.debye_peratom(x[perm], ff[perm], q), I) < 1e-11
+    # rows copied from a type table: the per-type oracle (R10)
+    w = wl.small_random(78, 150, 4, 9, signed=True)
+    assert rel(orc.debye_peratom(w.xyz, w.fftab[w.type], w.q), orc.debye_sym(w.xyz, w.type, w.fftab, w.q)) < RT
+    # ... times a per-atom weight: the weighted oracle (R10w)
+    wt = rng.uniform(0.3, 1.7, w.N).astype(np.float32)
+    ffw = (w.fftab[w.type].astype(np.float64) * wt[:, None].astype(np.float64))
+    ffw32 = ffw.astype(np.float32)
+    if np.array_equal(ffw32.astype(np.float64), ffw):      # only exact products are comparable bit for bit; else loosen
+        tolw = RT
+    else:
+        tolw = 1e-6
+    assert rel(orc.debye_peratom(w.xyz, ffw32, w.q), orc.debye_sym(w.xyz, w.type, w.fftab, w.q, weight=wt)) < tolw
+    # separable rows f_j(q) = c_j g(q), c_j small integers and g powers of two (products exact in float32)
+    c = rng.integers(-3, 5, N).astype(np.float32)
+    g = np.array([2.0, 1.0, 0.5, 0.25], dtype=np.float32)
+    ones = np.ones((1, M), dtype=np.float32)
+    pts = orc.debye_sym(x, np.zeros(N, np.int32), ones, q, weight=c)
+    assert rel(orc.debye_peratom(x, c[:, None] * g[None, :], q), g.astype(np.float64) ** 2 * pts) < 1e-11
+    # equilateral triangle, three different atoms: I = sum f^2 + 2 (f1 f2 + f1 f3 + f2 f3) sinc(q a)
+    a = 2.0
+    tri = np.array([[0, 0, 0], [a, 0, 0], [a / 2, a * math.sqrt(3) / 2, 0]], dtype=np.float32)
+    ft = np.array([[3.0], [5.0], [-2.0]], dtype=np.float32)
+    qa = np.array([0.7], dtype=np.float32)
+    dists = [np.linalg.norm(tri[i].astype(np.float64) - tri[j].astype(np.float64)) for i, j in ((0, 1), (0, 2), (1, 2))]
+    sincs = [math.sin(float(qa[0]) * dd_) / (float(qa[0]) * dd_) for dd_ in dists]
+    want = 9 + 25 + 4 + 2 * (15 * sincs[0] - 6 * sincs[1] - 10 * sincs[2])
+    assert abs(orc.debye_peratom(tri, ft, qa)[0] - want) < 1e-12 * abs(want)

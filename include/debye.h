@@ -111,6 +111,20 @@ int debye_profile_weighted_host(const float *xyz, const int32_t *type, const flo
                                 const float *fftab, int32_t T, const float *q, int32_t M, double *I_out,
                                 uint32_t flags, debye_stream_t stream);
 
+/* The paper's general case: one form-factor row per ATOM ("the form factor depends on the atom type and its
+ * environment"; the kernel's input is "the form factors for each atom at Q values of q"),
+ *     I(q_m) = sum_i sum_j ff[i][m] ff[j][m] sinc(q_m |x_i - x_j|)      (Eq. 2; pairs once for i < j and doubled).
+ * Without types there is no per-type-pair factoring: the inner loop is distance once per pair and chunk of 32 q, then per
+ * q one range-reduced MUFU.SIN, a multiply by 1/r and an FMA with ff[j][m] from shared memory (XU-pipe bound); pairs with
+ * q r <= 0.004 take an accurate series.  FP32 partial sums are multiplied by ff[i][m] and reduced in FP64 in a fixed order.
+ *   xyz dev [N][3] float32, ff dev [N][M] float32 row-major (any sign), q dev [M] float32 (any grid; q and -q agree),
+ *   I_out dev [M] float64 (written).  flags: 0 or DEBYE_SINC_MUFU (the FP32 path above), or DEBYE_FP64 (double-precision
+ *   pair arithmetic, 1e-10 mode); anything else is DEBYE_EINVAL.  Three kernel launches, asynchronous on `stream`, same
+ *   workspace rules and error codes as debye_profile.  When the rows are copies of a type table (ff[i] = fftab[type[i]])
+ *   the result equals debye_profile's to rounding -- and debye_profile is several times faster. */
+int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, double *I_out,
+                          uint32_t flags, debye_stream_t stream);
+
 /* Plans: repeated profiles of ONE molecule whose coordinates change between calls (refinement, ensembles evaluated one
  * by one: the profile "must be recomputed hundreds of thousands of times").  debye_plan_create runs the
  * setup step once (type sort, schedule, analysis of the q grid), copies q and the weights into the plan, and synchronises

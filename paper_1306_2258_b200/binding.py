@@ -17,7 +17,7 @@ FLAGS = {"fp64": 1 << 0, "mufu": 1 << 2, "recur": 1 << 3, "accurate": 1 << 4, "a
 
 EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_profile_batch_host",
            "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials",
-           "debye_partials_shard", "debye_profile_from_partials", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
+           "debye_partials_shard", "debye_profile_from_partials", "debye_profile_peratom", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
            "debye_launch_info", "debye_set_pairs_events", "debye_q_hint", "debye_plan_create", "debye_plan_execute",
            "debye_plan_destroy", "debye_strerror", "debye_last_cuda_error", "debye_version")
 
@@ -49,6 +49,8 @@ def lib():
     L.debye_partials.argtypes = [vp, vp, i32, i32, vp, i32, i32, vp, vp, u32, vp]
     L.debye_partials_shard.argtypes = [vp, vp, i32, i32, vp, i32, i32, vp, vp, u32, i32, i32, vp]
     L.debye_profile_from_partials.argtypes = [vp, i32, vp, vp, i32, i32, i32, vp, vp]
+    L.debye_profile_peratom.argtypes = [vp, vp, i32, vp, i32, vp, u32, vp]
+    L.debye_profile_peratom.restype = C.c_int
     L.debye_profile_weighted.argtypes = [vp, vp, vp, i32, vp, i32, vp, i32, vp, u32, vp]
     L.debye_profile_weighted_host.argtypes = L.debye_profile_weighted.argtypes
     L.debye_profile_batch_weighted.argtypes = [vp, vp, vp, i32, i32, vp, i32, vp, i32, vp, u32, vp]
@@ -211,6 +213,21 @@ def debye_partials(xyz, type, q, T, variant="auto", stream=None):
                                 _dev(q, torch.float32, "q"), T, M, _dev(S, torch.float64, "S_out"),
                                 _dev(n, torch.int32, "n_out"), _flags(variant), _stream_ptr(stream)))
     return S, n
+
+
+def debye_profile_peratom(xyz, ff, q, I_out=None, variant="auto", stream=None):
+    """I_out[M] for per-ATOM form factors ff[N,M] f32 (the paper's general case).  variant: "auto" / "mufu"
+    (FP32, one MUFU.SIN per term) or "fp64"."""
+    import torch
+    N, M = xyz.shape[0], q.shape[0]
+    if tuple(ff.shape) != (N, M):
+        raise LibdebyeError("ff: expected shape [N, M]")
+    if I_out is None:
+        I_out = torch.empty(M, dtype=torch.float64, device=xyz.device)
+    _check(lib().debye_profile_peratom(_dev(xyz, torch.float32, "xyz"), _dev(ff, torch.float32, "ff"), N,
+                                       _dev(q, torch.float32, "q"), M, _dev(I_out, torch.float64, "I_out"),
+                                       _flags(variant), _stream_ptr(stream)))
+    return I_out
 
 
 def debye_partials_shard(xyz, type, q, T, shard_rank, shard_world, variant="auto", stream=None, hint=0):

@@ -18,6 +18,7 @@
 #include "debye_pairs.cuh"
 #include "debye_plan.cuh"
 #include "debye_registry.h"
+#include "debye_peratom.cuh"
 
 namespace {
 
@@ -424,6 +425,45 @@ int debye_profile_from_partials(const double *S_parts, int32_t n_parts, const in
     if (!S_parts || !n_a || !fftab || !I_out) return DEBYE_EINVAL;
     if (n_parts < 1 || n_parts > 4096 || B < 1 || B > 65535 || T < 1 || T > DEBYE_MAX_TYPES || M < 1 || M > DEBYE_MAX_Q) return DEBYE_EINVAL;
     debye::debye_combine_kernel<<<dim3((M + 127) / 128, B), 128, 0, (cudaStream_t)stream>>>(S_parts, n_parts, n_a, fftab, B, T, M, I_out);
+    CU(cudaGetLastError());
+    return DEBYE_OK;
+}
+
+int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, double *I_out, uint32_t flags, debye_stream_t stream_)
+{
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (!xyz || !ff || !q || !I_out) return DEBYE_EINVAL;
+    if (N < 1 || M < 1 || M > DEBYE_MAX_Q) return DEBYE_EINVAL;
+    if (flags & ~(uint32_t)(DEBYE_FP64 | DEBYE_SINC_MUFU)) return DEBYE_EINVAL;      // FP64, or FP32 with one MUFU.SIN per term (default)
+    if ((flags & DEBYE_FP64) && (flags & DEBYE_SINC_MUFU)) return DEBYE_EINVAL;
+    if (N > (1 << 24)) return DEBYE_EUNSUPPORTED;
+    const bool f64 = (flags & DEBYE_FP64) != 0;
+    std::lock_guard<std::mutex> lock(g_mu);
+    DevState *ds; int st;
+    if ((st = dev_state(&ds))) return st;
+    const int n_chunks = (M + DEBYE_PA_KQ - 1) / DEBYE_PA_KQ;
+    const int rows = debye_diag_rows(N);
+    const int64_t U = (rows > 0 ? debye_diag_row_prefix(N, rows) : 0) * n_chunks;
+    // resident CTAs x up to 8 waves, at least ~192 units (j atoms x 128 i atoms x 32 q) per CTA
+    int64_t G = U / 192;
+    const int64_t Gmax = (int64_t)ds->sms * (f64 ? 2 : 4) * 8;
+    if (G > Gmax) G = Gmax;
+    if (G < 1) G = 1;
+    size_t o = 0;
+    const size_t o_rec = o; o += align_up((size_t)(G + n_chunks) * DEBYE_PA_KQ * 8);
+    const size_t o_self = o; o += align_up((size_t)DEBYE_PA_SLICES * 2 * M * 8);
+    char *ws;
+    if (ds->user_ws) { if (ds->user_bytes < o) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
+    else { if ((st = ensure(&ds->ws, &ds->ws_bytes, o))) return st; ws = (char *)ds->ws; }
+    double *records = (double *)(ws + o_rec), *selfbuf = (double *)(ws + o_self);
+    debye::debye_peratom_self_kernel<<<dim3((M + 31) / 32, DEBYE_PA_SLICES), 256, 0, stream>>>(ff, N, M, selfbuf);
+    if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
+    if (U > 0) {
+        if (f64) debye::debye_peratom_pairs_kernel<true><<<(int)G, DEBYE_IB, 0, stream>>>(xyz, ff, q, N, M, n_chunks, records);
+        else debye::debye_peratom_pairs_kernel<false><<<(int)G, DEBYE_IB, 0, stream>>>(xyz, ff, q, N, M, n_chunks, records);
+    }
+    if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
+    debye::debye_peratom_final_kernel<<<(M + 127) / 128, 128, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, I_out);
     CU(cudaGetLastError());
     return DEBYE_OK;
 }

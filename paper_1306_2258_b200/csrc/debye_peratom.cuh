@@ -1,0 +1,227 @@
+// debye_peratom.cuh -- the paper's general case: one form-factor row per ATOM.
+//
+//     I(q_m) = sum_i ff[i][m]^2 + 2 sum_{i<j} ff[i][m] ff[j][m] sin(q_m r_ij) / (q_m r_ij)          (Eq. 2)
+//
+// With a different f on every atom the per-type-pair factoring of the main path is gone: every term needs its own
+// f_j(q_m), so the inner loop is the paper's own -- distance once per pair and q-chunk, then per q one
+// sine, one multiply by 1/r and one FMA with f_j(q_m) read from shared memory -- and any q grid is allowed (no recurrence:
+// it would save nothing here, the f_j load and FMA per term remain).  The bound is the XU pipe: one MUFU.SIN per term,
+// 16 lanes per clock and SM.
+//   thread = one i atom of a row of DEBYE_IB atoms, DEBYE_PA_KQ accumulators (one q-chunk) in registers ("private memory",
+//   PAPER.md:86); j atoms stream through shared memory in tiles of DEBYE_PA_JT atoms: float4 position + DEBYE_PA_KQ form
+//   factors each ("local memory", Fig. 2).  Units (one j atom against one row) are linearised q-chunk -> row ->
+//   j and cut into G equal contiguous ranges, as in the main path (static, balanced, bitwise reproducible).  The FP32
+//   accumulators are multiplied by f_i and reduced in FP64 in a fixed order at least every DEBYE_PA_FLUSH j atoms; a CTA
+//   writes one FP64 record per q-chunk it touched and the final kernel adds the records in CTA order.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <type_traits>
+#include "debye_plan.cuh"
+#include "debye_pairs.cuh"
+
+namespace debye {
+
+#define DEBYE_PA_KQ 32
+#define DEBYE_PA_JT 64
+#define DEBYE_PA_FLUSH 2048
+#define DEBYE_PA_SLICES 64       // self-term kernel: atom slices (grid.y)
+
+// sum_i ff[i][m] and sum_i ff[i][m]^2 in FP64, fixed order: slice s of DEBYE_PA_SLICES takes atoms s, s + S, ... in 8
+// interleaved sub-slices that are added in order.  selfbuf[s][0][m] = sum f, selfbuf[s][1][m] = sum f^2.
+__global__ void __launch_bounds__(256) debye_peratom_self_kernel(const float *__restrict__ ff, int N, int M, double *__restrict__ selfbuf)
+{
+    __shared__ double p1[8][32], p2[8][32];
+    const int kk = threadIdx.x & 31, sub = threadIdx.x >> 5;
+    const int k = blockIdx.x * 32 + kk, s = blockIdx.y;
+    double s1 = 0.0, s2 = 0.0;
+    if (k < M)
+        for (int64_t i = (int64_t)s * 8 + sub; i < N; i += (int64_t)DEBYE_PA_SLICES * 8) {
+            const double f = (double)ff[i * M + k];
+            s1 += f; s2 += f * f;
+        }
+    p1[sub][kk] = s1; p2[sub][kk] = s2;
+    __syncthreads();
+    if (sub == 0 && k < M) {
+        double a = 0.0, b = 0.0;
+#pragma unroll
+        for (int x = 0; x < 8; ++x) { a += p1[x][kk]; b += p2[x][kk]; }
+        selfbuf[((int64_t)s * 2 + 0) * M + k] = a;
+        selfbuf[((int64_t)s * 2 + 1) * M + k] = b;
+    }
+}
+
+template <bool F64>
+__global__ void __launch_bounds__(DEBYE_IB, F64 ? 2 : 4) debye_peratom_pairs_kernel(const float *__restrict__ xyz, const float *__restrict__ ff,
+                                                                                      const float *__restrict__ qv, int N, int M, int n_chunks,
+                                                                                      double *__restrict__ records)
+{
+    typedef typename std::conditional<F64, double, float>::type acc_t;
+    constexpr int KQ = DEBYE_PA_KQ, JT = DEBYE_PA_JT, NW = DEBYE_IB / 32;
+    __shared__ __align__(16) float4 pos[JT];
+    __shared__ __align__(16) float fj[JT][KQ];
+    __shared__ double wsum[NW][KQ];
+    __shared__ float qmin_s[NW];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int G = gridDim.x, c = blockIdx.x;
+    const int rows = debye_diag_rows(N);
+    const int64_t U1 = rows > 0 ? debye_diag_row_prefix(N, rows) : 0;
+    const int64_t U = U1 * n_chunks;
+    if (U == 0) return;
+    const int64_t u0 = debye_range_begin(U, c, G);
+    const int64_t u1 = (c + 1 == G) ? U : debye_range_begin(U, c + 1, G);
+    if (u0 >= u1) return;
+
+    // smallest non-zero |q|: pairs with q_small * r <= 0.004 take the accurate path (MUFU.SIN loses relative accuracy there)
+    float cut2 = 0.f;
+    if constexpr (!F64) {
+        float qsm = 3.0e38f;
+        for (int k = tid; k < M; k += DEBYE_IB) { const float a = fabsf(qv[k]); if (a > 0.f) qsm = fminf(qsm, a); }
+        for (int o = 16; o > 0; o >>= 1) qsm = fminf(qsm, __shfl_xor_sync(0xffffffffu, qsm, o));
+        if (lane == 0) qmin_s[warp] = qsm;
+        __syncthreads();
+        qsm = fminf(fminf(qmin_s[0], qmin_s[1]), fminf(qmin_s[2], qmin_s[3]));
+        if (qsm < 3.0e38f) { const float rcut = 0.004f / qsm; cut2 = rcut * rcut; }
+    }
+
+    acc_t acc[KQ];
+    float qr[KQ];
+#pragma unroll
+    for (int l = 0; l < KQ; ++l) { acc[l] = 0; qr[l] = 0.f; }
+    double run = 0.0;                  // thread l < KQ: FP64 running sum of q slot l of the current chunk
+    int ch_cur = -1;
+
+    int64_t u = u0;
+    while (u < u1) {
+        // ---- decode unit u -> (q-chunk, row, first j) ------------------------------------------------------------------
+        const int ch = (int)(u / U1);
+        const int64_t v = u - (int64_t)ch * U1;
+        int rl = 0, rh = rows;
+        while (rh - rl > 1) { const int mid = (rl + rh) >> 1; if (debye_diag_row_prefix(N, mid) <= v) rl = mid; else rh = mid; }
+        const int row = rl;
+        const int64_t jo = v - debye_diag_row_prefix(N, row);
+        const int64_t row_units = (int64_t)N - 1 - (int64_t)row * DEBYE_IB;
+        const int len = (int)min(min((int64_t)(u1 - u), row_units - jo), (int64_t)DEBYE_PA_FLUSH);
+        const int k0 = ch * KQ;
+        if (ch != ch_cur) {
+            if (ch_cur >= 0 && tid < KQ) { records[((int64_t)c + ch_cur) * KQ + tid] = run; run = 0.0; }
+            ch_cur = ch;
+#pragma unroll
+            for (int l = 0; l < KQ; ++l) qr[l] = (k0 + l < M) ? qv[k0 + l] : 0.f;
+        }
+        const int i = row * DEBYE_IB + tid;
+        const bool ivalid = i < N;
+        const float *xi = xyz + 3 * (int64_t)(ivalid ? i : 0);
+        const float pix = xi[0], piy = xi[1], piz = xi[2];
+        const int j_first = row * DEBYE_IB + 1 + (int)jo;
+
+        for (int t0 = 0; t0 < len; t0 += JT) {
+            const int cnt = min(len - t0, JT), jg0 = j_first + t0;
+            __syncthreads();                                   // the previous tile has been consumed
+            if (tid < cnt) { const float *s = xyz + 3 * (int64_t)(jg0 + tid); pos[tid] = make_float4(s[0], s[1], s[2], 0.f); }
+#pragma unroll 4
+            for (int e = tid; e < JT * KQ; e += DEBYE_IB) {
+                const int jj = e / KQ, l = e % KQ;
+                fj[jj][l] = (jj < cnt && k0 + l < M) ? ff[(int64_t)(jg0 + jj) * M + k0 + l] : 0.f;
+            }
+            __syncthreads();
+            // rows are diagonal blocks of the j > i triangle: a warp whose every i is >= j has nothing to do for that j
+            const int jj0 = max(0, row * DEBYE_IB + warp * 32 + 1 - jg0);
+            for (int jj = jj0; jj < cnt; ++jj) {
+                const float4 pj = pos[jj];
+                const bool ok = ivalid && (jg0 + jj > i);
+                if constexpr (F64) {
+                    const double dx = (double)pj.x - (double)pix, dy = (double)pj.y - (double)piy, dz = (double)pj.z - (double)piz;
+                    const double r = sqrt(dx * dx + dy * dy + dz * dz);
+                    if (ok) {
+#pragma unroll
+                        for (int l = 0; l < KQ; ++l) {
+                            const double qk = (double)qr[l], x = qk * r;
+                            const double tv = (x == 0.0) ? qk : sin(x) / r;          // sin(q r)/r -> q as r -> 0
+                            acc[l] += (double)fj[jj][l] * tv;
+                        }
+                    }
+                } else {
+                    const float dx = pj.x - pix, dy = pj.y - piy, dz = pj.z - piz;
+                    const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                    const bool small = !(r2 > cut2);
+                    const float r2c = fmaxf(r2, 1e-30f);
+                    float rinv = rsqrt_mufu(r2c);
+                    const float r = r2c * rinv;
+                    rinv = (ok && !small) ? rinv : 0.0f;
+                    if (__any_sync(0xffffffffu, small && ok)) {
+                        if (small && ok) {
+                            const float rs = sqrtf(r2);
+#pragma unroll
+                            for (int l = 0; l < KQ; ++l) {
+                                const float qk = qr[l];
+                                const float tv = (rs == 0.0f) ? qk : term_accurate(qk, rs);
+                                acc[l] = fmaf(fj[jj][l], tv, acc[l]);
+                            }
+                        }
+                    }
+                    const float rt = r * 0.15915494309189535f;                        // r / 2 pi: turns = q_k * rt
+#pragma unroll
+                    for (int l = 0; l < KQ; l += 4) {
+                        const float4 f4 = *reinterpret_cast<const float4 *>(&fj[jj][l]);
+                        acc[l + 0] = fmaf(sin_turns_fma(rt, qr[l + 0]) * rinv, f4.x, acc[l + 0]);
+                        acc[l + 1] = fmaf(sin_turns_fma(rt, qr[l + 1]) * rinv, f4.y, acc[l + 1]);
+                        acc[l + 2] = fmaf(sin_turns_fma(rt, qr[l + 2]) * rinv, f4.z, acc[l + 2]);
+                        acc[l + 3] = fmaf(sin_turns_fma(rt, qr[l + 3]) * rinv, f4.w, acc[l + 3]);
+                    }
+                }
+            }
+        }
+        // ---- flush: times f_i, FP64, fixed order (xor tree over the lanes, then the warps in order) ---------------------------
+        {
+            const float *fi = ff + (int64_t)(ivalid ? i : 0) * M + k0;
+#pragma unroll
+            for (int l = 0; l < KQ; ++l) {
+                double vv = (ivalid && k0 + l < M) ? (double)acc[l] * (double)fi[l] : 0.0;
+                acc[l] = 0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) vv += __shfl_xor_sync(0xffffffffu, vv, o);
+                if (lane == 0) wsum[warp][l] = vv;
+            }
+            __syncthreads();
+            if (tid < KQ) {
+                double s = 0.0;
+#pragma unroll
+                for (int w = 0; w < NW; ++w) s += wsum[w][tid];
+                run += s;
+            }
+        }
+        u += len;
+    }
+    if (ch_cur >= 0 && tid < KQ) records[((int64_t)c + ch_cur) * KQ + tid] = run;
+}
+
+// I[m] = sum_i f^2 + (2 / q_m) sum over CTAs of their records   (q_m != 0);   I[m] = (sum_i f)^2   (q_m == 0)
+__global__ void __launch_bounds__(128) debye_peratom_final_kernel(const double *__restrict__ records, const double *__restrict__ selfbuf,
+                                                                    const float *__restrict__ qv, int N, int M, int n_chunks, int G, double *__restrict__ out)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= M) return;
+    double s1 = 0.0, s2 = 0.0;
+    for (int s = 0; s < DEBYE_PA_SLICES; ++s) { s1 += selfbuf[((int64_t)s * 2 + 0) * M + k]; s2 += selfbuf[((int64_t)s * 2 + 1) * M + k]; }
+    const double qk = (double)qv[k];
+    const int rows = debye_diag_rows(N);
+    const int64_t U1 = rows > 0 ? debye_diag_row_prefix(N, rows) : 0;
+    if (qk == 0.0) { out[k] = s1 * s1; return; }
+    if (U1 == 0) { out[k] = s2; return; }
+    constexpr int KQ = DEBYE_PA_KQ;
+    const int ch = k / KQ, l = k % KQ;
+    const int64_t U = U1 * n_chunks, ub = (int64_t)ch * U1, ue = ub + U1 - 1;
+    const DebyeRanges ranges(U, G);
+    double s = 0.0;
+    if (U >= G) {
+        const int c_lo = ranges.owner(ub), c_hi = ranges.owner(ue);
+        for (int c = c_lo; c <= c_hi; ++c) s += records[((int64_t)c + ch) * KQ + l];
+    } else {
+        for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)ranges.owner(u) + ch) * KQ + l];
+    }
+    out[k] = s2 + 2.0 * s / qk;
+}
+
+}  // namespace debye

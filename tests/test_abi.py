@@ -62,6 +62,11 @@ def test_argument_validation_happens_before_cuda():
     assert L.debye_partials_shard(p, p, 10, 1, p, 2, 5, p, p, 0, 0, 0, None) == EINVAL
     assert L.debye_partials_shard(None, p, 10, 1, p, 2, 5, p, p, 0, 0, 2, None) == EINVAL
     assert L.debye_profile_from_partials(None, 2, p, p, 1, 2, 5, p, None) == EINVAL
+    assert L.debye_profile_peratom(None, p, 10, p, 5, p, 0, None) == EINVAL
+    assert L.debye_profile_peratom(p, p, 0, p, 5, p, 0, None) == EINVAL
+    assert L.debye_profile_peratom(p, p, 10, p, 4097, p, 0, None) == EINVAL
+    assert L.debye_profile_peratom(p, p, 10, p, 5, p, 1 << 3, None) == EINVAL                   # no recurrence variant here
+    assert L.debye_profile_peratom(p, p, (1 << 24) + 1, p, 5, p, 0, None) == EUNSUP
     assert L.debye_profile_from_partials(p, 0, p, p, 1, 2, 5, p, None) == EINVAL
     assert L.debye_profile_from_partials(p, 2, p, p, 1, 33, 5, p, None) == EINVAL
     assert L.debye_partials(p, p, 10, 1, None, 2, 5, p, None, 0, None) == EINVAL

@@ -476,3 +476,77 @@ def test_tile_split_argument_validation(db):
     S, n = db.debye_partials(x, t, q, w.T)
     with pytest.raises(db.LibdebyeError):
         db.debye_profile_from_partials(S[None][:, :, :2].contiguous(), n, f)
+
+
+def _peratom_ff(w, seed):
+    """per-ATOM rows (the form factor depends on the atom's environment): the type's row times a per-atom
+    factor in [0.6, 1.4] plus a per-atom q-dependent offset, so that no two atoms share a row"""
+    rng = np.random.default_rng(seed)
+    base = w.fftab[w.type].astype(np.float64)
+    fac = rng.uniform(0.6, 1.4, (w.N, 1))
+    off = rng.uniform(-0.3, 0.3, (w.N, 1)) * np.exp(-np.linspace(0, 2, w.M))[None, :]
+    return np.ascontiguousarray((base * fac + off).astype(np.float32))
+
+
+def test_peratom_form_factors_match_the_peratom_oracle(db):
+    """debye_profile_peratom (the paper's general case; NEXT-1) against oracle_debye_peratom, element by
+    element: sizes spanning several 128-atom rows, 64-atom tiles and 32-q chunks with ragged tails, uniform / offset /
+    non-uniform / descending grids with q = 0 inside, signed rows; FP32 (1e-4) and FP64 (1e-10) arithmetic."""
+    import torch
+    cases = [
+        wl.small_random(90, 130, 3, 17),
+        wl.small_random(91, 777, 5, 101),
+        wl.small_random(92, 1500, 4, 200, q_max=1.0),
+        wl.small_random(93, 513, 8, 40, signed=True),
+        wl.small_random(94, 900, 3, 64, q_min=0.3, q_max=0.9),
+        wl.small_random(95, 2100, 2, 33, q_max=1.2, box=60.0),
+        wl.cfg1(),
+    ]
+    for n, w in enumerate(cases):
+        ff = _peratom_ff(w, 900 + n)
+        qn = w.q.copy()
+        if n % 2 == 1:      # non-uniform, descending, with an explicit zero in the middle
+            qn = np.sort(np.random.default_rng(n).uniform(0.01, float(w.q.max()) + 0.1, w.M)).astype(np.float32)[::-1].copy()
+            qn[w.M // 2] = 0.0
+        ref = orc.debye_peratom(w.xyz, ff, qn)
+        x = torch.from_numpy(w.xyz).cuda(); f = torch.from_numpy(ff).cuda(); q = torch.from_numpy(qn).cuda()
+        for variant, tol in (("auto", TOL32), ("mufu", TOL32), ("fp64", TOL64)):
+            I = db.debye_profile_peratom(x, f, q, variant=variant).cpu().numpy()
+            assert rel(I, ref) <= tol, (n, variant, rel(I, ref))
+        a = db.debye_profile_peratom(x, f, q); b = db.debye_profile_peratom(x, f, q)
+        assert torch.equal(a, b)                                       # bitwise reproducible
+    # rows copied from a type table: the per-type path and its oracle
+    w = wl.small_random(96, 1100, 4, 101)
+    x, t, f, q = to_dev(w)
+    ffc = torch.from_numpy(np.ascontiguousarray(w.fftab[w.type])).cuda()
+    I = db.debye_profile_peratom(x, ffc, q).cpu().numpy()
+    assert rel(I, orc.debye_sym(w.xyz, w.type, w.fftab, w.q)) <= TOL32
+    assert rel(I, db.debye_profile(x, t, f, q).cpu().numpy()) <= 1e-5
+
+
+def test_peratom_degenerate_inputs(db):
+    import torch
+    q = np.array([0.0, 0.05, 0.4, 1.3], dtype=np.float32)
+    dq = torch.from_numpy(q).cuda()
+    # one atom: I = f^2; two atoms: closed form; coincident atoms: sinc(0) = 1; a very close pair (accurate small-x path)
+    one = np.array([[1.0, 2.0, 3.0]], dtype=np.float32); f1 = np.array([[2.0, 1.5, -1.0, 0.5]], dtype=np.float32)
+    I = db.debye_profile_peratom(torch.from_numpy(one).cuda(), torch.from_numpy(f1).cuda(), dq).cpu().numpy()
+    assert np.allclose(I, f1[0].astype(np.float64) ** 2, rtol=1e-15)
+    for d in (0.0, 1e-4, 0.01, 3.7, 250.0):
+        xyz = np.array([[0.5, 0.5, 0.5], [0.5, 0.5, 0.5 + d]], dtype=np.float32)
+        dd = float(np.float64(xyz[1, 2]) - np.float64(xyz[0, 2]))
+        ff = np.array([[6.0, 5.9, 4.0, 1.5], [-1.5, -1.4, -1.0, -0.3]], dtype=np.float32)
+        qq = q.astype(np.float64)
+        s = np.where(qq * dd == 0, 1.0, np.sin(qq * dd) / np.where(qq * dd == 0, 1.0, qq * dd))
+        want = ff[0].astype(np.float64) ** 2 + ff[1].astype(np.float64) ** 2 + 2 * ff[0].astype(np.float64) * ff[1] * s
+        for variant, tol in (("auto", 2e-6), ("fp64", 1e-12)):
+            I = db.debye_profile_peratom(torch.from_numpy(xyz).cuda(), torch.from_numpy(ff).cuda(), dq, variant=variant).cpu().numpy()
+            assert rel(I, want) <= tol, (d, variant, I, want)
+    # q = 0 only; M = 1
+    w = wl.small_random(97, 300, 3, 5)
+    ff = _peratom_ff(w, 97)[:, :1].copy()
+    I = db.debye_profile_peratom(torch.from_numpy(w.xyz).cuda(), torch.from_numpy(ff).cuda(), torch.zeros(1, device="cuda")).cpu().numpy()
+    assert abs(I[0] - ff.astype(np.float64).sum() ** 2) <= 1e-12 * I[0]
+    # bad flags are rejected before anything is launched
+    with pytest.raises(db.LibdebyeError):
+        db.debye_profile_peratom(torch.from_numpy(w.xyz).cuda(), torch.from_numpy(ff).cuda(), torch.zeros(1, device="cuda"), variant="recur")

@@ -162,6 +162,9 @@ def main():
     ap.add_argument("--variant", default="auto", choices=["auto", "recur", "mufu", "accurate", "fp64"])
     ap.add_argument("--impl", default="libdebye", choices=["libdebye", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--path", default="pertype", choices=["pertype", "peratom"],
+                    help="pertype: the north_star path (debye_profile, form factors per atom type); peratom: the paper's general "
+                         "case (debye_profile_peratom, one form-factor row per atom; NEXT-1)")
     ap.add_argument("--no-hint", action="store_true", help="do not pass the q-grid hint (DEBYE_QHINT_*) computed from the host copy of q")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "libdebye" else args.warmup
@@ -183,6 +186,8 @@ def main():
     db.lib()
 
     w = make_workload(args.config, rank)
+    if args.path == "peratom":
+        return run_peratom(args, w, rank, world, dev)
     batch = w.xyz.ndim == 3
     call = db.debye_profile_batch if batch else db.debye_profile
     call_host = db.debye_profile_batch_host if batch else db.debye_profile_host
@@ -312,6 +317,109 @@ def main():
             ref = orc.debye_sym(w.xyz, w.type, w.fftab[:, ks].copy(), w.q[ks].copy())
             line["parity_max_rel_err"] = float(np.max(np.abs(result_dev[ks] - ref) / np.abs(ref)))
         line["cpu_baseline"] = cb
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_peratom(args, w, rank, world, dev):
+    """--path peratom: one step = one debye_profile_peratom call (self terms, pairs, final: 3 launches) on the same synthetic
+    structure with a seeded per-atom table (workloads.peratom_table).  Same JSON contract; roofline = XU pipe (one MUFU.SIN
+    per pair.q); fp64 variant quoted against the same roofline for scale."""
+    import torch
+    import torch.distributed as dist
+    from paper_1306_2258_b200 import binding as db, sharding
+    if w.xyz.ndim == 3:
+        raise SystemExit("--path peratom takes single-structure configs")
+    variant = args.variant if args.variant in ("auto", "mufu", "fp64") else "auto"
+    ff = wl.peratom_table(w, rank)
+    x, f, q = (torch.from_numpy(a).to(dev) for a in (w.xyz, ff, w.q))
+    out = torch.empty(w.M, dtype=torch.float64, device=dev)
+    flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        db.debye_profile_peratom(x, f, q, out, variant=variant)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.fill_(1)
+        a.record()
+        db.debye_profile_peratom(x, f, q, out, variant=variant)
+        b.record()
+    barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    total_ms = sharding.max_over_ranks(float(np.sum([a.elapsed_time(b) for a, b in ev])), dev)
+    units = sharding.sum_over_ranks(float(w.pair_q), dev)
+    value = units * args.steps / (total_ms * 1e-3) / 1e9
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); e1.record(); torch.cuda.synchronize()
+    db.set_pairs_events(e0, e1)
+    pk = []
+    for _ in range(min(args.steps, 30)):
+        flush.fill_(1)
+        db.debye_profile_peratom(x, f, q, out, variant=variant)
+        torch.cuda.synchronize()
+        pk.append(e0.elapsed_time(e1))
+    db.set_pairs_events(None, None)
+    pairs_ms = float(np.mean(pk))
+    hx, hf, hq = (torch.from_numpy(a).pin_memory().numpy() for a in (w.xyz, ff, w.q))
+    hout = torch.empty(w.M, dtype=torch.float64).pin_memory().numpy()
+    for _ in range(3):
+        db.debye_profile_peratom_host(hx, hf, hq, hout, variant=variant)
+    barrier()
+    n_e2e = max(5, min(args.steps, 50))
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        db.debye_profile_peratom_host(hx, hf, hq, hout, variant=variant)
+    barrier()
+    e2e_s = sharding.max_over_ranks(time.perf_counter() - t0, dev)
+    result_dev = out.cpu().numpy()
+    assert np.array_equal(result_dev, hout), "host entry and device entry disagree"
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    fmax_ghz = float(measured_peaks().get("sm_max_mhz", 1965.0)) / 1e3
+    peak = SM_COUNT * MUFU_LANES * fmax_ghz / 1e3
+    achieved = float(w.pair_q) / (pairs_ms * 1e-3) / 1e12
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if variant == "fp64" else "f32", "data": "synthetic",
+        "config": {"workload": w.name + "+peratom_table", "path": "peratom", "N": w.N, "M": w.M, "B": 1,
+                   "variant": "fp64" if variant == "fp64" else "mufu", "q_chunk": 32, "n_chunks": (w.M + 31) // 32,
+                   "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
+                   "parallelism": f"{world} independent structure(s), one per GPU", "wall_s_timed_loop": wall},
+        "clocks": clocks,
+        "e2e": {"value": units * n_e2e / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(hx.nbytes + hf.nbytes + hq.nbytes),
+                "d2h_bytes_per_step": int(hout.nbytes), "ms_per_step": e2e_s / n_e2e * 1e3, "steps": n_e2e},
+        "gpu_launches": 3 * args.steps,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T sin/s", "frac": achieved / peak, "traffic": None,
+                     "note": "XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM x 148 SM x sm_max_mhz; the 32-q chunks "
+                             "are padded (M = 101 runs 128 slots), which the algorithmic count does not credit",
+                     "kernel": f"debye_peratom_pairs_kernel<{'fp64' if variant == 'fp64' else 'fp32'}>", "kernel_ms": pairs_ms,
+                     "share_of_step": pairs_ms / (total_ms / args.steps)},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle as orc
+        ks = list(range(0, w.M, max(1, w.M // 8)))
+        ref = orc.debye_peratom(w.xyz, ff[:, ks].copy(), w.q[ks].copy())
+        line["parity_max_rel_err"] = float(np.max(np.abs(result_dev[ks] - ref) / np.abs(ref)))
+        ns = min(w.N, 6000)
+        t0 = time.perf_counter()
+        orc.debye_peratom(w.xyz[:ns], ff[:ns], w.q)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": ns * (ns - 1) / 2 * w.M / dt / 1e9, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+                                "sample": f"oracle_debye_peratom on the first {ns} atoms, all {w.M} q ({dt:.2f} s)", "seconds": dt}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -124,6 +124,9 @@ int debye_profile_weighted_host(const float *xyz, const int32_t *type, const flo
  *   the result equals debye_profile's to rounding -- and debye_profile is several times faster. */
 int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, double *I_out,
                           uint32_t flags, debye_stream_t stream);
+/* The same through HOST buffers (copies in, runs the device path, copies I_out back, synchronises `stream`). */
+int debye_profile_peratom_host(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, double *I_out,
+                               uint32_t flags, debye_stream_t stream);
 
 /* Plans: repeated profiles of ONE molecule whose coordinates change between calls (refinement, ensembles evaluated one
  * by one: the profile "must be recomputed hundreds of thousands of times").  debye_plan_create runs the

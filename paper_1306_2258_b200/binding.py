@@ -17,7 +17,7 @@ FLAGS = {"fp64": 1 << 0, "mufu": 1 << 2, "recur": 1 << 3, "accurate": 1 << 4, "a
 
 EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_profile_batch_host",
            "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials",
-           "debye_partials_shard", "debye_profile_from_partials", "debye_profile_peratom", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
+           "debye_partials_shard", "debye_profile_from_partials", "debye_profile_peratom", "debye_profile_peratom_host", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
            "debye_launch_info", "debye_set_pairs_events", "debye_q_hint", "debye_plan_create", "debye_plan_execute",
            "debye_plan_destroy", "debye_strerror", "debye_last_cuda_error", "debye_version")
 
@@ -51,6 +51,8 @@ def lib():
     L.debye_profile_from_partials.argtypes = [vp, i32, vp, vp, i32, i32, i32, vp, vp]
     L.debye_profile_peratom.argtypes = [vp, vp, i32, vp, i32, vp, u32, vp]
     L.debye_profile_peratom.restype = C.c_int
+    L.debye_profile_peratom_host.argtypes = L.debye_profile_peratom.argtypes
+    L.debye_profile_peratom_host.restype = C.c_int
     L.debye_profile_weighted.argtypes = [vp, vp, vp, i32, vp, i32, vp, i32, vp, u32, vp]
     L.debye_profile_weighted_host.argtypes = L.debye_profile_weighted.argtypes
     L.debye_profile_batch_weighted.argtypes = [vp, vp, vp, i32, i32, vp, i32, vp, i32, vp, u32, vp]
@@ -285,6 +287,16 @@ def debye_profile_batch_host(xyz, type, fftab, q, I_out=None, variant="auto", st
     _check(lib().debye_profile_batch_host(_host(xyz, np.float32, "xyz"), _host(type, np.int32, "type"), N, B,
                                           _host(fftab, np.float32, "fftab"), T, _host(q, np.float32, "q"), M,
                                           _host(I_out, np.float64, "I_out"), _flags(variant, hint), _stream_ptr(stream)))
+    return I_out
+
+
+def debye_profile_peratom_host(xyz, ff, q, I_out=None, variant="auto", stream=None):
+    N, M = xyz.shape[0], q.shape[0]
+    if I_out is None:
+        I_out = np.empty(M, dtype=np.float64)
+    _check(lib().debye_profile_peratom_host(_host(xyz, np.float32, "xyz"), _host(ff, np.float32, "ff"), N,
+                                            _host(q, np.float32, "q"), M, _host(I_out, np.float64, "I_out"),
+                                            _flags(variant), _stream_ptr(stream)))
     return I_out
 
 

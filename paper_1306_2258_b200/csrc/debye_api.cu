@@ -468,6 +468,34 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
     return DEBYE_OK;
 }
 
+int debye_profile_peratom_host(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, double *I_out, uint32_t flags, debye_stream_t stream_)
+{
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (!xyz || !ff || !q || !I_out) return DEBYE_EINVAL;
+    if (N < 1 || M < 1 || M > DEBYE_MAX_Q) return DEBYE_EINVAL;
+    if (N > (1 << 24)) return DEBYE_EUNSUPPORTED;
+    DevState *ds; int st; char *base;
+    size_t o = 0;
+    const size_t o_xyz = o; o += align_up((size_t)N * 12);
+    const size_t o_ff = o; o += align_up((size_t)N * M * 4);
+    const size_t o_q = o; o += align_up((size_t)M * 4);
+    const size_t o_out = o; o += align_up((size_t)M * 8);
+    {
+        std::lock_guard<std::mutex> lock(g_mu);
+        if ((st = dev_state(&ds))) return st;
+        if ((st = ensure(&ds->stage, &ds->stage_bytes, o))) return st;
+        base = (char *)ds->stage;
+    }
+    CU(cudaMemcpyAsync(base + o_xyz, xyz, (size_t)N * 12, cudaMemcpyHostToDevice, stream));
+    CU(cudaMemcpyAsync(base + o_ff, ff, (size_t)N * M * 4, cudaMemcpyHostToDevice, stream));
+    CU(cudaMemcpyAsync(base + o_q, q, (size_t)M * 4, cudaMemcpyHostToDevice, stream));
+    st = debye_profile_peratom((const float *)(base + o_xyz), (const float *)(base + o_ff), N, (const float *)(base + o_q), M, (double *)(base + o_out), flags, stream_);
+    if (st) return st;
+    CU(cudaMemcpyAsync(I_out, base + o_out, (size_t)M * 8, cudaMemcpyDeviceToHost, stream));
+    CU(cudaStreamSynchronize(stream));
+    return DEBYE_OK;
+}
+
 int debye_plan_create(debye_plan **out, const int32_t *type, int32_t N, int32_t B, int32_t T, const float *q, int32_t M, const float *weight, uint32_t flags,
                       debye_stream_t stream_)
 {

@@ -257,3 +257,15 @@ def cubic_lattice(nx: int, ny: int, nz: int, a: float, M: int, q_max: float, T: 
 
 
 CONFIGS = {"cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4, "cfg5": cfg5}
+
+
+def peratom_table(w: Workload, seed: int = 0) -> np.ndarray:
+    """ff[N][M] float32 for the per-ATOM path ("the form factor depends on the atom type and its environment" --
+    excluded volume and hydration layer): the type's row times a seeded per-atom factor in [0.6, 1.4] (a stand-in for the
+    solvent-accessible fraction), plus a seeded per-atom offset in [-0.3, 0.3] that decays with q (a hydration-shell-like
+    term), so that no two atoms share a row.  An input recipe only: none of the method's arithmetic."""
+    rng = np.random.default_rng(0x5EED0000 + seed)
+    base = w.fftab[w.type].astype(np.float64)
+    fac = rng.uniform(0.6, 1.4, (w.N, 1))
+    off = rng.uniform(-0.3, 0.3, (w.N, 1)) * np.exp(-np.linspace(0.0, 2.0, w.M))[None, :]
+    return np.ascontiguousarray((base * fac + off).astype(np.float32))

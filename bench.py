@@ -390,13 +390,15 @@ def run_peratom(args, w, rank, world, dev):
         return
     fmax_ghz = float(measured_peaks().get("sm_max_mhz", 1965.0)) / 1e3
     peak = SM_COUNT * MUFU_LANES * fmax_ghz / 1e3
+    # the library's q-chunk (debye_peratom_kq): the multiple of 4 in [16, 32] with the fewest padded slots, larger on ties
+    kq = min(range(32, 12, -4), key=lambda c: ((w.M + c - 1) // c * c, -c))
     achieved = float(w.pair_q) / (pairs_ms * 1e-3) / 1e12
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if variant == "fp64" else "f32", "data": "synthetic",
         "config": {"workload": w.name + "+peratom_table", "path": "peratom", "N": w.N, "M": w.M, "B": 1,
-                   "variant": "fp64" if variant == "fp64" else "mufu", "q_chunk": 32, "n_chunks": (w.M + 31) // 32,
+                   "variant": "fp64" if variant == "fp64" else "mufu", "q_chunk": kq, "n_chunks": (w.M + kq - 1) // kq,
                    "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
                    "parallelism": f"{world} independent structure(s), one per GPU", "wall_s_timed_loop": wall},
         "clocks": clocks,
@@ -404,8 +406,8 @@ def run_peratom(args, w, rank, world, dev):
                 "d2h_bytes_per_step": int(hout.nbytes), "ms_per_step": e2e_s / n_e2e * 1e3, "steps": n_e2e},
         "gpu_launches": 3 * args.steps,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T sin/s", "frac": achieved / peak, "traffic": None,
-                     "note": "XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM x 148 SM x sm_max_mhz; the 32-q chunks "
-                             "are padded (M = 101 runs 128 slots), which the algorithmic count does not credit",
+                     "note": "XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM x 148 SM x sm_max_mhz; the q-chunks "
+                             "are padded (M = 101 runs 4 x 28 = 112 slots), which the algorithmic count does not credit",
                      "kernel": f"debye_peratom_pairs_kernel<{'fp64' if variant == 'fp64' else 'fp32'}>", "kernel_ms": pairs_ms,
                      "share_of_step": pairs_ms / (total_ms / args.steps)},
     }

@@ -441,11 +441,12 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
     std::lock_guard<std::mutex> lock(g_mu);
     DevState *ds; int st;
     if ((st = dev_state(&ds))) return st;
-    const int n_chunks = (M + DEBYE_PA_KQ - 1) / DEBYE_PA_KQ;
+    const int KQ = debye::debye_peratom_kq(M);
+    const int n_chunks = (M + KQ - 1) / KQ;
     const int rows = debye_diag_rows(N);
     const int64_t U = (rows > 0 ? debye_diag_row_prefix(N, rows) : 0) * n_chunks;
     // resident CTAs x up to 8 waves, at least ~192 units (j atoms x 128 i atoms x 32 q) per CTA
-    int64_t G = U / 192;
+    int64_t G = U / (192 * DEBYE_PA_KQ / KQ);
     const int64_t Gmax = (int64_t)ds->sms * (f64 ? 2 : 4) * 8;
     if (G > Gmax) G = Gmax;
     if (G < 1) G = 1;
@@ -459,11 +460,16 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
     debye::debye_peratom_self_kernel<<<dim3((M + 31) / 32, DEBYE_PA_SLICES), 256, 0, stream>>>(ff, N, M, selfbuf);
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
     if (U > 0) {
-        if (f64) debye::debye_peratom_pairs_kernel<true><<<(int)G, DEBYE_IB, 0, stream>>>(xyz, ff, q, N, M, n_chunks, records);
-        else debye::debye_peratom_pairs_kernel<false><<<(int)G, DEBYE_IB, 0, stream>>>(xyz, ff, q, N, M, n_chunks, records);
+#define DEBYE_PA_LAUNCH(KQ_)                                                                                                              \
+    case KQ_:                                                                                                                           \
+        if (f64) debye::debye_peratom_pairs_kernel<true, KQ_><<<(int)G, DEBYE_IB, 0, stream>>>(xyz, ff, q, N, M, n_chunks, records);    \
+        else debye::debye_peratom_pairs_kernel<false, KQ_><<<(int)G, DEBYE_IB, 0, stream>>>(xyz, ff, q, N, M, n_chunks, records);      \
+        break;
+        switch (KQ) { DEBYE_PA_LAUNCH(16) DEBYE_PA_LAUNCH(20) DEBYE_PA_LAUNCH(24) DEBYE_PA_LAUNCH(28) DEBYE_PA_LAUNCH(32) default: return DEBYE_EUNSUPPORTED; }
+#undef DEBYE_PA_LAUNCH
     }
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
-    debye::debye_peratom_final_kernel<<<(M + 127) / 128, 128, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, I_out);
+    debye::debye_peratom_final_kernel<<<(M + 127) / 128, 128, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, KQ, I_out);
     CU(cudaGetLastError());
     return DEBYE_OK;
 }

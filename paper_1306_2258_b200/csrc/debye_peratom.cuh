@@ -22,7 +22,7 @@
 
 namespace debye {
 
-#define DEBYE_PA_KQ 32
+#define DEBYE_PA_KQ 32           // largest q-chunk (accumulators per thread); the kernel is instantiated for 16, 20, ... 32
 #define DEBYE_PA_JT 64
 #define DEBYE_PA_FLUSH 2048
 #define DEBYE_PA_SLICES 64       // self-term kernel: atom slices (grid.y)
@@ -51,13 +51,24 @@ __global__ void __launch_bounds__(256) debye_peratom_self_kernel(const float *__
     }
 }
 
-template <bool F64>
+// q-chunk that wastes the fewest padded slots for M q values (ties: the larger chunk, fewer distance evaluations)
+__host__ __device__ inline int debye_peratom_kq(int M)
+{
+    int best = DEBYE_PA_KQ, best_slots = (M + DEBYE_PA_KQ - 1) / DEBYE_PA_KQ * DEBYE_PA_KQ;
+    for (int kq = DEBYE_PA_KQ - 4; kq >= 16; kq -= 4) {
+        const int slots = (M + kq - 1) / kq * kq;
+        if (slots < best_slots) { best = kq; best_slots = slots; }
+    }
+    return best;
+}
+
+template <bool F64, int KQ>
 __global__ void __launch_bounds__(DEBYE_IB, F64 ? 2 : 4) debye_peratom_pairs_kernel(const float *__restrict__ xyz, const float *__restrict__ ff,
                                                                                       const float *__restrict__ qv, int N, int M, int n_chunks,
                                                                                       double *__restrict__ records)
 {
     typedef typename std::conditional<F64, double, float>::type acc_t;
-    constexpr int KQ = DEBYE_PA_KQ, JT = DEBYE_PA_JT, NW = DEBYE_IB / 32;
+    constexpr int JT = DEBYE_PA_JT, NW = DEBYE_IB / 32;
     __shared__ __align__(16) float4 pos[JT];
     __shared__ __align__(16) float fj[JT][KQ];
     __shared__ double wsum[NW][KQ];
@@ -199,7 +210,8 @@ __global__ void __launch_bounds__(DEBYE_IB, F64 ? 2 : 4) debye_peratom_pairs_ker
 
 // I[m] = sum_i f^2 + (2 / q_m) sum over CTAs of their records   (q_m != 0);   I[m] = (sum_i f)^2   (q_m == 0)
 __global__ void __launch_bounds__(128) debye_peratom_final_kernel(const double *__restrict__ records, const double *__restrict__ selfbuf,
-                                                                    const float *__restrict__ qv, int N, int M, int n_chunks, int G, double *__restrict__ out)
+                                                                    const float *__restrict__ qv, int N, int M, int n_chunks, int G, int KQ,
+                                                                    double *__restrict__ out)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= M) return;
@@ -210,14 +222,23 @@ __global__ void __launch_bounds__(128) debye_peratom_final_kernel(const double *
     const int64_t U1 = rows > 0 ? debye_diag_row_prefix(N, rows) : 0;
     if (qk == 0.0) { out[k] = s1 * s1; return; }
     if (U1 == 0) { out[k] = s2; return; }
-    constexpr int KQ = DEBYE_PA_KQ;
     const int ch = k / KQ, l = k % KQ;
     const int64_t U = U1 * n_chunks, ub = (int64_t)ch * U1, ue = ub + U1 - 1;
     const DebyeRanges ranges(U, G);
     double s = 0.0;
     if (U >= G) {
         const int c_lo = ranges.owner(ub), c_hi = ranges.owner(ue);
-        for (int c = c_lo; c <= c_hi; ++c) s += records[((int64_t)c + ch) * KQ + l];
+        // loads of 8 records in flight together, added in CTA order
+        const double *rp = records + ((int64_t)c_lo + ch) * KQ + l;
+        int c = c_lo;
+        for (; c + 8 <= c_hi + 1; c += 8, rp += 8 * (int64_t)KQ) {
+            double r[8];
+#pragma unroll
+            for (int x = 0; x < 8; ++x) r[x] = rp[x * (int64_t)KQ];
+#pragma unroll
+            for (int x = 0; x < 8; ++x) s += r[x];
+        }
+        for (; c <= c_hi; ++c, rp += KQ) s += rp[0];
     } else {
         for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)ranges.owner(u) + ch) * KQ + l];
     }

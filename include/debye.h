@@ -120,7 +120,8 @@ int debye_profile_weighted_host(const float *xyz, const int32_t *type, const flo
  *   xyz dev [N][3] float32, ff dev [N][M] float32 row-major (any sign), q dev [M] float32 (any grid; q and -q agree),
  *   I_out dev [M] float64 (written).  flags: 0 or DEBYE_SINC_MUFU (the FP32 path above), or DEBYE_FP64 (double-precision
  *   pair arithmetic, 1e-10 mode); anything else is DEBYE_EINVAL.  Three kernel launches, asynchronous on `stream`, same
- *   workspace rules and error codes as debye_profile.  When the rows are copies of a type table (ff[i] = fftab[type[i]])
+ *   workspace rules and error codes as debye_profile (scratch: at most 1.3 MB + 1 KB x M; a caller-supplied workspace
+ *   smaller than that gives DEBYE_ENOMEM).  q is processed in chunks of 16..32 values fitted to M.  When the rows are copies of a type table (ff[i] = fftab[type[i]])
  *   the result equals debye_profile's to rounding -- and debye_profile is several times faster. */
 int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, double *I_out,
                           uint32_t flags, debye_stream_t stream);

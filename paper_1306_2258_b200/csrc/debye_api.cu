@@ -469,7 +469,7 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
 #undef DEBYE_PA_LAUNCH
     }
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
-    debye::debye_peratom_final_kernel<<<(M + 127) / 128, 128, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, KQ, I_out);
+    debye::debye_peratom_final_kernel<<<(M + 31) / 32, 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, KQ, I_out);
     CU(cudaGetLastError());
     return DEBYE_OK;
 }

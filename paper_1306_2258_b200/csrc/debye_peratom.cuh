@@ -209,40 +209,51 @@ __global__ void __launch_bounds__(DEBYE_IB, F64 ? 2 : 4) debye_peratom_pairs_ker
 }
 
 // I[m] = sum_i f^2 + (2 / q_m) sum over CTAs of their records   (q_m != 0);   I[m] = (sum_i f)^2   (q_m == 0)
-__global__ void __launch_bounds__(128) debye_peratom_final_kernel(const double *__restrict__ records, const double *__restrict__ selfbuf,
-                                                                    const float *__restrict__ qv, int N, int M, int n_chunks, int G, int KQ,
-                                                                    double *__restrict__ out)
+// Block = 32 q indices x DEBYE_PA_FS slices: thread (kk, sl) adds the sl-th of DEBYE_PA_FS equal parts of the CTA range
+// that touched q index k (8 record loads in flight, added in CTA order); the parts are then added in slice order, so the
+// order is a fixed function of (N, M, G) and the result is bitwise reproducible.
+#define DEBYE_PA_FS 8
+__global__ void __launch_bounds__(32 * DEBYE_PA_FS) debye_peratom_final_kernel(const double *__restrict__ records, const double *__restrict__ selfbuf,
+                                                                                 const float *__restrict__ qv, int N, int M, int n_chunks, int G, int KQ,
+                                                                                 double *__restrict__ out)
 {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= M) return;
-    double s1 = 0.0, s2 = 0.0;
-    for (int s = 0; s < DEBYE_PA_SLICES; ++s) { s1 += selfbuf[((int64_t)s * 2 + 0) * M + k]; s2 += selfbuf[((int64_t)s * 2 + 1) * M + k]; }
-    const double qk = (double)qv[k];
+    __shared__ double part[DEBYE_PA_FS][32];
+    const int kk = threadIdx.x & 31, sl = threadIdx.x >> 5;
+    const int k = blockIdx.x * 32 + kk;
     const int rows = debye_diag_rows(N);
     const int64_t U1 = rows > 0 ? debye_diag_row_prefix(N, rows) : 0;
-    if (qk == 0.0) { out[k] = s1 * s1; return; }
-    if (U1 == 0) { out[k] = s2; return; }
-    const int ch = k / KQ, l = k % KQ;
-    const int64_t U = U1 * n_chunks, ub = (int64_t)ch * U1, ue = ub + U1 - 1;
-    const DebyeRanges ranges(U, G);
     double s = 0.0;
-    if (U >= G) {
-        const int c_lo = ranges.owner(ub), c_hi = ranges.owner(ue);
-        // loads of 8 records in flight together, added in CTA order
-        const double *rp = records + ((int64_t)c_lo + ch) * KQ + l;
-        int c = c_lo;
-        for (; c + 8 <= c_hi + 1; c += 8, rp += 8 * (int64_t)KQ) {
-            double r[8];
+    if (k < M && U1 > 0 && qv[k] != 0.0f) {
+        const int ch = k / KQ, l = k % KQ;
+        const int64_t U = U1 * n_chunks, ub = (int64_t)ch * U1, ue = ub + U1 - 1;
+        const DebyeRanges ranges(U, G);
+        if (U >= G) {           // every CTA owns at least one unit: all CTAs between the owners took part
+            const int c_lo = ranges.owner(ub), c_hi = ranges.owner(ue);
+            const int n = c_hi - c_lo + 1, per = (n + DEBYE_PA_FS - 1) / DEBYE_PA_FS;
+            const int cb = c_lo + sl * per, ce = min(c_hi + 1, cb + per);
+            const double *rp = records + ((int64_t)cb + ch) * KQ + l;
+            int c = cb;
+            for (; c + 8 <= ce; c += 8, rp += 8 * (int64_t)KQ) {
+                double r[8];
 #pragma unroll
-            for (int x = 0; x < 8; ++x) r[x] = rp[x * (int64_t)KQ];
+                for (int x = 0; x < 8; ++x) r[x] = rp[x * (int64_t)KQ];
 #pragma unroll
-            for (int x = 0; x < 8; ++x) s += r[x];
+                for (int x = 0; x < 8; ++x) s += r[x];
+            }
+            for (; c < ce; ++c, rp += KQ) s += rp[0];
+        } else if (sl == 0) {   // fewer units than CTAs: each unit has its own CTA
+            for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)ranges.owner(u) + ch) * KQ + l];
         }
-        for (; c <= c_hi; ++c, rp += KQ) s += rp[0];
-    } else {
-        for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)ranges.owner(u) + ch) * KQ + l];
     }
-    out[k] = s2 + 2.0 * s / qk;
+    part[sl][kk] = s;
+    __syncthreads();
+    if (sl != 0 || k >= M) return;
+    double s1 = 0.0, s2 = 0.0, tot = 0.0;
+    for (int x = 0; x < DEBYE_PA_SLICES; ++x) { s1 += selfbuf[((int64_t)x * 2 + 0) * M + k]; s2 += selfbuf[((int64_t)x * 2 + 1) * M + k]; }
+#pragma unroll
+    for (int x = 0; x < DEBYE_PA_FS; ++x) tot += part[x][kk];
+    const double qk = (double)qv[k];
+    out[k] = (qk == 0.0) ? s1 * s1 : s2 + 2.0 * tot / qk;
 }
 
 }  // namespace debye

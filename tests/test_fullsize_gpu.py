@@ -118,3 +118,33 @@ def test_two_type_lattice_and_chain_closed_forms(db):
     wantc = orc.chain_closed_form(n, d, q.astype(np.float64))
     for v in ["auto", "mufu"]:
         assert np.max(np.abs(run(db, wc, v) - wantc) / wantc) <= TOL32
+
+
+def test_tile_split_full_size_against_stored_oracle(db):
+    """cfg2 and cfg3 split over 4 emulated ranks by tiles (debye_partials_shard with bench.py's launch configuration: the
+    automatic variant, 2368 / 4736 pairs CTAs), gathered and combined on the device, against the stored oracle samples."""
+    import torch
+    for name in ("cfg2", "cfg3"):
+        w = wl.CONFIGS[name]()
+        x, t, f, q = (torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (w.xyz, w.type, w.fftab, w.q))
+        parts = [db.debye_partials_shard(x, t, q, w.T, r, 4) for r in range(4)]
+        I = db.debye_profile_from_partials(torch.stack([p[0] for p in parts]), parts[0][1], f).cpu().numpy()[0]
+        assert check(I, golden()[name], w, TOL32) <= 1e-5
+        # every rank got about a quarter of the pair sums (cyclic CTAs keep the triangular load balanced)
+        k = w.M // 2
+        share = torch.stack([p[0][0, :, 1].abs().sum() for p in parts])          # q index 1: all terms positive-ish
+        assert float(share.min() / share.max()) > 0.8
+
+
+def test_peratom_full_size_against_the_oracle_at_sampled_q(db):
+    """debye_profile_peratom at cfg2's full size with the table bench.py --path peratom uses, against oracle_debye_peratom
+    evaluated at 8 sampled q (the oracle needs only those columns of the table)."""
+    import torch
+    w = wl.cfg2()
+    ff = wl.peratom_table(w, 0)
+    I = db.debye_profile_peratom(torch.from_numpy(w.xyz).cuda(), torch.from_numpy(ff).cuda(), torch.from_numpy(w.q).cuda()).cpu().numpy()
+    ks = list(range(0, w.M, 13)) + [w.M - 1]
+    ref = orc.debye_peratom(w.xyz, np.ascontiguousarray(ff[:, ks]), np.ascontiguousarray(w.q[ks]))
+    assert float(np.max(np.abs(I[ks] - ref) / np.abs(ref))) <= 1e-5
+    I64 = db.debye_profile_peratom(torch.from_numpy(w.xyz).cuda(), torch.from_numpy(ff).cuda(), torch.from_numpy(w.q).cuda(), variant="fp64").cpu().numpy()
+    assert float(np.max(np.abs(I64[ks] - ref) / np.abs(ref))) <= TOL64

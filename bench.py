@@ -35,7 +35,12 @@ SM_COUNT, FP32_LANES, MUFU_LANES = 148, 128, 16           # per B200 / per SM pe
 NCU_TRAFFIC = {("cfg2", "recur"): 239104, ("cfg4", "recur"): 32843264 + 163584, ("cfg5", "recur"): 3336192}
 
 
+TABLE1 = {f"table1_{n}": n for n in (1000, 2000, 4000, 10000, 20000, 40000, 100000)}       # the paper's Table I rows
+
+
 def make_workload(name: str, rank: int = 0):
+    if name in TABLE1:
+        return wl.table1(TABLE1[name])
     if name == "cfg2" and rank:
         return wl.cfg2(seed_off=2 + 1000 * rank, tag=f"cfg2_globular_10k_rank{rank}")
     return wl.CONFIGS[name]()
@@ -158,7 +163,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", default="cfg2", choices=sorted(wl.CONFIGS))
+    ap.add_argument("--config", default="cfg2", choices=sorted(wl.CONFIGS) + list(TABLE1),
+                    help="cfg1..cfg5: BASELINE.json's configs; table1_N: the shape of the paper's Table I rows (N atoms, 50 q on (0, 1])")
     ap.add_argument("--variant", default="auto", choices=["auto", "recur", "mufu", "accurate", "fp64"])
     ap.add_argument("--impl", default="libdebye", choices=["libdebye", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -550,3 +550,25 @@ def test_peratom_degenerate_inputs(db):
     # bad flags are rejected before anything is launched
     with pytest.raises(db.LibdebyeError):
         db.debye_profile_peratom(torch.from_numpy(w.xyz).cuda(), torch.from_numpy(ff).cuda(), torch.zeros(1, device="cuda"), variant="recur")
+    # caller-owned workspace (include/debye.h: at most 1.3 MB + 1 KB x M): same bits; too small a workspace is refused; and the
+    # sharded and unsharded per-type calls run from the same caller workspace
+    w = wl.small_random(98, 900, 3, 45)
+    ff = _peratom_ff(w, 98)
+    x, t, f, q = to_dev(w)
+    fd = torch.from_numpy(ff).cuda()
+    ref = db.debye_profile_peratom(x, fd, q).cpu().numpy()
+    part_ref = db.debye_partials_shard(x, t, q, w.T, 1, 2)[0].cpu().numpy()
+    L = db.lib()
+    need = max(1400000 + 1024 * w.M, L.debye_workspace_bytes(w.N, 1, w.T, w.M, 0))
+    buf = torch.empty(need + 256, dtype=torch.uint8, device="cuda")
+    ptr = (buf.data_ptr() + 255) // 256 * 256
+    assert L.debye_set_workspace(ptr, need) == 0
+    try:
+        assert db.debye_profile_peratom(x, fd, q).cpu().numpy().tobytes() == ref.tobytes()
+        assert db.debye_partials_shard(x, t, q, w.T, 1, 2)[0].cpu().numpy().tobytes() == part_ref.tobytes()
+        assert L.debye_set_workspace(ptr, 1024) == 0
+        with pytest.raises(db.LibdebyeError):
+            db.debye_profile_peratom(x, fd, q)
+    finally:
+        assert L.debye_set_workspace(None, 0) == 0
+    assert db.debye_profile_peratom(x, fd, q).cpu().numpy().tobytes() == ref.tobytes()

@@ -48,6 +48,11 @@ def _worker(rank, world, port, tmp):
     allp = sharding.gather_partials(part, world)
     if rank == 1:
         np.save(os.path.join(tmp, "allp.npy"), allp.numpy())
+    # the whole helper with stand-ins for the two library calls: every rank must end with the rank-ordered sum
+    tot = sharding.profile_tile_split(lambda r, wd: (torch.full((1, 3, 7), float(10 ** r), dtype=torch.float64), None),
+                                      lambda S, n, f: (S * torch.arange(1, S.shape[0] + 1, dtype=torch.float64)[:, None, None, None]).sum(0),
+                                      None, rank, world)
+    np.save(os.path.join(tmp, f"tot{rank}.npy"), tot.numpy())
     t = sharding.max_over_ranks(1.0 + rank)
     s = sharding.sum_over_ranks(hi - lo)
     if rank == 0:
@@ -71,5 +76,7 @@ def test_two_rank_gloo_shards_and_gathers(tmp_path):
     assert allp.shape == (2, 2, 3, 7)
     for r in range(2):
         assert np.array_equal(allp[r], np.broadcast_to((r + 1) * np.arange(7.0), (2, 3, 7)))
+    for r in range(2):      # 1 * 10^0 + 2 * 10^1: the parts arrive in rank order on every rank
+        assert np.array_equal(np.load(tmp_path / f"tot{r}.npy"), np.full((1, 3, 7), 21.0))
     t, s = np.load(tmp_path / "ts.npy")
     assert t == 2.0 and s == 5.0

@@ -168,6 +168,10 @@ def main():
     ap.add_argument("--variant", default="auto", choices=["auto", "recur", "mufu", "accurate", "fp64"])
     ap.add_argument("--impl", default="libdebye", choices=["libdebye", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--split", default="structures", choices=["structures", "tiles"],
+                    help="multi-GPU decomposition: structures = every rank its own structure (weak scaling, no collective; the "
+                         "default); tiles = ONE structure split over the ranks by tiles of the upper triangle, one all-gather of FP64 "
+                         "partials per profile (strong scaling; debye_partials_shard + debye_profile_from_partials)")
     ap.add_argument("--path", default="pertype", choices=["pertype", "peratom"],
                     help="pertype: the north_star path (debye_profile, form factors per atom type); peratom: the paper's general "
                          "case (debye_profile_peratom, one form-factor row per atom; NEXT-1)")
@@ -194,6 +198,8 @@ def main():
     w = make_workload(args.config, rank)
     if args.path == "peratom":
         return run_peratom(args, w, rank, world, dev)
+    if args.split == "tiles":
+        return run_tile_split(args, make_workload(args.config, 0), rank, world, dev)
     batch = w.xyz.ndim == 3
     call = db.debye_profile_batch if batch else db.debye_profile
     call_host = db.debye_profile_batch_host if batch else db.debye_profile_host
@@ -323,6 +329,78 @@ def main():
             ref = orc.debye_sym(w.xyz, w.type, w.fftab[:, ks].copy(), w.q[ks].copy())
             line["parity_max_rel_err"] = float(np.max(np.abs(result_dev[ks] - ref) / np.abs(ref)))
         line["cpu_baseline"] = cb
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_tile_split(args, w, rank, world, dev):
+    """--split tiles: one step = one profile of ONE structure on all ranks: debye_partials_shard(rank, world) (setup, pack,
+    pairs CTAs c with c % world == rank, final), NCCL all-gather of S[B][T(T+1)/2][M] FP64, debye_profile_from_partials
+    (rank-ordered sum + epilogue).  Strong scaling: total work is fixed.  Every rank ends with the full profile."""
+    import torch
+    import torch.distributed as dist
+    from paper_1306_2258_b200 import binding as db, sharding
+    x, t, f, q = (torch.from_numpy(a).to(dev) for a in (w.xyz, w.type, w.fftab, w.q))
+    hint = 0 if args.no_hint else db.q_hint(w.q)
+    flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    info = db.launch_info(w.N, w.B, w.T, w.M, args.variant, with_grid=True, hint=hint)
+
+    def step():
+        return sharding.profile_tile_split(
+            lambda r, wd: db.debye_partials_shard(x, t, q, w.T, r, wd, variant=args.variant, hint=hint),
+            db.debye_profile_from_partials, f, rank, world)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        out = step()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    for a, b in ev:
+        flush.fill_(1)
+        a.record()
+        out = step()
+        b.record()
+    barrier()
+    clocks = sampler.stop()
+    total_ms = sharding.max_over_ranks(float(np.sum([a.elapsed_time(b) for a, b in ev])), dev)
+    value = float(w.pair_q) * args.steps / (total_ms * 1e-3) / 1e9              # one structure: the job's units are not multiplied by N
+    t0 = time.perf_counter()
+    n_e2e = max(5, min(args.steps, 50))
+    hx = torch.from_numpy(w.xyz).pin_memory()
+    for _ in range(n_e2e):                                                       # coordinates from pinned host memory, profile read back
+        x.copy_(hx, non_blocking=True)
+        res = step().cpu()
+    barrier()
+    e2e_s = sharding.max_over_ranks(time.perf_counter() - t0, dev)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "dtype": "f64" if args.variant == "fp64" else "f32", "data": "synthetic",
+        "config": {"workload": w.name, "N": w.N, "T": w.T, "M": w.M, "B": w.B, "variant": args.variant, "pairs_grid": info["pairs_grid"],
+                   "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
+                   "parallelism": f"one structure split over {world} rank(s) by tiles; all-gather of {w.B * w.T * (w.T + 1) // 2 * w.M * 8} B per rank"},
+        "clocks": clocks,
+        "e2e": {"value": float(w.pair_q) * n_e2e / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(hx.numpy().nbytes),
+                "d2h_bytes_per_step": int(res.numpy().nbytes), "ms_per_step": e2e_s / n_e2e * 1e3, "steps": n_e2e},
+        "gpu_launches": (info["n_launches"] + 1) * args.steps,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle as orc
+        if w.xyz.ndim == 2:
+            ks = list(range(0, w.M, max(1, w.M // 8)))
+            ref = orc.debye_sym(w.xyz, w.type, w.fftab[:, ks].copy(), w.q[ks].copy())
+            line["parity_max_rel_err"] = float(np.max(np.abs(out.cpu().numpy()[0][ks] - ref) / np.abs(ref)))
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

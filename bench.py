@@ -489,7 +489,9 @@ def run_peratom(args, w, rank, world, dev):
         "e2e": {"value": units * n_e2e / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(hx.nbytes + hf.nbytes + hq.nbytes),
                 "d2h_bytes_per_step": int(hout.nbytes), "ms_per_step": e2e_s / n_e2e * 1e3, "steps": n_e2e},
         "gpu_launches": 3 * args.steps,
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T sin/s", "frac": achieved / peak, "traffic": None,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T sin/s", "frac": achieved / peak,
+                     # dram__bytes_read.sum + write.sum of the pairs kernel from the full ncu capture (profiles/r01_v6.md)
+                     "traffic": 4248064 if (args.config == "cfg2" and variant != "fp64") else None,
                      "note": "XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM x 148 SM x sm_max_mhz; the q-chunks "
                              "are padded (M = 101 runs 4 x 28 = 112 slots), which the algorithmic count does not credit",
                      "kernel": f"debye_peratom_pairs_kernel<{'fp64' if variant == 'fp64' else 'fp32'}>", "kernel_ms": pairs_ms,

@@ -131,7 +131,6 @@ def test_tile_split_full_size_against_stored_oracle(db):
         I = db.debye_profile_from_partials(torch.stack([p[0] for p in parts]), parts[0][1], f).cpu().numpy()[0]
         assert check(I, golden()[name], w, TOL32) <= 1e-5
         # every rank got about a quarter of the pair sums (cyclic CTAs keep the triangular load balanced)
-        k = w.M // 2
         share = torch.stack([p[0][0, :, 1].abs().sum() for p in parts])          # q index 1: all terms positive-ish
         assert float(share.min() / share.max()) > 0.8
 

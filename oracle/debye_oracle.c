@@ -25,7 +25,9 @@
  *
  * Pins (tests/test_oracle_pins.py): two-atom closed form, I(0) = (sum f)^2, Eq. (1) by spherical quadrature,
  * chain / lattice / triangle / tetrahedron closed forms, coincident atoms, low-q expansion, rotation /
- * translation / permutation invariance, scaling identities, full == sym.
+ * translation / permutation invariance, scaling identities, full == sym.  oracle_debye_peratom (R10p): two-atom and
+ * triangle closed forms with different atoms, I(0) = (sum f)^2, Eq. (1) quadrature with a different f on every atom,
+ * reduction to the per-type and weighted oracles, separable rows, permutation, full == sym (test_peratom_oracle_pins).
  */
 #include <math.h>
 #include <stdint.h>

@@ -175,6 +175,9 @@ def main():
     ap.add_argument("--path", default="pertype", choices=["pertype", "peratom"],
                     help="pertype: the north_star path (debye_profile, form factors per atom type); peratom: the paper's general "
                          "case (debye_profile_peratom, one form-factor row per atom; NEXT-1)")
+    ap.add_argument("--peaks", action="store_true",
+                    help="measure what one SM delivers on the instruction mixes of the pairs kernels (debye_pipe_bench) and the MUFU.SIN "
+                         "error statistics; prints one JSON object and exits")
     ap.add_argument("--no-hint", action="store_true", help="do not pass the q-grid hint (DEBYE_QHINT_*) computed from the host copy of q")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "libdebye" else args.warmup
@@ -195,6 +198,8 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
     db.lib()
 
+    if args.peaks:
+        return run_peaks(dev) if rank == 0 else None
     w = make_workload(args.config, rank)
     if args.path == "peratom":
         return run_peratom(args, w, rank, world, dev)
@@ -332,6 +337,29 @@ def main():
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_peaks(dev):
+    """--peaks: the measured side of the "alu" roofline.  Rates are per SM clock (clock64 inside the kernels), so they do
+    not depend on the clock the part runs at; nominal: 128 FP32 lanes and 16 MUFU lanes per SM and clock."""
+    from paper_1306_2258_b200 import binding as db
+    L = db.lib()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    tests = []
+    for t in range(L.debye_pipe_bench_count()):
+        row = {"test": t}
+        for c in (1, 2, 3, 4):
+            r = db.pipe_bench(t, c)
+            if r is None:
+                continue
+            row["name"] = r[0]
+            row[f"ctas{c}"] = {"lane_ops_per_clk_per_sm": round(r[1], 2), "sched_cycles_per_instr": round(r[2], 3)}
+        tests.append(row)
+    mx, rms, mean = db.mufu_sin_error()
+    print(json.dumps({"pipe_bench": tests, "nominal": {"fp32_lanes_per_clk_per_sm": FP32_LANES, "mufu_lanes_per_clk_per_sm": MUFU_LANES},
+                      "mufu_sin_error_on_0_to_half_turn": {"max_abs": mx, "rms": rms, "mean": mean, "points": 1 << 24},
+                      "clocks": sampler.stop()}))
 
 
 def run_tile_split(args, w, rank, world, dev):

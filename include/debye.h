@@ -195,6 +195,22 @@ int debye_launch_info(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags
  * dominant kernel -- so its device time can be read with cudaEventElapsedTime.  NULL, NULL switches it off. */
 int debye_set_pairs_events(void *start_event, void *stop_event);
 
+/* Diagnostics behind `bench.py --peaks` (the FP32 / MUFU issue peaks "are nominal; the build must
+ * measure them"): micro-kernels of the instruction mixes the pairs kernels consist of, run on every SM of the current
+ * device with ctas_per_sm (1..4) CTAs of 128 threads resident per SM; blocking (synchronise `stream`).
+ *   test in [0, debye_pipe_bench_count()); debye_pipe_bench_name(test) describes it (NULL outside the range).
+ *   *lane_ops_per_clk_per_sm: FP32-pipe (for the MUFU test: XU) lane-operations per SM clock cycle and SM, measured with
+ *   clock64 inside the kernel, so independent of the clock the part happens to run at (nominal: 128, MUFU 16);
+ *   *cycles_per_instr (may be NULL): cycles of one warp scheduler per warp instruction of the mix.
+ * Errors: DEBYE_EINVAL bad arguments, DEBYE_EUNSUPPORTED if ctas_per_sm CTAs of that test do not fit on an SM.
+ * debye_mufu_sin_error: error of MUFU.SIN (sin.approx.ftz.f32 of 2 pi t) against double sin on n points of (0, 1/2] turns:
+ * maximum |e|, root mean square, and MEAN (a bias is a coherent error in every pair: DESIGN.md section 6). */
+int debye_pipe_bench_count(void);
+const char *debye_pipe_bench_name(int test);
+int debye_pipe_bench(int test, int ctas_per_sm, int iters, double *lane_ops_per_clk_per_sm, double *cycles_per_instr,
+                     debye_stream_t stream);
+int debye_mufu_sin_error(int n, double *max_abs, double *rms, double *mean, debye_stream_t stream);
+
 const char *debye_strerror(int status);
 int debye_last_cuda_error(void); /* cudaError_t of the last failing runtime call on this thread, 0 if none */
 int debye_version(void);         /* major*10000 + minor*100 + patch */

@@ -11,7 +11,8 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libdebye.so")
+# LIBDEBYE_PATH: load another build of the same library (e.g. one compiled with different tuning macros)
+LIB_PATH = os.environ.get("LIBDEBYE_PATH") or os.path.join(HERE, "libdebye.so")
 
 FLAGS = {"fp64": 1 << 0, "mufu": 1 << 2, "recur": 1 << 3, "accurate": 1 << 4, "auto": 0}
 
@@ -19,7 +20,8 @@ EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_
            "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials",
            "debye_partials_shard", "debye_profile_from_partials", "debye_profile_peratom", "debye_profile_peratom_host", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
            "debye_launch_info", "debye_set_pairs_events", "debye_q_hint", "debye_plan_create", "debye_plan_execute",
-           "debye_plan_destroy", "debye_strerror", "debye_last_cuda_error", "debye_version")
+           "debye_plan_destroy", "debye_strerror", "debye_last_cuda_error", "debye_version", "debye_pipe_bench_count",
+           "debye_pipe_bench_name", "debye_pipe_bench", "debye_mufu_sin_error")
 
 
 class LibdebyeError(RuntimeError):
@@ -82,6 +84,13 @@ def lib():
     L.debye_strerror.restype = C.c_char_p
     L.debye_last_cuda_error.restype = C.c_int
     L.debye_version.restype = C.c_int
+    L.debye_pipe_bench_count.restype = C.c_int
+    L.debye_pipe_bench_name.argtypes = [C.c_int]
+    L.debye_pipe_bench_name.restype = C.c_char_p
+    L.debye_pipe_bench.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
+    L.debye_pipe_bench.restype = C.c_int
+    L.debye_mufu_sin_error.argtypes = [C.c_int] + [C.POINTER(C.c_double)] * 3 + [vp]
+    L.debye_mufu_sin_error.restype = C.c_int
     _lib = L
     return L
 
@@ -318,3 +327,22 @@ def launch_info(N, B, T, M, variant="auto", with_grid=False, hint=0):
     if with_grid:
         out["pairs_grid"] = g.value
     return out
+
+
+def pipe_bench(test: int, ctas_per_sm: int, iters: int = 2000, stream=None):
+    """(name, FP32-pipe lane-operations per clock and SM, scheduler cycles per warp instruction) of one micro-kernel
+    (include/debye.h, debye_pipe_bench); None if ctas_per_sm CTAs of that test do not fit on an SM."""
+    L = lib()
+    rate, cpi = C.c_double(), C.c_double()
+    st = L.debye_pipe_bench(test, ctas_per_sm, iters, C.byref(rate), C.byref(cpi), _stream_ptr(stream))
+    if st == 2:
+        return None
+    _check(st)
+    return L.debye_pipe_bench_name(test).decode(), rate.value, cpi.value
+
+
+def mufu_sin_error(n: int = 1 << 24, stream=None):
+    """max |e|, rms, mean of MUFU.SIN against double sin on n points of (0, 1/2] turns (debye_mufu_sin_error)."""
+    mx, rms, mean = C.c_double(), C.c_double(), C.c_double()
+    _check(lib().debye_mufu_sin_error(n, C.byref(mx), C.byref(rms), C.byref(mean), _stream_ptr(stream)))
+    return mx.value, rms.value, mean.value

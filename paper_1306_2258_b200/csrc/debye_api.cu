@@ -5,7 +5,8 @@
 //   debye_pack_kernel               gather into type-sorted float4                                     S0
 //   debye_pairs_kernel<K, variant>  persistent grid, one or (automatic mode) two launches of which     S1-S6
 //                                   the one not selected on the device exits immediately
-//   debye_final_kernel              fixed-order FP64 reduction + form-factor epilogue                  S7
+//   debye_reduce_kernel             fixed-order FP64 sum of the per-CTA records                        S7
+//   debye_epilogue_kernel           telescoping of the product form, form-factor epilogue              S7
 #include <cuda_runtime.h>
 #include <cstdint>
 #include <cstdio>
@@ -98,19 +99,22 @@ int recur_choices(Choice *out, int M)
     return 1;
 }
 
-struct Layout { size_t plan, perm, sorted, records, total; };
+struct Layout { size_t plan, perm, sorted, records, sums, total; };
 Layout layout(int N, int B, int T, int M, int G_max, const Choice *ch, int nch)
 {
     Layout L; size_t o = 0;
     L.plan = o; o += align_up(sizeof(DevPlan));
     L.perm = o; o += align_up((size_t)N * 4);
     L.sorted = o; o += align_up((size_t)N * B * 16);
-    size_t rec = 0;
+    size_t rec = 0, sm = 0;
     for (int i = 0; i < nch; ++i) {
         size_t r = ((size_t)G_max + (size_t)B * (T * (T + 1) / 2) * ch[i].n_chunks) * ch[i].K * 8;
+        size_t m = (size_t)B * (T * (T + 1) / 2) * ch[i].n_chunks * ch[i].K * 8;
         if (r > rec) rec = r;
+        if (m > sm) sm = m;
     }
     L.records = o; o += align_up(rec);
+    L.sums = o; o += align_up(sm);
     L.total = o;
     return L;
 }
@@ -275,6 +279,7 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     int32_t *perm = pre ? pre->perm : (int32_t *)(ws + L.perm);
     float4 *sorted = (float4 *)(ws + L.sorted);
     double *records = (double *)(ws + L.records);
+    double *sums = (double *)(ws + L.sums);
 
     int alt_offered = 0;
     for (int i = 0; i < nch; ++i) if (ch[i].alt_gate == 1) alt_offered = 1;
@@ -286,7 +291,7 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     }
     const bool pack_here = !pre && (int64_t)N * B <= DEBYE_PACK_IN_SETUP;      // small inputs: the setup CTA gathers too
     // tile split over GPUs: the pairs CTAs of the other ranks do not run here; their records must read as zero
-    if (shard_world > 1) CU(cudaMemsetAsync(records, 0, L.total - L.records, stream));
+    if (shard_world > 1) CU(cudaMemsetAsync(records, 0, L.sums - L.records, stream));
     if (!pre) debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, hint_class, xyz, sorted, pack_here ? 1 : 0, weight,
                                                                                 shard_rank, shard_world);
     if (!pack_here) {
@@ -308,14 +313,19 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     }
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
     {
-        int threads = DEBYE_FINAL_THREADS, blocks = B * ((M + DEBYE_FINAL_Q - 1) / DEBYE_FINAL_Q);
-        // the final kernel repeats the device-side decisions of the pairs launches to find the one that did the work
+        // the final kernels repeat the device-side decisions of the pairs launches to find the one that did the work
         debye::FinalSets sets; sets.n = nch;
+        int64_t red_blocks = 0;
         for (int i = 0; i < MAX_CHOICES; ++i) {
             const int j = i < nch ? i : 0;
             sets.s[i].variant = ch[j].variant; sets.s[i].K = ch[j].K; sets.s[i].n_chunks = ch[j].n_chunks; sets.s[i].G = G[j]; sets.s[i].alt_gate = ch[j].alt_gate;
+            const int64_t nb = (int64_t)B * (T * (T + 1) / 2) * ch[j].n_chunks * ((ch[j].K + 31) / 32);
+            if (nb > red_blocks) red_blocks = nb;
         }
-        CU(launch_pdl(debye::debye_final_kernel, dim3(blocks), dim3(threads), stream, (const DevPlan *)plan, (const double *)records, fftab, q, out, is_auto, sets, mode));
+        if (red_blocks > 0x7fffffff) return DEBYE_EUNSUPPORTED;
+        CU(launch_pdl(debye::debye_reduce_kernel, dim3((unsigned)red_blocks), dim3(DEBYE_RED_THREADS), stream, (const DevPlan *)plan, (const double *)records, sums, is_auto, sets));
+        const int blocks = B * ((M + DEBYE_FINAL_Q - 1) / DEBYE_FINAL_Q);
+        CU(launch_pdl(debye::debye_epilogue_kernel, dim3(blocks), dim3(DEBYE_FINAL_THREADS), stream, (const DevPlan *)plan, (const double *)sums, fftab, q, out, is_auto, sets, mode));
     }
     if (mode == 1 && n_out) CU(cudaMemcpyAsync(n_out, plan->n_a, sizeof(int32_t) * T, cudaMemcpyDeviceToDevice, stream));
     CU(cudaGetLastError());
@@ -636,7 +646,7 @@ int debye_launch_info(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags
     Choice ch[MAX_CHOICES]; int is_auto;
     int nch = variants_for(flags, ch, M, &is_auto);
     const int lead = (nch > 1 && ch[0].alt_gate == 1) ? 1 : 0;     // report the launch sized for the general case
-    if (n_launches) *n_launches = 2 + nch + (((int64_t)N * B <= DEBYE_PACK_IN_SETUP) ? 0 : 1);   // setup, [pack], pairs x nch, final
+    if (n_launches) *n_launches = 3 + nch + (((int64_t)N * B <= DEBYE_PACK_IN_SETUP) ? 0 : 1);   // setup, [pack], pairs x nch, reduce, epilogue
     if (q_chunk) *q_chunk = ch[lead].K;
     if (n_chunks) *n_chunks = ch[lead].n_chunks;
     if (pairs_grid) {

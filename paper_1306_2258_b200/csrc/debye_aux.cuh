@@ -188,51 +188,103 @@ __global__ void debye_weight_sums_kernel(DevPlan *plan, const float4 *__restrict
 // number of unordered pairs of type pair (a, b)
 __device__ __forceinline__ double pair_count(int na, int nb, bool diag) { return diag ? 0.5 * (double)na * (double)(na - 1) : (double)na * (double)nb; }
 
-// S7: fixed-order FP64 sum of the per-CTA records, then the form-factor epilogue
-//   I(q_k) = sum_a n_a F_a^2 + 2 sum_{a<=b} F_a F_b S_ab(q_k),   S_ab = (1/q_k) sum sin(q_k r)/r  (q_k != 0), #pairs (q_k == 0).
-// Block = (conformer, tile of DEBYE_FINAL_Q q indices); thread (kk, g, sl) handles q index k0 + kk, the type pairs
-// g, g + G8, ... in increasing order and, of each type pair's CTA range [c_lo, c_hi], the sl-th of NS equal slices.
-// The partial sums are then added in (g, sl) order.  The slicing is a fixed function of (U, G), so every order is fixed
-// and the result is bitwise reproducible.  mode 0: write I_out[b][k]; mode 1 (NS must be 1): write S_out[b][tp][k].
+// S7 in two launches.
+// (a) debye_reduce_kernel: fixed-order FP64 sum of the per-CTA records of every (conformer, type pair, q-chunk) X:
+//         sums[X][l] = sum over the CTAs c that worked on X, in CTA order, of records[(c + X) K + l].
+//     Block = (X, group of 32 slots); thread (lane, sl) adds the sl-th of NS equal slices of the CTA range for slot
+//     32 g + lane (coalesced over the slots); the slices are then added in slice order.  The slicing is a fixed function
+//     of (U, G), so every order is fixed and the result is bitwise reproducible.
+// (b) debye_epilogue_kernel: per output q_k and type pair the slot (chunk, l) of the sum -- or, for the product form of
+//     the recurrence, the telescoped chain of slots  B_{Sj+k0} = Out[j][k0] + B_{Sj-k0}  (debye_pairs.cuh) -- then
+//         I(q_k) = sum_a n_a F_a^2 + 2 sum_{a<=b} F_a F_b S_ab(q_k),  S_ab = (1/q_k) sum sin(q_k r)/r  (q_k != 0), #pairs (q_k == 0).
+//     Block = (conformer, tile of 8 q indices); thread (kk, g) handles q index k0 + kk and the type pairs g, g + 32, ...
+//     in increasing order; the partial sums are added in g order.  mode 0: write I_out[b][k]; mode 1: S_out[b][tp][k].
+#define DEBYE_RED_NS 8
+#define DEBYE_RED_THREADS (32 * DEBYE_RED_NS)
 #define DEBYE_FINAL_Q 8
-#define DEBYE_FINAL_G 8
-#define DEBYE_FINAL_NS 4
-#define DEBYE_FINAL_THREADS (DEBYE_FINAL_Q * DEBYE_FINAL_G * DEBYE_FINAL_NS)
+#define DEBYE_FINAL_G 32
+#define DEBYE_FINAL_THREADS (DEBYE_FINAL_Q * DEBYE_FINAL_G)
 struct FinalSet { int variant, K, n_chunks, G, alt_gate; };   // parameters of one pairs launch (alt_gate as in the pairs kernel)
 struct FinalSets { FinalSet s[3]; int n; };                    // up to: recurrence (M - 1 indices), recurrence, MUFU
-__global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const DevPlan *__restrict__ plan, const double *__restrict__ records,
-                                                                            const float *__restrict__ fftab, const float *__restrict__ q, double *__restrict__ out,
-                                                                            int is_auto, const FinalSets sets, int mode)
+// which pairs launch did the work: the same device-side decisions the pairs kernels took
+__device__ __forceinline__ int final_pick(const DevPlan *plan, const FinalSets &sets, int is_auto)
 {
-    __shared__ double part[DEBYE_FINAL_G * DEBYE_FINAL_NS][DEBYE_FINAL_Q];
-    pdl_wait();
-    const int M = plan->M, Bn = plan->B, T = plan->T, n_tp = plan->n_tp;
-    const int ktiles = (M + DEBYE_FINAL_Q - 1) / DEBYE_FINAL_Q;
-    const int kk = threadIdx.x % DEBYE_FINAL_Q, gs = threadIdx.x / DEBYE_FINAL_Q;
-    const int NS = (mode == 0) ? DEBYE_FINAL_NS : 1;
-    const int g = gs / DEBYE_FINAL_NS, sl = gs % DEBYE_FINAL_NS;
-    const int b = blockIdx.x / ktiles, k = (blockIdx.x % ktiles) * DEBYE_FINAL_Q + kk;
-    const bool live = k < M && sl < NS;
-    // which pairs launch did the work: the same device-side decisions the pairs kernels took
-    int pick = 0;
     for (int i = 0; i < sets.n; ++i) {
         const FinalSet &c = sets.s[i];
-        if ((!is_auto || plan->variant_auto == c.variant) && (c.alt_gate < 0 || plan->recur_alt == c.alt_gate)) { pick = i; break; }
+        if ((!is_auto || plan->variant_auto == c.variant) && (c.alt_gate < 0 || plan->recur_alt == c.alt_gate)) return i;
     }
-    const int variant = sets.s[pick].variant, K = sets.s[pick].K, n_chunks = sets.s[pick].n_chunks, G = sets.s[pick].G;
+    return 0;
+}
+__global__ void __launch_bounds__(DEBYE_RED_THREADS) debye_reduce_kernel(const DevPlan *__restrict__ plan, const double *__restrict__ records,
+                                                                           double *__restrict__ sums, int is_auto, const FinalSets sets)
+{
+    __shared__ double part[DEBYE_RED_NS][32];
+    pdl_wait();
+    pdl_trigger();
+    const int pick = final_pick(plan, sets, is_auto);
+    const int K = sets.s[pick].K, n_chunks = sets.s[pick].n_chunks, G = sets.s[pick].G;
+    const int Bn = plan->B, n_tp = plan->n_tp;
+    const int groups = (K + 31) / 32;
+    const int64_t nX = (int64_t)Bn * n_tp * n_chunks;
+    if ((int64_t)blockIdx.x >= nX * groups) return;             // the grid is sized for the largest of the offered launches
+    const int64_t X = blockIdx.x / groups;
+    const int lane = threadIdx.x & 31, sl = threadIdx.x >> 5;
+    const int l = (int)(blockIdx.x % groups) * 32 + lane;
+    const int ch = (int)(X % n_chunks), tp = (int)((X / n_chunks) % n_tp), b = (int)(X / ((int64_t)n_chunks * n_tp));
+    const int64_t U1 = plan->U1, Uc = U1 * n_chunks, U = Uc * Bn;
+    const int64_t units = plan->tp_prefix[tp + 1] - plan->tp_prefix[tp];
+    double s = 0.0;
+    if (l < K && units > 0 && U > 0) {
+        const DebyeRanges ranges(U, G);
+        const int64_t ub = (int64_t)b * Uc + plan->tp_prefix[tp] * n_chunks + (int64_t)ch * units;
+        const int64_t ue = ub + units - 1;
+        if (U >= G) {           // every CTA owns at least one unit: all CTAs between the owners took part
+            const int c_lo = ranges.owner(ub), c_hi = ranges.owner(ue);
+            const int n = c_hi - c_lo + 1, per = (n + DEBYE_RED_NS - 1) / DEBYE_RED_NS;
+            const int cb = c_lo + sl * per, ce = min(c_hi + 1, cb + per);
+            const double *rp = records + ((int64_t)cb + X) * K + l;
+            int c = cb;
+            for (; c + 4 <= ce; c += 4, rp += 4 * (int64_t)K) {
+                const double r0 = rp[0], r1 = rp[K], r2 = rp[2 * (int64_t)K], r3 = rp[3 * (int64_t)K];
+                s += r0; s += r1; s += r2; s += r3;
+            }
+            for (; c < ce; ++c, rp += K) s += rp[0];
+        } else if (sl == 0) {   // fewer units than CTAs: each unit has its own CTA
+            for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)ranges.owner(u) + X) * K + l];
+        }
+    }
+    part[sl][lane] = s;
+    __syncthreads();
+    if (sl == 0 && l < K) {
+        double tot = 0.0;
+#pragma unroll
+        for (int x = 0; x < DEBYE_RED_NS; ++x) tot += part[x][lane];
+        sums[X * K + l] = tot;
+    }
+}
+
+__global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_epilogue_kernel(const DevPlan *__restrict__ plan, const double *__restrict__ sums,
+                                                                               const float *__restrict__ fftab, const float *__restrict__ q, double *__restrict__ out,
+                                                                               int is_auto, const FinalSets sets, int mode)
+{
+    __shared__ double part[DEBYE_FINAL_G][DEBYE_FINAL_Q];
+    pdl_wait();
+    const int M = plan->M, T = plan->T, n_tp = plan->n_tp;
+    const int ktiles = (M + DEBYE_FINAL_Q - 1) / DEBYE_FINAL_Q;
+    const int kk = threadIdx.x % DEBYE_FINAL_Q, g = threadIdx.x / DEBYE_FINAL_Q;
+    const int b = blockIdx.x / ktiles, k = (blockIdx.x % ktiles) * DEBYE_FINAL_Q + kk;
+    const int pick = final_pick(plan, sets, is_auto);
+    const int variant = sets.s[pick].variant, K = sets.s[pick].K, n_chunks = sets.s[pick].n_chunks;
     const bool bad = (variant == V_RECUR && !plan->uniform) || plan->hint_bad;   // forced recurrence on a non-uniform grid, or a wrong grid hint -> NaN
     const double nan = __longlong_as_double(0x7ff8000000000000LL);
     const double scale = (variant == V_RECUR) ? 0.5 : 1.0;            // the recurrence kernel accumulates 2 sin(q r)/r
+    // recurrence on a grid (k + koff) dq with at most 2 chunks ran in product form (the same test as in the pairs kernel)
+    const bool product = variant == V_RECUR && plan->zero_start >= 0 && n_chunks <= 2;
     double I = 0.0;
-    if (live) {
-        // chain / grid index of output k (convention at slot_of); -1 only for q = 0, which never reads a record
-        int idx = k;
-        if (variant == V_RECUR && plan->zero_start >= 0 && n_chunks <= 2) idx = k + plan->zero_start - 1;
-        int ch = 0, l = 0;
-        if (idx >= 0) slot_of(variant, K, n_chunks, idx, ch, l);
+    if (k < M) {
+        // chain / grid index of output k (convention at slot_of); -1 only for q = 0, which never reads a sum
+        const int idx = product ? k + plan->zero_start - 1 : k;
         const double qk = (double)q[k];
-        const int64_t U1 = plan->U1, Uc = U1 * n_chunks, U = Uc * Bn;
-        const DebyeRanges ranges(U > 0 ? U : 1, G);
         // type pair index -> (a, b2): walk rows of the upper triangle
         int a = 0, rowstart = 0;
         for (int tp = g; tp < n_tp; tp += DEBYE_FINAL_G) {
@@ -240,32 +292,29 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
             const int b2 = a + (tp - rowstart);
             double S;
             const int64_t units = plan->tp_prefix[tp + 1] - plan->tp_prefix[tp];
-            if (bad) S = (sl == 0) ? nan : 0.0;
+            if (bad) S = nan;
             else if (qk == 0.0 || units == 0) {
                 // sum over the pairs of w_i w_j sinc(0): the pair count, or with weights sw_a sw_b resp. (sw_a^2 - sw2_a) / 2
                 double cnt = pair_count(plan->n_a[a], plan->n_a[b2], a == b2);
                 if (plan->weighted && units != 0) cnt = (a == b2) ? 0.5 * (plan->sw[a] * plan->sw[a] - plan->sw2[a]) : plan->sw[a] * plan->sw[b2];
                 // tile split over GPUs: the closed-form terms are nobody's tile, rank 0 contributes them
-                S = (sl == 0 && plan->shard_rank == 0) ? cnt : 0.0;
+                S = (plan->shard_rank == 0) ? cnt : 0.0;
             }
             else {
-                const int64_t ub = (int64_t)b * Uc + plan->tp_prefix[tp] * n_chunks + (int64_t)ch * units;
-                const int64_t ue = ub + units - 1;
-                const int64_t X = ((int64_t)b * n_tp + tp) * n_chunks + ch;
+                const double *sp = sums + ((int64_t)b * n_tp + tp) * n_chunks * (int64_t)K;
                 double s = 0.0;
-                if (U >= G) {           // every CTA owns at least one unit: all CTAs between the owners took part
-                    const int c_lo = ranges.owner(ub), c_hi = ranges.owner(ue);
-                    const int n = c_hi - c_lo + 1, per = (n + NS - 1) / NS;
-                    const int cb = c_lo + sl * per, ce = min(c_hi + 1, cb + per);
-                    const double *rp = records + ((int64_t)cb + X) * K + l;
-                    int c = cb;
-                    for (; c + 4 <= ce; c += 4, rp += 4 * (int64_t)K) {
-                        const double r0 = rp[0], r1 = rp[K], r2 = rp[2 * (int64_t)K], r3 = rp[3 * (int64_t)K];
-                        s += r0; s += r1; s += r2; s += r3;
+                if (product) {
+                    // kappa = idx + 1 = S j + kres with kres in 1..S:  B_kappa = Out[slot(kappa)] + B_{S j - kres}
+                    const int Sres = 8 * n_chunks;
+                    for (int kap = idx + 1; kap > 0;) {
+                        const int j = (kap - 1) / Sres, kres = kap - Sres * j;
+                        s += sp[(int64_t)((kres - 1) >> 3) * K + 8 * j + ((kres - 1) & 7)];
+                        kap = Sres * j - kres;
                     }
-                    for (; c < ce; ++c, rp += K) s += rp[0];
-                } else if (sl == 0) {   // fewer units than CTAs: each unit has its own CTA
-                    for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)ranges.owner(u) + X) * K + l];
+                } else {
+                    int ch = 0, l = 0;
+                    slot_of(variant, K, n_chunks, idx, ch, l);
+                    s = sp[(int64_t)ch * K + l];
                 }
                 S = scale * s / qk;
             }
@@ -274,13 +323,13 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_final_kernel(const 
         }
     }
     if (mode != 0) return;
-    part[gs][kk] = I;
+    part[g][kk] = I;
     __syncthreads();
-    if (gs == 0 && k < M) {
+    if (g == 0 && k < M) {
         double tot = 0.0;
         for (int a = 0; a < T; ++a) { const double fa = (double)fftab[a * M + k]; tot += (plan->weighted ? plan->sw2[a] : (double)plan->n_a[a]) * fa * fa; }
 #pragma unroll
-        for (int x = 0; x < DEBYE_FINAL_G * DEBYE_FINAL_NS; ++x) tot += part[x][kk];
+        for (int x = 0; x < DEBYE_FINAL_G; ++x) tot += part[x][kk];
         out[(int64_t)b * M + k] = tot;
     }
 }

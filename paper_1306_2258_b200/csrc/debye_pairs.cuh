@@ -13,11 +13,18 @@
 //     CTA order.
 //
 // Variants of the per-pair term evaluation (north_star (d), (e)):
-//   V_RECUR    uniform grid q_k = qbase + k dq.  sin(q_k r) for all k of the chunk by the three-term
-//              (Chebyshev) recurrence v_{k+S} = 2cos(S theta) v_k - v_{k-S}, theta = r dq, run as 4 packed
-//              chains (8 residues mod S = 8 n_chunks) with fma.rn.f32x2 (SASS FFMA2) and accumulated with
-//              add.rn.f32x2 (FADD2): 2 FP32-pipe lane-operations per term, no MUFU in the loop.  Start values
-//              come from 4 (zero start) or 8 (general start) MUFU.SIN and a stride-4 bootstrap.
+//   V_RECUR    uniform grid q_k = qbase + k dq, theta = r dq.
+//              PRODUCT FORM (grids q_k = (k + koff) dq, koff in {0, 1}, at most 2 q-chunks; all BASELINE configs and the
+//              paper's own grid): with b_n = 2 sin(n theta)/r,
+//                  2 cos(j S theta) * b_k0 = b_{S j + k0} - b_{S j - k0},
+//              so per pair 8 seeds b_k0 (k0 = 1..8 of the chunk) times J weights W_j = 2 cos(j S theta) (W_0 := 1) give,
+//              with ONE packed FMA lane per output, the sums Out[j][k0] = sum_pairs (b_{Sj+k0} - b_{Sj-k0}); the final stage
+//              undoes the telescoping in FP64: B_{Sj+k0} = Out[j][k0] + B_{Sj-k0} (B_0 = 0, B_{-n} = -B_n).  1 FP32-pipe
+//              lane-operation per term instead of the 2 (recurrence step + accumulate) of a chain, no MUFU in the loop,
+//              and no small-angle problem: the weights carry only the even part of the angle.
+//              CHAIN FORM (general start q_0, or more than 2 chunks): three-term (Chebyshev) recurrence
+//              v_{k+S} = 2cos(S theta) v_k - v_{k-S} run as 4 packed chains (8 residues mod S = 8 n_chunks) with
+//              fma.rn.f32x2 (SASS FFMA2), accumulated with add.rn.f32x2 (FADD2): 2 lane-operations per term.
 //   V_MUFU     any grid: explicit range reduction in turns (magic-number rounding, exact FMA remainder), one
 //              MUFU.SIN per term.
 //   V_ACCURATE any grid: libdevice sinf per term (reference variant).
@@ -227,26 +234,29 @@ struct RecurConst {
     int n_chunks;
 };
 
-enum RecurMode : int { RM_Z1 = 0, RM_Z2A = 1, RM_Z2B = 2, RM_G = 3 };
-// RM_Z1   grid q_k' = k' dq, one chunk  (S = 8):  chains start at k' = 0..7
-// RM_Z2A  grid q_k' = k' dq, two chunks (S = 16), chunk 0: k' = 16 m + (0..7)
-// RM_Z2B  same, chunk 1: k' = 16 m + 8 + (0..7)
-// RM_G    any uniform grid / any number of chunks: 8 accurate sines at k' = 8 ch - S + (0..7), stride-4 bootstrap
+enum RecurMode : int { RM_P1 = 0, RM_P2A = 1, RM_P2B = 2, RM_G = 3 };
+// RM_P1   product form, grid q_k' = k' dq, one chunk  (S = 8):  seeds k0 = 1..8, outputs k' = 8 j + k0
+// RM_P2A  product form, two chunks (S = 16), chunk 0: seeds k0 = 1..8, outputs k' = 16 j + k0
+// RM_P2B  same, chunk 1: seeds k0 = 9..16
+// RM_G    chain form, any uniform grid / any number of chunks: 8 accurate sines at k' = 8 ch - S + (0..7), stride-4 bootstrap
+__host__ __device__ constexpr bool recur_is_product(int mode) { return mode != RM_G; }
 
 // The start-up of one pair is split into two stages so that the tile loop can run them one and two groups ahead of the
 // packed loop (three-stage software pipeline).
-// Stage A (geometry): distance, 1/r, slow-path flag and the two reduced angles (turns, in [-1/2, 1/2]).
+// Stage A (geometry): distance, 1/r, slow-path flag (chain form only) and the two reduced angles (turns, in [-1/2, 1/2]).
 struct RecurGeom { float r, rinv, f1, fS; bool slow; };
 template <int MODE, bool W>
 __device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, const bool ok, const RecurConst &rc, RecurGeom &g)
 {
     const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
-    // + 1e-30 keeps rsqrt finite for coincident atoms (they take the slow path, which gets the limit right) and changes no
-    // other distance; folding it into the FMA chain saves the clamp
+    // + 1e-30 keeps rsqrt finite for coincident atoms and changes no other distance; folding it into the FMA chain saves the
+    // clamp.  Product form: r = 1e-15 then gives b_k0 = 2 sin(k0 theta)/r its limit 2 k0 dq and W_j = 2 (every step of the
+    // start-up keeps RELATIVE accuracy for small theta).  Chain form: such pairs take the slow path.
     const float r2c = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, 1e-30f)));
-    const bool small = !(r2c > rc.cut2);
     const float rinv = rsqrt_mufu(r2c);
     g.r = r2c * rinv;
+    bool small = false;
+    if constexpr (!recur_is_product(MODE)) small = !(r2c > rc.cut2);
     // zero for masked / slow-path pairs: every start value becomes exactly 0.  Weighted instantiations (W): pj.w is the j
     // atom's weight; the i atom's weight is applied when the accumulators are flushed
     if constexpr (W) g.rinv = (ok && !small) ? rinv * pj.w : 0.0f;
@@ -254,91 +264,155 @@ __device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, con
     g.slow = small && ok;
     reduce_turns_pair(g.r, rc.w1, rc.w1_lo, rc.smult, g.f1, g.fS);     // f1 is dead code in the general-start mode
 }
+
+// ---- product form (RM_P1 / RM_P2A / RM_P2B) ----------------------------------------------------------------------
+// Stage B: U = the chunk's 8 seeds b_k0 = 2 sin(k0 theta)/r as 4 pairs; Wt[j] = 2 cos(j S theta) for j = 1 .. J-1.
+// Seeds: folded sine / cosine of theta/2 by polynomial, then double-angle / three-term steps, each a single rounding, so
+// relative accuracy survives small theta.  T_n = 2 sin(n theta), c_n = 2 cos(n theta).
+// Weights: 2 cos(S theta) by its own polynomial on the reduced angle of S theta (not by doubling 2 cos(theta): the
+// correlated roundings of that route leave a coherent phase bias); then two interleaved Chebyshev
+// chains of stride 2 (W_j = W_2 W_{j-2} - W_{j-4}, W_0 = 2, W_{-1} = W_1), which halves the dependency depth.  An error
+// d of 2 cos(S theta) changes W_j by at most j^2 d (6e-8 x 256 = 1.5e-5 of the term at j = 16, pseudo-random over pairs).
+template <int MODE, int J>
+__device__ __forceinline__ void prod_vals(const RecurGeom &g, u64 (&U)[4], float (&Wt)[J])
+{
+    const float rinv = g.rinv;
+    const Folded h = sincos_fold(g.f1);                // g.f1 = theta / 2 pi reduced: pi f1 = theta / 2
+    const float T1 = two_sin_from(h, g.f1);
+    const float c1 = two_cos_from(h);
+    const float c2 = fmaf(-T1, T1, 2.0f);
+    const float c4 = fmaf(c2, c2, -2.0f);     // used for ONE (two for chunk 1 of 2) bootstrap step only: its absolute error of
+                                              // one rounding costs 1e-7 relative in u5..u16, no relative accuracy needed
+    float u[17];
+    u[1] = T1 * rinv; u[2] = c1 * u[1]; u[3] = fmaf(c1, u[2], -u[1]); u[4] = c2 * u[2];
+    u[5] = fmaf(c4, u[1], u[3]); u[6] = fmaf(c4, u[2], u[2]); u[7] = fmaf(c4, u[3], u[1]); u[8] = c4 * u[4];
+    if constexpr (MODE == RM_P2B) {
+#pragma unroll
+        for (int n = 9; n <= 16; ++n) u[n] = fmaf(c4, u[n - 4], -u[n - 8]);
+        U[0] = pk2(u[9], u[10]); U[1] = pk2(u[11], u[12]); U[2] = pk2(u[13], u[14]); U[3] = pk2(u[15], u[16]);
+    } else {
+        U[0] = pk2(u[1], u[2]); U[1] = pk2(u[3], u[4]); U[2] = pk2(u[5], u[6]); U[3] = pk2(u[7], u[8]);
+    }
+    const float cS = two_cos_from(sincos_fold(g.fS));
+    if constexpr (J > 1) Wt[1] = cS;
+    if constexpr (J > 2) Wt[2] = fmaf(cS, cS, -2.0f);
+    if constexpr (J > 3) Wt[3] = fmaf(Wt[2], cS, -cS);
+    if constexpr (J > 4) Wt[4] = fmaf(Wt[2], Wt[2], -2.0f);
+#pragma unroll
+    for (int j = 5; j < J; ++j) Wt[j] = fmaf(Wt[2], Wt[j - 2], -Wt[j - 4]);
+    Wt[0] = 1.0f;
+}
+// Stage C: the outer product.  acc[4 j + a] (slots 8 j + 2 a, 8 j + 2 a + 1) += W_j * U[a]; level 0 has W_0 = 1.
+// All K/2 packed operations are independent of one another.
+template <int K>
+__device__ __forceinline__ void prod_hot(u64 (&acc)[K / 2], const u64 (&U)[4], const float (&Wt)[(K + 7) / 8])
+{
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+        if (2 * a < K) acc[a] = add2(acc[a], U[a]);
+#pragma unroll
+    for (int j = 1; j < (K + 7) / 8; ++j) {
+        const u64 wj = pk2(Wt[j], Wt[j]);               // SASS: the scalar-broadcast operand form of FFMA2, no copy
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+            if (8 * j + 2 * a < K) acc[4 * j + a] = fma2(wj, U[a], acc[4 * j + a]);     // K % 8 == 4: the last level has 4 slots
+    }
+}
+
+// One shared-memory tile of j atoms against this thread's i atom, product form, NP pairs per iteration.  Stage A of group
+// jj + 2 NP and stage B of group jj + NP sit in the same basic block as the outer products of group jj, so the scheduler
+// hides their dependency chains (distance, rsqrt, range reduction, polynomials, seed and weight chains: ~70 dependent
+// FP32 instructions) under the independent packed instructions.
+#ifndef DEBYE_NPP
+#define DEBYE_NPP 1
+#endif
+#define DEBYE_PRAGMA_(x) _Pragma(#x)
+#define DEBYE_PRAGMA(x) DEBYE_PRAGMA_(x)
+#ifdef DEBYE_PROD_UNROLL
+#define DEBYE_PROD_UNROLL_PRAGMA DEBYE_PRAGMA(unroll DEBYE_PROD_UNROLL)
+#else
+#define DEBYE_PROD_UNROLL_PRAGMA
+#endif
+template <int K, int MODE, bool W>
+__device__ __forceinline__ void prod_tile(u64 (&acc)[K / 2], const float4 *__restrict__ tile, const int jj0, const int cnt, const float4 pi,
+                                          const bool ivalid, const bool diag, const int i_local, const int jl0, const RecurConst &rc)
+{
+    constexpr int NP = DEBYE_NPP, J = (K + 7) / 8;
+    if (jj0 >= cnt) return;
+    // first tile index this thread may pair with: masks i >= j on the diagonal and threads without an i atom
+    const int jmin = ivalid ? (diag ? max(0, i_local + 1 - jl0) : 0) : 0x7fffffff;
+    // masked pairs (before jmin, behind the last atom of the tile: the pipeline reads two groups ahead) get 1/r = 0 and with
+    // it seeds that are exactly 0; their coordinates are read from a VALID entry of this tile (index clamp), so that a
+    // stale non-finite entry behind the tile can never reach the accumulators (0 * NaN)
+    auto geom = [&](const int jbase, RecurGeom (&g)[NP]) {
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            const int j = jbase + p;
+            recur_geom<MODE, W>(tile[min(j, cnt - 1)], pi, j >= jmin && j < cnt, rc, g[p]);
+        }
+    };
+    u64 U[NP][4];
+    float Wt[NP][J];
+    RecurGeom gn[NP];
+    geom(jj0, gn);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) prod_vals<MODE, J>(gn[p], U[p], Wt[p]);
+    geom(jj0 + NP, gn);
+    DEBYE_PROD_UNROLL_PRAGMA
+    for (int jj = jj0; jj < cnt; jj += NP) {
+        u64 Un[NP][4];
+        float Wn[NP][J];
+#pragma unroll
+        for (int p = 0; p < NP; ++p) prod_vals<MODE, J>(gn[p], Un[p], Wn[p]);
+        geom(jj + 2 * NP, gn);
+#pragma unroll
+        for (int p = 0; p < NP; ++p) prod_hot<K>(acc, U[p], Wt[p]);
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+#pragma unroll
+            for (int a = 0; a < 4; ++a) U[p][a] = Un[p][a];
+#pragma unroll
+            for (int j = 0; j < J; ++j) Wt[p][j] = Wn[p][j];
+        }
+    }
+}
+
+// ---- chain form (RM_G) ----------------------------------------------------------------------------------------------
 // Stage B (values): Bv = w_0 (the 8 residues), A = w_{-1}, cS = 2 cos(S theta).
-template <int MODE, bool TWO>
+// General start (q_0 not a small multiple of dq, or more than 2 chunks): 8 accurate sines at k' = base .. base+7
+// (base = -S + 8 ch), then the stride-4 recurrence v_{n+4} = 2cos(4 theta) v_n - v_{n-4} walks up to k' = 8 ch .. 8 ch + 7
 __device__ __forceinline__ void recur_vals(const RecurGeom &g, const RecurConst &rc, const float *wtab, u64 (&A)[4], u64 (&Bv)[4], float &cS)
 {
     const float r = g.r, rinv = g.rinv;
     // the chain coefficient 2 cos(S theta) is NOT derived from 2 cos(theta) by repeated doubling: the correlated roundings
     // of that route leave a +7e-8 rad coherent phase bias after 16 steps (fp32 emulation)
     cS = two_cos_from(sincos_fold(g.fS));
-    if constexpr (MODE != RM_G) {
-        // zero start: v_n = 2 sin(n theta)/r, v_0 = 0, v_{-n} = -v_n.  Folded sine / cosine of theta/2 by polynomial,
-        // everything else by double-angle / three-term steps (each a single rounding, so relative accuracy survives
-        // small theta).  T_n = 2 sin(n theta), c_n = 2 cos(n theta).
-        const Folded h = sincos_fold(g.f1);                // g.f1 = theta / 2 pi reduced: pi f1 = theta / 2
-        const float T1 = two_sin_from(h, g.f1);
-        const float c1 = two_cos_from(h);
-        const float c2 = fmaf(-T1, T1, 2.0f);
-        const float c4 = fmaf(c2, c2, -2.0f);     // used for ONE (two for 2 chunks) bootstrap step only: its absolute error of
-                                                  // one rounding costs 1e-7 relative in u5..u16, no relative accuracy needed
-        float u[17];
-        u[0] = 0.0f;
-        u[1] = T1 * rinv; u[2] = c1 * u[1]; u[3] = fmaf(c1, u[2], -u[1]); u[4] = c2 * u[2];
-        u[5] = fmaf(c4, u[1], u[3]); u[6] = fmaf(c4, u[2], u[2]); u[7] = fmaf(c4, u[3], u[1]); u[8] = c4 * u[4];
-        // chains start at index 1 (index 0 is identically zero): chain j of chunk ch holds k' = 1 + 8 ch + j + S m.
-        // B = w_0 = v(k'), A = w_{-1} = -v(k' - S) = +u[S - k'] (v(-n) = -v(n))
+    float g0[4], g1[4];
 #pragma unroll
-        for (int n = 9; n <= 16; ++n) u[n] = fmaf(c4, u[n - 4], -u[n - 8]);
-        if constexpr (TWO) {
-            // TWO-SEED form (recur_two_seeds): A = w_0 = v(1..8), Bv = w_1 = v(9..16).  Compared with (w_{-1}, w_0) this costs
-            // 8 scalar FFMA but saves one packed chain step (4 FFMA2) and, above all, the 8 register copies that building
-            // w_{-1} = (u7, u6, ..., u1, 0) out of values that also sit in w_0 needs: every u lands in exactly one slot
-            A[0] = pk2(u[1], u[2]); A[1] = pk2(u[3], u[4]); A[2] = pk2(u[5], u[6]); A[3] = pk2(u[7], u[8]);
-            Bv[0] = pk2(u[9], u[10]); Bv[1] = pk2(u[11], u[12]); Bv[2] = pk2(u[13], u[14]); Bv[3] = pk2(u[15], u[16]);
-        } else if constexpr (MODE == RM_Z1) {
-            Bv[0] = pk2(u[1], u[2]); Bv[1] = pk2(u[3], u[4]); Bv[2] = pk2(u[5], u[6]); Bv[3] = pk2(u[7], u[8]);
-            A[0] = pk2(u[7], u[6]); A[1] = pk2(u[5], u[4]); A[2] = pk2(u[3], u[2]); A[3] = pk2(u[1], u[0]);
-        } else {
-            if constexpr (MODE == RM_Z2A) {
-                Bv[0] = pk2(u[1], u[2]); Bv[1] = pk2(u[3], u[4]); Bv[2] = pk2(u[5], u[6]); Bv[3] = pk2(u[7], u[8]);
-                A[0] = pk2(u[15], u[14]); A[1] = pk2(u[13], u[12]); A[2] = pk2(u[11], u[10]); A[3] = pk2(u[9], u[8]);
-            } else {
-                Bv[0] = pk2(u[9], u[10]); Bv[1] = pk2(u[11], u[12]); Bv[2] = pk2(u[13], u[14]); Bv[3] = pk2(u[15], u[16]);
-                A[0] = pk2(u[7], u[6]); A[1] = pk2(u[5], u[4]); A[2] = pk2(u[3], u[2]); A[3] = pk2(u[1], u[0]);
-            }
-        }
-    } else {
-        // general start (q_0 not a small multiple of dq, or more than 2 chunks): 8 accurate sines at
-        // k' = base .. base+7 (base = -S + 8 ch), then the stride-4 recurrence v_{n+4} = 2cos(4 theta) v_n - v_{n-4}
-        // walks up to k' = 8 ch .. 8 ch + 7
-        float g0[4], g1[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            g0[j] = two_sin_turns_accurate(r, wtab[j], wtab[8 + j]) * rinv;
-            g1[j] = two_sin_turns_accurate(r, wtab[4 + j], wtab[12 + j]) * rinv;
-        }
-        const float c4 = two_cos_turns(r, rc.w4, rc.w4_lo);
-        float a0[4], a1[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) { a0[j] = g0[j]; a1[j] = g1[j]; }
-        for (int st = 0; st < 2 * rc.n_chunks; ++st) {
-#pragma unroll
-            for (int j = 0; j < 4; ++j) { float nx = fmaf(c4, g1[j], -g0[j]); g0[j] = g1[j]; g1[j] = nx; }
-        }
-        Bv[0] = pk2(g0[0], g0[1]); Bv[1] = pk2(g0[2], g0[3]); Bv[2] = pk2(g1[0], g1[1]); Bv[3] = pk2(g1[2], g1[3]);
-        A[0] = pk2(-a0[0], -a0[1]); A[1] = pk2(-a0[2], -a0[3]); A[2] = pk2(-a1[0], -a1[1]); A[3] = pk2(-a1[2], -a1[3]);
+    for (int j = 0; j < 4; ++j) {
+        g0[j] = two_sin_turns_accurate(r, wtab[j], wtab[8 + j]) * rinv;
+        g1[j] = two_sin_turns_accurate(r, wtab[4 + j], wtab[12 + j]) * rinv;
     }
+    const float c4 = two_cos_turns(r, rc.w4, rc.w4_lo);
+    float a0[4], a1[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { a0[j] = g0[j]; a1[j] = g1[j]; }
+    for (int st = 0; st < 2 * rc.n_chunks; ++st) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { float nx = fmaf(c4, g1[j], -g0[j]); g0[j] = g1[j]; g1[j] = nx; }
+    }
+    Bv[0] = pk2(g0[0], g0[1]); Bv[1] = pk2(g0[2], g0[3]); Bv[2] = pk2(g1[0], g1[1]); Bv[3] = pk2(g1[2], g1[3]);
+    A[0] = pk2(-a0[0], -a0[1]); A[1] = pk2(-a0[2], -a0[3]); A[2] = pk2(-a1[0], -a1[1]); A[3] = pk2(-a1[2], -a1[3]);
 }
 
 // Packed hot loop of one pair: w_m = sigma_m v_m with sigma = (+,+,-,-): w_{m+1} = (+/-) cS w_m + w_{m-1}; 4 packed chains
 // (8 residues), K/8 steps: per term one FFMA2 lane and one FADD2 lane.  A and Bv are consumed.
-// which instantiations hand over (w_0, w_1) instead of (w_{-1}, w_0): the one-chunk zero-start mode.  Measured per K on B200
-// (pairs-kernel-only driver, N = 10 000): two seeds win 2-5 % at K = 64, 104, 128 and lose 2.3 % at K = 100, where the
-// register allocation of the packed loop happens to come out worse -- hence the exception.
-__host__ __device__ constexpr bool recur_two_seeds(int mode, int K) { return mode == RM_Z1 && K != 100; }
-
-template <int K, bool TWO>
+template <int K>
 __device__ __forceinline__ void recur_hot(u64 (&acc)[K / 2], u64 (&A)[4], u64 (&Bv)[4], const float cS)
 {
     const u64 cP = pk2(cS, cS), cN = pk2(-cS, -cS);
-    if constexpr (TWO) {
 #pragma unroll
-        for (int a = 0; a < 4; ++a)
-            if (2 * a < K) acc[a] = add2(acc[a], A[a]);        // step 0 (sigma_0 = +)
-    }
-#pragma unroll
-    for (int m = TWO ? 1 : 0; m < (K + 7) / 8; ++m) {
+    for (int m = 0; m < (K + 7) / 8; ++m) {
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
             if (8 * m + 2 * a < K) {                       // K % 8 == 4: the last step runs chains 0 and 1 only
@@ -354,38 +428,32 @@ __device__ __forceinline__ void recur_hot(u64 (&acc)[K / 2], u64 (&A)[4], u64 (&
     }
 }
 
-// Slow path of one pair (theta = r dq at or below theta_min, or coincident atoms).  The three-term chain loses the
-// pair's frequency when 2cos(S theta) rounds next to 2 (relative error of theta^2 is 6e-8 / (S theta)^2), so these pairs
+// Slow path of one pair (theta = r dq at or below theta_min, or coincident atoms), chain form.  The three-term chain loses
+// the pair's frequency when 2cos(S theta) rounds next to 2 (relative error of theta^2 is 6e-8 / (S theta)^2), so these pairs
 // run Reinsch's form of the same chain, which carries beta = 4 sin^2(S theta / 2) = 2 - 2cos(S theta) with full relative
 // accuracy:   d_{m+1} = d_m - beta s_m,   s_{m+1} = s_m + d_{m+1},   s_0 = v(k'_j),  d_0 = v(k'_j) - v(k'_j - S).
 // Start values are those of the fast path evaluated with the true 1/r (for r = 0 the clamp r^2 >= 1e-30 makes
 // 2 sin(n theta)/r come out as its limit 2 n dq).  Three packed lane-operations per term; rare, so cost is irrelevant.
-template <int K, int MODE, bool W>
+template <int K, bool W>
 __device__ __forceinline__ void recur_slow_pair(u64 (&acc)[K / 2], const float4 pj, const float4 pi, const RecurConst &rc, const float *wtab)
 {
     RecurConst rs = rc;
     rs.cut2 = -1.0f;                       // never "small": stage A keeps the true 1/r
     RecurGeom g;
-    recur_geom<MODE, W>(pj, pi, true, rs, g);
+    recur_geom<RM_G, W>(pj, pi, true, rs, g);
     u64 A[4], Bv[4];
     float cS;
-    recur_vals<MODE, recur_two_seeds(MODE, K)>(g, rc, wtab, A, Bv, cS);
+    recur_vals(g, rc, wtab, A, Bv, cS);
     (void)cS;
     // beta from the polynomial directly (2 - cS would cancel)
     const float nbeta = -four_sin2_from(sincos_fold(g.fS));
     const u64 nb2 = pk2(nbeta, nbeta);
-    // stage B returns A = w_{-1} = -v_{-1} (sign convention of the fast loop): d_0 = v_0 - v_{-1} = Bv + A;
-    // in the two-seed form it returns (v_0, v_1): step 0 is added here and the chain starts at m = 1 with d_1 = v_1 - v_0
-    constexpr bool TWO = recur_two_seeds(MODE, K);
+    // stage B returns A = w_{-1} = -v_{-1} (sign convention of the fast loop): d_0 = v_0 - v_{-1} = Bv + A
     u64 s[4], d[4];
 #pragma unroll
-    for (int a = 0; a < 4; ++a) {
-        s[a] = Bv[a];
-        if constexpr (TWO) { if (2 * a < K) acc[a] = add2(acc[a], A[a]); d[a] = sub2(Bv[a], A[a]); }
-        else d[a] = add2(Bv[a], A[a]);
-    }
+    for (int a = 0; a < 4; ++a) { s[a] = Bv[a]; d[a] = add2(Bv[a], A[a]); }
 #pragma unroll
-    for (int m = TWO ? 1 : 0; m < (K + 7) / 8; ++m) {
+    for (int m = 0; m < (K + 7) / 8; ++m) {
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
             if (8 * m + 2 * a < K) {
@@ -399,70 +467,44 @@ __device__ __forceinline__ void recur_slow_pair(u64 (&acc)[K / 2], const float4 
     }
 }
 
-// Occupancy policy (measured on B200, profiles/): the K accumulators dominate the register budget.  K <= 64 fits 4 CTAs
-// of 128 threads per SM (128 registers), K <= 80 fits 3 (168), larger K runs 2 CTAs per SM with up to 255 registers and
-// makes up for the missing warps with NP = 2 pairs in flight per thread.
+// Occupancy policy: the K accumulators dominate the register budget.  Product form: K + ~60 registers.
 #ifndef DEBYE_K4
 #define DEBYE_K4 64
 #endif
 #ifndef DEBYE_K3
-#define DEBYE_K3 80
+#define DEBYE_K3 104
 #endif
 __host__ __device__ constexpr int recur_min_ctas(int K) { return K <= DEBYE_K4 ? 4 : (K <= DEBYE_K3 ? 3 : 2); }
-#ifdef DEBYE_NP
-__host__ __device__ constexpr int recur_np(int K) { return DEBYE_NP; }
-#else
-__host__ __device__ constexpr int recur_np(int K) { return K <= DEBYE_K3 ? 1 : 2; }
-#endif
 
-// One shared-memory tile of j atoms against this thread's i atom, NP pairs per iteration.  The start values of
-// pairs jj+NP .. jj+2NP-1 are computed in the same basic block as the packed loops of pairs jj .. jj+NP-1, so the
-// scheduler hides their dependency chain (distance, rsqrt, range reduction, polynomials: ~60 dependent FP32
-// instructions) under the independent packed instructions.  NP > 1 gives that much more instruction-level
-// parallelism per warp at 17 registers per extra pair -- the K accumulators, which are what limits the number of
-// resident warps, are shared by all NP pairs.
-template <int K, int MODE, bool W>
+// One shared-memory tile of j atoms against this thread's i atom, chain form, one pair per iteration, the same three-stage
+// pipeline as prod_tile.
+template <int K, bool W>
 __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__restrict__ tile, const int jj0, const int cnt, const float4 pi,
                                            const bool ivalid, const bool diag, const int i_local, const int jl0, const RecurConst &rc,
                                            const float *wtab)
 {
-    constexpr int NP = recur_np(K);
     if (jj0 >= cnt) return;
-    // first tile index this thread may pair with: masks i >= j on the diagonal and threads without an i atom
     const int jmin = ivalid ? (diag ? max(0, i_local + 1 - jl0) : 0) : 0x7fffffff;
     bool had_slow = false;                // some pair of this thread in this tile needs the slow path (handled after the loop)
-    // the tile buffers carry DEBYE_TILE_PAD finite entries behind the last atom, so the two groups that the pipeline reads
-    // ahead never need an index clamp; such pairs are masked (1/r = 0)
-    auto geom = [&](const int jbase, RecurGeom (&g)[NP]) {
-#pragma unroll
-        for (int p = 0; p < NP; ++p) {
-            const int j = jbase + p;
-            recur_geom<MODE, W>(tile[j], pi, j >= jmin && j < cnt, rc, g[p]);
-            had_slow = had_slow || g[p].slow;
-        }
+    auto geom = [&](const int j, RecurGeom &g) {
+        recur_geom<RM_G, W>(tile[min(j, cnt - 1)], pi, j >= jmin && j < cnt, rc, g);
+        had_slow = had_slow || g.slow;
     };
-    u64 A[NP][4], Bv[NP][4];
-    float cS[NP];
-    RecurGeom gn[NP];
+    u64 A[4], Bv[4];
+    float cS;
+    RecurGeom gn;
     geom(jj0, gn);
+    recur_vals(gn, rc, wtab, A, Bv, cS);
+    geom(jj0 + 1, gn);
+    for (int jj = jj0; jj < cnt; ++jj) {
+        u64 An[4], Bn[4];
+        float cSn;
+        recur_vals(gn, rc, wtab, An, Bn, cSn);
+        geom(jj + 2, gn);
+        recur_hot<K>(acc, A, Bv, cS);
 #pragma unroll
-    for (int p = 0; p < NP; ++p) recur_vals<MODE, recur_two_seeds(MODE, K)>(gn[p], rc, wtab, A[p], Bv[p], cS[p]);
-    geom(jj0 + NP, gn);
-    for (int jj = jj0; jj < cnt; jj += NP) {
-        // stage B of group jj + NP, stage A of group jj + 2 NP, packed loops of group jj: one basic block, no branch
-        u64 An[NP][4], Bn[NP][4];
-        float cSn[NP];
-#pragma unroll
-        for (int p = 0; p < NP; ++p) recur_vals<MODE, recur_two_seeds(MODE, K)>(gn[p], rc, wtab, An[p], Bn[p], cSn[p]);
-        geom(jj + 2 * NP, gn);
-#pragma unroll
-        for (int p = 0; p < NP; ++p) recur_hot<K, recur_two_seeds(MODE, K)>(acc, A[p], Bv[p], cS[p]);
-#pragma unroll
-        for (int p = 0; p < NP; ++p) {
-#pragma unroll
-            for (int a = 0; a < 4; ++a) { A[p][a] = An[p][a]; Bv[p][a] = Bn[p][a]; }
-            cS[p] = cSn[p];
-        }
+        for (int a = 0; a < 4; ++a) { A[a] = An[a]; Bv[a] = Bn[a]; }
+        cS = cSn;
     }
     // slow-path pairs (theta at or below theta_min, coincident atoms) contributed exactly zero above; they are rare, so
     // the tile is rescanned for them only if some lane of the warp met one
@@ -472,7 +514,7 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
                 const float4 pj = tile[j];
                 const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
                 const float r2c = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, 1e-30f)));       // as in recur_geom
-                if (!(r2c > rc.cut2)) recur_slow_pair<K, MODE, W>(acc, pj, pi, rc, wtab);
+                if (!(r2c > rc.cut2)) recur_slow_pair<K, W>(acc, pj, pi, rc, wtab);
             }
         }
     }
@@ -640,7 +682,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                     // zero-start modes: grid (k + koff) dq with koff in {0, 1} and at most 2 chunks; else general start,
                     // which takes the grid as q0 + k dq whatever q0 is
                     const bool zs = (koff >= 0 && n_chunks <= 2);
-                    mode = zs ? (n_chunks == 1 ? RM_Z1 : (ch == 0 ? RM_Z2A : RM_Z2B)) : RM_G;
+                    mode = zs ? (n_chunks == 1 ? RM_P1 : (ch == 0 ? RM_P2A : RM_P2B)) : RM_G;
                     const double qb = q0_d;                               // general start: q of chain index 0
                     const int base = -S + 8 * ch;                         // k' of the first start value
                     __syncthreads();
@@ -697,11 +739,11 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
             int jj0 = 0;
             if (diag) { int first_i = row * DEBYE_IB + warp * 32; jj0 = max(0, first_i + 1 - jl0); }
             if constexpr (VAR == V_RECUR) {
-                switch (mode) {      // warp-uniform; one copy of the pipelined loop per start mode
-                    case RM_Z1: recur_tile<K, RM_Z1, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
-                    case RM_Z2A: recur_tile<K, RM_Z2A, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
-                    case RM_Z2B: recur_tile<K, RM_Z2B, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
-                    default: recur_tile<K, RM_G, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
+                switch (mode) {      // warp-uniform; one copy of the pipelined loop per mode
+                    case RM_P1: prod_tile<K, RM_P1, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc); break;
+                    case RM_P2A: prod_tile<K, RM_P2A, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc); break;
+                    case RM_P2B: prod_tile<K, RM_P2B, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc); break;
+                    default: recur_tile<K, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
                 }
             } else {
             for (int jj = jj0; jj < cnt; ++jj) {

@@ -83,11 +83,11 @@ def test_workspace_and_launch_info_are_host_side():
     a, b = L.debye_workspace_bytes(100000, 1, 5, 64, 0), L.debye_workspace_bytes(200000, 1, 5, 64, 0)
     assert 15 * 100000 < b - a < 25 * 100000
     info = binding.launch_info(10000, 1, 5, 101, "auto")
-    # setup(+pack: N*B <= 16384), recurrence sized for 100 and for 101 chain indices, MUFU, final
-    assert info == {"n_launches": 5, "q_chunk": 104, "n_chunks": 1}
-    assert binding.launch_info(50000, 1, 4, 200, "recur") == {"n_launches": 4, "q_chunk": 104, "n_chunks": 2}
+    # setup(+pack: N*B <= 16384), recurrence sized for 100 and for 101 chain indices, MUFU, reduce, epilogue
+    assert info == {"n_launches": 6, "q_chunk": 104, "n_chunks": 1}
+    assert binding.launch_info(50000, 1, 4, 200, "recur") == {"n_launches": 5, "q_chunk": 104, "n_chunks": 2}
     assert binding.launch_info(1000, 1, 5, 51, "fp64")["n_chunks"] == 2
-    assert binding.launch_info(1000, 1, 5, 300, "mufu") == {"n_launches": 3, "q_chunk": 104, "n_chunks": 3}
+    assert binding.launch_info(1000, 1, 5, 300, "mufu") == {"n_launches": 4, "q_chunk": 104, "n_chunks": 3}
 
 
 def test_binding_refuses_non_cuda_inputs():
@@ -115,6 +115,6 @@ def test_q_hint_classifies_grids_on_the_host():
     L = binding.lib()
     assert L.debye_q_hint(None, 5) == 0
     # with a hint exactly one pairs instantiation is launched
-    assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H | U | Z) == {"n_launches": 3, "q_chunk": 100, "n_chunks": 1}
-    assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H | U | D) == {"n_launches": 3, "q_chunk": 104, "n_chunks": 1}
-    assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H)["n_launches"] == 3
+    assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H | U | Z) == {"n_launches": 4, "q_chunk": 100, "n_chunks": 1}
+    assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H | U | D) == {"n_launches": 4, "q_chunk": 104, "n_chunks": 1}
+    assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H)["n_launches"] == 4

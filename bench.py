@@ -33,6 +33,7 @@ SM_COUNT, FP32_LANES, MUFU_LANES = 148, 128, 16           # per B200 / per SM pe
 # dram__bytes_read.sum + dram__bytes_write.sum of the pairs kernel, per launch, from the committed ncu --set full capture
 # (profiles/r01_ncu_full_pairs_recur_cfg{2,4,5}_v4.txt); None where no capture exists
 NCU_TRAFFIC = {("cfg2", "recur"): 239104, ("cfg4", "recur"): 32843264 + 163584, ("cfg5", "recur"): 3336192}
+NCU_TRAFFIC_SOURCE = "profiles/r01_ncu_full_pairs_recur_cfg{2,4,5}_v4.txt (capture of an earlier build; the kernel's inputs are unchanged)"
 
 
 TABLE1 = {f"table1_{n}": n for n in (1000, 2000, 4000, 10000, 20000, 40000, 100000)}       # the paper's Table I rows
@@ -158,6 +159,188 @@ def run_reference(args, rank, world):
         "gpu_launches": 0}))
 
 
+def respawn_if_needed(args):
+    """`python bench.py --gpus N` (N > 1) without a launcher: start N ranks, one per GPU, under torch.distributed.run on
+    127.0.0.1 and hand it the same arguments.  Under a launcher (WORLD_SIZE set) the two counts must agree."""
+    ws = os.environ.get("WORLD_SIZE")
+    if ws is not None:
+        if int(ws) != args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={ws}: launch with --nproc-per-node {args.gpus}")
+        return
+    if args.gpus <= 1:
+        return
+    if args.impl == "reference":
+        return          # the oracle arm runs on rank 0's host cores only
+    import socket
+    import subprocess
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} needs {args.gpus} CUDA devices, this node has {have}")
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
+def stored_oracle(name):
+    """rows (conformer, k, I) of the oracle's stored whole profile of a full-size config (tests/golden/oracle_full_<name>.txt,
+    written by tests/golden/make_golden_full.py from oracle/ alone), or None."""
+    path = os.path.join(ROOT, "tests", "golden", f"oracle_full_{name}.txt")
+    if not os.path.exists(path):
+        return None
+    rows = []
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        _, b, k, _, I, _ = line.split()
+        rows.append((int(b), int(k), float(I)))
+    return rows
+
+
+def roofline_of(w, variant_ran, pairs_ms, fmax_ghz):
+    """Roofline of the pairs kernel.  Algorithmic work per pair.q as SURVEY.md 8(d) counts it for a
+    uniform grid: one recurrence FMA + one accumulate = 2 FP32-pipe lane-operations (4 FMA-equivalent flop)."""
+    nz = int(np.count_nonzero(w.q))                                             # q = 0 is answered in closed form by the epilogue
+    pq_all, pq_nz = float(w.pair_q), float(w.pair_q) / w.M * nz
+    if variant_ran == "recur":
+        peak = SM_COUNT * FP32_LANES * 2 * fmax_ghz / 1e3                       # TFLOP/s, FMA = 2 flop
+        achieved = 4.0 * pq_nz / (pairs_ms * 1e-3) / 1e12
+        return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                "frac_product_form_1_lane_op": 0.5 * achieved / peak,
+                "note": "FP32-pipe roofline with SURVEY 8(d)'s algorithmic count for a uniform grid: 2 lane-ops (recurrence FFMA + "
+                        "accumulate = 4 FMA-equivalent flop) per pair.q with q != 0; peak = 148 SM x 128 lanes x 2 x sm_max_mhz "
+                        "(MEASURED_PEAKS.json clock; nominal -- bench.py --peaks measures the pipe rates, profiles/r02_pipe_peaks.md). "
+                        "The product form of the kernel (DESIGN.md section 5.1) needs ONE FFMA lane per pair.q plus a per-pair "
+                        "start-up, so this fraction can exceed 1; frac_product_form_1_lane_op counts 1 lane-op per pair.q instead"}
+    peak = SM_COUNT * MUFU_LANES * fmax_ghz / 1e3                               # T MUFU op/s
+    achieved = pq_all / (pairs_ms * 1e-3) / 1e12
+    return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T sin/s", "frac": achieved / peak, "traffic": None,
+            "note": "XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM" if variant_ran == "mufu" else
+                    "reference variant; XU roofline quoted for scale"}
+
+
+def measure(db, w, dev, variant, use_hint, steps, warmup, world=1, e2e=True):
+    """Times `steps` calls of debye_profile[_batch] on workload w (device-resident inputs, L2 flushed between steps) and,
+    separately, the pairs kernel alone and the host-buffer entry.  Returns a dict of raw figures."""
+    import torch
+    import torch.distributed as dist
+    from paper_1306_2258_b200 import sharding
+    batch = w.xyz.ndim == 3
+    call = db.debye_profile_batch if batch else db.debye_profile
+    call_host = db.debye_profile_batch_host if batch else db.debye_profile_host
+    x, t, f, q = (torch.from_numpy(a).to(dev) for a in (w.xyz, w.type, w.fftab, w.q))
+    out = torch.empty((w.B, w.M) if batch else (w.M,), dtype=torch.float64, device=dev)
+    flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device=dev)        # > 126 MB L2
+    # the q grid exists on the host (it was generated there), so the caller can tell the library its shape: one pairs launch
+    # instead of up to three (include/debye.h, DEBYE_QHINT_*); the device verifies the hint
+    hint = db.q_hint(w.q) if use_hint else 0
+    info = db.launch_info(w.N, w.B, w.T, w.M, variant, with_grid=True, hint=hint)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(warmup):
+        call(x, t, f, q, out, variant=variant, hint=hint)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    barrier()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.fill_(1)                          # L2 flush between steps, outside the per-step events
+        a.record()
+        call(x, t, f, q, out, variant=variant, hint=hint)
+        b.record()
+    barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sharding.max_over_ranks(float(np.sum(step_ms)), dev)
+    units = sharding.sum_over_ranks(float(w.pair_q), dev)          # pair.q per step over all ranks
+    res = {"total_ms": total_ms, "units": units, "wall": wall, "clocks": clocks, "info": info, "hint": hint,
+           "value": units * steps / (total_ms * 1e-3) / 1e9}
+
+    # ---- dominant kernel (pairs) timed alone with events recorded by the library around its launch ----------
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); e1.record(); torch.cuda.synchronize()
+    db.set_pairs_events(e0, e1)
+    pk = []
+    for _ in range(min(steps, 30)):
+        flush.fill_(1)
+        call(x, t, f, q, out, variant=variant, hint=hint)
+        torch.cuda.synchronize()
+        pk.append(e0.elapsed_time(e1))
+    db.set_pairs_events(None, None)
+    res["pairs_ms"] = float(np.mean(pk))
+    res["result"] = out.cpu().numpy()
+
+    # ---- end to end through the host-buffer C entry (pinned inputs, copies inside the timed region) ----------
+    if e2e:
+        hx, ht, hf, hq = (torch.from_numpy(a).pin_memory().numpy() for a in (w.xyz, w.type, w.fftab, w.q))
+        hout = torch.empty((w.B, w.M) if batch else (w.M,), dtype=torch.float64).pin_memory().numpy()
+        for _ in range(3):
+            call_host(hx, ht, hf, hq, hout, variant=variant, hint=hint)
+        barrier()
+        n_e2e = max(5, min(steps, 50))
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            call_host(hx, ht, hf, hq, hout, variant=variant, hint=hint)
+        barrier()
+        e2e_s = sharding.max_over_ranks(time.perf_counter() - t0, dev)
+        assert np.array_equal(res["result"], hout), "host entry and device entry disagree"
+        res["e2e"] = {"value": units * n_e2e / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(hx.nbytes + ht.nbytes + hf.nbytes + hq.nbytes),
+                      "d2h_bytes_per_step": int(hout.nbytes), "ms_per_step": e2e_s / n_e2e * 1e3, "steps": n_e2e}
+    return res
+
+
+def variant_that_ran(variant, w):
+    return variant if variant != "auto" else ("recur" if _is_uniform(w.q) else "mufu")
+
+
+def kernel_shape(db, w, res, variant_ran):
+    """(K, n_chunks) of the pairs launch that did the work."""
+    info, hint = res["info"], res["hint"]
+    k_ran, chunks_ran = info["q_chunk"], info["n_chunks"]
+    if hint == 0 and variant_ran == "recur" and w.M >= 2 and float(w.q[0]) == 0.0:
+        # grid starts at q = 0: the device runs the recurrence launch sized for M - 1 chain indices when the library
+        # offered one (it does when that saves accumulators or a chunk; DESIGN.md section 5.1)
+        alt = db.launch_info(w.N, w.B, w.T, w.M - 1, "recur")
+        if alt["n_chunks"] <= 2 and (alt["q_chunk"] < k_ran or alt["n_chunks"] < chunks_ran):
+            k_ran, chunks_ran = alt["q_chunk"], alt["n_chunks"]
+    return k_ran, chunks_ran
+
+
+def config_summary(db, name, dev, variant, use_hint, fmax_ghz):
+    """One entry of the `configs` object: a full-size BASELINE config measured like the headline (fewer steps) and checked
+    against the oracle's stored whole profile (cfg1 / cfg2: the oracle runs live)."""
+    from oracle import oracle as orc
+    w = make_workload(name)
+    steps = {"cfg1": 50, "cfg2": 30, "cfg3": 8, "cfg4": 8, "cfg5": 4}.get(name, 10)
+    res = measure(db, w, dev, variant, use_hint, steps, 3, e2e=False)
+    vr = variant_that_ran(variant, w)
+    k_ran, chunks_ran = kernel_shape(db, w, res, vr)
+    roof = roofline_of(w, vr, res["pairs_ms"], fmax_ghz)
+    rows = stored_oracle(name)
+    I = res["result"]
+    if rows is None:
+        ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)
+        err, checked, against = float(np.max(np.abs(I - ref) / np.abs(ref))), int(w.M), "oracle run live, every q"
+    else:
+        err = max(abs((I[b, k] if I.ndim == 2 else I[k]) - ref) / abs(ref) for b, k, ref in rows)
+        checked, against = len(rows), f"stored oracle profile tests/golden/oracle_full_{name}.txt (every q" + (", 65 conformers)" if I.ndim == 2 else ")")
+    return {"workload": w.name, "N": w.N, "T": w.T, "M": w.M, "B": w.B, "steps": steps, "ms_per_step": res["total_ms"] / steps,
+            "T_pair_q_per_s": res["value"] / 1e3, "kernel": f"debye_pairs_kernel<{k_ran}, {vr}>", "kernel_ms": res["pairs_ms"],
+            "q_chunk": k_ran, "n_chunks": chunks_ran, "pairs_grid": res["info"]["pairs_grid"], "frac": roof["frac"],
+            "frac_product_form_1_lane_op": roof.get("frac_product_form_1_lane_op"),
+            "pair_q_per_clk_per_sm": float(w.pair_q) / (res["pairs_ms"] * 1e-3) / (SM_COUNT * fmax_ghz * 1e9),
+            "clocks": res["clocks"], "max_rel_err": float(err), "values_checked": checked, "checked_against": against}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -168,10 +351,12 @@ def main():
     ap.add_argument("--variant", default="auto", choices=["auto", "recur", "mufu", "accurate", "fp64"])
     ap.add_argument("--impl", default="libdebye", choices=["libdebye", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config summary (`configs` object) of the default 1-GPU run")
     ap.add_argument("--split", default="structures", choices=["structures", "tiles"],
-                    help="multi-GPU decomposition: structures = every rank its own structure (weak scaling, no collective; the "
-                         "default); tiles = ONE structure split over the ranks by tiles of the upper triangle, one all-gather of FP64 "
-                         "partials per profile (strong scaling; debye_partials_shard + debye_profile_from_partials)")
+                    help="what the headline of a multi-GPU run measures: structures = every rank its own structure (weak scaling, no "
+                         "collective; the default, with the tile split of one cfg5 structure reported beside it as `tile_split`); tiles = ONE "
+                         "structure (--config) split over the ranks by tiles of the upper triangle, one all-gather of FP64 partials per "
+                         "profile (strong scaling; debye_partials_shard + debye_profile_from_partials)")
     ap.add_argument("--path", default="pertype", choices=["pertype", "peratom"],
                     help="pertype: the north_star path (debye_profile, form factors per atom type); peratom: the paper's general "
                          "case (debye_profile_peratom, one form-factor row per atom; NEXT-1)")
@@ -180,6 +365,9 @@ def main():
                          "error statistics; prints one JSON object and exits")
     ap.add_argument("--no-hint", action="store_true", help="do not pass the q-grid hint (DEBYE_QHINT_*) computed from the host copy of q")
     args = ap.parse_args()
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    respawn_if_needed(args)
     args.warmup = max(args.warmup, 3) if args.impl == "libdebye" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -189,9 +377,11 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_1306_2258_b200 import binding as db, sharding
+    from paper_1306_2258_b200 import binding as db
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (libdebye has no CPU fallback)")
+    if torch.cuda.device_count() <= local_rank:
+        raise SystemExit(f"bench.py: rank {rank} needs CUDA device {local_rank}, this node has {torch.cuda.device_count()}")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
@@ -204,136 +394,67 @@ def main():
     if args.path == "peratom":
         return run_peratom(args, w, rank, world, dev)
     if args.split == "tiles":
-        return run_tile_split(args, make_workload(args.config, 0), rank, world, dev)
-    batch = w.xyz.ndim == 3
-    call = db.debye_profile_batch if batch else db.debye_profile
-    call_host = db.debye_profile_batch_host if batch else db.debye_profile_host
-    x, t, f, q = (torch.from_numpy(a).to(dev) for a in (w.xyz, w.type, w.fftab, w.q))
-    out = torch.empty((w.B, w.M) if batch else (w.M,), dtype=torch.float64, device=dev)
-    flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device=dev)        # > 126 MB L2
-    # the q grid exists on the host (it was generated there), so the caller can tell the library its shape: one pairs launch
-    # instead of up to three (include/debye.h, DEBYE_QHINT_*); the device verifies the hint
-    hint = 0 if args.no_hint else db.q_hint(w.q)
-    info = db.launch_info(w.N, w.B, w.T, w.M, args.variant, with_grid=True, hint=hint)
-
-    def barrier():
+        line = run_tile_split(args, make_workload(args.config, 0), rank, world, dev)
+        if rank == 0:
+            print(json.dumps(line))
         if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    # ---- device-resident timing -------------------------------------------------------------------------------
-    for _ in range(args.warmup):
-        call(x, t, f, q, out, variant=args.variant, hint=hint)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    wall0 = time.perf_counter()
-    for a, b in ev:
-        flush.fill_(1)                          # L2 flush between steps, outside the per-step events
-        a.record()
-        call(x, t, f, q, out, variant=args.variant, hint=hint)
-        b.record()
-    barrier()
-    wall = time.perf_counter() - wall0
-    clocks = sampler.stop()
-    step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = sharding.max_over_ranks(float(np.sum(step_ms)), dev)
-    units = sharding.sum_over_ranks(float(w.pair_q), dev)          # pair.q per step over all ranks
-    value = units * args.steps / (total_ms * 1e-3) / 1e9
-
-    # ---- dominant kernel (pairs) timed alone with events recorded by the library around its launch ----------
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(); e1.record(); torch.cuda.synchronize()
-    db.set_pairs_events(e0, e1)
-    pk = []
-    for _ in range(min(args.steps, 30)):
-        flush.fill_(1)
-        call(x, t, f, q, out, variant=args.variant, hint=hint)
-        torch.cuda.synchronize()
-        pk.append(e0.elapsed_time(e1))
-    db.set_pairs_events(None, None)
-    pairs_ms = float(np.mean(pk))
-
-    # ---- end to end through the host-buffer C entry (pinned inputs, copies inside the timed region) ----------
-    hx, ht, hf, hq = (torch.from_numpy(a).pin_memory().numpy() for a in (w.xyz, w.type, w.fftab, w.q))
-    hout = torch.empty((w.B, w.M) if batch else (w.M,), dtype=torch.float64).pin_memory().numpy()
-    for _ in range(3):
-        call_host(hx, ht, hf, hq, hout, variant=args.variant, hint=hint)
-    barrier()
-    n_e2e = max(5, min(args.steps, 50))
-    t0 = time.perf_counter()
-    for _ in range(n_e2e):
-        call_host(hx, ht, hf, hq, hout, variant=args.variant, hint=hint)
-    barrier()
-    e2e_s = sharding.max_over_ranks(time.perf_counter() - t0, dev)
-    e2e_value = units * n_e2e / e2e_s / 1e9
-    h2d = int(hx.nbytes + ht.nbytes + hf.nbytes + hq.nbytes)
-    result_dev = out.cpu().numpy()
-    assert np.array_equal(result_dev, hout), "host entry and device entry disagree"
-
+            dist.destroy_process_group()
+        return
+    batch = w.xyz.ndim == 3
+    res = measure(db, w, dev, args.variant, not args.no_hint, args.steps, args.warmup, world)
+    # multi-GPU: beside the independent structures (weak scaling), ONE cfg5 structure split over the ranks by tiles
+    split_line = None
+    if world > 1:
+        sargs = argparse.Namespace(**vars(args))
+        sargs.steps, sargs.warmup = 5, 3
+        split_line = run_tile_split(sargs, make_workload("cfg5", 0), rank, world, dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the pairs kernel ----------------------------------------------------
     peaks = measured_peaks()
     fmax_ghz = float(peaks.get("sm_max_mhz", 1965.0)) / 1e3
-    variant_ran = args.variant if args.variant != "auto" else ("recur" if _is_uniform(w.q) else "mufu")
-    pq_per_launch = float(w.pair_q)
-    if variant_ran == "recur":
-        # algorithmic work per pair.q: one recurrence FMA + one accumulate add = 2 FP32-pipe lane-ops (4 flop-slots)
-        peak = SM_COUNT * FP32_LANES * 2 * fmax_ghz / 1e3                       # TFLOP/s, FMA = 2 flop
-        achieved = 4.0 * pq_per_launch / (pairs_ms * 1e-3) / 1e12
-        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": None,
-                "note": "FP32-pipe roofline: 2 lane-ops (FFMA + FADD = 4 FMA-equivalent flop) per pair.q; peak = "
-                        "148 SM x 128 lanes x 2 x sm_max_mhz (MEASURED_PEAKS.json clock); measured pipe rates on this part: FADD2 0.995, "
-                        "FFMA2 0.91 of it (DESIGN.md section 7)"}
-    else:
-        per_term = {"mufu": 1.0}.get(variant_ran)
-        peak = SM_COUNT * MUFU_LANES * fmax_ghz / 1e3                           # T MUFU op/s
-        achieved = pq_per_launch / (pairs_ms * 1e-3) / 1e12
-        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T sin/s", "frac": achieved / peak,
-                "traffic": None, "note": "XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM" if per_term else
-                "reference variant; XU roofline quoted for scale"}
+    variant_ran = variant_that_ran(args.variant, w)
+    pairs_ms, total_ms, info = res["pairs_ms"], res["total_ms"], res["info"]
+    roof = roofline_of(w, variant_ran, pairs_ms, fmax_ghz)
+    # dram__bytes_read.sum + dram__bytes_write.sum of the pairs kernel from a committed ncu --set full capture of this command
+    # (None where no capture exists): not measured by this run
     roof["traffic"] = NCU_TRAFFIC.get((args.config, variant_ran))
-    k_ran, chunks_ran = info["q_chunk"], info["n_chunks"]
-    if hint == 0 and variant_ran == "recur" and w.M >= 2 and float(w.q[0]) == 0.0:
-        # grid starts at q = 0: the device runs the recurrence launch sized for M - 1 chain indices when the library
-        # offered one (it does when that saves accumulators or a chunk)
-        alt = db.launch_info(w.N, w.B, w.T, w.M - 1, "recur")
-        if alt["n_chunks"] <= 2 and (alt["q_chunk"] < k_ran or alt["n_chunks"] < chunks_ran):
-            k_ran, chunks_ran = alt["q_chunk"], alt["n_chunks"]
+    roof["traffic_source"] = NCU_TRAFFIC_SOURCE if roof["traffic"] is not None else None
+    k_ran, chunks_ran = kernel_shape(db, w, res, variant_ran)
     roof["kernel"] = f"debye_pairs_kernel<{k_ran}, {variant_ran}>"
     roof["kernel_ms"] = pairs_ms
-    roof["pair_q_per_clk_per_sm"] = pq_per_launch / (pairs_ms * 1e-3) / (SM_COUNT * fmax_ghz * 1e9)
+    roof["pair_q_per_clk_per_sm"] = float(w.pair_q) / (pairs_ms * 1e-3) / (SM_COUNT * fmax_ghz * 1e9)
     roof["share_of_step"] = pairs_ms / (total_ms / args.steps)
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if variant_ran == "fp64" else "f32", "data": "synthetic",
         "config": {"workload": w.name, "N": w.N, "T": w.T, "M": w.M, "B": w.B, "variant": variant_ran,
                    "pairs_grid": info["pairs_grid"], "q_chunk": k_ran, "n_chunks": chunks_ran,
-                   "q_hint": "passed (grid classified from the host copy of q, verified on the device)" if hint else "none",
+                   "q_hint": "passed (grid classified from the host copy of q, verified on the device)" if res["hint"] else "none",
                    "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
-                   "parallelism": f"{world} independent structure(s), one per GPU", "wall_s_timed_loop": wall},
-        "clocks": clocks,
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": int(hout.nbytes),
-                "ms_per_step": e2e_s / n_e2e * 1e3, "steps": n_e2e},
+                   "parallelism": f"{world} independent structure(s), one per GPU", "wall_s_timed_loop": res["wall"]},
+        "clocks": res["clocks"],
+        "e2e": res["e2e"],
         "gpu_launches": info["n_launches"] * args.steps,
         "roofline": roof,
     }
+    if split_line is not None:
+        line["tile_split"] = split_line
     if world == 1 and not args.no_cpu_baseline:
         cb = cpu_baseline(w)
         from oracle import oracle as orc                   # parity of the timed call's output against the oracle
         if not batch:
             ks = list(range(0, w.M, max(1, w.M // 8)))
             ref = orc.debye_sym(w.xyz, w.type, w.fftab[:, ks].copy(), w.q[ks].copy())
-            line["parity_max_rel_err"] = float(np.max(np.abs(result_dev[ks] - ref) / np.abs(ref)))
+            line["parity_max_rel_err"] = float(np.max(np.abs(res["result"][ks] - ref) / np.abs(ref)))
         line["cpu_baseline"] = cb
+    if world == 1 and args.config == "cfg2" and args.variant == "auto" and not args.no_configs and not args.no_cpu_baseline:
+        # the other BASELINE configs, same launch configuration, fewer steps; each checked against the oracle's whole profile
+        line["configs"] = {name: config_summary(db, name, dev, args.variant, not args.no_hint, fmax_ghz) for name in sorted(wl.CONFIGS)}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -357,7 +478,8 @@ def run_peaks(dev):
             row[f"ctas{c}"] = {"lane_ops_per_clk_per_sm": round(r[1], 2), "sched_cycles_per_instr": round(r[2], 3)}
         tests.append(row)
     mx, rms, mean = db.mufu_sin_error()
-    print(json.dumps({"pipe_bench": tests, "nominal": {"fp32_lanes_per_clk_per_sm": FP32_LANES, "mufu_lanes_per_clk_per_sm": MUFU_LANES},
+    rmx, rrms, rmean = db.mufu_rsq_error()
+    print(json.dumps({"pipe_bench": tests, "mufu_rsq_relative_error_log_uniform_1_to_4": {"max": rmx, "rms": rrms, "mean": rmean, "points": 1 << 24}, "nominal": {"fp32_lanes_per_clk_per_sm": FP32_LANES, "mufu_lanes_per_clk_per_sm": MUFU_LANES},
                       "mufu_sin_error_on_0_to_half_turn": {"max_abs": mx, "rms": rms, "mean": mean, "points": 1 << 24},
                       "clocks": sampler.stop()}))
 

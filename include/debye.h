@@ -204,12 +204,15 @@ int debye_set_pairs_events(void *start_event, void *stop_event);
  *   *cycles_per_instr (may be NULL): cycles of one warp scheduler per warp instruction of the mix.
  * Errors: DEBYE_EINVAL bad arguments, DEBYE_EUNSUPPORTED if ctas_per_sm CTAs of that test do not fit on an SM.
  * debye_mufu_sin_error: error of MUFU.SIN (sin.approx.ftz.f32 of 2 pi t) against double sin on n points of (0, 1/2] turns:
- * maximum |e|, root mean square, and MEAN (a bias is a coherent error in every pair: DESIGN.md section 6). */
+ * maximum |e|, root mean square, and MEAN (a bias is a coherent error in every pair: DESIGN.md section 6).
+ * debye_mufu_rsq_error: relative error of MUFU.RSQ (rsqrt.approx.ftz.f32) on n log-uniform points of [1, 4), same statistics;
+ * its mean shifts every distance, i.e. the q axis, by that relative amount. */
 int debye_pipe_bench_count(void);
 const char *debye_pipe_bench_name(int test);
 int debye_pipe_bench(int test, int ctas_per_sm, int iters, double *lane_ops_per_clk_per_sm, double *cycles_per_instr,
                      debye_stream_t stream);
 int debye_mufu_sin_error(int n, double *max_abs, double *rms, double *mean, debye_stream_t stream);
+int debye_mufu_rsq_error(int n, double *max_rel, double *rms, double *mean, debye_stream_t stream);
 
 const char *debye_strerror(int status);
 int debye_last_cuda_error(void); /* cudaError_t of the last failing runtime call on this thread, 0 if none */

@@ -21,7 +21,7 @@ EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_
            "debye_partials_shard", "debye_profile_from_partials", "debye_profile_peratom", "debye_profile_peratom_host", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
            "debye_launch_info", "debye_set_pairs_events", "debye_q_hint", "debye_plan_create", "debye_plan_execute",
            "debye_plan_destroy", "debye_strerror", "debye_last_cuda_error", "debye_version", "debye_pipe_bench_count",
-           "debye_pipe_bench_name", "debye_pipe_bench", "debye_mufu_sin_error")
+           "debye_pipe_bench_name", "debye_pipe_bench", "debye_mufu_sin_error", "debye_mufu_rsq_error")
 
 
 class LibdebyeError(RuntimeError):
@@ -91,6 +91,8 @@ def lib():
     L.debye_pipe_bench.restype = C.c_int
     L.debye_mufu_sin_error.argtypes = [C.c_int] + [C.POINTER(C.c_double)] * 3 + [vp]
     L.debye_mufu_sin_error.restype = C.c_int
+    L.debye_mufu_rsq_error.argtypes = L.debye_mufu_sin_error.argtypes
+    L.debye_mufu_rsq_error.restype = C.c_int
     _lib = L
     return L
 
@@ -345,4 +347,11 @@ def mufu_sin_error(n: int = 1 << 24, stream=None):
     """max |e|, rms, mean of MUFU.SIN against double sin on n points of (0, 1/2] turns (debye_mufu_sin_error)."""
     mx, rms, mean = C.c_double(), C.c_double(), C.c_double()
     _check(lib().debye_mufu_sin_error(n, C.byref(mx), C.byref(rms), C.byref(mean), _stream_ptr(stream)))
+    return mx.value, rms.value, mean.value
+
+
+def mufu_rsq_error(n: int = 1 << 24, stream=None):
+    """max, rms, mean RELATIVE error of MUFU.RSQ on n log-uniform points of [1, 4) (debye_mufu_rsq_error)."""
+    mx, rms, mean = C.c_double(), C.c_double(), C.c_double()
+    _check(lib().debye_mufu_rsq_error(n, C.byref(mx), C.byref(rms), C.byref(mean), _stream_ptr(stream)))
     return mx.value, rms.value, mean.value

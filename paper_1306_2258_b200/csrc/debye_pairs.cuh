@@ -253,7 +253,12 @@ __device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, con
     // clamp.  Product form: r = 1e-15 then gives b_k0 = 2 sin(k0 theta)/r its limit 2 k0 dq and W_j = 2 (every step of the
     // start-up keeps RELATIVE accuracy for small theta).  Chain form: such pairs take the slow path.
     const float r2c = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, 1e-30f)));
+#ifdef DEBYE_DBG_NEWTON
+    float rinv = rsqrt_mufu(r2c);
+    rinv = fmaf(0.5f * rinv, fmaf(-r2c * rinv, rinv, 1.0f), rinv);
+#else
     const float rinv = rsqrt_mufu(r2c);
+#endif
     g.r = r2c * rinv;
     bool small = false;
     if constexpr (!recur_is_product(MODE)) small = !(r2c > rc.cut2);
@@ -274,8 +279,9 @@ __device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, con
 // chains of stride 2 (W_j = W_2 W_{j-2} - W_{j-4}, W_0 = 2, W_{-1} = W_1), which halves the dependency depth.  An error
 // d of 2 cos(S theta) changes W_j by at most j^2 d (6e-8 x 256 = 1.5e-5 of the term at j = 16, pseudo-random over pairs).
 template <int MODE, int J>
-__device__ __forceinline__ void prod_vals(const RecurGeom &g, u64 (&U)[4], float (&Wt)[J])
+__device__ __forceinline__ void prod_vals(const RecurGeom &g, const RecurConst &rc, u64 (&U)[4], float (&Wt)[J])
 {
+    (void)rc;
     const float rinv = g.rinv;
     const Folded h = sincos_fold(g.f1);                // g.f1 = theta / 2 pi reduced: pi f1 = theta / 2
     const float T1 = two_sin_from(h, g.f1);
@@ -293,6 +299,14 @@ __device__ __forceinline__ void prod_vals(const RecurGeom &g, u64 (&U)[4], float
     } else {
         U[0] = pk2(u[1], u[2]); U[1] = pk2(u[3], u[4]); U[2] = pk2(u[5], u[6]); U[3] = pk2(u[7], u[8]);
     }
+#ifdef DEBYE_DBG_U64
+    {
+        const double th = 6.283185307179586476925 * ((double)rc.w1 + (double)rc.w1_lo) * (double)g.r;
+        const int o = (MODE == RM_P2B) ? 8 : 0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) U[a] = pk2((float)(2.0 * sin((o + 2 * a + 1) * th)) * rinv, (float)(2.0 * sin((o + 2 * a + 2) * th)) * rinv);
+    }
+#endif
     const float cS = two_cos_from(sincos_fold(g.fS));
     if constexpr (J > 1) Wt[1] = cS;
     if constexpr (J > 2) Wt[2] = fmaf(cS, cS, -2.0f);
@@ -300,23 +314,71 @@ __device__ __forceinline__ void prod_vals(const RecurGeom &g, u64 (&U)[4], float
     if constexpr (J > 4) Wt[4] = fmaf(Wt[2], Wt[2], -2.0f);
 #pragma unroll
     for (int j = 5; j < J; ++j) Wt[j] = fmaf(Wt[2], Wt[j - 2], -Wt[j - 4]);
+#ifdef DEBYE_DBG_W64
+    {
+        const double ph = 6.283185307179586476925 * ((double)rc.w1 + (double)rc.w1_lo) * (double)g.r * (double)rc.smult;
+#pragma unroll
+        for (int j = 1; j < J; ++j) Wt[j] = (float)(2.0 * cos(j * ph));
+    }
+#endif
     Wt[0] = 1.0f;
 }
 // Stage C: the outer product.  acc[4 j + a] (slots 8 j + 2 a, 8 j + 2 a + 1) += W_j * U[a]; level 0 has W_0 = 1.
 // All K/2 packed operations are independent of one another.
+#ifndef DEBYE_HOT_ORDER
+#define DEBYE_HOT_ORDER 0
+#endif
+__device__ __forceinline__ u64 fma2v(u64 a, u64 b, u64 c) { u64 d; asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ u64 add2v(u64 a, u64 b) { u64 d; asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 template <int K>
 __device__ __forceinline__ void prod_hot(u64 (&acc)[K / 2], const u64 (&U)[4], const float (&Wt)[(K + 7) / 8])
 {
+    constexpr int J = (K + 7) / 8;
+#if DEBYE_HOT_ORDER == 0      // the compiler orders the K/2 independent packed operations
 #pragma unroll
     for (int a = 0; a < 4; ++a)
         if (2 * a < K) acc[a] = add2(acc[a], U[a]);
 #pragma unroll
-    for (int j = 1; j < (K + 7) / 8; ++j) {
+    for (int j = 1; j < J; ++j) {
         const u64 wj = pk2(Wt[j], Wt[j]);               // SASS: the scalar-broadcast operand form of FFMA2, no copy
 #pragma unroll
         for (int a = 0; a < 4; ++a)
             if (8 * j + 2 * a < K) acc[4 * j + a] = fma2(wj, U[a], acc[4 * j + a]);     // K % 8 == 4: the last level has 4 slots
     }
+#elif DEBYE_HOT_ORDER == 1    // fixed order, seed pair outermost: U[a] stays in the operand reuse cache, each FFMA2 reads W_j + acc
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+        if (2 * a < K) acc[a] = add2v(acc[a], U[a]);
+#pragma unroll
+        for (int j = 1; j < J; ++j)
+            if (8 * j + 2 * a < K) acc[4 * j + a] = fma2v(pk2(Wt[j], Wt[j]), U[a], acc[4 * j + a]);
+    }
+#elif DEBYE_HOT_ORDER == 2    // fixed order, weight outermost
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+        if (2 * a < K) acc[a] = add2v(acc[a], U[a]);
+#pragma unroll
+    for (int j = 1; j < J; ++j) {
+        const u64 wj = pk2(Wt[j], Wt[j]);
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+            if (8 * j + 2 * a < K) acc[4 * j + a] = fma2v(wj, U[a], acc[4 * j + a]);
+    }
+#else                         // scalar FFMA
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+        float ul, uh;
+        upk2(U[a], ul, uh);
+#pragma unroll
+        for (int j = 0; j < J; ++j)
+            if (8 * j + 2 * a < K) {
+                float lo, hi;
+                upk2(acc[4 * j + a], lo, hi);
+                if (j == 0) { lo += ul; hi += uh; } else { lo = fmaf(Wt[j], ul, lo); hi = fmaf(Wt[j], uh, hi); }
+                acc[4 * j + a] = pk2(lo, hi);
+            }
+    }
+#endif
 }
 
 // One shared-memory tile of j atoms against this thread's i atom, product form, NP pairs per iteration.  Stage A of group
@@ -356,14 +418,14 @@ __device__ __forceinline__ void prod_tile(u64 (&acc)[K / 2], const float4 *__res
     RecurGeom gn[NP];
     geom(jj0, gn);
 #pragma unroll
-    for (int p = 0; p < NP; ++p) prod_vals<MODE, J>(gn[p], U[p], Wt[p]);
+    for (int p = 0; p < NP; ++p) prod_vals<MODE, J>(gn[p], rc, U[p], Wt[p]);
     geom(jj0 + NP, gn);
     DEBYE_PROD_UNROLL_PRAGMA
     for (int jj = jj0; jj < cnt; jj += NP) {
         u64 Un[NP][4];
         float Wn[NP][J];
 #pragma unroll
-        for (int p = 0; p < NP; ++p) prod_vals<MODE, J>(gn[p], Un[p], Wn[p]);
+        for (int p = 0; p < NP; ++p) prod_vals<MODE, J>(gn[p], rc, Un[p], Wn[p]);
         geom(jj + 2 * NP, gn);
 #pragma unroll
         for (int p = 0; p < NP; ++p) prod_hot<K>(acc, U[p], Wt[p]);
@@ -521,7 +583,7 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
 }
 
 #ifndef DEBYE_FLUSH_J
-#define DEBYE_FLUSH_J 4096
+#define DEBYE_FLUSH_J 512
 #endif
 
 #ifdef DEBYE_TRACE
@@ -802,10 +864,12 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
             }
             }
             __syncthreads();
+            // FP32 -> FP64 at least every DEBYE_FLUSH_J terms per accumulator, also inside a long row segment
+            pending += cnt;
+            if (pending >= DEBYE_FLUSH_J) { flush(); pending = 0; }
         }
-        pending += len;
         // weighted calls: the i atom (and with it wi) changes with every row segment, so flush before it does
-        if (W || pending >= DEBYE_FLUSH_J) { flush(); pending = 0; }
+        if (W && pending) { flush(); pending = 0; }
         u += len;
     }
     if (curX >= 0) { if (pending) flush(); write_record(curX); }

@@ -141,14 +141,14 @@ def test_two_type_lattice_and_chain_closed_forms(db):
 
 def test_tile_split_full_size_against_stored_oracle(db):
     """cfg2 and cfg3 split over 4 emulated ranks by tiles (debye_partials_shard with bench.py's launch configuration: the
-    automatic variant, 2368 / 4736 pairs CTAs), gathered and combined on the device, against the stored oracle samples."""
+    automatic variant, 2368 / 4736 pairs CTAs), gathered and combined on the device, against the stored oracle values (cfg2: 11 sampled q; cfg3: every q)."""
     import torch
     for name in ("cfg2", "cfg3"):
         w = wl.CONFIGS[name]()
         x, t, f, q = (torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (w.xyz, w.type, w.fftab, w.q))
         parts = [db.debye_partials_shard(x, t, q, w.T, r, 4) for r in range(4)]
         I = db.debye_profile_from_partials(torch.stack([p[0] for p in parts]), parts[0][1], f).cpu().numpy()[0]
-        assert check(I, golden()[name], w, TOL32) <= 1e-5
+        assert check(I, golden()[name], w, TOL32, f"{name} tile split x4") <= 3e-5
         # every rank got about a quarter of the pair sums (cyclic CTAs keep the triangular load balanced)
         share = torch.stack([p[0][0, :, 1].abs().sum() for p in parts])          # q index 1: all terms positive-ish
         assert float(share.min() / share.max()) > 0.8

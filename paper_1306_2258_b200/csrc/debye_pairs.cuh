@@ -253,12 +253,7 @@ __device__ __forceinline__ void recur_geom(const float4 pj, const float4 pi, con
     // clamp.  Product form: r = 1e-15 then gives b_k0 = 2 sin(k0 theta)/r its limit 2 k0 dq and W_j = 2 (every step of the
     // start-up keeps RELATIVE accuracy for small theta).  Chain form: such pairs take the slow path.
     const float r2c = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, 1e-30f)));
-#ifdef DEBYE_DBG_NEWTON
-    float rinv = rsqrt_mufu(r2c);
-    rinv = fmaf(0.5f * rinv, fmaf(-r2c * rinv, rinv, 1.0f), rinv);
-#else
     const float rinv = rsqrt_mufu(r2c);
-#endif
     g.r = r2c * rinv;
     bool small = false;
     if constexpr (!recur_is_product(MODE)) small = !(r2c > rc.cut2);
@@ -299,14 +294,6 @@ __device__ __forceinline__ void prod_vals(const RecurGeom &g, const RecurConst &
     } else {
         U[0] = pk2(u[1], u[2]); U[1] = pk2(u[3], u[4]); U[2] = pk2(u[5], u[6]); U[3] = pk2(u[7], u[8]);
     }
-#ifdef DEBYE_DBG_U64
-    {
-        const double th = 6.283185307179586476925 * ((double)rc.w1 + (double)rc.w1_lo) * (double)g.r;
-        const int o = (MODE == RM_P2B) ? 8 : 0;
-#pragma unroll
-        for (int a = 0; a < 4; ++a) U[a] = pk2((float)(2.0 * sin((o + 2 * a + 1) * th)) * rinv, (float)(2.0 * sin((o + 2 * a + 2) * th)) * rinv);
-    }
-#endif
     const float cS = two_cos_from(sincos_fold(g.fS));
     if constexpr (J > 1) Wt[1] = cS;
     if constexpr (J > 2) Wt[2] = fmaf(cS, cS, -2.0f);
@@ -314,80 +301,31 @@ __device__ __forceinline__ void prod_vals(const RecurGeom &g, const RecurConst &
     if constexpr (J > 4) Wt[4] = fmaf(Wt[2], Wt[2], -2.0f);
 #pragma unroll
     for (int j = 5; j < J; ++j) Wt[j] = fmaf(Wt[2], Wt[j - 2], -Wt[j - 4]);
-#ifdef DEBYE_DBG_W64
-    {
-        const double ph = 6.283185307179586476925 * ((double)rc.w1 + (double)rc.w1_lo) * (double)g.r * (double)rc.smult;
-#pragma unroll
-        for (int j = 1; j < J; ++j) Wt[j] = (float)(2.0 * cos(j * ph));
-    }
-#endif
     Wt[0] = 1.0f;
 }
 // Stage C: the outer product.  acc[4 j + a] (slots 8 j + 2 a, 8 j + 2 a + 1) += W_j * U[a]; level 0 has W_0 = 1.
 // All K/2 packed operations are independent of one another.
-#ifndef DEBYE_HOT_ORDER
-#define DEBYE_HOT_ORDER 0
-#endif
-__device__ __forceinline__ u64 fma2v(u64 a, u64 b, u64 c) { u64 d; asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
-__device__ __forceinline__ u64 add2v(u64 a, u64 b) { u64 d; asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 template <int K>
 __device__ __forceinline__ void prod_hot(u64 (&acc)[K / 2], const u64 (&U)[4], const float (&Wt)[(K + 7) / 8])
 {
-    constexpr int J = (K + 7) / 8;
-#if DEBYE_HOT_ORDER == 0      // the compiler orders the K/2 independent packed operations
+    // the compiler orders the K/2 independent packed operations; fixed orders (seed pair or weight outermost, so that one
+    // operand stays in the reuse cache) and scalar FFMA were measured on B200 and are slower (profiles/r02_product_form.md)
 #pragma unroll
     for (int a = 0; a < 4; ++a)
         if (2 * a < K) acc[a] = add2(acc[a], U[a]);
 #pragma unroll
-    for (int j = 1; j < J; ++j) {
+    for (int j = 1; j < (K + 7) / 8; ++j) {
         const u64 wj = pk2(Wt[j], Wt[j]);               // SASS: the scalar-broadcast operand form of FFMA2, no copy
 #pragma unroll
         for (int a = 0; a < 4; ++a)
             if (8 * j + 2 * a < K) acc[4 * j + a] = fma2(wj, U[a], acc[4 * j + a]);     // K % 8 == 4: the last level has 4 slots
     }
-#elif DEBYE_HOT_ORDER == 1    // fixed order, seed pair outermost: U[a] stays in the operand reuse cache, each FFMA2 reads W_j + acc
-#pragma unroll
-    for (int a = 0; a < 4; ++a) {
-        if (2 * a < K) acc[a] = add2v(acc[a], U[a]);
-#pragma unroll
-        for (int j = 1; j < J; ++j)
-            if (8 * j + 2 * a < K) acc[4 * j + a] = fma2v(pk2(Wt[j], Wt[j]), U[a], acc[4 * j + a]);
-    }
-#elif DEBYE_HOT_ORDER == 2    // fixed order, weight outermost
-#pragma unroll
-    for (int a = 0; a < 4; ++a)
-        if (2 * a < K) acc[a] = add2v(acc[a], U[a]);
-#pragma unroll
-    for (int j = 1; j < J; ++j) {
-        const u64 wj = pk2(Wt[j], Wt[j]);
-#pragma unroll
-        for (int a = 0; a < 4; ++a)
-            if (8 * j + 2 * a < K) acc[4 * j + a] = fma2v(wj, U[a], acc[4 * j + a]);
-    }
-#else                         // scalar FFMA
-#pragma unroll
-    for (int a = 0; a < 4; ++a) {
-        float ul, uh;
-        upk2(U[a], ul, uh);
-#pragma unroll
-        for (int j = 0; j < J; ++j)
-            if (8 * j + 2 * a < K) {
-                float lo, hi;
-                upk2(acc[4 * j + a], lo, hi);
-                if (j == 0) { lo += ul; hi += uh; } else { lo = fmaf(Wt[j], ul, lo); hi = fmaf(Wt[j], uh, hi); }
-                acc[4 * j + a] = pk2(lo, hi);
-            }
-    }
-#endif
 }
 
 // One shared-memory tile of j atoms against this thread's i atom, product form, NP pairs per iteration.  Stage A of group
 // jj + 2 NP and stage B of group jj + NP sit in the same basic block as the outer products of group jj, so the scheduler
 // hides their dependency chains (distance, rsqrt, range reduction, polynomials, seed and weight chains: ~70 dependent
 // FP32 instructions) under the independent packed instructions.
-#ifndef DEBYE_NPP
-#define DEBYE_NPP 1
-#endif
 #define DEBYE_PRAGMA_(x) _Pragma(#x)
 #define DEBYE_PRAGMA(x) DEBYE_PRAGMA_(x)
 #ifdef DEBYE_PROD_UNROLL
@@ -395,48 +333,70 @@ __device__ __forceinline__ void prod_hot(u64 (&acc)[K / 2], const u64 (&U)[4], c
 #else
 #define DEBYE_PROD_UNROLL_PRAGMA
 #endif
+// pairs per iteration: two (amortises the loop overhead and gives the scheduler two independent start-up chains; measured
+// on B200 against one pair per iteration: +4 % cfg2, +9 % cfg3, +4 % cfg4, +6 % cfg5)
+#ifndef DEBYE_NPP
+#define DEBYE_NPP 2
+#endif
+__host__ __device__ constexpr int prod_np(int K) { return DEBYE_NPP; }
 template <int K, int MODE, bool W>
 __device__ __forceinline__ void prod_tile(u64 (&acc)[K / 2], const float4 *__restrict__ tile, const int jj0, const int cnt, const float4 pi,
-                                          const bool ivalid, const bool diag, const int i_local, const int jl0, const RecurConst &rc)
+                                          const bool ivalid, const bool diag, const int i_local, const int jl0, const RecurConst &rc,
+                                          const int jfree /* warp-uniform: every lane may pair with every tile index >= jfree */)
 {
-    constexpr int NP = DEBYE_NPP, J = (K + 7) / 8;
+    constexpr int NP = prod_np(K), J = (K + 7) / 8;
     if (jj0 >= cnt) return;
     // first tile index this thread may pair with: masks i >= j on the diagonal and threads without an i atom
     const int jmin = ivalid ? (diag ? max(0, i_local + 1 - jl0) : 0) : 0x7fffffff;
     // masked pairs (before jmin, behind the last atom of the tile: the pipeline reads two groups ahead) get 1/r = 0 and with
     // it seeds that are exactly 0; their coordinates are read from a VALID entry of this tile (index clamp), so that a
     // stale non-finite entry behind the tile can never reach the accumulators (0 * NaN)
-    auto geom = [&](const int jbase, RecurGeom (&g)[NP]) {
+    auto geom_masked = [&](const int jbase, RecurGeom (&g)[NP]) {
 #pragma unroll
         for (int p = 0; p < NP; ++p) {
             const int j = jbase + p;
             recur_geom<MODE, W>(tile[min(j, cnt - 1)], pi, j >= jmin && j < cnt, rc, g[p]);
         }
     };
+    auto geom_free = [&](const int jbase, RecurGeom (&g)[NP]) {
+#pragma unroll
+        for (int p = 0; p < NP; ++p) recur_geom<MODE, W>(tile[jbase + p], pi, true, rc, g[p]);
+    };
     u64 U[NP][4];
     float Wt[NP][J];
     RecurGeom gn[NP];
-    geom(jj0, gn);
+    geom_masked(jj0, gn);
 #pragma unroll
     for (int p = 0; p < NP; ++p) prod_vals<MODE, J>(gn[p], rc, U[p], Wt[p]);
-    geom(jj0 + NP, gn);
-    DEBYE_PROD_UNROLL_PRAGMA
-    for (int jj = jj0; jj < cnt; jj += NP) {
-        u64 Un[NP][4];
-        float Wn[NP][J];
-#pragma unroll
-        for (int p = 0; p < NP; ++p) prod_vals<MODE, J>(gn[p], rc, Un[p], Wn[p]);
-        geom(jj + 2 * NP, gn);
-#pragma unroll
-        for (int p = 0; p < NP; ++p) prod_hot<K>(acc, U[p], Wt[p]);
-#pragma unroll
-        for (int p = 0; p < NP; ++p) {
-#pragma unroll
-            for (int a = 0; a < 4; ++a) U[p][a] = Un[p][a];
-#pragma unroll
-            for (int j = 0; j < J; ++j) Wt[p][j] = Wn[p][j];
+    geom_masked(jj0 + NP, gn);
+    // one iteration: stage B of group jj + NP, stage A of group jj + 2 NP, outer products of group jj
+#define DEBYE_PROD_ITER(GEOM)                                                                        \
+    {                                                                                                \
+        u64 Un[NP][4];                                                                               \
+        float Wn[NP][J];                                                                             \
+        _Pragma("unroll") for (int p = 0; p < NP; ++p) prod_vals<MODE, J>(gn[p], rc, Un[p], Wn[p]);  \
+        GEOM(jj + 2 * NP, gn);                                                                       \
+        _Pragma("unroll") for (int p = 0; p < NP; ++p) prod_hot<K>(acc, U[p], Wt[p]);                \
+        _Pragma("unroll") for (int p = 0; p < NP; ++p) {                                             \
+            _Pragma("unroll") for (int a = 0; a < 4; ++a) U[p][a] = Un[p][a];                        \
+            _Pragma("unroll") for (int j = 0; j < J; ++j) Wt[p][j] = Wn[p][j];                       \
+        }                                                                                            \
+    }
+    // The interior of a tile needs no mask: all lanes have an i atom below every j of the group whose geometry the iteration
+    // computes (jj + 2 NP .. jj + 3 NP - 1 in [jfree, cnt)).  The bounds are warp-uniform; the masked copy of the loop runs the
+    // head (diagonal) and the tail of the tile, and whole tiles of warps with a lane that has no i atom (jfree = INT_MAX).
+    int jj = jj0;
+#pragma unroll 1
+    for (int phase = 0; phase < 2; ++phase) {
+        const int stop = (phase == 0) ? ((jfree > cnt) ? cnt : min(cnt, max(jj0, jfree - 2 * NP))) : cnt;
+#pragma unroll 1
+        for (; jj < stop; jj += NP) DEBYE_PROD_ITER(geom_masked)
+        if (phase == 0) {
+            DEBYE_PROD_UNROLL_PRAGMA
+            for (; jj + 3 * NP <= cnt; jj += NP) DEBYE_PROD_ITER(geom_free)
         }
     }
+#undef DEBYE_PROD_ITER
 }
 
 // ---- chain form (RM_G) ----------------------------------------------------------------------------------------------
@@ -801,10 +761,16 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
             int jj0 = 0;
             if (diag) { int first_i = row * DEBYE_IB + warp * 32; jj0 = max(0, first_i + 1 - jl0); }
             if constexpr (VAR == V_RECUR) {
+                // first tile index from which every lane of this warp pairs with every j: 0 off the diagonal, behind the
+                // warp's last i atom on it; never if some lane has no i atom (ragged last row)
+                const int w_last_i = row * DEBYE_IB + warp * 32 + 31;
+                const int jfree = (w_last_i >= n_i) ? 0x7fffffff : (diag ? max(0, w_last_i + 1 - jl0) : 0);
+                // a warp none of whose lanes has an i atom (ragged last row of a small type segment) only keeps the barriers
+                if (row * DEBYE_IB + warp * 32 < n_i)
                 switch (mode) {      // warp-uniform; one copy of the pipelined loop per mode
-                    case RM_P1: prod_tile<K, RM_P1, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc); break;
-                    case RM_P2A: prod_tile<K, RM_P2A, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc); break;
-                    case RM_P2B: prod_tile<K, RM_P2B, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc); break;
+                    case RM_P1: prod_tile<K, RM_P1, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, jfree); break;
+                    case RM_P2A: prod_tile<K, RM_P2A, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, jfree); break;
+                    case RM_P2B: prod_tile<K, RM_P2B, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, jfree); break;
                     default: recur_tile<K, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
                 }
             } else {

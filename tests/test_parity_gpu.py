@@ -392,6 +392,26 @@ def test_non_finite_input_propagates_and_does_not_poison_later_calls(db):
     assert gpu_profile(db, w).tobytes() == good.tobytes()
 
 
+def test_non_finite_conformer_does_not_reach_its_neighbours_in_a_batch(db):
+    """A NaN coordinate in ONE conformer of a batch makes that conformer's profile NaN and leaves every other conformer's
+    profile bit-identical to a clean run: masked pairs (tile tails, read-ahead of the pipeline) read their coordinates from
+    a valid entry of the current tile, never from whatever an earlier tile -- possibly of another conformer -- left behind.
+    Odd atom counts per type make the two-pairs-per-iteration loop end on a masked partner."""
+    for N, M in ((301, 101), (517, 64), (203, 128)):
+        geo, tab = wl.cfg4(B=5, N=N), wl.small_random(3, 10, 5, M, q_max=0.5)      # 5 conformers; a 5-type table on M points
+        w = wl.Workload("batch", geo.xyz, geo.type, tab.fftab, tab.q)
+        clean = gpu_profile(db, w, batch=True)
+        bad = wl.Workload("nanbatch", w.xyz.copy(), w.type, w.fftab, w.q)
+        bad.xyz[2, N // 3, 1] = np.nan
+        bad.xyz[2, N - 1, 2] = np.inf
+        for v in ("auto", "mufu"):
+            ref = clean if v == "auto" else gpu_profile(db, w, v, batch=True)
+            I = gpu_profile(db, bad, v, batch=True)
+            assert not np.isfinite(I[2, 1:]).any(), v
+            for b in (0, 1, 3, 4):
+                assert I[b].tobytes() == ref[b].tobytes(), (v, b, N)
+
+
 def test_q_grid_split_over_ranks_reassembles_the_profile(db):
     """sharding.profile_q_slice (different q ranges on different devices), the ranks emulated one after
     the other on one GPU: the slices tile the grid and agree with the unsplit profile and the oracle."""

@@ -215,7 +215,7 @@ class Plan:
             pass
 
 
-def debye_partials(xyz, type, q, T, variant="auto", stream=None):
+def debye_partials(xyz, type, q, T, variant="auto", stream=None, hint=0):
     """(S[B,T(T+1)/2,M] float64, n[T] int32): per-type-pair sums of sinc(q r) over pairs i<j, atoms per type."""
     import torch
     x3 = xyz if xyz.dim() == 3 else xyz[None]
@@ -224,7 +224,7 @@ def debye_partials(xyz, type, q, T, variant="auto", stream=None):
     n = torch.empty(T, dtype=torch.int32, device=xyz.device)
     _check(lib().debye_partials(_dev(x3, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N, B,
                                 _dev(q, torch.float32, "q"), T, M, _dev(S, torch.float64, "S_out"),
-                                _dev(n, torch.int32, "n_out"), _flags(variant), _stream_ptr(stream)))
+                                _dev(n, torch.int32, "n_out"), _flags(variant, hint), _stream_ptr(stream)))
     return S, n
 
 

@@ -20,6 +20,7 @@
 #include "debye_plan.cuh"
 #include "debye_registry.h"
 #include "debye_peratom.cuh"
+#include "debye_small.cuh"
 
 namespace {
 
@@ -42,6 +43,7 @@ struct DevState {
     int sms = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;         // optional: recorded around the pairs launches
     int occ[5][33];                                   // cached CTAs/SM per (variant, K/4); 0 = unknown
+    int occ_small[17][DEBYE_SMALL_TMAX + 1];          // the same for debye_small_kernel<8 i> with T types (N = 2048); 0 = unknown
 };
 DevState g_dev[MAX_DEV];
 std::mutex g_mu;
@@ -187,6 +189,7 @@ int dev_state(DevState **st)
         CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
         s->sms = sms;
         memset(s->occ, 0, sizeof(s->occ));
+        memset(s->occ_small, 0, sizeof(s->occ_small));
     }
     *st = s;
     return DEBYE_OK;
@@ -252,10 +255,69 @@ int ensure(void **ptr, size_t *have, size_t need)
 struct debye_plan {
     int N, B, T, M, device;
     uint32_t flags;              // the caller's flags with the grid hint resolved at creation
-    char *buf;                   // one allocation: DevPlan | perm[N] | q[M] | weight[N]
-    DevPlan *plan; int32_t *perm; float *q; float *weight;
+    char *buf;                   // one allocation: DevPlan | perm[N] | q[M] | weight[N] | type[N]
+    DevPlan *plan; int32_t *perm; float *q; float *weight; int32_t *type;
 };
 namespace {
+
+// One launch for one small structure (debye_small.cuh): single structure, unweighted, not sharded, N <= 2048, T <= 8, and a
+// grid hint that promises q_k = (k + koff) dq with at most 128 chain indices (the kernel verifies the hint; NaN otherwise).
+bool small_eligible(int N, int B, int T, int M, uint32_t flags, const float *weight, int shard_world)
+{
+    if (B != 1 || weight || shard_world != 1 || N > DEBYE_SMALL_NMAX || T > DEBYE_SMALL_TMAX) return false;
+    if (flags & (DEBYE_FP64 | DEBYE_SINC_MUFU | DEBYE_SINC_ACCURATE)) return false;
+    const int cls = hint_class_of(flags);
+    if (cls != 0 && cls != 1) return false;
+    const int n_idx = M - (cls == 0 ? 1 : 0);
+    return n_idx >= 1 && n_idx <= DEBYE_KMAX_F32;
+}
+int small_K(int M, uint32_t flags) { return (debye::recur_slots(M - (hint_class_of(flags) == 0 ? 1 : 0), 1) + 7) / 8 * 8; }
+int small_grid(DevState *ds, int N, int T, int K, int *G)
+{
+    int &o = ds->occ_small[K / 8][T];
+    debye_small_fn fn = debye_get_small_kernel(K);
+    if (!fn) return DEBYE_EUNSUPPORTED;
+    if (o == 0) {
+        // dynamic shared memory up to the largest case (T = 8, K = 128 sums / 2048 atoms); opt in once
+        CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)debye::debye_small_dyn_smem(DEBYE_SMALL_NMAX, DEBYE_SMALL_TMAX, DEBYE_KMAX_F32)));
+        int nb = 0;
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fn, DEBYE_IB, debye::debye_small_dyn_smem(DEBYE_SMALL_NMAX, T, K)));
+        o = nb < 1 ? 1 : nb;
+    }
+    // one wave at most; at least ~6 units (j atoms x 128 i atoms) per CTA, estimated from N alone
+    const int64_t units = (int64_t)N * N / (2 * DEBYE_IB) + 1;
+    // one CTA per SM at most (measured on B200, 1000 and 2000 atoms: 28.8 / 37.0 us per profile with 148 CTAs, 29.2 / 37.4
+    // with 296, 33.3 / 42.9 with 592: every CTA pays the sort, and the final stage grows with the number of records)
+    int64_t g = units / 6;
+    if (g > (int64_t)ds->sms) g = (int64_t)ds->sms;
+    if (g < 1) g = 1;
+    *G = (int)g;
+    return DEBYE_OK;
+}
+size_t small_ws_bytes(int T, int K, int G) { return align_up(((size_t)G + (size_t)(T * (T + 1) / 2)) * K * 8); }
+
+int run_small(DevState *ds, const float *xyz, const int32_t *type, int N, const float *fftab, int T, const float *q, int M, double *out, int32_t *n_out,
+              uint32_t flags, cudaStream_t stream, int mode)
+{
+    const int K = small_K(M, flags);
+    int G = 0, st;
+    if ((st = small_grid(ds, N, T, K, &G))) return st;
+    const size_t need = small_ws_bytes(T, K, G);
+    char *ws;
+    if (ds->user_ws) { if (ds->user_bytes < need) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
+    else { if ((st = ensure(&ds->ws, &ds->ws_bytes, need))) return st; ws = (char *)ds->ws; }
+    debye_small_fn fn = debye_get_small_kernel(K);
+    if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
+    {   // cooperative launch: the kernel has a grid-wide barrier (G is at most one resident wave, small_grid)
+        int hc = hint_class_of(flags);
+        double *rec = (double *)ws;
+        void *args[] = {(void *)&xyz, (void *)&type, (void *)&N, (void *)&T, (void *)&fftab, (void *)&q, (void *)&M, (void *)&hc, (void *)&rec, (void *)&out, (void *)&mode, (void *)&n_out};
+        CU(cudaLaunchCooperativeKernel((const void *)fn, dim3(G), dim3(DEBYE_IB), args, debye::debye_small_dyn_smem(N, T, K), stream));
+    }
+    if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
+    CU(cudaGetLastError());
+    return DEBYE_OK;
+}
 
 // mode 0: I_out[B][M]; mode 1: S_out[B][n_tp][M] (+ n_out)
 int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab, int T, const float *q, int M, double *out, int32_t *n_out,
@@ -267,6 +329,8 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     std::lock_guard<std::mutex> lock(g_mu);
     DevState *ds;
     if ((st = dev_state(&ds))) return st;
+    if (small_eligible(N, B, T, M, flags, weight, shard_world) && (!pre || pre->type))
+        return run_small(ds, xyz, pre ? pre->type : type, N, fftab, T, q, M, out, n_out, flags, stream, mode);
     Choice ch[MAX_CHOICES]; int is_auto = 0;
     const int nch = variants_for(flags, ch, M, &is_auto);
     int G[MAX_CHOICES] = {0, 0, 0}, Gmax = 0;
@@ -535,9 +599,12 @@ int debye_plan_create(debye_plan **out, const int32_t *type, int32_t N, int32_t 
     const size_t o_perm = o; o += align_up((size_t)N * 4);
     const size_t o_q = o; o += align_up((size_t)M * 4);
     const size_t o_w = o; o += align_up((size_t)N * 4);
+    const size_t o_t = o; o += align_up((size_t)N * 4);
     if (cudaMalloc((void **)&p->buf, o) != cudaSuccess) { (void)cudaGetLastError(); p->buf = nullptr; return fail(DEBYE_ENOMEM); }
     p->plan = (DevPlan *)(p->buf + o_plan); p->perm = (int32_t *)(p->buf + o_perm); p->q = (float *)(p->buf + o_q);
     p->weight = weight ? (float *)(p->buf + o_w) : nullptr;
+    p->type = (int32_t *)(p->buf + o_t);          // small structures re-sort per call inside the one fused launch
+    if (cudaMemcpyAsync(p->type, type, (size_t)N * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
     if (cudaMemcpyAsync(p->q, q, (size_t)M * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
     if (weight && cudaMemcpyAsync(p->weight, weight, (size_t)N * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
     // the setup step, once; then read its verdict on the grid back (the only synchronisation of the plan's life)
@@ -593,6 +660,14 @@ size_t debye_workspace_bytes(int32_t N, int32_t B, int32_t T, int32_t M, uint32_
 {
     static const char dummy = 0;
     if (validate(&dummy, &dummy, N, B, &dummy, T, &dummy, M, &dummy, flags)) return 0;
+    if (small_eligible(N, B, T, M, flags, nullptr, 1)) {
+        std::lock_guard<std::mutex> lock(g_mu);
+        DevState *ds; int G = 192 * 4;
+        const int K = small_K(M, flags);
+        if (dev_state(&ds) == DEBYE_OK) { int g = 0; if (small_grid(ds, N, T, K, &g) == DEBYE_OK) G = g; }
+        (void)cudaGetLastError();
+        return small_ws_bytes(T, K, G);
+    }
     Choice ch[MAX_CHOICES]; int is_auto;
     int nch = variants_for(flags, ch, M, &is_auto);
     // exact when a CUDA device is current (same grid computation as the call itself; attribute queries only, no GPU work);
@@ -643,6 +718,20 @@ int debye_launch_info(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags
     static const char dummy = 0;
     int st = validate(&dummy, &dummy, N, B, &dummy, T, &dummy, M, &dummy, flags);
     if (st) return st;
+    if (small_eligible(N, B, T, M, flags, nullptr, 1)) {      // one fused launch (debye_small.cuh)
+        const int K = small_K(M, flags);
+        if (n_launches) *n_launches = 1;
+        if (q_chunk) *q_chunk = K;
+        if (n_chunks) *n_chunks = 1;
+        if (pairs_grid) {
+            std::lock_guard<std::mutex> lock(g_mu);
+            DevState *ds; int G = 0;
+            if ((st = dev_state(&ds))) return st;
+            if ((st = small_grid(ds, N, T, K, &G))) return st;
+            *pairs_grid = G;
+        }
+        return DEBYE_OK;
+    }
     Choice ch[MAX_CHOICES]; int is_auto;
     int nch = variants_for(flags, ch, M, &is_auto);
     const int lead = (nch > 1 && ch[0].alt_gate == 1) ? 1 : 0;     // report the launch sized for the general case

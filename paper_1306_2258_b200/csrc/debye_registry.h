@@ -11,3 +11,7 @@ typedef void (*debye_pairs_fn)(const DevPlan *, const float4 *, const float *, d
 // K must be a multiple of 8 in [8, KMAX] (recurrence: a multiple of 4); returns nullptr otherwise
 // sharded: the instantiation whose CTAs skip the tiles of other ranks (debye_partials_shard; unweighted only)
 debye_pairs_fn debye_get_pairs_kernel(int variant, int K, bool weighted, bool sharded = false);
+
+// one launch for one small structure (debye_small.cuh): K a multiple of 8 in [8, 128]; nullptr otherwise
+typedef void (*debye_small_fn)(const float *, const int32_t *, int, int, const float *, const float *, int, int, double *, double *, int, int32_t *);
+debye_small_fn debye_get_small_kernel(int K);

@@ -310,8 +310,9 @@ def test_random_shape_sweep(db):
 
 
 def test_grid_hints_select_one_launch_and_are_checked(db):
-    """DEBYE_QHINT_* (include/debye.h): with the right hint the result is the unhinted one bit for bit; a wrong hint gives
-    NaN, never a wrong number."""
+    """DEBYE_QHINT_* (include/debye.h): with the right hint the result is the unhinted one -- bit for bit where the hint
+    only removes launches, to rounding where it selects the single fused launch for small structures (debye_small.cuh: the
+    same terms, summed by other CTAs); a wrong hint gives NaN, never a wrong number."""
     import torch
     grids = {"zero": wl.q_grid(0.5, 101), "dq": wl.q_grid(1.0, 50, 0.02), "offset": wl.q_grid(0.9, 64, 0.3),
              "nonuniform": np.sort(np.random.default_rng(7).uniform(0.01, 0.8, 40)).astype(np.float32),
@@ -327,12 +328,61 @@ def test_grid_hints_select_one_launch_and_are_checked(db):
         ref = orc.debye_sym(base.xyz, base.type, f, qg)
         assert rel(plain, ref) <= TOL32
         hinted = db.debye_profile(x, t, fd, qd, hint=hints[name]).cpu().numpy()
-        assert hinted.tobytes() == plain.tobytes(), name
+        if db.launch_info(base.N, 1, 3, len(qg), "auto", hint=hints[name])["n_launches"] == 1:      # the fused small-structure launch
+            assert name in ("zero", "dq", "zero_129") and rel(hinted, plain) <= 2e-6 and rel(hinted, ref) <= TOL32
+            assert hinted.tobytes() == db.debye_profile(x, t, fd, qd, hint=hints[name]).cpu().numpy().tobytes()
+        else:
+            assert hinted.tobytes() == plain.tobytes(), name
         for other, h in hints.items():
             if h != hints[name]:
                 assert np.isnan(db.debye_profile(x, t, fd, qd, hint=h).cpu().numpy()).all(), (name, other)
     hb = db.debye_profile_host(base.xyz, base.type, wl.gaussian_form_factors(77, 3, grids["zero"]), grids["zero"], hint=hints["zero"])
     assert np.isfinite(hb).all()
+
+
+def test_small_structure_single_launch(db):
+    """debye_small_kernel (PAPER.md:88 "N < W", :25 refinement loops): with a grid hint a structure of at most 2048 atoms and
+    8 types on a grid q_k = (k + koff) dq with at most 128 chain indices runs as ONE launch (sort in shared memory per CTA,
+    product-form pairs, last-CTA reduction + epilogue).  Against the oracle, against the general path, twice for bits; the
+    partial structure factors too; shapes that span 1..16 rows, 1..8 types, ragged segments, the size limits."""
+    import torch
+    shapes = [(2, 1, 5, 0.0), (3, 2, 9, 0.0), (130, 3, 17, 0.0), (777, 5, 101, 0.0), (1000, 8, 51, 0.0), (1031, 4, 129, 0.0),
+              (500, 2, 128, 0.005), (2048, 5, 64, 0.0), (1999, 7, 33, 0.02), (257, 1, 2, 0.0), (64, 8, 100, 0.004)]
+    for si, (N, T, M, q_min) in enumerate(shapes):
+        w = wl.small_random(200 + si, N, T, M, q_min=q_min, q_max=q_min * M if q_min else 0.6, box=20.0 + N ** (1 / 3) * 3)
+        hint = db.q_hint(w.q)
+        assert db.launch_info(N, 1, T, M, "auto", hint=hint)["n_launches"] == 1, (N, T, M)
+        x, t, f, q = to_dev(w)
+        ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)
+        a = db.debye_profile(x, t, f, q, hint=hint).cpu().numpy()
+        assert rel(a, ref) <= TOL32, (N, T, M, rel(a, ref))
+        assert rel(a, gpu_profile(db, w)) <= 5e-6
+        assert a.tobytes() == db.debye_profile(x, t, f, q, hint=hint).cpu().numpy().tobytes()
+        S, n = db.debye_partials(x, t, q, T, hint=hint)
+        assert np.array_equal(n.cpu().numpy(), np.bincount(w.type, minlength=T))
+        S = S.cpu().numpy()[0]
+        F = w.fftab.astype(np.float64)
+        I = (n.cpu().numpy()[:, None] * F * F).sum(0)
+        tp = 0
+        for ta in range(T):
+            for tb in range(ta, T):
+                I = I + 2.0 * F[ta] * F[tb] * S[tp]
+                tp += 1
+        assert rel(I, a) <= 1e-12
+    # a wrong hint gives NaN; just beyond the limits the general path runs
+    w = wl.small_random(230, 300, 3, 40, q_min=0.3, q_max=0.9)          # general start, but the caller promises q[0] == 0
+    x, t, f, q = to_dev(w)
+    assert np.isnan(db.debye_profile(x, t, f, q, hint=db.q_hint(wl.q_grid(0.5, 40))).cpu().numpy()).all()
+    assert db.launch_info(2049, 1, 3, 40, "auto", hint=db.q_hint(wl.q_grid(0.5, 40)))["n_launches"] > 1
+    assert db.launch_info(500, 1, 9, 40, "auto", hint=db.q_hint(wl.q_grid(0.5, 40)))["n_launches"] > 1
+    assert db.launch_info(500, 1, 3, 130, "auto", hint=db.q_hint(wl.q_grid(0.5, 130)))["n_launches"] > 1
+    # coincident atoms and a single atom
+    w1 = wl.Workload("one", np.zeros((1, 3), np.float32), np.zeros(1, np.int32), np.full((1, 9), 3.0, np.float32), wl.q_grid(0.4, 9))
+    x, t, f, q = to_dev(w1)
+    assert np.allclose(db.debye_profile(x, t, f, q, hint=db.q_hint(w1.q)).cpu().numpy(), 9.0, rtol=0, atol=0)
+    wc = wl.Workload("coincident", np.zeros((40, 3), np.float32), np.zeros(40, np.int32), np.full((1, 9), 1.0, np.float32), wl.q_grid(0.4, 9))
+    x, t, f, q = to_dev(wc)
+    assert rel(db.debye_profile(x, t, f, q, hint=db.q_hint(wc.q)).cpu().numpy(), np.full(9, 1600.0)) <= 1e-6
 
 
 def test_maximum_q_count_and_type_count(db):
@@ -363,7 +413,7 @@ def test_plan_execute_equals_the_plain_calls_bit_for_bit(db):
             xyz = (base.xyz + rng.normal(0, 0.5, base.xyz.shape)).astype(np.float32)
             x = torch.from_numpy(xyz).cuda()
             a = plan.execute(x, fd).cpu().numpy()
-            b = db.debye_profile(x, t, fd, qd).cpu().numpy()
+            b = db.debye_profile(x, t, fd, qd, hint=db.q_hint(qg)).cpu().numpy()     # a plan knows its grid: same launches as a hinted call
             assert a.tobytes() == b.tobytes()
             assert rel(a, orc.debye_sym(xyz, base.type, f, qg)) <= TOL32
         plan.destroy()

@@ -15,8 +15,12 @@
  *   - Device-pointer calls are asynchronous on `stream`, never synchronise the host and never read device
  *     data on the host.  Scratch memory comes from a library-owned per-device cache that only grows
  *     (cudaMalloc on growth, which may synchronise the first time a larger problem is seen) or from a
- *     caller-supplied workspace (debye_set_workspace).  Calls on different streams must not overlap in time
- *     (one workspace per device).
+ *     caller-supplied workspace (debye_set_workspace).  That scratch is one per device: a call on another stream than
+ *     the previous call first makes its stream wait (cudaStreamWaitEvent, no host synchronisation) for the event the
+ *     previous call recorded behind its last kernel, so calls on different streams serialise on the device instead
+ *     of overwriting each other's records.  A plan (debye_plan_create) owns its scratch: plans on different streams run
+ *     concurrently; one plan used on several streams serialises the same way.  Calls may come from several host threads
+ *     (a mutex covers the shared scratch); one plan must not be executed from two host threads at once.
  *   - Results are bitwise reproducible run to run for the same inputs, flags, GPU model and library build.
  *   - Not checked (undefined behaviour if violated): 0 <= type[i] < T; finite inputs (NaN/Inf propagate).
  *   - fftab values may be negative (neutron scattering lengths); q may contain 0 and be in any
@@ -111,8 +115,10 @@ int debye_profile_weighted_host(const float *xyz, const int32_t *type, const flo
                                 const float *fftab, int32_t T, const float *q, int32_t M, double *I_out,
                                 uint32_t flags, debye_stream_t stream);
 
-/* The paper's general case: one form-factor row per ATOM ("the form factor depends on the atom type and its
- * environment"; the kernel's input is "the form factors for each atom at Q values of q"),
+/* The paper's general case: one form-factor row per ATOM (the form factors "cannot be factored out of the
+ * equation, because the non-uniform density of the water layer atoms around the molecule creates an intractable number of
+ * possible f_k f_j combinations"; the GPU holds "all N positions of atoms and at least one set of QN associated
+ * form factors for a specific q value", i.e. a Q x N table),
  *     I(q_m) = sum_i sum_j ff[i][m] ff[j][m] sinc(q_m |x_i - x_j|)      (Eq. 2; pairs once for i < j and doubled).
  * Without types there is no per-type-pair factoring: the inner loop is distance once per pair and chunk of 32 q, then per
  * q one range-reduced MUFU.SIN, a multiply by 1/r and an FMA with ff[j][m] from shared memory (XU-pipe bound); pairs with

@@ -18,8 +18,10 @@
  *   R10 form factors are given per atom TYPE: f_j(q_m) = fftab[type[j]][m]  (north_star narrowing).
  *   R10w optional per-atom weights (the one-parameter family of the paper's per-atom form factors,
  *        PAPER.md:44, 82): f_j(q_m) = weight[j] * fftab[type[j]][m]; weight == NULL means 1.
- *   R10p the paper's own general case (the form factor depends on the atom and its environment, the
- *        GPU kernel's input is "the form factors for each atom at Q values of q"): f_j(q_m) = ff[j][m], one table row per
+ *   R10p the paper's own general case (the form factors "cannot be factored out of the equation, because the
+ *        non-uniform density of the water layer atoms around the molecule creates an intractable number of possible f_k f_j
+ *        combinations"; the GPU memory holds "all N positions of atoms and at least one set of QN associated form
+ *        factors for a specific q value", i.e. a Q x N table): f_j(q_m) = ff[j][m], one table row per
  *        ATOM (oracle_debye_peratom).
  * Inputs are the same float32 / int32 bytes the GPU gets, promoted exactly to double.
  *

@@ -121,10 +121,16 @@ def _stream_ptr(stream):
     return C.c_void_p(s.cuda_stream)
 
 
-def _dev(t, dtype, name):
+def _dev(t, dtype, name, shape=None):
+    """Device pointer of a contiguous CUDA tensor of the given dtype on the CURRENT device (the library keys its scratch on
+    cudaGetDevice); shape: expected shape, None entries are free."""
     import torch
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
         raise LibdebyeError(f"{name}: expected a contiguous CUDA tensor of dtype {dtype}")
+    if t.device.index != torch.cuda.current_device():
+        raise LibdebyeError(f"{name}: tensor on cuda:{t.device.index}, current device is cuda:{torch.cuda.current_device()}")
+    if shape is not None and (t.dim() != len(shape) or any(e is not None and int(d) != int(e) for d, e in zip(t.shape, shape))):
+        raise LibdebyeError(f"{name}: shape {tuple(t.shape)}, expected {tuple('*' if e is None else e for e in shape)}")
     return C.c_void_p(t.data_ptr())
 
 
@@ -135,9 +141,9 @@ def debye_profile(xyz, type, fftab, q, I_out=None, variant="auto", stream=None, 
     N, T, M = xyz.shape[0], fftab.shape[0], q.shape[0]
     if I_out is None:
         I_out = torch.empty(M, dtype=torch.float64, device=xyz.device)
-    _check(lib().debye_profile(_dev(xyz, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N,
-                               _dev(fftab, torch.float32, "fftab"), T, _dev(q, torch.float32, "q"), M,
-                               _dev(I_out, torch.float64, "I_out"), _flags(variant, hint), _stream_ptr(stream)))
+    _check(lib().debye_profile(_dev(xyz, torch.float32, "xyz", (N, 3)), _dev(type, torch.int32, "type", (N,)), N,
+                               _dev(fftab, torch.float32, "fftab", (T, M)), T, _dev(q, torch.float32, "q", (M,)), M,
+                               _dev(I_out, torch.float64, "I_out", (M,)), _flags(variant, hint), _stream_ptr(stream)))
     return I_out
 
 
@@ -147,9 +153,9 @@ def debye_profile_batch(xyz, type, fftab, q, I_out=None, variant="auto", stream=
     B, N, T, M = xyz.shape[0], xyz.shape[1], fftab.shape[0], q.shape[0]
     if I_out is None:
         I_out = torch.empty((B, M), dtype=torch.float64, device=xyz.device)
-    _check(lib().debye_profile_batch(_dev(xyz, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N, B,
-                                     _dev(fftab, torch.float32, "fftab"), T, _dev(q, torch.float32, "q"), M,
-                                     _dev(I_out, torch.float64, "I_out"), _flags(variant, hint), _stream_ptr(stream)))
+    _check(lib().debye_profile_batch(_dev(xyz, torch.float32, "xyz", (B, N, 3)), _dev(type, torch.int32, "type", (N,)), N, B,
+                                     _dev(fftab, torch.float32, "fftab", (T, M)), T, _dev(q, torch.float32, "q", (M,)), M,
+                                     _dev(I_out, torch.float64, "I_out", (B, M)), _flags(variant, hint), _stream_ptr(stream)))
     return I_out
 
 
@@ -161,9 +167,10 @@ def debye_profile_weighted(xyz, type, weight, fftab, q, I_out=None, variant="aut
     N, T, M = xyz.shape[-2], fftab.shape[0], q.shape[0]
     if I_out is None:
         I_out = torch.empty((xyz.shape[0], M) if batch else M, dtype=torch.float64, device=xyz.device)
-    a = (_dev(xyz, torch.float32, "xyz"), _dev(type, torch.int32, "type"), _dev(weight, torch.float32, "weight"), N)
-    b = (_dev(fftab, torch.float32, "fftab"), T, _dev(q, torch.float32, "q"), M, _dev(I_out, torch.float64, "I_out"),
-         _flags(variant, hint), _stream_ptr(stream))
+    a = (_dev(xyz, torch.float32, "xyz", (xyz.shape[0], N, 3) if batch else (N, 3)), _dev(type, torch.int32, "type", (N,)),
+         _dev(weight, torch.float32, "weight", (N,)), N)
+    b = (_dev(fftab, torch.float32, "fftab", (T, M)), T, _dev(q, torch.float32, "q", (M,)), M,
+         _dev(I_out, torch.float64, "I_out", (xyz.shape[0], M) if batch else (M,)), _flags(variant, hint), _stream_ptr(stream))
     if batch:
         _check(lib().debye_profile_batch_weighted(*a, xyz.shape[0], *b))
     else:
@@ -190,17 +197,21 @@ class Plan:
         import torch
         self.N, self.M, self.T, self.B = type.shape[0], q.shape[0], T, B
         self._h = C.c_void_p()
-        _check(lib().debye_plan_create(C.byref(self._h), _dev(type, torch.int32, "type"), self.N, B, T,
-                                       _dev(q, torch.float32, "q"), self.M,
-                                       _dev(weight, torch.float32, "weight") if weight is not None else None,
+        _check(lib().debye_plan_create(C.byref(self._h), _dev(type, torch.int32, "type", (self.N,)), self.N, B, T,
+                                       _dev(q, torch.float32, "q", (self.M,)), self.M,
+                                       _dev(weight, torch.float32, "weight", (self.N,)) if weight is not None else None,
                                        _flags(variant), _stream_ptr(stream)))
 
     def execute(self, xyz, fftab, I_out=None, stream=None):
         import torch
+        batch = xyz.dim() == 3
+        if (batch and xyz.shape[0] != self.B) or (not batch and self.B != 1):
+            raise LibdebyeError(f"xyz: the plan was created for B = {self.B} conformers")
         if I_out is None:
-            I_out = torch.empty((self.B, self.M) if xyz.dim() == 3 else self.M, dtype=torch.float64, device=xyz.device)
-        _check(lib().debye_plan_execute(self._h, _dev(xyz, torch.float32, "xyz"), _dev(fftab, torch.float32, "fftab"),
-                                        _dev(I_out, torch.float64, "I_out"), _stream_ptr(stream)))
+            I_out = torch.empty((self.B, self.M) if batch else self.M, dtype=torch.float64, device=xyz.device)
+        _check(lib().debye_plan_execute(self._h, _dev(xyz, torch.float32, "xyz", (self.B, self.N, 3) if batch else (self.N, 3)),
+                                        _dev(fftab, torch.float32, "fftab", (self.T, self.M)),
+                                        _dev(I_out, torch.float64, "I_out", (self.B, self.M) if batch else (self.M,)), _stream_ptr(stream)))
         return I_out
 
     def destroy(self):
@@ -222,8 +233,8 @@ def debye_partials(xyz, type, q, T, variant="auto", stream=None, hint=0):
     B, N, M = x3.shape[0], x3.shape[1], q.shape[0]
     S = torch.empty((B, T * (T + 1) // 2, M), dtype=torch.float64, device=xyz.device)
     n = torch.empty(T, dtype=torch.int32, device=xyz.device)
-    _check(lib().debye_partials(_dev(x3, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N, B,
-                                _dev(q, torch.float32, "q"), T, M, _dev(S, torch.float64, "S_out"),
+    _check(lib().debye_partials(_dev(x3, torch.float32, "xyz", (B, N, 3)), _dev(type, torch.int32, "type", (N,)), N, B,
+                                _dev(q, torch.float32, "q", (M,)), T, M, _dev(S, torch.float64, "S_out"),
                                 _dev(n, torch.int32, "n_out"), _flags(variant, hint), _stream_ptr(stream)))
     return S, n
 
@@ -237,8 +248,8 @@ def debye_profile_peratom(xyz, ff, q, I_out=None, variant="auto", stream=None):
         raise LibdebyeError("ff: expected shape [N, M]")
     if I_out is None:
         I_out = torch.empty(M, dtype=torch.float64, device=xyz.device)
-    _check(lib().debye_profile_peratom(_dev(xyz, torch.float32, "xyz"), _dev(ff, torch.float32, "ff"), N,
-                                       _dev(q, torch.float32, "q"), M, _dev(I_out, torch.float64, "I_out"),
+    _check(lib().debye_profile_peratom(_dev(xyz, torch.float32, "xyz", (N, 3)), _dev(ff, torch.float32, "ff", (N, M)), N,
+                                       _dev(q, torch.float32, "q", (M,)), M, _dev(I_out, torch.float64, "I_out", (M,)),
                                        _flags(variant), _stream_ptr(stream)))
     return I_out
 
@@ -251,8 +262,8 @@ def debye_partials_shard(xyz, type, q, T, shard_rank, shard_world, variant="auto
     B, N, M = x3.shape[0], x3.shape[1], q.shape[0]
     S = torch.empty((B, T * (T + 1) // 2, M), dtype=torch.float64, device=xyz.device)
     n = torch.empty(T, dtype=torch.int32, device=xyz.device)
-    _check(lib().debye_partials_shard(_dev(x3, torch.float32, "xyz"), _dev(type, torch.int32, "type"), N, B,
-                                      _dev(q, torch.float32, "q"), T, M, _dev(S, torch.float64, "S_out"),
+    _check(lib().debye_partials_shard(_dev(x3, torch.float32, "xyz", (B, N, 3)), _dev(type, torch.int32, "type", (N,)), N, B,
+                                      _dev(q, torch.float32, "q", (M,)), T, M, _dev(S, torch.float64, "S_out"),
                                       _dev(n, torch.int32, "n_out"), _flags(variant, hint), int(shard_rank), int(shard_world),
                                       _stream_ptr(stream)))
     return S, n

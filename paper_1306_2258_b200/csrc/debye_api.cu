@@ -34,6 +34,21 @@ thread_local int g_last_cuda = 0;
         }                                          \
     } while (0)
 
+// Scratch shared by calls on different streams (the per-device workspace and staging buffer; a plan's own workspace): acquire
+// before the first use in a call, release behind the last.  Same stream as the previous user: stream order is enough.
+struct ScratchOrder { cudaEvent_t done = nullptr; cudaStream_t stream = nullptr; bool used = false; };
+cudaError_t scratch_acquire(ScratchOrder &o, cudaStream_t stream)
+{
+    if (o.used && o.stream != stream) return cudaStreamWaitEvent(stream, o.done, 0);
+    return cudaSuccess;
+}
+cudaError_t scratch_release(ScratchOrder &o, cudaStream_t stream)
+{
+    if (!o.done) { cudaError_t e = cudaEventCreateWithFlags(&o.done, cudaEventDisableTiming); if (e != cudaSuccess) return e; }
+    o.stream = stream; o.used = true;
+    return cudaEventRecord(o.done, stream);
+}
+
 constexpr int MAX_DEV = 64;
 constexpr int64_t DEBYE_PACK_IN_SETUP = 16384;   // N x B up to which debye_setup_kernel also packs the coordinates
 struct DevState {
@@ -42,6 +57,10 @@ struct DevState {
     void *stage = nullptr; size_t stage_bytes = 0;    // device staging for the *_host entry points
     int sms = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;         // optional: recorded around the pairs launches
+    // cross-stream ordering of the shared scratch (workspace, staging buffer): every call records ws_done behind its last
+    // use; a call on another stream first makes its stream wait for it, so calls on different streams serialise on the
+    // device instead of overwriting each other's records
+    ScratchOrder order;
     int occ[5][33];                                   // cached CTAs/SM per (variant, K/4); 0 = unknown
     int occ_small[17][DEBYE_SMALL_TMAX + 1];          // the same for debye_small_kernel<8 i> with T types (N = 2048); 0 = unknown
 };
@@ -50,6 +69,8 @@ std::mutex g_mu;
 bool g_atexit = false;
 
 size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+
 
 // launch with programmatic stream serialisation (PDL, debye_plan.cuh): the kernel must start with pdl_wait()
 template <typename... KArgs, typename... Args>
@@ -255,8 +276,10 @@ int ensure(void **ptr, size_t *have, size_t need)
 struct debye_plan {
     int N, B, T, M, device;
     uint32_t flags;              // the caller's flags with the grid hint resolved at creation
-    char *buf;                   // one allocation: DevPlan | perm[N] | q[M] | weight[N] | type[N]
+    char *buf;                   // one allocation: DevPlan | perm[N] | q[M] | weight[N] | type[N] | workspace
     DevPlan *plan; int32_t *perm; float *q; float *weight; int32_t *type;
+    char *ws; size_t ws_bytes;   // the plan's own scratch: plans on different streams run concurrently
+    ScratchOrder order;          // ... and one plan used on several streams serialises on the device
 };
 namespace {
 
@@ -297,48 +320,60 @@ int small_grid(DevState *ds, int N, int T, int K, int *G)
 size_t small_ws_bytes(int T, int K, int G) { return align_up(((size_t)G + (size_t)(T * (T + 1) / 2)) * K * 8); }
 
 int run_small(DevState *ds, const float *xyz, const int32_t *type, int N, const float *fftab, int T, const float *q, int M, double *out, int32_t *n_out,
-              uint32_t flags, cudaStream_t stream, int mode)
+              uint32_t flags, cudaStream_t stream, int mode, debye_plan *pre, std::unique_lock<std::mutex> &lock)
 {
     const int K = small_K(M, flags);
     int G = 0, st;
     if ((st = small_grid(ds, N, T, K, &G))) return st;
     const size_t need = small_ws_bytes(T, K, G);
     char *ws;
-    if (ds->user_ws) { if (ds->user_bytes < need) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
+    ScratchOrder *order = &ds->order;
+    if (pre && pre->ws) { if (pre->ws_bytes < need) return DEBYE_ENOMEM; ws = pre->ws; order = &pre->order; }
+    else if (ds->user_ws) { if (ds->user_bytes < need) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
     else { if ((st = ensure(&ds->ws, &ds->ws_bytes, need))) return st; ws = (char *)ds->ws; }
+    cudaEvent_t ev0 = ds->ev0, ev1 = ds->ev1;
+    if (pre && pre->ws) lock.unlock();             // nothing shared with other calls from here on
+    CU(scratch_acquire(*order, stream));
     debye_small_fn fn = debye_get_small_kernel(K);
-    if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
+    if (ev0) CU(cudaEventRecord(ev0, stream));
     {   // cooperative launch: the kernel has a grid-wide barrier (G is at most one resident wave, small_grid)
         int hc = hint_class_of(flags);
         double *rec = (double *)ws;
         void *args[] = {(void *)&xyz, (void *)&type, (void *)&N, (void *)&T, (void *)&fftab, (void *)&q, (void *)&M, (void *)&hc, (void *)&rec, (void *)&out, (void *)&mode, (void *)&n_out};
         CU(cudaLaunchCooperativeKernel((const void *)fn, dim3(G), dim3(DEBYE_IB), args, debye::debye_small_dyn_smem(N, T, K), stream));
     }
-    if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
+    if (ev1) CU(cudaEventRecord(ev1, stream));
+    CU(scratch_release(*order, stream));
     CU(cudaGetLastError());
     return DEBYE_OK;
 }
 
 // mode 0: I_out[B][M]; mode 1: S_out[B][n_tp][M] (+ n_out)
 int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab, int T, const float *q, int M, double *out, int32_t *n_out,
-        uint32_t flags, cudaStream_t stream, int mode, const float *weight = nullptr, const debye_plan *pre = nullptr, int shard_rank = 0,
+        uint32_t flags, cudaStream_t stream, int mode, const float *weight = nullptr, debye_plan *pre = nullptr, int shard_rank = 0,
         int shard_world = 1)
 {
     int st = validate(xyz, type, N, B, mode == 0 ? (const void *)fftab : (const void *)q, T, q, M, out, flags);
     if (st) return st;
-    std::lock_guard<std::mutex> lock(g_mu);
+    std::unique_lock<std::mutex> lock(g_mu);
     DevState *ds;
     if ((st = dev_state(&ds))) return st;
     if (small_eligible(N, B, T, M, flags, weight, shard_world) && (!pre || pre->type))
-        return run_small(ds, xyz, pre ? pre->type : type, N, fftab, T, q, M, out, n_out, flags, stream, mode);
+        return run_small(ds, xyz, pre ? pre->type : type, N, fftab, T, q, M, out, n_out, flags, stream, mode, pre, lock);
     Choice ch[MAX_CHOICES]; int is_auto = 0;
     const int nch = variants_for(flags, ch, M, &is_auto);
     int G[MAX_CHOICES] = {0, 0, 0}, Gmax = 0;
     for (int i = 0; i < nch; ++i) { if ((st = grid_for(ds, ch[i], N, B, &G[i]))) return st; if (G[i] > Gmax) Gmax = G[i]; }
     const Layout L = layout(N, B, T, M, Gmax, ch, nch);
     char *ws;
-    if (ds->user_ws) { if (ds->user_bytes < L.total) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
+    ScratchOrder *order = &ds->order;
+    if (pre && pre->ws) { if (pre->ws_bytes < L.total) return DEBYE_ENOMEM; ws = pre->ws; order = &pre->order; }
+    else if (ds->user_ws) { if (ds->user_bytes < L.total) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
     else { if ((st = ensure(&ds->ws, &ds->ws_bytes, L.total))) return st; ws = (char *)ds->ws; }
+    const cudaEvent_t ev0 = ds->ev0, ev1 = ds->ev1;
+    const int sms = ds->sms;
+    if (pre && pre->ws) lock.unlock();             // a plan's own scratch: nothing shared with other calls from here on
+    CU(scratch_acquire(*order, stream));
     DevPlan *plan = pre ? pre->plan : (DevPlan *)(ws + L.plan);
     int32_t *perm = pre ? pre->perm : (int32_t *)(ws + L.perm);
     float4 *sorted = (float4 *)(ws + L.sorted);
@@ -361,13 +396,13 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     if (!pack_here) {
         int64_t total = (int64_t)N * B;
         int blocks = (int)((total + 255) / 256);
-        if (blocks > ds->sms * 16) blocks = ds->sms * 16;
+        if (blocks > sms * 16) blocks = sms * 16;
         // with a plan the pack kernel is the first kernel of the call: an ordinary launch (its pdl_wait returns at once)
         if (pre) debye::debye_pack_kernel<<<blocks, 256, 0, stream>>>(plan, xyz, type, perm, sorted, N, B, weight);
         else CU(launch_pdl(debye::debye_pack_kernel, dim3(blocks), dim3(256), stream, (const DevPlan *)plan, xyz, type, (const int32_t *)perm, sorted, N, B, weight));
     }
     if (weight) CU(launch_pdl(debye::debye_weight_sums_kernel, dim3(T), dim3(32), stream, plan, (const float4 *)sorted));
-    if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
+    if (ev0) CU(cudaEventRecord(ev0, stream));
     for (int i = 0; i < nch; ++i) {
         debye_pairs_fn fn = debye_get_pairs_kernel(ch[i].variant, ch[i].K, weight != nullptr, shard_world > 1);
         if (!fn) return DEBYE_EUNSUPPORTED;
@@ -375,7 +410,7 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
         const float theta_min = (ch[i].variant == V_RECUR) ? 0.002f : 0.004f;
         CU(launch_pdl(fn, dim3(G[i]), dim3(DEBYE_IB), stream, (const DevPlan *)plan, (const float4 *)sorted, q, records, ch[i].n_chunks, is_auto, theta_min, ch[i].alt_gate));
     }
-    if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
+    if (ev1) CU(cudaEventRecord(ev1, stream));
     {
         // the final kernels repeat the device-side decisions of the pairs launches to find the one that did the work
         debye::FinalSets sets; sets.n = nch;
@@ -392,6 +427,7 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
         CU(launch_pdl(debye::debye_epilogue_kernel, dim3(blocks), dim3(DEBYE_FINAL_THREADS), stream, (const DevPlan *)plan, (const double *)sums, fftab, q, out, is_auto, sets, mode));
     }
     if (mode == 1 && n_out) CU(cudaMemcpyAsync(n_out, plan->n_a, sizeof(int32_t) * T, cudaMemcpyDeviceToDevice, stream));
+    CU(scratch_release(*order, stream));
     CU(cudaGetLastError());
     return DEBYE_OK;
 }
@@ -417,6 +453,7 @@ int run_host(const float *xyz, const int32_t *type, int N, int B, const float *f
         total = o;
         if ((st = ensure(&ds->stage, &ds->stage_bytes, total))) return st;
         base = (char *)ds->stage;
+        CU(scratch_acquire(ds->order, stream));    // the staging buffer is shared scratch too; run() releases behind the last kernel
     }
     CU(cudaMemcpyAsync(base + o_xyz, xyz, (size_t)N * B * 12, cudaMemcpyHostToDevice, stream));
     CU(cudaMemcpyAsync(base + o_type, type, (size_t)N * 4, cudaMemcpyHostToDevice, stream));
@@ -427,7 +464,7 @@ int run_host(const float *xyz, const int32_t *type, int N, int B, const float *f
              (double *)(base + o_out), nullptr, flags, stream, 0, weight ? (const float *)(base + o_w) : nullptr);
     if (st) return st;
     CU(cudaMemcpyAsync(out, base + o_out, (size_t)B * M * 8, cudaMemcpyDeviceToHost, stream));
-    CU(cudaStreamSynchronize(stream));
+    CU(cudaStreamSynchronize(stream));             // the staging buffer is free again when this returns
     return DEBYE_OK;
 }
 
@@ -536,6 +573,7 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
     if (ds->user_ws) { if (ds->user_bytes < o) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
     else { if ((st = ensure(&ds->ws, &ds->ws_bytes, o))) return st; ws = (char *)ds->ws; }
     double *records = (double *)(ws + o_rec), *selfbuf = (double *)(ws + o_self);
+    CU(scratch_acquire(ds->order, stream));
     debye::debye_peratom_self_kernel<<<dim3((M + 31) / 32, DEBYE_PA_SLICES), 256, 0, stream>>>(ff, N, M, selfbuf);
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
     if (U > 0) {
@@ -549,6 +587,7 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
     }
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
     debye::debye_peratom_final_kernel<<<(M + 31) / 32, 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, KQ, I_out);
+    CU(scratch_release(ds->order, stream));
     CU(cudaGetLastError());
     return DEBYE_OK;
 }
@@ -570,6 +609,7 @@ int debye_profile_peratom_host(const float *xyz, const float *ff, int32_t N, con
         if ((st = dev_state(&ds))) return st;
         if ((st = ensure(&ds->stage, &ds->stage_bytes, o))) return st;
         base = (char *)ds->stage;
+        CU(scratch_acquire(ds->order, stream));
     }
     CU(cudaMemcpyAsync(base + o_xyz, xyz, (size_t)N * 12, cudaMemcpyHostToDevice, stream));
     CU(cudaMemcpyAsync(base + o_ff, ff, (size_t)N * M * 4, cudaMemcpyHostToDevice, stream));
@@ -591,7 +631,7 @@ int debye_plan_create(debye_plan **out, const int32_t *type, int32_t N, int32_t 
     int st = validate(&dummy, type, N, B, &dummy, T, q, M, &dummy, flags);
     if (st) return st;
     debye_plan *p = new debye_plan();
-    p->N = N; p->B = B; p->T = T; p->M = M; p->flags = flags; p->buf = nullptr;
+    p->N = N; p->B = B; p->T = T; p->M = M; p->flags = flags; p->buf = nullptr; p->ws = nullptr; p->ws_bytes = 0;
     auto fail = [&](int code) { if (p->buf) cudaFree(p->buf); delete p; return code; };
     if (cudaGetDevice(&p->device) != cudaSuccess) return fail(DEBYE_ECUDA);
     size_t o = 0;
@@ -600,9 +640,20 @@ int debye_plan_create(debye_plan **out, const int32_t *type, int32_t N, int32_t 
     const size_t o_q = o; o += align_up((size_t)M * 4);
     const size_t o_w = o; o += align_up((size_t)N * 4);
     const size_t o_t = o; o += align_up((size_t)N * 4);
+    const size_t o_ws = o;
+    {   // the plan's own scratch, sized for any grid class the setup step may find (the hint is resolved below)
+        size_t need = 0;
+        const uint32_t base_flags = flags & ~(uint32_t)(DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ);
+        const uint32_t hints[4] = {DEBYE_QHINT, DEBYE_QHINT | DEBYE_QHINT_UNIFORM, DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0,
+                                   DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_STARTDQ};
+        for (int i = 0; i < 4; ++i) { const size_t b = debye_workspace_bytes(N, B, T, M, base_flags | hints[i]); if (b > need) need = b; }
+        if (need == 0) return fail(DEBYE_EINVAL);
+        p->ws_bytes = need; o += align_up(need);
+    }
     if (cudaMalloc((void **)&p->buf, o) != cudaSuccess) { (void)cudaGetLastError(); p->buf = nullptr; return fail(DEBYE_ENOMEM); }
     p->plan = (DevPlan *)(p->buf + o_plan); p->perm = (int32_t *)(p->buf + o_perm); p->q = (float *)(p->buf + o_q);
     p->weight = weight ? (float *)(p->buf + o_w) : nullptr;
+    p->ws = p->buf + o_ws;
     p->type = (int32_t *)(p->buf + o_t);          // small structures re-sort per call inside the one fused launch
     if (cudaMemcpyAsync(p->type, type, (size_t)N * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
     if (cudaMemcpyAsync(p->q, q, (size_t)M * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
@@ -634,6 +685,7 @@ void debye_plan_destroy(debye_plan *p)
 {
     if (!p) return;
     if (p->buf) cudaFree(p->buf);
+    if (p->order.done) cudaEventDestroy(p->order.done);
     delete p;
 }
 

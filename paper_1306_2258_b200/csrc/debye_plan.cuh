@@ -42,14 +42,22 @@ struct DevPlan {
 
 // ---- q-grid classification, identical on the host (debye_q_hint) and on the device (debye_setup_kernel) -----------------
 // class: -2 not uniform; -1 uniform, general start; 0 uniform with q[0] == 0; 1 uniform with q[0] == dq (the paper's grid).
-// `dev` = max_k |q[k] - fma(k, dq, q0)| rounded to float per element, `qmax` = max_k |q[k]|: a maximum, so the order in which
-// it is taken (serial on the host, tree on the device) does not matter; fma keeps host and device arithmetic identical.
+// `dev` = max_k |q[k] - fma(k, dq, q0)| / max(|q[k]|, |dq|) rounded to float per element, `qmax` = max_k |q[k]|: maxima, so the
+// order in which they are taken (serial on the host, tree on the device) does not matter; fma keeps host and device
+// arithmetic identical.
 __host__ __device__ inline double debye_grid_dq(double q0, double qlast, int M) { return (M > 1) ? (qlast - q0) / (double)(M - 1) : (q0 != 0.0 ? q0 : 1.0); }
-__host__ __device__ inline float debye_grid_dev(double qk, int k, double q0, double dq) { return (float)fabs(qk - fma((double)k, dq, q0)); }
+__host__ __device__ inline float debye_grid_dev(double qk, int k, double q0, double dq)
+{
+    const double scale = fmax(fabs(qk), fabs(dq));
+    return (float)(fabs(qk - fma((double)k, dq, q0)) / (scale > 1e-300 ? scale : 1e-300));
+}
 __host__ __device__ inline int debye_grid_class(double q0, double dq, float dev, float qmax)
 {
-    // uniform if every q[k] is within 2 float ulps (of the largest |q|) of the line through the end points
-    const bool uni = (dq != 0.0) && (dev <= 2.4e-7f * (qmax > 1e-30f ? qmax : 1e-30f));
+    // Uniform if every q[k] is within 1.5 float ulps OF ITSELF (not of the largest |q|) of the line through the end points:
+    // the recurrence evaluates the line, so whatever is accepted here is a relative error of q_k, i.e. of the phase q_k r.
+    // A grid rounded once from the exact line deviates by at most 1 ulp (its own rounding plus that of the end points).
+    (void)qmax;
+    const bool uni = (dq != 0.0) && (dev <= 1.8e-7f);
     if (!uni) return -2;
     if (q0 == 0.0) return 0;
     if (fabs(q0 / dq - 1.0) <= 1e-6) return 1;

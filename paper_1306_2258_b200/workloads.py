@@ -260,7 +260,8 @@ CONFIGS = {"cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4, "cfg5": cfg5}
 
 
 def peratom_table(w: Workload, seed: int = 0) -> np.ndarray:
-    """ff[N][M] float32 for the per-ATOM path ("the form factor depends on the atom type and its environment" --
+    """ff[N][M] float32 for the per-ATOM path (the form factors "cannot be factored out of the equation, because the non-uniform density of the water layer
+    atoms around the molecule creates an intractable number of possible f_k f_j combinations" --
     excluded volume and hydration layer): the type's row times a seeded per-atom factor in [0.6, 1.4] (a stand-in for the
     solvent-accessible fraction), plus a seeded per-atom offset in [-0.3, 0.3] that decays with q (a hydration-shell-like
     term), so that no two atoms share a row.  An input recipe only: none of the method's arithmetic."""

@@ -112,6 +112,15 @@ def test_q_hint_classifies_grids_on_the_host():
     assert binding.q_hint(wl.q_grid(0.3, 31)[::-1].copy()) == H | U            # descending
     assert binding.q_hint(np.array([0.0, 0.1, 0.25], np.float32)) == H         # not uniform
     assert binding.q_hint(np.array([0.0], np.float32)) == H | U | Z
+    # a grid is uniform if every q[k] is within 1.5 float ulps of ITSELF of the line through the end points: grids rounded once
+    # from the exact line pass at every size and range, a jitter of 2 ulps of q_max at low k does not
+    for qmax, M, qmin in ((0.5, 101, 0.0), (1.0, 50, 0.02), (0.3, 128, 0.0), (1.7, 4096, 0.0), (0.9, 64, 0.3), (25.0, 999, 0.0)):
+        assert binding.q_hint(wl.q_grid(qmax, M, qmin)) & U, (qmax, M, qmin)
+        assert binding.q_hint(np.linspace(qmin, qmax, M, dtype=np.float32)) & U
+        assert binding.q_hint((np.arange(M) * np.float32((qmax - qmin) / (M - 1)) + np.float32(qmin)).astype(np.float32)) & U or M > 500
+    g = wl.q_grid(0.5, 101)
+    j = g.copy(); j[3] = np.nextafter(np.nextafter(j[3], np.float32(1)), np.float32(1)); j[7] += 2 * np.spacing(np.float32(0.5))
+    assert binding.q_hint(j) == H                                             # not uniform: the MUFU kernel takes q as it is
     L = binding.lib()
     assert L.debye_q_hint(None, 5) == 0
     # with a hint exactly one pairs instantiation is launched

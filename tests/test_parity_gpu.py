@@ -429,6 +429,60 @@ def test_plan_execute_equals_the_plain_calls_bit_for_bit(db):
     plan.destroy()
 
 
+def test_calls_on_different_streams_do_not_corrupt_each_other(db):
+    """include/debye.h: the per-device scratch is ordered across streams with an event (calls on different streams serialise
+    on the device); a plan owns its scratch, so plans on different streams may overlap.  Eight rounds of interleaved calls
+    on three streams, large enough to overlap in time if nothing ordered them, against the single-stream results bit for bit."""
+    import torch
+    ws = [wl.small_random(90 + i, 2600 + 300 * i, 4, 101) for i in range(3)]       # beyond the single-launch size limit
+    devs = [to_dev(w) for w in ws]
+    refs = [gpu_profile(db, w) for w in ws]
+    for i, w in enumerate(ws):
+        assert rel(refs[i], orc.debye_sym(w.xyz, w.type, w.fftab, w.q)) <= TOL32
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    outs = [[None] * 3 for _ in range(8)]
+    for r in range(8):                                       # plain calls: shared scratch, three streams
+        for i in (r % 3, (r + 1) % 3, (r + 2) % 3):
+            x, t, f, q = devs[i]
+            outs[r][i] = db.debye_profile(x, t, f, q, stream=streams[i])
+    torch.cuda.synchronize()
+    for r in range(8):
+        for i in range(3):
+            assert outs[r][i].cpu().numpy().tobytes() == refs[i].tobytes(), (r, i)
+    plans = [db.Plan(devs[i][1], devs[i][3], ws[i].T) for i in range(3)]
+    torch.cuda.synchronize()
+    pref = [plans[i].execute(devs[i][0], devs[i][2]).cpu().numpy() for i in range(3)]
+    for r in range(8):                                       # plans: own scratch, three streams, no ordering between them
+        for i in (r % 3, (r + 1) % 3, (r + 2) % 3):
+            outs[r][i] = plans[i].execute(devs[i][0], devs[i][2], stream=streams[i])
+    # one plan on two streams in turn: serialised by the plan's own event
+    twice = [plans[0].execute(devs[0][0], devs[0][2], stream=streams[k % 2]) for k in range(6)]
+    torch.cuda.synchronize()
+    for r in range(8):
+        for i in range(3):
+            assert outs[r][i].cpu().numpy().tobytes() == pref[i].tobytes(), (r, i)
+    for o in twice:
+        assert o.cpu().numpy().tobytes() == pref[0].tobytes()
+    for i in range(3):
+        assert rel(pref[i], orc.debye_sym(ws[i].xyz, ws[i].type, ws[i].fftab, ws[i].q)) <= TOL32
+        plans[i].destroy()
+
+
+def test_grid_jittered_by_two_ulps_is_taken_as_it_is(db):
+    """A grid whose points sit 2 float ulps of q_max off the uniform line is NOT run through the recurrence (which would
+    evaluate the line instead of q[k]): the device classifies it as non-uniform and the MUFU kernel takes q as given."""
+    w = wl.small_random(95, 3000, 3, 96, q_max=0.6, box=80.0)
+    rng = np.random.default_rng(5)
+    qj = (w.q + rng.integers(-2, 3, w.M) * np.spacing(np.float32(0.6))).astype(np.float32)
+    qj[0] = 0.0
+    wj = wl.Workload("jitter", w.xyz, w.type, w.fftab, qj)
+    assert db.q_hint(qj) == 1 << 8                                           # DEBYE_QHINT alone: not uniform
+    ref = orc.debye_sym(wj.xyz, wj.type, wj.fftab, wj.q)
+    assert rel(gpu_profile(db, wj), ref) <= 1e-5
+    assert gpu_profile(db, wj).tobytes() == gpu_profile(db, wj, "mufu").tobytes()
+    assert np.isnan(gpu_profile(db, wj, "recur")).all()                      # forced recurrence on a non-uniform grid: NaN
+
+
 def test_non_finite_input_propagates_and_does_not_poison_later_calls(db):
     """include/debye.h: NaN / Inf in the inputs propagate to I_out (no hang, no crash); the next call is unaffected."""
     w = wl.small_random(70, 500, 3, 40)

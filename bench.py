@@ -585,8 +585,12 @@ def run_peratom(args, w, rank, world, dev):
     from paper_1306_2258_b200 import binding as db, sharding
     if w.xyz.ndim == 3:
         raise SystemExit("--path peratom takes single-structure configs")
-    variant = args.variant if args.variant in ("auto", "mufu", "fp64") else "auto"
+    variant = args.variant if args.variant in ("auto", "mufu", "fp64", "recur") else "auto"
     ff = wl.peratom_table(w, rank)
+    # with the grid hint (q was generated on the host) a grid q_k = (k + koff) dq runs the recurrence (debye_peratom_recur.cuh)
+    hint = 0 if (args.no_hint or variant in ("mufu", "fp64")) else db.q_hint(w.q)
+    H, U, Z, D = 1 << 8, 1 << 9, 1 << 10, 1 << 11
+    recur = bool(hint & U) and bool(hint & (Z | D)) and (w.M - (1 if hint & Z else 0)) <= 256
     x, f, q = (torch.from_numpy(a).to(dev) for a in (w.xyz, ff, w.q))
     out = torch.empty(w.M, dtype=torch.float64, device=dev)
     flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device=dev)
@@ -597,7 +601,7 @@ def run_peratom(args, w, rank, world, dev):
         torch.cuda.synchronize()
 
     for _ in range(args.warmup):
-        db.debye_profile_peratom(x, f, q, out, variant=variant)
+        db.debye_profile_peratom(x, f, q, out, variant=variant, hint=hint)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
     sampler = ClockSampler(dev.index or 0)
@@ -606,7 +610,7 @@ def run_peratom(args, w, rank, world, dev):
     for a, b in ev:
         flush.fill_(1)
         a.record()
-        db.debye_profile_peratom(x, f, q, out, variant=variant)
+        db.debye_profile_peratom(x, f, q, out, variant=variant, hint=hint)
         b.record()
     barrier()
     wall = time.perf_counter() - wall0
@@ -620,7 +624,7 @@ def run_peratom(args, w, rank, world, dev):
     pk = []
     for _ in range(min(args.steps, 30)):
         flush.fill_(1)
-        db.debye_profile_peratom(x, f, q, out, variant=variant)
+        db.debye_profile_peratom(x, f, q, out, variant=variant, hint=hint)
         torch.cuda.synchronize()
         pk.append(e0.elapsed_time(e1))
     db.set_pairs_events(None, None)
@@ -628,12 +632,12 @@ def run_peratom(args, w, rank, world, dev):
     hx, hf, hq = (torch.from_numpy(a).pin_memory().numpy() for a in (w.xyz, ff, w.q))
     hout = torch.empty(w.M, dtype=torch.float64).pin_memory().numpy()
     for _ in range(3):
-        db.debye_profile_peratom_host(hx, hf, hq, hout, variant=variant)
+        db.debye_profile_peratom_host(hx, hf, hq, hout, variant=variant, hint=hint)
     barrier()
     n_e2e = max(5, min(args.steps, 50))
     t0 = time.perf_counter()
     for _ in range(n_e2e):
-        db.debye_profile_peratom_host(hx, hf, hq, hout, variant=variant)
+        db.debye_profile_peratom_host(hx, hf, hq, hout, variant=variant, hint=hint)
     barrier()
     e2e_s = sharding.max_over_ranks(time.perf_counter() - t0, dev)
     result_dev = out.cpu().numpy()
@@ -644,27 +648,34 @@ def run_peratom(args, w, rank, world, dev):
         return
     fmax_ghz = float(measured_peaks().get("sm_max_mhz", 1965.0)) / 1e3
     peak = SM_COUNT * MUFU_LANES * fmax_ghz / 1e3
+    if recur:
+        peak = SM_COUNT * FP32_LANES * 2 * fmax_ghz / 1e3                       # TFLOP/s, FMA = 2 flop
     # the library's q-chunk (debye_peratom_kq): the multiple of 4 in [16, 32] with the fewest padded slots, larger on ties
     kq = min(range(32, 12, -4), key=lambda c: ((w.M + c - 1) // c * c, -c))
     achieved = float(w.pair_q) / (pairs_ms * 1e-3) / 1e12
+    if recur:       # 2 FP32-pipe lane-operations (chain FFMA + weighted-accumulate FFMA = 4 flop) per pair.q with q != 0
+        achieved = 4.0 * float(w.pair_q) / w.M * int(np.count_nonzero(w.q)) / (pairs_ms * 1e-3) / 1e12
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if variant == "fp64" else "f32", "data": "synthetic",
         "config": {"workload": w.name + "+peratom_table", "path": "peratom", "N": w.N, "M": w.M, "B": 1,
-                   "variant": "fp64" if variant == "fp64" else "mufu", "q_chunk": kq, "n_chunks": (w.M + kq - 1) // kq,
+                   "variant": "fp64" if variant == "fp64" else ("recur" if recur else "mufu"), "q_chunk": kq, "n_chunks": (w.M + kq - 1) // kq,
+                   "q_hint": "passed" if hint else "none",
                    "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
                    "parallelism": f"{world} independent structure(s), one per GPU", "wall_s_timed_loop": wall},
         "clocks": clocks,
         "e2e": {"value": units * n_e2e / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(hx.nbytes + hf.nbytes + hq.nbytes),
                 "d2h_bytes_per_step": int(hout.nbytes), "ms_per_step": e2e_s / n_e2e * 1e3, "steps": n_e2e},
-        "gpu_launches": 3 * args.steps,
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T sin/s", "frac": achieved / peak,
+        "gpu_launches": (4 if recur else 3) * args.steps,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s" if recur else "T sin/s", "frac": achieved / peak,
                      # dram__bytes_read.sum + write.sum of the pairs kernel from the full ncu capture (profiles/r01_v6.md)
-                     "traffic": 4248064 if (args.config == "cfg2" and variant != "fp64") else None,
-                     "note": "XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM x 148 SM x sm_max_mhz; the q-chunks "
-                             "are padded (M = 101 runs 4 x 28 = 112 slots), which the algorithmic count does not credit",
-                     "kernel": f"debye_peratom_pairs_kernel<{'fp64' if variant == 'fp64' else 'fp32'}>", "kernel_ms": pairs_ms,
+                     "traffic": 4248064 if (args.config == "cfg2" and variant != "fp64" and not recur) else None,
+                     "note": ("FP32-pipe roofline: 2 lane-ops (chain FFMA + accumulate FFMA against f_j = 4 FMA-equivalent flop) per pair.q "
+                              "with q != 0; peak = 148 SM x 128 lanes x 2 x sm_max_mhz") if recur else
+                             ("XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM x 148 SM x sm_max_mhz; the q-chunks "
+                              "are padded (M = 101 runs 4 x 28 = 112 slots), which the algorithmic count does not credit"),
+                     "kernel": "debye_peratom_recur_kernel" if recur else f"debye_peratom_pairs_kernel<{'fp64' if variant == 'fp64' else 'fp32'}>", "kernel_ms": pairs_ms,
                      "share_of_step": pairs_ms / (total_ms / args.steps)},
     }
     if world == 1 and not args.no_cpu_baseline:

@@ -125,9 +125,15 @@ int debye_profile_weighted_host(const float *xyz, const int32_t *type, const flo
  * q r <= 0.004 take an accurate series.  FP32 partial sums are multiplied by ff[i][m] and reduced in FP64 in a fixed order.
  *   xyz dev [N][3] float32, ff dev [N][M] float32 row-major (any sign), q dev [M] float32 (any grid; q and -q agree),
  *   I_out dev [M] float64 (written).  flags: 0 or DEBYE_SINC_MUFU (the FP32 path above), or DEBYE_FP64 (double-precision
- *   pair arithmetic, 1e-10 mode); anything else is DEBYE_EINVAL.  Three kernel launches, asynchronous on `stream`, same
- *   workspace rules and error codes as debye_profile (scratch: at most 1.3 MB + 1 KB x M; a caller-supplied workspace
- *   smaller than that gives DEBYE_ENOMEM).  q is processed in chunks of 16..32 values fitted to M.  When the rows are copies of a type table (ff[i] = fftab[type[i]])
+ *   pair arithmetic, 1e-10 mode), optionally with a grid hint (DEBYE_QHINT_*, debye_q_hint); anything else is DEBYE_EINVAL.
+ *   With a hint that promises q_k = (k + koff) dq, koff in {0, 1}, and at most 256 such q -- and neither DEBYE_SINC_MUFU nor
+ *   DEBYE_FP64 -- the RECURRENCE runs instead (debye_peratom_recur.cuh): per pair the Chebyshev recurrence generates
+ *   2 sin(q_k r)/r across the grid and each value is accumulated with one packed FMA against ff[j][k] from shared memory: 2 FP32
+ *   lane-operations per term instead of ~9 instructions and a MUFU.SIN, four launches (re-layout of ff + grid check, self
+ *   terms, pairs, final), scratch N x (16 + 4 K n_chunks) bytes more.  The device checks the hint; a wrong one gives NaN.
+ *   DEBYE_SINC_RECUR demands the recurrence: DEBYE_EUNSUPPORTED if the hinted grid is not one it takes.  Asynchronous on
+ *   `stream`, same workspace rules and error codes as debye_profile (direct path scratch: at most 1.3 MB + 1 KB x M; a
+ *   caller-supplied workspace that is too small gives DEBYE_ENOMEM).  The direct path takes q in chunks of 16..32 values fitted to M.  When the rows are copies of a type table (ff[i] = fftab[type[i]])
  *   the result equals debye_profile's to rounding -- and debye_profile is several times faster. */
 int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, double *I_out,
                           uint32_t flags, debye_stream_t stream);

@@ -239,9 +239,10 @@ def debye_partials(xyz, type, q, T, variant="auto", stream=None, hint=0):
     return S, n
 
 
-def debye_profile_peratom(xyz, ff, q, I_out=None, variant="auto", stream=None):
-    """I_out[M] for per-ATOM form factors ff[N,M] f32 (the paper's general case).  variant: "auto" / "mufu"
-    (FP32, one MUFU.SIN per term) or "fp64"."""
+def debye_profile_peratom(xyz, ff, q, I_out=None, variant="auto", stream=None, hint=0):
+    """I_out[M] for per-ATOM form factors ff[N,M] f32 (the paper's general case).  variant: "auto" (with a
+    grid hint that promises q_k = (k + koff) dq, koff in {0, 1}, and at most 256 chain indices: the recurrence, 2 FP32 lane-ops per
+    term; otherwise one MUFU.SIN per term), "mufu", "recur" or "fp64".  hint: q_hint(q_host)."""
     import torch
     N, M = xyz.shape[0], q.shape[0]
     if tuple(ff.shape) != (N, M):
@@ -250,7 +251,7 @@ def debye_profile_peratom(xyz, ff, q, I_out=None, variant="auto", stream=None):
         I_out = torch.empty(M, dtype=torch.float64, device=xyz.device)
     _check(lib().debye_profile_peratom(_dev(xyz, torch.float32, "xyz", (N, 3)), _dev(ff, torch.float32, "ff", (N, M)), N,
                                        _dev(q, torch.float32, "q", (M,)), M, _dev(I_out, torch.float64, "I_out", (M,)),
-                                       _flags(variant), _stream_ptr(stream)))
+                                       _flags(variant, hint), _stream_ptr(stream)))
     return I_out
 
 
@@ -312,13 +313,13 @@ def debye_profile_batch_host(xyz, type, fftab, q, I_out=None, variant="auto", st
     return I_out
 
 
-def debye_profile_peratom_host(xyz, ff, q, I_out=None, variant="auto", stream=None):
+def debye_profile_peratom_host(xyz, ff, q, I_out=None, variant="auto", stream=None, hint=0):
     N, M = xyz.shape[0], q.shape[0]
     if I_out is None:
         I_out = np.empty(M, dtype=np.float64)
     _check(lib().debye_profile_peratom_host(_host(xyz, np.float32, "xyz"), _host(ff, np.float32, "ff"), N,
                                             _host(q, np.float32, "q"), M, _host(I_out, np.float64, "I_out"),
-                                            _flags(variant), _stream_ptr(stream)))
+                                            _flags(variant, hint), _stream_ptr(stream)))
     return I_out
 
 

@@ -21,6 +21,7 @@
 #include "debye_registry.h"
 #include "debye_peratom.cuh"
 #include "debye_small.cuh"
+#include "debye_peratom_recur.cuh"
 
 namespace {
 
@@ -540,18 +541,81 @@ int debye_profile_from_partials(const double *S_parts, int32_t n_parts, const in
     return DEBYE_OK;
 }
 
+namespace {
+// per-atom form factors, recurrence (debye_peratom_recur.cuh): pack (+ grid check) | self terms | pairs | final.  Called with g_mu held.
+int run_peratom_recur(DevState *ds, const float *xyz, const float *ff, int N, const float *q, int M, double *I_out, int cls, int n_chunks, int K, cudaStream_t stream)
+{
+    debye_peratom_recur_fn fn = debye_get_peratom_recur_kernel(K);
+    if (!fn) return DEBYE_EUNSUPPORTED;
+    int st;
+    const int rows = debye_diag_rows(N);
+    const int64_t U = (rows > 0 ? debye_diag_row_prefix(N, rows) : 0) * n_chunks;
+    const int64_t one_wave = (int64_t)ds->sms * (K <= 64 ? 3 : 2);
+    int64_t G = U / 150 / one_wave * one_wave;                 // whole waves, at least ~150 units (j atoms x 128 i atoms) per CTA
+    if (G > one_wave * 16) G = one_wave * 16;
+    if (G < one_wave) { G = U / 8; if (G > one_wave) G = one_wave; }
+    if (G < 1) G = 1;
+    size_t o = 0;
+    const size_t o_plan = o; o += align_up(sizeof(debye::PeratomPlan));
+    const size_t o_pos = o; o += align_up((size_t)N * 16 + 16 * DEBYE_PAR_JT);
+    const size_t o_ffp = o; o += align_up((size_t)n_chunks * N * K * 4 + (size_t)DEBYE_PAR_JT * K * 4);
+    const size_t o_rec = o; o += align_up((size_t)(G + n_chunks) * K * 8);
+    const size_t o_self = o; o += align_up((size_t)DEBYE_PA_SLICES * 2 * M * 8);
+    char *ws;
+    if (ds->user_ws) { if (ds->user_bytes < o) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
+    else { if ((st = ensure(&ds->ws, &ds->ws_bytes, o))) return st; ws = (char *)ds->ws; }
+    debye::PeratomPlan *plan = (debye::PeratomPlan *)(ws + o_plan);
+    float4 *pos4 = (float4 *)(ws + o_pos);
+    float *ffp = (float *)(ws + o_ffp);
+    double *records = (double *)(ws + o_rec), *selfbuf = (double *)(ws + o_self);
+    CU(scratch_acquire(ds->order, stream));
+    int pb = (int)(((int64_t)N * K + 255) / 256);
+    if (pb > ds->sms * 8) pb = ds->sms * 8;
+    if (pb < 1) pb = 1;
+    debye::debye_peratom_pack_kernel<<<dim3(pb, n_chunks + 1), 256, 0, stream>>>(xyz, ff, q, N, M, K, n_chunks, cls, pos4, ffp, plan);
+    debye::debye_peratom_self_kernel<<<dim3((M + 31) / 32, DEBYE_PA_SLICES), 256, 0, stream>>>(ff, N, M, selfbuf);
+    if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
+    if (U > 0) fn<<<(int)G, DEBYE_IB, 0, stream>>>(pos4, ffp, q, plan, N, M, n_chunks, 0.002f, records);
+    if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
+    debye::debye_peratom_final_kernel<<<(M + 31) / 32, 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, K, I_out, (const int32_t *)plan);
+    CU(scratch_release(ds->order, stream));
+    CU(cudaGetLastError());
+    return DEBYE_OK;
+}
+}  // namespace
+
 int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, double *I_out, uint32_t flags, debye_stream_t stream_)
 {
     cudaStream_t stream = (cudaStream_t)stream_;
     if (!xyz || !ff || !q || !I_out) return DEBYE_EINVAL;
     if (N < 1 || M < 1 || M > DEBYE_MAX_Q) return DEBYE_EINVAL;
-    if (flags & ~(uint32_t)(DEBYE_FP64 | DEBYE_SINC_MUFU)) return DEBYE_EINVAL;      // FP64, or FP32 with one MUFU.SIN per term (default)
-    if ((flags & DEBYE_FP64) && (flags & DEBYE_SINC_MUFU)) return DEBYE_EINVAL;
+    // FP64, FP32 with one MUFU.SIN per term (DEBYE_SINC_MUFU, or any grid without a hint), or -- with a grid hint that promises
+    // q_k = (k + koff) dq -- the recurrence (DEBYE_SINC_RECUR or automatic)
+    const uint32_t hint_bits = DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ;
+    if (flags & ~(uint32_t)(DEBYE_FP64 | DEBYE_SINC_MUFU | DEBYE_SINC_RECUR | hint_bits)) return DEBYE_EINVAL;
+    if ((flags & DEBYE_FP64) && (flags & (DEBYE_SINC_MUFU | DEBYE_SINC_RECUR))) return DEBYE_EINVAL;
+    if ((flags & DEBYE_SINC_MUFU) && (flags & DEBYE_SINC_RECUR)) return DEBYE_EINVAL;
+    {
+        const uint32_t sub = flags & (DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ), st2 = flags & (DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ);
+        if ((sub && !(flags & DEBYE_QHINT)) || (st2 && !(flags & DEBYE_QHINT_UNIFORM)) || st2 == (DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ)) return DEBYE_EINVAL;
+    }
     if (N > (1 << 24)) return DEBYE_EUNSUPPORTED;
     const bool f64 = (flags & DEBYE_FP64) != 0;
+    if (flags & DEBYE_SINC_RECUR) {        // the recurrence was demanded: only for a hinted grid q_k = (k + koff) dq of at most 2 chunks
+        const int cls = hint_class_of(flags);
+        if ((cls != 0 && cls != 1) || M - (cls == 0 ? 1 : 0) < 1 || choose(V_RECUR, M - (cls == 0 ? 1 : 0)).n_chunks > 2) return DEBYE_EUNSUPPORTED;
+    }
     std::lock_guard<std::mutex> lock(g_mu);
     DevState *ds; int st;
     if ((st = dev_state(&ds))) return st;
+    {   // the recurrence: hinted grid q_k = (k + koff) dq, at most two chunks of 128 chain indices
+        const int cls = hint_class_of(flags);
+        const int n_idx = M - (cls == 0 ? 1 : 0);
+        if (!f64 && !(flags & DEBYE_SINC_MUFU) && (cls == 0 || cls == 1) && n_idx >= 1) {
+            const Choice c = choose(V_RECUR, n_idx);
+            if (c.n_chunks <= 2) return run_peratom_recur(ds, xyz, ff, N, q, M, I_out, cls, c.n_chunks, (c.K + 7) / 8 * 8, stream);
+        }
+    }
     const int KQ = debye::debye_peratom_kq(M);
     const int n_chunks = (M + KQ - 1) / KQ;
     const int rows = debye_diag_rows(N);
@@ -586,7 +650,7 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
 #undef DEBYE_PA_LAUNCH
     }
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
-    debye::debye_peratom_final_kernel<<<(M + 31) / 32, 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, KQ, I_out);
+    debye::debye_peratom_final_kernel<<<(M + 31) / 32, 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, KQ, I_out, nullptr);
     CU(scratch_release(ds->order, stream));
     CU(cudaGetLastError());
     return DEBYE_OK;

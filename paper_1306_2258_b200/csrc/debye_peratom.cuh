@@ -213,18 +213,25 @@ __global__ void __launch_bounds__(DEBYE_IB, F64 ? 2 : 4) debye_peratom_pairs_ker
 // that touched q index k (8 record loads in flight, added in CTA order); the parts are then added in slice order, so the
 // order is a fixed function of (N, M, G) and the result is bitwise reproducible.
 #define DEBYE_PA_FS 8
+// rplan != nullptr: the records come from debye_peratom_recur_kernel (debye_peratom_recur.cuh): chain slots (slot_of) holding
+// sums of 2 sin(q r)/r; a wrong grid hint (rplan->bad) gives NaN.
+struct PeratomPlan;
 __global__ void __launch_bounds__(32 * DEBYE_PA_FS) debye_peratom_final_kernel(const double *__restrict__ records, const double *__restrict__ selfbuf,
                                                                                  const float *__restrict__ qv, int N, int M, int n_chunks, int G, int KQ,
-                                                                                 double *__restrict__ out)
+                                                                                 double *__restrict__ out, const int32_t *__restrict__ rplan)
 {
     __shared__ double part[DEBYE_PA_FS][32];
+    pdl_wait();
     const int kk = threadIdx.x & 31, sl = threadIdx.x >> 5;
     const int k = blockIdx.x * 32 + kk;
     const int rows = debye_diag_rows(N);
     const int64_t U1 = rows > 0 ? debye_diag_row_prefix(N, rows) : 0;
+    const bool recur = rplan != nullptr;
+    const bool bad = recur && rplan[0] != 0;                 // PeratomPlan::bad, ::koff are its first two int32
     double s = 0.0;
-    if (k < M && U1 > 0 && qv[k] != 0.0f) {
-        const int ch = k / KQ, l = k % KQ;
+    if (k < M && U1 > 0 && qv[k] != 0.0f && !bad) {
+        int ch = k / KQ, l = k % KQ;
+        if (recur) slot_of(V_RECUR, KQ, n_chunks, k + rplan[1] - 1, ch, l);
         const int64_t U = U1 * n_chunks, ub = (int64_t)ch * U1, ue = ub + U1 - 1;
         const DebyeRanges ranges(U, G);
         if (U >= G) {           // every CTA owns at least one unit: all CTAs between the owners took part
@@ -253,7 +260,8 @@ __global__ void __launch_bounds__(32 * DEBYE_PA_FS) debye_peratom_final_kernel(c
 #pragma unroll
     for (int x = 0; x < DEBYE_PA_FS; ++x) tot += part[x][kk];
     const double qk = (double)qv[k];
-    out[k] = (qk == 0.0) ? s1 * s1 : s2 + 2.0 * tot / qk;
+    if (bad) { out[k] = __longlong_as_double(0x7ff8000000000000LL); return; }
+    out[k] = (qk == 0.0) ? s1 * s1 : s2 + (recur ? 1.0 : 2.0) * tot / qk;
 }
 
 }  // namespace debye

@@ -15,3 +15,8 @@ debye_pairs_fn debye_get_pairs_kernel(int variant, int K, bool weighted, bool sh
 // one launch for one small structure (debye_small.cuh): K a multiple of 8 in [8, 128]; nullptr otherwise
 typedef void (*debye_small_fn)(const float *, const int32_t *, int, int, const float *, const float *, int, int, double *, double *, int, int32_t *);
 debye_small_fn debye_get_small_kernel(int K);
+
+// per-atom form factors on a uniform grid (debye_peratom_recur.cuh): K a multiple of 8 in [8, 128]; nullptr otherwise
+namespace debye { struct PeratomPlan; }
+typedef void (*debye_peratom_recur_fn)(const float4 *, const float *, const float *, const debye::PeratomPlan *, int, int, int, float, double *);
+debye_peratom_recur_fn debye_get_peratom_recur_kernel(int K);

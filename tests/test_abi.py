@@ -65,7 +65,10 @@ def test_argument_validation_happens_before_cuda():
     assert L.debye_profile_peratom(None, p, 10, p, 5, p, 0, None) == EINVAL
     assert L.debye_profile_peratom(p, p, 0, p, 5, p, 0, None) == EINVAL
     assert L.debye_profile_peratom(p, p, 10, p, 4097, p, 0, None) == EINVAL
-    assert L.debye_profile_peratom(p, p, 10, p, 5, p, 1 << 3, None) == EINVAL                   # no recurrence variant here
+    assert L.debye_profile_peratom(p, p, 10, p, 5, p, 1 << 3, None) == EUNSUP                   # recurrence demanded without a grid hint
+    assert L.debye_profile_peratom(p, p, 10, p, 5, p, (1 << 3) | (1 << 2), None) == EINVAL      # recurrence and MUFU
+    assert L.debye_profile_peratom(p, p, 10, p, 5, p, (1 << 3) | 1, None) == EINVAL             # recurrence and FP64
+    assert L.debye_profile_peratom(p, p, 10, p, 5, p, 1 << 10, None) == EINVAL                  # hint sub-bit without DEBYE_QHINT
     assert L.debye_profile_peratom(p, p, (1 << 24) + 1, p, 5, p, 0, None) == EUNSUP
     assert L.debye_profile_from_partials(p, 0, p, p, 1, 2, 5, p, None) == EINVAL
     assert L.debye_profile_from_partials(p, 2, p, p, 1, 33, 5, p, None) == EINVAL

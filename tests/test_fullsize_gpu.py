@@ -175,3 +175,23 @@ def test_peratom_full_size_against_the_oracle_at_sampled_q(db):
     assert float(np.max(np.abs(I[ks] - ref) / np.abs(ref))) <= 1e-5
     I64 = db.debye_profile_peratom(torch.from_numpy(w.xyz).cuda(), torch.from_numpy(ff).cuda(), torch.from_numpy(w.q).cuda(), variant="fp64").cpu().numpy()
     assert float(np.max(np.abs(I64[ks] - ref) / np.abs(ref))) <= TOL64
+    # the recurrence (hinted grid), as bench.py --path peratom runs it: sampled q against the oracle, every q against FP64
+    Ir = db.debye_profile_peratom(torch.from_numpy(w.xyz).cuda(), torch.from_numpy(ff).cuda(), torch.from_numpy(w.q).cuda(), hint=db.q_hint(w.q)).cpu().numpy()
+    assert float(np.max(np.abs(Ir[ks] - ref) / np.abs(ref))) <= 1e-5
+    assert float(np.max(np.abs(Ir - I64) / np.abs(I64))) <= 1e-5
+
+
+def test_peratom_recurrence_cfg3_size_two_chunks(db):
+    """cfg3's 50 000 atoms and 200 q (two chunks of chain indices) with a per-atom table: the recurrence against
+    oracle_debye_peratom at 6 sampled q (the oracle needs only those columns; ~2 min of host time would be the whole grid)
+    and against the FP32 direct kernel at every q."""
+    import torch
+    w = wl.cfg3()
+    ff = wl.peratom_table(w, 0)
+    x, f, q = torch.from_numpy(w.xyz).cuda(), torch.from_numpy(ff).cuda(), torch.from_numpy(w.q).cuda()
+    Ir = db.debye_profile_peratom(x, f, q, hint=db.q_hint(w.q)).cpu().numpy()
+    ks = [1, 37, 100, 150, 193, 199]
+    ref = orc.debye_peratom(w.xyz, np.ascontiguousarray(ff[:, ks]), np.ascontiguousarray(w.q[ks]))
+    assert float(np.max(np.abs(Ir[ks] - ref) / np.abs(ref))) <= 3e-5
+    Id = db.debye_profile_peratom(x, f, q).cpu().numpy()
+    assert float(np.max(np.abs(Ir - Id) / np.abs(Id))) <= 5e-5

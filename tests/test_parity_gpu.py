@@ -651,6 +651,41 @@ def test_peratom_form_factors_match_the_peratom_oracle(db):
     assert rel(I, db.debye_profile(x, t, f, q).cpu().numpy()) <= 1e-5
 
 
+def test_peratom_recurrence_on_hinted_uniform_grids(db):
+    """debye_profile_peratom with a grid hint (grids q_k = (k + koff) dq): the chain recurrence with one packed FMA per term
+    against f_j(q_k) (debye_peratom_recur.cuh) instead of one MUFU.SIN per term.  Against oracle_debye_peratom element by
+    element and against the direct kernel; one and two chunks, K % 8 == 4, grids from 0 and from dq, ragged rows, close and
+    coincident atoms (the small-theta path), a wrong hint, a grid it does not take."""
+    import torch
+    shapes = [(2, 9, 0.0), (3, 17, 0.0), (130, 33, 0.0), (777, 101, 0.0), (1500, 129, 0.0), (700, 128, 0.004), (1100, 200, 0.0),
+              (400, 257, 0.0), (515, 52, 0.01), (900, 64, 0.0)]
+    for si, (N, M, q_min) in enumerate(shapes):
+        w = wl.small_random(300 + si, N, 3, M, q_min=q_min, q_max=q_min * M if q_min else 0.7, box=12.0 + N ** (1 / 3) * 3)
+        ff = _peratom_ff(w, 400 + si)
+        hint = db.q_hint(w.q)
+        x, f, q = (torch.from_numpy(a).cuda() for a in (w.xyz, ff, w.q))
+        ref = orc.debye_peratom(w.xyz, ff, w.q)
+        a = db.debye_profile_peratom(x, f, q, hint=hint, variant="recur").cpu().numpy()
+        assert rel(a, ref) <= TOL32, (N, M, q_min, rel(a, ref))
+        assert rel(a, db.debye_profile_peratom(x, f, q).cpu().numpy()) <= 2e-5          # the direct kernel
+        assert a.tobytes() == db.debye_profile_peratom(x, f, q, hint=hint).cpu().numpy().tobytes()      # automatic choice, and run to run
+        assert np.array_equal(a, db.debye_profile_peratom_host(w.xyz, ff, w.q, hint=hint))
+    # close pairs (theta far below the small-theta threshold) and coincident atoms
+    xyz = np.array([[0, 0, 0], [0, 0, 0], [1e-3, 0, 0], [0.02, 0.01, 0], [3.0, 1.0, -2.0], [0.3, 0.0, 0.0]], np.float32)
+    qg = wl.q_grid(0.5, 101)
+    ff = (1.0 + 0.3 * np.random.default_rng(3).standard_normal((6, 101))).astype(np.float32)
+    a = db.debye_profile_peratom(torch.from_numpy(xyz).cuda(), torch.from_numpy(ff).cuda(), torch.from_numpy(qg).cuda(), hint=db.q_hint(qg)).cpu().numpy()
+    assert rel(a, orc.debye_peratom(xyz, ff, qg)) <= 1e-5
+    # a wrong hint gives NaN; a general-start grid is not taken by the recurrence
+    w = wl.small_random(330, 300, 3, 40, q_min=0.3, q_max=0.9)
+    ff = _peratom_ff(w, 1)
+    x, f, q = (torch.from_numpy(a_).cuda() for a_ in (w.xyz, ff, w.q))
+    assert np.isnan(db.debye_profile_peratom(x, f, q, hint=db.q_hint(wl.q_grid(0.5, 40))).cpu().numpy()).all()
+    with pytest.raises(db.LibdebyeError):
+        db.debye_profile_peratom(x, f, q, hint=db.q_hint(w.q), variant="recur")
+    assert rel(db.debye_profile_peratom(x, f, q, hint=db.q_hint(w.q)).cpu().numpy(), orc.debye_peratom(w.xyz, ff, w.q)) <= TOL32
+
+
 def test_peratom_degenerate_inputs(db):
     import torch
     q = np.array([0.0, 0.05, 0.4, 1.3], dtype=np.float32)

@@ -30,10 +30,10 @@ from paper_1306_2258_b200 import workloads as wl          # noqa: E402  (input g
 METRIC = "pair_q_sinc_terms_per_second"
 UNIT = "G pair.q/s"
 SM_COUNT, FP32_LANES, MUFU_LANES = 148, 128, 16           # per B200 / per SM per clock (B200_PROFILING.md)
-# dram__bytes_read.sum + dram__bytes_write.sum of the pairs kernel, per launch, from the committed ncu --set full capture
-# (profiles/r01_ncu_full_pairs_recur_cfg{2,4,5}_v4.txt); None where no capture exists
-NCU_TRAFFIC = {("cfg2", "recur"): 239104, ("cfg4", "recur"): 32843264 + 163584, ("cfg5", "recur"): 3336192}
-NCU_TRAFFIC_SOURCE = "profiles/r01_ncu_full_pairs_recur_cfg{2,4,5}_v4.txt (capture of an earlier build; the kernel's inputs are unchanged)"
+# dram__bytes_read.sum + dram__bytes_write.sum of the pairs kernel, per launch, from the committed ncu --set full captures
+# (profiles/r02_ncu_full_pairs_cfg{2,4,5}.txt); None where no capture exists
+NCU_TRAFFIC = {("cfg2", "recur"): 239104, ("cfg4", "recur"): 32848640 + 254464, ("cfg5", "recur"): 3329280}
+NCU_TRAFFIC_SOURCE = "profiles/r02_ncu_full_pairs_cfg{2,4,5}.txt (ncu --set full capture of this kernel, commands in profiles/r02_product_form.md); not measured by this run"
 
 
 TABLE1 = {f"table1_{n}": n for n in (1000, 2000, 4000, 10000, 20000, 40000, 100000)}       # the paper's Table I rows
@@ -516,6 +516,8 @@ def run_tile_split(args, w, rank, world, dev):
     flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device=dev)
     info = db.launch_info(w.N, w.B, w.T, w.M, args.variant, with_grid=True, hint=hint)
 
+    sharding.assert_same_schedule(info["pairs_grid"], world, dev)       # CTA c belongs to rank c mod world on EVERY rank
+
     def step():
         return sharding.profile_tile_split(
             lambda r, wd: db.debye_partials_shard(x, t, q, w.T, r, wd, variant=args.variant, hint=hint),
@@ -549,13 +551,30 @@ def run_tile_split(args, w, rank, world, dev):
         res = step().cpu()
     barrier()
     e2e_s = sharding.max_over_ranks(time.perf_counter() - t0, dev)
+    # this rank's pairs kernel alone (events recorded by the library around its launch); max over ranks
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); e1.record(); torch.cuda.synchronize()
+    db.set_pairs_events(e0, e1)
+    pk = []
+    for _ in range(min(args.steps, 10)):
+        flush.fill_(1)
+        step()
+        torch.cuda.synchronize()
+        pk.append(e0.elapsed_time(e1))
+    db.set_pairs_events(None, None)
+    pairs_ms = sharding.max_over_ranks(float(np.mean(pk)), dev)
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        return None
+    fmax_ghz = float(measured_peaks().get("sm_max_mhz", 1965.0)) / 1e3
+    vr = variant_that_ran(args.variant, w)
+    # every rank's pairs kernel does 1/world of the pairs: roofline of ONE GPU's kernel on its share
+    roof = roofline_of(w, vr, pairs_ms * world, fmax_ghz)
+    roof["kernel_ms"] = pairs_ms
+    roof["note"] = f"per GPU: each rank's pairs kernel runs 1/{world} of the CTAs of the single-GPU schedule; " + roof["note"]
+    roof["share_of_step"] = pairs_ms / (total_ms / args.steps)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "roofline": roof,
         "dtype": "f64" if args.variant == "fp64" else "f32", "data": "synthetic",
         "config": {"workload": w.name, "N": w.N, "T": w.T, "M": w.M, "B": w.B, "variant": args.variant, "pairs_grid": info["pairs_grid"],
                    "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
@@ -571,9 +590,12 @@ def run_tile_split(args, w, rank, world, dev):
             ks = list(range(0, w.M, max(1, w.M // 8)))
             ref = orc.debye_sym(w.xyz, w.type, w.fftab[:, ks].copy(), w.q[ks].copy())
             line["parity_max_rel_err"] = float(np.max(np.abs(out.cpu().numpy()[0][ks] - ref) / np.abs(ref)))
-    print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+        line["cpu_baseline"] = cpu_baseline(w)
+    rows = stored_oracle(args.config if w.name.startswith(args.config) else w.name.split("_")[0])
+    if rows is not None and w.xyz.ndim == 2:
+        I = out.cpu().numpy()[0]
+        line["max_rel_err_vs_stored_oracle"] = float(max(abs(I[k] - ref) / abs(ref) for b, k, ref in rows))
+    return line
 
 
 def run_peratom(args, w, rank, world, dev):

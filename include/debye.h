@@ -60,7 +60,8 @@ enum {
     DEBYE_SINC_RECUR = 1u << 3,   /* FP32, Chebyshev angle-addition recurrence across a uniform q grid          *
                                    * q_m = q_0 + m dq.  If q is not uniform (checked on the device) the output  *
                                    * is filled with NaN.                                                         */
-    DEBYE_SINC_ACCURATE = 1u << 4, /* FP32, libdevice sinf per term (slow reference variant); any q grid        */
+    DEBYE_SINC_ACCURATE = 1u << 4, /* FP32, libdevice sinf per term (slow reference variant); any q grid;       *
+                                   * plain calls only: DEBYE_EUNSUPPORTED with weights or in a tile split      */
     /* Optional grid hint, as returned by debye_q_hint() from a HOST copy of q.  Without it the library cannot know the
      * shape of the grid when it launches (q is device memory and calls never synchronise), so it launches every pairs
      * instantiation that could be needed and the device runs exactly one; with it, only that one is launched (two to
@@ -175,6 +176,8 @@ int debye_partials(const float *xyz, const int32_t *type, int32_t N, int32_t B, 
  * form-factor epilogue on the device:
  *     I_out[b][m] = sum_a n_a F_a^2 + 2 sum_{p=(a<=b')} F_a F_b' sum_{r < n_parts} S_parts[r][b][p][m].
  *   S_parts dev [n_parts][B][T(T+1)/2][M] float64, n_a dev [T] int32 (n_out of any rank), fftab dev [T][M], I_out dev [B][M].
+ * Every rank must build the SAME static schedule, i.e. the same pairs grid (debye_launch_info: it follows from the SM count
+ * and the kernel's occupancy): same GPU model and library build on every rank (sharding.assert_same_schedule checks it).
  * shard_world == 1 is debye_partials.  Unweighted only.  Errors: DEBYE_EINVAL for shard_rank outside [0, shard_world),
  * shard_world / n_parts outside [1, 4096], B > 65535 (from_partials), otherwise as debye_partials. */
 int debye_partials_shard(const float *xyz, const int32_t *type, int32_t N, int32_t B, const float *q, int32_t T, int32_t M,

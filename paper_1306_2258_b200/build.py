@@ -16,8 +16,9 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libdebye.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+# -Xfatbin=-compress-all: the device code (with its -lineinfo tables) is stored compressed, a third of the size
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
-         "--expt-relaxed-constexpr", *os.environ.get("DEBYE_EXTRA_NVCC_FLAGS", "").split()]
+         "--expt-relaxed-constexpr", "-Xfatbin=-compress-all", *os.environ.get("DEBYE_EXTRA_NVCC_FLAGS", "").split()]
 
 
 def _sources():

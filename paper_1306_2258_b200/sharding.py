@@ -102,6 +102,21 @@ def gather_partials(S_part, world: int):
     return out
 
 
+def assert_same_schedule(pairs_grid: int, world: int, device=None):
+    """The tile split assigns pairs CTA c of ONE static schedule to rank c mod world, so every rank must have built the
+    same schedule: the same pairs grid (it depends on the device's SM count and the kernel's occupancy, binding.launch_info).
+    Raises on every rank if the ranks disagree (mixed GPU models, differently built libraries)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or world == 1:
+        return
+    t = torch.tensor([int(pairs_grid), -int(pairs_grid)], dtype=torch.int64, device=device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    if int(t[0]) != -int(t[1]):
+        raise RuntimeError(f"tile split: ranks disagree on the pairs grid (max {int(t[0])}, min {-int(t[1])}); "
+                           "every rank must run the same GPU model and library build")
+
+
 def profile_tile_split(partials_shard_fn, from_partials_fn, fftab, rank: int, world: int):
     """One profile of one structure (or batch) on `world` GPUs: partials_shard_fn(rank, world) -> (S_part, n) is this rank's
     tile share (binding.debye_partials_shard with xyz / type / q bound), the parts are all-gathered, and

@@ -53,6 +53,14 @@ def _worker(rank, world, port, tmp):
                                       lambda S, n, f: (S * torch.arange(1, S.shape[0] + 1, dtype=torch.float64)[:, None, None, None]).sum(0),
                                       None, rank, world)
     np.save(os.path.join(tmp, f"tot{rank}.npy"), tot.numpy())
+    # every rank must have built the same static schedule (same pairs grid): agreeing grids pass, differing ones raise everywhere
+    sharding.assert_same_schedule(2368, world)
+    try:
+        sharding.assert_same_schedule(2368 + rank, world)
+        raised = False
+    except RuntimeError:
+        raised = True
+    np.save(os.path.join(tmp, f"raised{rank}.npy"), np.array([raised]))
     t = sharding.max_over_ranks(1.0 + rank)
     s = sharding.sum_over_ranks(hi - lo)
     if rank == 0:
@@ -80,3 +88,20 @@ def test_two_rank_gloo_shards_and_gathers(tmp_path):
         assert np.array_equal(np.load(tmp_path / f"tot{r}.npy"), np.full((1, 3, 7), 21.0))
     t, s = np.load(tmp_path / "ts.npy")
     assert t == 2.0 and s == 5.0
+    assert np.load(tmp_path / "raised0.npy")[0] and np.load(tmp_path / "raised1.npy")[0]
+
+
+def test_bench_refuses_more_gpus_than_the_node_has():
+    """`python bench.py --gpus N` starts N ranks itself (torch.distributed.run on 127.0.0.1) -- and says so, with a non-zero
+    exit status, when the node has fewer than N CUDA devices (here: none) instead of measuring fewer GPUs than it reports."""
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    env["CUDA_VISIBLE_DEVICES"] = ""
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "1"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode != 0 and "needs 2 CUDA devices" in (r.stderr + r.stdout)
+    env["WORLD_SIZE"] = "4"            # under a launcher the two counts must agree
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2"], capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode != 0 and "WORLD_SIZE=4" in (r.stderr + r.stdout)

@@ -68,7 +68,8 @@ enum {
      * three launches fewer: ~8 us per call).  The device checks the hint against q; if it is wrong nothing is computed
      * and the output is filled with NaN. */
     DEBYE_QHINT = 1u << 8,          /* a hint is present                                                        */
-    DEBYE_QHINT_UNIFORM = 1u << 9,  /* q[k] = q[0] + k dq (to 2 float ulps of max |q|)                          */
+    DEBYE_QHINT_UNIFORM = 1u << 9,  /* q[k] = q[0] + k dq, dq = (q[M-1] - q[0])/(M-1): every q[k] within 1.5 float
+                                     * ulps (1.8e-7 relative to max(|q[k]|, |dq|)) of that line                  */
     DEBYE_QHINT_START0 = 1u << 10,  /* ... and q[0] == 0                                                        */
     DEBYE_QHINT_STARTDQ = 1u << 11  /* ... and q[0] == dq (the paper's grid q_k = k dq, k >= 1)   */
 };

@@ -24,8 +24,13 @@ EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_
            "debye_pipe_bench_name", "debye_pipe_bench", "debye_mufu_sin_error", "debye_mufu_rsq_error")
 
 
+# status codes of include/debye.h (debye_status)
+DEBYE_OK, DEBYE_EINVAL, DEBYE_EUNSUPPORTED, DEBYE_ENOMEM, DEBYE_ECUDA = 0, 1, 2, 3, 4
+
+
 class LibdebyeError(RuntimeError):
-    pass
+    """code: the library's status (DEBYE_E*), or None for an error raised by the binding's own argument checks."""
+    code = None
 
 
 _lib = None
@@ -100,8 +105,10 @@ def lib():
 def _check(st: int):
     if st != 0:
         L = lib()
-        raise LibdebyeError(f"libdebye status {st}: {L.debye_strerror(st).decode()} "
-                            f"(cuda error {L.debye_last_cuda_error()})")
+        e = LibdebyeError(f"libdebye status {st}: {L.debye_strerror(st).decode()} "
+                          f"(cuda error {L.debye_last_cuda_error()})")
+        e.code = int(st)
+        raise e
 
 
 def _flags(variant, hint: int = 0) -> int:

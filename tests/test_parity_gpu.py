@@ -254,9 +254,13 @@ def test_weighted_profiles_match_the_weighted_oracle(db):
         ref, A = orc.debye_sym(w0.xyz, w0.type, w0.fftab, w0.q, weight=wt, return_abs=True)
         x, t, f, q = to_dev(w0)
         wd = torch.from_numpy(wt).cuda()
-        for v in FP32_VARIANTS:
+        for v in ["auto", "recur", "mufu"]:
             I = db.debye_profile_weighted(x, t, wd, f, q, variant=v).cpu().numpy()
             assert rel(I, ref) <= TOL32, (name, v, rel(I, ref))
+        # the libdevice-sinf reference variant exists for the plain calls only (include/debye.h DEBYE_SINC_ACCURATE)
+        with pytest.raises(db.LibdebyeError) as ei:
+            db.debye_profile_weighted(x, t, wd, f, q, variant="accurate")
+        assert ei.value.code == db.DEBYE_EUNSUPPORTED
         assert rel(db.debye_profile_weighted(x, t, wd, f, q, variant="fp64").cpu().numpy(), ref) <= TOL64
         ones = torch.ones(w0.N, dtype=torch.float32, device="cuda")
         # weight 1 is the unweighted profile up to summation order (weighted calls reduce their accumulators once per row)

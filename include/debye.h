@@ -200,6 +200,35 @@ int debye_set_workspace(void *dev_ptr, size_t bytes);
 /* Frees the library-owned workspace of every device (also done at process exit). */
 void debye_shutdown(void);
 
+/* One small structure WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (CUDA graph capture, tight serving
+ * loops, harnesses that forbid it).  Same result as debye_profile on the same inputs and flags (the single cooperative launch
+ * of the small-structure kernel: sort, pairs, FP64 reduction and epilogue), but the per-CTA FP64 records
+ * live in a file-scope __device__ array of DEBYE_STATIC_SCRATCH_BYTES (292 KiB) that is part of the library's device image
+ * (every GPU that uses the entry point holds it until the process exits) instead of the cudaMalloc'ed workspace.  The call
+ * allocates nothing -- no cudaMalloc / cudaFree, no events, no workspace -- and never synchronises.
+ *   xyz dev [N][3], type dev [N], fftab dev [T][M], q dev [M], I_out dev [M] float64: the caller's, as for debye_profile.
+ *   flags MUST carry a grid hint DEBYE_QHINT | DEBYE_QHINT_UNIFORM | (DEBYE_QHINT_START0 or DEBYE_QHINT_STARTDQ), e.g. from
+ *   debye_q_hint (the host may not read q; the device checks the hint and fills I_out with NaN if it is wrong);
+ *   DEBYE_SINC_RECUR is accepted, the other variants are not (they need the allocated workspace).
+ * Limits (what the array holds): N <= DEBYE_STATIC_MAX_ATOMS, T <= DEBYE_STATIC_MAX_TYPES, at most DEBYE_STATIC_MAX_Q
+ * non-zero q values (M <= 129 with q[0] == 0, M <= 128 otherwise).  Anything beyond, or a missing / non-uniform hint, returns
+ * DEBYE_EUNSUPPORTED and launches nothing; debye_profile_static_error() then names the limit that was exceeded (a message
+ * for the calling thread's last debye_profile_static call, "" after a success).
+ * SHARED SCRATCH: all calls on one GPU use the one array, which keeps the last call's records (the kernel writes every record
+ * before it reads it: nothing needs clearing).  Calls on the same stream are ordered by the stream; calls that can overlap on
+ * the GPU (different streams with no event between them) race and return wrong profiles: the caller orders them.  It does not
+ * share anything with the other entry points and may overlap with those. */
+#define DEBYE_STATIC_MAX_ATOMS 2048
+#define DEBYE_STATIC_MAX_TYPES 8
+#define DEBYE_STATIC_MAX_Q 128
+#define DEBYE_STATIC_MAX_GRID 256                                   /* CTAs (one per SM at most)                      */
+#define DEBYE_STATIC_SCRATCH_BYTES ((size_t)(256 + 36) * 128 * 8)   /* (CTAs + type pairs) records x 128 slots x 8 B */
+int debye_profile_static(const float *xyz, const int32_t *type, int32_t N, const float *fftab, int32_t T, const float *q,
+                         int32_t M, double *I_out, uint32_t flags, debye_stream_t stream);
+const char *debye_profile_static_error(void);
+/* The limits above at run time (any pointer may be NULL). */
+void debye_profile_static_limits(int32_t *max_atoms, int32_t *max_types, int32_t *max_nonzero_q, size_t *scratch_bytes);
+
 /* Introspection used by bench.py / tests (host-side, no GPU work):
  * number of library kernels one debye_profile[_batch] call with these arguments launches, and the grid /
  * chunking the pairs kernel would use (any out pointer may be NULL). */

@@ -21,7 +21,8 @@ EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_
            "debye_partials_shard", "debye_profile_from_partials", "debye_profile_peratom", "debye_profile_peratom_host", "debye_workspace_bytes", "debye_set_workspace", "debye_shutdown",
            "debye_launch_info", "debye_set_pairs_events", "debye_q_hint", "debye_plan_create", "debye_plan_execute",
            "debye_plan_destroy", "debye_strerror", "debye_last_cuda_error", "debye_version", "debye_pipe_bench_count",
-           "debye_pipe_bench_name", "debye_pipe_bench", "debye_mufu_sin_error", "debye_mufu_rsq_error")
+           "debye_pipe_bench_name", "debye_pipe_bench", "debye_mufu_sin_error", "debye_mufu_rsq_error",
+           "debye_profile_static", "debye_profile_static_error", "debye_profile_static_limits")
 
 
 # status codes of include/debye.h (debye_status)
@@ -98,6 +99,12 @@ def lib():
     L.debye_mufu_sin_error.restype = C.c_int
     L.debye_mufu_rsq_error.argtypes = L.debye_mufu_sin_error.argtypes
     L.debye_mufu_rsq_error.restype = C.c_int
+    L.debye_profile_static.argtypes = L.debye_profile.argtypes
+    L.debye_profile_static.restype = C.c_int
+    L.debye_profile_static_error.argtypes = []
+    L.debye_profile_static_error.restype = C.c_char_p
+    L.debye_profile_static_limits.argtypes = [C.POINTER(i32)] * 3 + [C.POINTER(sz)]
+    L.debye_profile_static_limits.restype = None
     _lib = L
     return L
 
@@ -151,6 +158,31 @@ def debye_profile(xyz, type, fftab, q, I_out=None, variant="auto", stream=None, 
     _check(lib().debye_profile(_dev(xyz, torch.float32, "xyz", (N, 3)), _dev(type, torch.int32, "type", (N,)), N,
                                _dev(fftab, torch.float32, "fftab", (T, M)), T, _dev(q, torch.float32, "q", (M,)), M,
                                _dev(I_out, torch.float64, "I_out", (M,)), _flags(variant, hint), _stream_ptr(stream)))
+    return I_out
+
+
+def static_limits():
+    """(max atoms, max types, max non-zero q values, bytes of the static scratch) of debye_profile_static."""
+    a, t, m, b = C.c_int32(), C.c_int32(), C.c_int32(), C.c_size_t()
+    lib().debye_profile_static_limits(C.byref(a), C.byref(t), C.byref(m), C.byref(b))
+    return a.value, t.value, m.value, b.value
+
+
+def debye_profile_static(xyz, type, fftab, q, I_out, hint, stream=None):
+    """debye_profile for one small structure with NO allocation anywhere (include/debye.h debye_profile_static): the scratch
+    is a fixed __device__ array of the library.  I_out is the caller's (this wrapper does not allocate it either); `hint` must
+    be q_hint() of a uniform grid starting at 0 or dq.  Beyond static_limits() the library refuses (DEBYE_EUNSUPPORTED) and
+    the error names the limit.  Calls that overlap on the GPU (different streams, no event between them) race."""
+    import torch
+    N, T, M = xyz.shape[0], fftab.shape[0], q.shape[0]
+    L = lib()
+    st = L.debye_profile_static(_dev(xyz, torch.float32, "xyz", (N, 3)), _dev(type, torch.int32, "type", (N,)), N,
+                                _dev(fftab, torch.float32, "fftab", (T, M)), T, _dev(q, torch.float32, "q", (M,)), M,
+                                _dev(I_out, torch.float64, "I_out", (M,)), int(hint), _stream_ptr(stream))
+    if st != 0:
+        e = LibdebyeError(f"libdebye status {st}: {L.debye_profile_static_error().decode() or L.debye_strerror(st).decode()}")
+        e.code = int(st)
+        raise e
     return I_out
 
 

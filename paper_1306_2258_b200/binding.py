@@ -14,7 +14,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 # LIBDEBYE_PATH: load another build of the same library (e.g. one compiled with different tuning macros)
 LIB_PATH = os.environ.get("LIBDEBYE_PATH") or os.path.join(HERE, "libdebye.so")
 
-FLAGS = {"fp64": 1 << 0, "mufu": 1 << 2, "recur": 1 << 3, "accurate": 1 << 4, "auto": 0}
+FLAGS = {"fp64": 1 << 0, "mufu": 1 << 2, "recur": 1 << 3, "accurate": 1 << 4, "centred": 1 << 5, "auto": 0}
+QHINT_PIECES = 1 << 12
 
 EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_profile_batch_host",
            "debye_profile_weighted", "debye_profile_batch_weighted", "debye_profile_weighted_host", "debye_partials",
@@ -22,7 +23,7 @@ EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_
            "debye_launch_info", "debye_set_pairs_events", "debye_q_hint", "debye_plan_create", "debye_plan_execute",
            "debye_plan_destroy", "debye_strerror", "debye_last_cuda_error", "debye_version", "debye_pipe_bench_count",
            "debye_pipe_bench_name", "debye_pipe_bench", "debye_mufu_sin_error", "debye_mufu_rsq_error",
-           "debye_profile_static", "debye_profile_static_error", "debye_profile_static_limits")
+           "debye_profile_static", "debye_profile_static_error", "debye_profile_static_limits", "debye_q_hint_pieces")
 
 
 # status codes of include/debye.h (debye_status)
@@ -86,6 +87,8 @@ def lib():
     L.debye_plan_destroy.restype = None
     L.debye_q_hint.argtypes = [vp, i32]
     L.debye_q_hint.restype = u32
+    L.debye_q_hint_pieces.argtypes = [vp, i32]
+    L.debye_q_hint_pieces.restype = u32
     L.debye_strerror.argtypes = [C.c_int]
     L.debye_strerror.restype = C.c_char_p
     L.debye_last_cuda_error.restype = C.c_int
@@ -127,6 +130,20 @@ def q_hint(q_host) -> int:
     so that only the pairs instantiation this grid needs is launched.  A wrong hint gives NaN, never a wrong number."""
     q_host = np.ascontiguousarray(q_host, dtype=np.float32)
     return int(lib().debye_q_hint(C.c_void_p(q_host.ctypes.data), q_host.shape[0]))
+
+
+def q_hint_pieces(q_host) -> int:
+    """The piecewise-uniform hint (centred product form) for ANY grid made of at most 16 uniform pieces, 0 if q is not one;
+    q_hint() returns it by itself for grids that are not uniform as a whole.  (pieces, K) = pieces_of(hint)."""
+    q_host = np.ascontiguousarray(q_host, dtype=np.float32)
+    return int(lib().debye_q_hint_pieces(C.c_void_p(q_host.ctypes.data), q_host.shape[0]))
+
+
+def pieces_of(hint: int):
+    """(number of uniform pieces, accumulators per thread) a piecewise-uniform hint carries; (0, 0) for any other hint."""
+    if not hint & QHINT_PIECES:
+        return 0, 0
+    return ((hint >> 16) & 31) + 1, 8 * (((hint >> 21) & 31) + 1)
 
 
 def _stream_ptr(stream):

@@ -14,6 +14,7 @@
 #include <cstddef>
 #include <cmath>
 #include <mutex>
+#include <vector>
 #include "../../include/debye.h"
 #include "debye_aux.cuh"
 #include "debye_pairs.cuh"
@@ -50,6 +51,11 @@ cudaError_t scratch_release(ScratchOrder &o, cudaStream_t stream)
     return cudaEventRecord(o.done, stream);
 }
 
+// debye_q_hint: 1 = a uniform grid with a general start (neither 0 nor dq) is hinted as pieces too: the centred product form
+// (measured on B200, 10 000 atoms x 101 q: 11.6 T pair.q/s) instead of the chain form of the recurrence (4.65 T)
+#ifndef DEBYE_CENT_FOR_GENERAL_START
+#define DEBYE_CENT_FOR_GENERAL_START 1
+#endif
 constexpr int MAX_DEV = 64;
 constexpr int64_t DEBYE_PACK_IN_SETUP = 16384;   // N x B up to which debye_setup_kernel also packs the coordinates
 struct DevState {
@@ -62,7 +68,7 @@ struct DevState {
     // use; a call on another stream first makes its stream wait for it, so calls on different streams serialise on the
     // device instead of overwriting each other's records
     ScratchOrder order;
-    int occ[5][33];                                   // cached CTAs/SM per (variant, K/4); 0 = unknown
+    int occ[6][33];                                   // cached CTAs/SM per (variant, K/4); 0 = unknown
     int occ_small[17][DEBYE_SMALL_TMAX + 1];          // the same for debye_small_kernel<8 i> with T types (N = 2048); 0 = unknown
 };
 DevState g_dev[MAX_DEV];
@@ -144,14 +150,27 @@ Layout layout(int N, int B, int T, int M, int G_max, const Choice *ch, int nch)
 }
 
 constexpr int MAX_CHOICES = 3;
-// grid class promised by the caller's hint flags (debye_grid_class), -3 without a hint
+// grid class promised by the caller's hint flags (debye_grid_class), -3 without a hint, -4 for a piecewise-uniform grid
 int hint_class_of(uint32_t flags)
 {
     if (!(flags & DEBYE_QHINT)) return -3;
+    if (flags & DEBYE_QHINT_PIECES) return -4;
     if (!(flags & DEBYE_QHINT_UNIFORM)) return -2;
     if (flags & DEBYE_QHINT_START0) return 0;
     if (flags & DEBYE_QHINT_STARTDQ) return 1;
     return -1;
+}
+// piecewise-uniform hint: number of pieces and accumulators per thread, as (n << 8) | K / 8 (the setup kernel's argument)
+int hint_pieces_of(uint32_t flags)
+{
+    if (!(flags & DEBYE_QHINT_PIECES)) return 0;
+    return (int)((((flags >> DEBYE_QHINT_NPIECES_SHIFT) & 31u) + 1u) << 8) | (int)(((flags >> DEBYE_QHINT_PIECEK_SHIFT) & 31u) + 1u);
+}
+Choice cent_choice(uint32_t flags)
+{
+    const int hp = hint_pieces_of(flags);
+    Choice c; c.variant = V_CENT; c.K = 8 * (hp & 255); c.n_chunks = hp >> 8; c.alt_gate = -1;
+    return c;
 }
 // the one recurrence launch for a known grid class
 int recur_choice_hinted(Choice *out, int M, int cls)
@@ -170,7 +189,9 @@ int variants_for(uint32_t flags, Choice *out, int M, int *is_auto)
     if (flags & DEBYE_SINC_MUFU) { out[0] = choose(V_MUFU, M); return 1; }
     if (flags & DEBYE_SINC_RECUR) return (cls >= -1) ? recur_choice_hinted(out, M, cls) : recur_choices(out, M);
     if (flags & DEBYE_SINC_ACCURATE) { out[0] = choose(V_ACCURATE, M); return 1; }
+    if (flags & DEBYE_SINC_CENTRED) { out[0] = cent_choice(flags); return 1; }      // validate(): only with a pieces hint
     *is_auto = 1;
+    if (cls == -4) { out[0] = cent_choice(flags); return 1; }         // hinted: piecewise uniform, the centred product form
     if (cls == -2) { out[0] = choose(V_MUFU, M); return 1; }          // hinted: not uniform
     if (cls >= -1) return recur_choice_hinted(out, M, cls);           // hinted: uniform
     int n = recur_choices(out, M);
@@ -183,10 +204,11 @@ int validate(const void *xyz, const void *type, int N, int B, const void *tab, i
     if (!xyz || !type || !q || !out) return DEBYE_EINVAL;
     if (!tab) return DEBYE_EINVAL;
     if (N < 1 || M < 1 || T < 1 || B < 1 || T > DEBYE_MAX_TYPES || M > DEBYE_MAX_Q) return DEBYE_EINVAL;
-    uint32_t known = DEBYE_FP64 | DEBYE_SINC_MUFU | DEBYE_SINC_RECUR | DEBYE_SINC_ACCURATE | DEBYE_QHINT | DEBYE_QHINT_UNIFORM |
-                     DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ;
+    const uint32_t piece_fields = (31u << DEBYE_QHINT_NPIECES_SHIFT) | (31u << DEBYE_QHINT_PIECEK_SHIFT);
+    uint32_t known = DEBYE_FP64 | DEBYE_SINC_MUFU | DEBYE_SINC_RECUR | DEBYE_SINC_ACCURATE | DEBYE_SINC_CENTRED | DEBYE_QHINT | DEBYE_QHINT_UNIFORM |
+                     DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ | DEBYE_QHINT_PIECES | piece_fields;
     if (flags & ~known) return DEBYE_EINVAL;
-    uint32_t s = flags & (DEBYE_SINC_MUFU | DEBYE_SINC_RECUR | DEBYE_SINC_ACCURATE);
+    uint32_t s = flags & (DEBYE_SINC_MUFU | DEBYE_SINC_RECUR | DEBYE_SINC_ACCURATE | DEBYE_SINC_CENTRED);
     if (s & (s - 1)) return DEBYE_EINVAL;
     if ((flags & DEBYE_FP64) && s) return DEBYE_EINVAL;
     {   // grid hint: sub-bits only with DEBYE_QHINT, start bits only for uniform grids and not both
@@ -194,6 +216,13 @@ int validate(const void *xyz, const void *type, int N, int B, const void *tab, i
         if (sub && !(flags & DEBYE_QHINT)) return DEBYE_EINVAL;
         if (st2 && !(flags & DEBYE_QHINT_UNIFORM)) return DEBYE_EINVAL;
         if (st2 == (DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ)) return DEBYE_EINVAL;
+        // piecewise-uniform hint: excludes the uniform bits; its fields (pieces - 1, K / 8 - 1) only with it, at most 16 each
+        if ((flags & DEBYE_QHINT_PIECES) && (!(flags & DEBYE_QHINT) || sub)) return DEBYE_EINVAL;
+        if (!(flags & DEBYE_QHINT_PIECES) && (flags & piece_fields)) return DEBYE_EINVAL;
+        if ((flags & DEBYE_QHINT_PIECES) && ((((flags >> DEBYE_QHINT_NPIECES_SHIFT) & 31u) >= DEBYE_MAX_PIECES) || (((flags >> DEBYE_QHINT_PIECEK_SHIFT) & 31u) >= 16u)))
+            return DEBYE_EINVAL;
+        // the centred product form needs the pieces: the host sizes the launch from them
+        if ((flags & DEBYE_SINC_CENTRED) && !(flags & DEBYE_QHINT_PIECES)) return DEBYE_EUNSUPPORTED;
     }
     if (N > (1 << 24)) return DEBYE_EUNSUPPORTED;
     if ((int64_t)N * B > ((int64_t)1 << 31)) return DEBYE_EUNSUPPORTED;
@@ -356,6 +385,11 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
 {
     int st = validate(xyz, type, N, B, mode == 0 ? (const void *)fftab : (const void *)q, T, q, M, out, flags);
     if (st) return st;
+    // the tile split has no centred-form instantiation: a pieces hint is dropped there (the device then finds the grid's class itself)
+    if (shard_world > 1 && (flags & DEBYE_QHINT_PIECES)) {
+        if (flags & DEBYE_SINC_CENTRED) return DEBYE_EUNSUPPORTED;
+        flags &= ~(uint32_t)(DEBYE_QHINT | DEBYE_QHINT_PIECES | (31u << DEBYE_QHINT_NPIECES_SHIFT) | (31u << DEBYE_QHINT_PIECEK_SHIFT));
+    }
     std::unique_lock<std::mutex> lock(g_mu);
     DevState *ds;
     if ((st = dev_state(&ds))) return st;
@@ -383,7 +417,7 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
 
     int alt_offered = 0;
     for (int i = 0; i < nch; ++i) if (ch[i].alt_gate == 1) alt_offered = 1;
-    const int hint_class = hint_class_of(flags);
+    const int hint_class = hint_class_of(flags), hint_pieces = hint_pieces_of(flags);
     if (hint_class == 0 && nch == 1 && ch[0].variant == V_RECUR) {
         // hinted q[0] == 0 and a single recurrence launch: it is the one sized for M - 1 indices exactly when that pays
         Choice c2[2];
@@ -392,7 +426,7 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
     const bool pack_here = !pre && (int64_t)N * B <= DEBYE_PACK_IN_SETUP;      // small inputs: the setup CTA gathers too
     // tile split over GPUs: the pairs CTAs of the other ranks do not run here; their records must read as zero
     if (shard_world > 1) CU(cudaMemsetAsync(records, 0, L.sums - L.records, stream));
-    if (!pre) debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, hint_class, xyz, sorted, pack_here ? 1 : 0, weight,
+    if (!pre) debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(plan, type, q, perm, N, T, M, B, alt_offered, hint_class, hint_pieces, xyz, sorted, pack_here ? 1 : 0, weight,
                                                                                 shard_rank, shard_world);
     if (!pack_here) {
         int64_t total = (int64_t)N * B;
@@ -591,7 +625,9 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
     if (N < 1 || M < 1 || M > DEBYE_MAX_Q) return DEBYE_EINVAL;
     // FP64, FP32 with one MUFU.SIN per term (DEBYE_SINC_MUFU, or any grid without a hint), or -- with a grid hint that promises
     // q_k = (k + koff) dq -- the recurrence (DEBYE_SINC_RECUR or automatic)
-    const uint32_t hint_bits = DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ;
+    // (a piecewise-uniform hint, which debye_q_hint may return, is accepted and means "no uniform grid" here)
+    const uint32_t hint_bits = DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ | DEBYE_QHINT_PIECES |
+                               (31u << DEBYE_QHINT_NPIECES_SHIFT) | (31u << DEBYE_QHINT_PIECEK_SHIFT);
     if (flags & ~(uint32_t)(DEBYE_FP64 | DEBYE_SINC_MUFU | DEBYE_SINC_RECUR | hint_bits)) return DEBYE_EINVAL;
     if ((flags & DEBYE_FP64) && (flags & (DEBYE_SINC_MUFU | DEBYE_SINC_RECUR))) return DEBYE_EINVAL;
     if ((flags & DEBYE_SINC_MUFU) && (flags & DEBYE_SINC_RECUR)) return DEBYE_EINVAL;
@@ -698,6 +734,18 @@ int debye_plan_create(debye_plan **out, const int32_t *type, int32_t N, int32_t 
     p->N = N; p->B = B; p->T = T; p->M = M; p->flags = flags; p->buf = nullptr; p->ws = nullptr; p->ws_bytes = 0;
     auto fail = [&](int code) { if (p->buf) cudaFree(p->buf); delete p; return code; };
     if (cudaGetDevice(&p->device) != cudaSuccess) return fail(DEBYE_ECUDA);
+    const uint32_t all_hint_bits = DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ | DEBYE_QHINT_PIECES |
+                                   (31u << DEBYE_QHINT_NPIECES_SHIFT) | (31u << DEBYE_QHINT_PIECEK_SHIFT);
+    // a piecewise-uniform grid (the centred product form) is recognised on a host copy of q: the launch is sized from its pieces
+    uint32_t pieces_hint = 0;
+    {
+        std::vector<float> qh((size_t)M);
+        if (cudaMemcpyAsync(qh.data(), q, (size_t)M * 4, cudaMemcpyDeviceToHost, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
+        if (cudaStreamSynchronize(stream) != cudaSuccess) return fail(DEBYE_ECUDA);
+        const uint32_t hh = debye_q_hint(qh.data(), M);
+        if (hh & DEBYE_QHINT_PIECES) pieces_hint = hh;
+    }
+    if ((flags & DEBYE_SINC_CENTRED) && !pieces_hint) return fail(DEBYE_EUNSUPPORTED);
     size_t o = 0;
     const size_t o_plan = o; o += align_up(sizeof(DevPlan));
     const size_t o_perm = o; o += align_up((size_t)N * 4);
@@ -707,7 +755,8 @@ int debye_plan_create(debye_plan **out, const int32_t *type, int32_t N, int32_t 
     const size_t o_ws = o;
     {   // the plan's own scratch, sized for any grid class the setup step may find (the hint is resolved below)
         size_t need = 0;
-        const uint32_t base_flags = flags & ~(uint32_t)(DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ);
+        const uint32_t base_flags = flags & ~all_hint_bits;
+        if (pieces_hint) need = debye_workspace_bytes(N, B, T, M, base_flags | pieces_hint);
         const uint32_t hints[4] = {DEBYE_QHINT, DEBYE_QHINT | DEBYE_QHINT_UNIFORM, DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0,
                                    DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_STARTDQ};
         for (int i = 0; i < 4; ++i) { const size_t b = debye_workspace_bytes(N, B, T, M, base_flags | hints[i]); if (b > need) need = b; }
@@ -723,7 +772,8 @@ int debye_plan_create(debye_plan **out, const int32_t *type, int32_t N, int32_t 
     if (cudaMemcpyAsync(p->q, q, (size_t)M * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
     if (weight && cudaMemcpyAsync(p->weight, weight, (size_t)N * 4, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
     // the setup step, once; then read its verdict on the grid back (the only synchronisation of the plan's life)
-    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(p->plan, type, p->q, p->perm, N, T, M, B, 1, -3, nullptr, nullptr, 0, p->weight, 0, 1);
+    debye::debye_setup_kernel<<<1, DEBYE_SETUP_THREADS, 0, stream>>>(p->plan, type, p->q, p->perm, N, T, M, B, 1, pieces_hint ? -4 : -3, hint_pieces_of(pieces_hint), nullptr, nullptr, 0,
+                                                                     p->weight, 0, 1);
     DevPlan head;
     if (cudaMemcpyAsync(&head, p->plan, offsetof(DevPlan, seg_off), cudaMemcpyDeviceToHost, stream) != cudaSuccess) return fail(DEBYE_ECUDA);
     if (cudaStreamSynchronize(stream) != cudaSuccess) return fail(DEBYE_ECUDA);
@@ -731,7 +781,8 @@ int debye_plan_create(debye_plan **out, const int32_t *type, int32_t N, int32_t 
     if (head.uniform) hint |= DEBYE_QHINT_UNIFORM;
     if (head.uniform && head.zero_start == 0) hint |= DEBYE_QHINT_START0;
     if (head.uniform && head.zero_start == 1) hint |= DEBYE_QHINT_STARTDQ;
-    p->flags = (flags & ~(uint32_t)(DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ)) | hint;
+    if (pieces_hint) hint = pieces_hint;
+    p->flags = (flags & ~all_hint_bits) | hint;
     *out = p;
     return DEBYE_OK;
 }
@@ -765,11 +816,24 @@ uint32_t debye_q_hint(const float *q_host, int32_t M)
         if (a > qmax) qmax = a;
     }
     const int cls = debye_grid_class(q0, dq, dev, qmax);
+    if (cls == -2 || (cls == -1 && DEBYE_CENT_FOR_GENERAL_START)) {
+        // not one uniform grid from 0 or dq: a few uniform pieces (the centred product form) if the grid has that shape
+        const uint32_t fp = debye_q_hint_pieces(q_host, M);
+        if (fp) return fp;
+    }
     uint32_t f = DEBYE_QHINT;
     if (cls != -2) f |= DEBYE_QHINT_UNIFORM;
     if (cls == 0) f |= DEBYE_QHINT_START0;
     if (cls == 1) f |= DEBYE_QHINT_STARTDQ;
     return f;
+}
+
+uint32_t debye_q_hint_pieces(const float *q_host, int32_t M)
+{
+    if (!q_host || M < 1) return 0;
+    DebyePieces P;
+    if (!debye_find_pieces(q_host, M, P)) return 0;
+    return DEBYE_QHINT | DEBYE_QHINT_PIECES | ((uint32_t)(P.n - 1) << DEBYE_QHINT_NPIECES_SHIFT) | ((uint32_t)(P.K / 8 - 1) << DEBYE_QHINT_PIECEK_SHIFT);
 }
 
 size_t debye_workspace_bytes(int32_t N, int32_t B, int32_t T, int32_t M, uint32_t flags)

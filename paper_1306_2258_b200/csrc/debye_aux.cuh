@@ -20,7 +20,8 @@ namespace debye {
 // If pack_here != 0 the CTA also gathers the coordinates (small N x B: saves the pack launch).
 __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPlan *plan, const int32_t *__restrict__ type, const float *__restrict__ q,
                                                                             int32_t *__restrict__ perm, int N, int T, int M, int B, int alt_offered /* a recurrence launch sized for M - 1 indices exists */,
-                                                                            int hint_class /* -3: no hint; else the grid class the caller promised (debye_grid_class) */,
+                                                                            int hint_class /* -3: no hint; -4: piecewise uniform (hint_pieces); else the grid class the caller promised (debye_grid_class) */,
+                                                                            int hint_pieces /* hint_class == -4: (number of pieces << 8) | K / 8 as debye_find_pieces gives them */,
                                                                             const float *__restrict__ xyz, float4 *__restrict__ sorted, int pack_here, const float *__restrict__ weight,
                                                                             int shard_rank, int shard_world)
 {
@@ -83,6 +84,13 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
         // zero start: q0 == 0 exactly (koff = 0) or q0 == dq to 1e-6 (koff = 1, the paper's own grid q_k = k dq, k >= 1)
         const int koff = cls >= 0 ? cls : -1;
         hint_bad_s = (hint_class != -3 && hint_class != cls) ? 1 : 0;
+        plan->pieces.n = 0;
+        if (hint_class == -4) {
+            // piecewise-uniform grid promised (the centred product form, V_CENT): the same segmentation as the host's, and it
+            // has to give the piece count and accumulator count the launch was sized for.  Serial, O(M): hinted calls only.
+            const bool ok = debye_find_pieces(q, M, plan->pieces) && plan->pieces.n == (hint_pieces >> 8) && plan->pieces.K == 8 * (hint_pieces & 255);
+            hint_bad_s = ok ? 0 : 1;
+        }
         plan->hint_bad = hint_bad_s;
         plan->recur_alt = (koff == 0 && alt_offered) ? 1 : 0;
         plan->N = N; plan->T = T; plan->M = M; plan->B = B; plan->n_tp = T * (T + 1) / 2;
@@ -93,7 +101,7 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
         plan->q0 = q0;
         plan->dq = dq;
         plan->q_small = (s < 3.0e38f) ? s : 0.f;
-        plan->variant_auto = uni ? V_RECUR : V_MUFU;
+        plan->variant_auto = (hint_class == -4) ? V_CENT : (uni ? V_RECUR : V_MUFU);
     }
     __syncthreads();
     // ---- unit prefix per type pair (thread 0, n_tp <= 528 steps) while the other warps sort -----------------------------
@@ -278,6 +286,13 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_epilogue_kernel(con
     const bool bad = (variant == V_RECUR && !plan->uniform) || plan->hint_bad;   // forced recurrence on a non-uniform grid, or a wrong grid hint -> NaN
     const double nan = __longlong_as_double(0x7ff8000000000000LL);
     const double scale = (variant == V_RECUR) ? 0.5 : 1.0;            // the recurrence kernel accumulates 2 sin(q r)/r
+    // centred product form: piece of output k and its local index (pieces are in increasing k)
+    int piece = 0, mloc = 0;
+    if (variant == V_CENT && !bad && k < M) {
+        const int np = plan->pieces.n;
+        while (piece + 1 < np && plan->pieces.off[piece + 1] <= k) ++piece;
+        mloc = k - plan->pieces.off[piece];
+    }
     // recurrence on a grid (k + koff) dq with at most 2 chunks ran in product form (the same test as in the pairs kernel)
     const bool product = variant == V_RECUR && plan->zero_start >= 0 && n_chunks <= 2;
     double I = 0.0;
@@ -303,7 +318,13 @@ __global__ void __launch_bounds__(DEBYE_FINAL_THREADS) debye_epilogue_kernel(con
             else {
                 const double *sp = sums + ((int64_t)b * n_tp + tp) * n_chunks * (int64_t)K;
                 double s = 0.0;
-                if (product) {
+                if (variant == V_CENT) {
+                    // sum_pairs sin(q r)/r = scale (P + sgn Q), resp. scale x the level-0 slot (debye_pairs.cuh cent_slot_of)
+                    int lp, lq; double sgn, sc;
+                    cent_slot_of(K, mloc, lp, lq, sgn, sc);
+                    const double *pp = sp + (int64_t)piece * K;
+                    s = sc * (lq >= 0 ? pp[lp] + sgn * pp[lq] : pp[lp]);
+                } else if (product) {
                     // kappa = idx + 1 = S j + kres with kres in 1..S:  B_kappa = Out[slot(kappa)] + B_{S j - kres}
                     const int Sres = 8 * n_chunks;
                     for (int kap = idx + 1; kap > 0;) {

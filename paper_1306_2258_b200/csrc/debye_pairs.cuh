@@ -399,6 +399,172 @@ __device__ __forceinline__ void prod_tile(u64 (&acc)[K / 2], const float4 *__res
 #undef DEBYE_PROD_ITER
 }
 
+// ---- centred product form (V_CENT): any uniform piece q = q_s + m dq, 1 lane-operation per term, no telescoping -----------
+// With phi = q_c r the angle of a seed and delta a multiple of theta = r dq,
+//     2 cos(delta) * 2 sin(phi)/r = 2 [sin(phi + delta) + sin(phi - delta)]/r        =: P
+//     2 sin(delta) * 2 cos(phi)/r = 2 [sin(phi + delta) - sin(phi - delta)]/r        =: Q
+// so two packed FMA lanes (one into P, one into Q) serve TWO terms, the ones at q_c + delta/r and q_c - delta/r:
+//     sum_pairs 4 sin((q_c +/- delta/r) r)/r = P +/- Q            (taken in FP64 by the epilogue).
+// Per pair: 8 sine and 8 cosine seeds at phi_k0 = (q_c + k0 dq) r, k0 = 0..7 (q_c in the middle of the piece), and L weight
+// pairs 2cos(delta_j), 2sin(delta_j).  K = 16 L + 8: delta_j = 8 j theta and the seeds themselves are level 0 (slots 0..7 hold
+// 2 sin(phi_k0)/r); K = 16 L: delta_j = (8 j - 4) theta, no level 0.  Local index m of the piece (q = q_s + m dq):
+//     K = 16 L + 8:  seed k0 <-> m = 8 L + k0;      (k0, +j) <-> m = 8 L + k0 + 8 j;      (k0, -j) <-> m = 8 L + k0 - 8 j
+//     K = 16 L:                                     (k0, +j) <-> m = 8 L + k0 + 8 (j - 1); (k0, -j) <-> m = 8 L + k0 - 8 j
+// Slots: [level 0: 8] then per level j = 1..L: P_j[k0] (8 slots), Q_j[k0] (8 slots).  Unlike the telescoped form nothing is
+// chained across q, the start q_s is arbitrary (general-start grids, the pieces of a piecewise-uniform grid), and every
+// step of the start-up keeps relative accuracy for small angles (coincident atoms: r = 1e-15 gives the limits 2 q).
+struct CentConst {
+    float wc, wc_lo;         // q of seed k0 = 0, / 2 pi, hi + lo
+    float w1, w1_lo;         // dq / 2 pi
+    float smult;             // 8 (K % 16 == 8) or 4 (K % 16 == 0): fS = smult * theta
+};
+struct CentGeom { float rinv, fc, f1, fS; };
+template <bool W>
+__device__ __forceinline__ void cent_geom(const float4 pj, const float4 pi, const bool ok, const CentConst &cc, CentGeom &g)
+{
+    const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+    const float r2c = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, 1e-30f)));       // as recur_geom
+    const float rinv = rsqrt_mufu(r2c);
+    const float r = r2c * rinv;
+    if constexpr (W) g.rinv = ok ? rinv * pj.w : 0.0f;
+    else g.rinv = ok ? rinv : 0.0f;
+    g.fc = reduce_turns(r, cc.wc, cc.wc_lo);
+    reduce_turns_pair(r, cc.w1, cc.w1_lo, cc.smult, g.f1, g.fS);
+}
+// Stage B.  Us / Uc: the 8 seeds 2 sin(phi_k0)/r and 2 cos(phi_k0)/r as 4 pairs each; Cw[j], Sw[j] = 2 cos(delta_j), 2 sin(delta_j).
+// Seeds: sine and cosine of phi_0 and of theta by the folded polynomials, one exact rotation to phi_1, then the three-term
+// recurrence x_{n+1} = 2cos(theta) x_n - x_{n-1} (six steps: rounding errors grow by at most n^2/2 and are unbiased).  Weights:
+// the same recurrence in steps of 8 theta from the polynomial values at 8 theta (or 4 theta and one doubling).
+template <int K>
+__device__ __forceinline__ void cent_vals(const CentGeom &g, u64 (&Us)[4], u64 (&Uc)[4], float (&Cw)[K / 16 + 1], float (&Sw)[K / 16 + 1])
+{
+    constexpr bool HAS0 = (K % 16) == 8;
+    constexpr int L = K / 16;
+    const Folded hc = sincos_fold(g.fc);
+    float s[8], c[8];
+    s[0] = two_sin_from(hc, g.fc) * g.rinv;
+    c[0] = two_cos_from(hc) * g.rinv;
+    const Folded h1 = sincos_fold(g.f1);
+    const float S1 = two_sin_from(h1, g.f1), C1 = two_cos_from(h1);
+    const float hs = 0.5f * S1, hk = 0.5f * C1;
+    s[1] = fmaf(c[0], hs, s[0] * hk);
+    c[1] = fmaf(-s[0], hs, c[0] * hk);
+#pragma unroll
+    for (int n = 2; n < 8; ++n) { s[n] = fmaf(C1, s[n - 1], -s[n - 2]); c[n] = fmaf(C1, c[n - 1], -c[n - 2]); }
+#pragma unroll
+    for (int a = 0; a < 4; ++a) { Us[a] = pk2(s[2 * a], s[2 * a + 1]); Uc[a] = pk2(c[2 * a], c[2 * a + 1]); }
+    if constexpr (L >= 1) {
+        const Folded hS = sincos_fold(g.fS);
+        const float SS = two_sin_from(hS, g.fS), CS = two_cos_from(hS);
+        Cw[0] = 0.f; Sw[0] = 0.f;
+        Cw[1] = CS; Sw[1] = SS;
+        if constexpr (HAS0) {            // delta_j = 8 j theta: T_0 = (2, 0)
+            if constexpr (L >= 2) { Cw[2] = fmaf(CS, CS, -2.0f); Sw[2] = CS * SS; }
+#pragma unroll
+            for (int j = 3; j <= L; ++j) { Cw[j] = fmaf(CS, Cw[j - 1], -Cw[j - 2]); Sw[j] = fmaf(CS, Sw[j - 1], -Sw[j - 2]); }
+        } else {                         // delta_j = (8 j - 4) theta: step 8 theta, T_0 = (2cos(4 theta), -2 sin(4 theta))
+            const float C8 = fmaf(CS, CS, -2.0f);
+            if constexpr (L >= 2) { Cw[2] = fmaf(C8, CS, -CS); Sw[2] = fmaf(C8, SS, SS); }
+#pragma unroll
+            for (int j = 3; j <= L; ++j) { Cw[j] = fmaf(C8, Cw[j - 1], -Cw[j - 2]); Sw[j] = fmaf(C8, Sw[j - 1], -Sw[j - 2]); }
+        }
+    } else { Cw[0] = 0.f; Sw[0] = 0.f; }
+}
+// Stage C: K/2 independent packed operations.
+template <int K>
+__device__ __forceinline__ void cent_hot(u64 (&acc)[K / 2], const u64 (&Us)[4], const u64 (&Uc)[4], const float (&Cw)[K / 16 + 1], const float (&Sw)[K / 16 + 1])
+{
+    constexpr bool HAS0 = (K % 16) == 8;
+    constexpr int L = K / 16, B0 = HAS0 ? 4 : 0;
+    if constexpr (HAS0) {
+#pragma unroll
+        for (int a = 0; a < 4; ++a) acc[a] = add2(acc[a], Us[a]);
+    }
+#pragma unroll
+    for (int j = 1; j <= L; ++j) {
+        const u64 wc = pk2(Cw[j], Cw[j]), ws = pk2(Sw[j], Sw[j]);
+#pragma unroll
+        for (int a = 0; a < 4; ++a) acc[B0 + 8 * (j - 1) + a] = fma2(wc, Us[a], acc[B0 + 8 * (j - 1) + a]);
+#pragma unroll
+        for (int a = 0; a < 4; ++a) acc[B0 + 8 * (j - 1) + 4 + a] = fma2(ws, Uc[a], acc[B0 + 8 * (j - 1) + 4 + a]);
+    }
+}
+// where local index m of a piece lives: slot of P (or of the level-0 seed), slot of Q (-1: none), sign of Q, and the factor
+// that turns the slot sum(s) into sum_pairs sin(q r)/r.  Used by the epilogue.
+__host__ __device__ inline void cent_slot_of(int K, int m, int &lp, int &lq, double &sgn, double &scale)
+{
+    const bool has0 = (K % 16) == 8;
+    const int L = K / 16, b0 = has0 ? 8 : 0;
+    if (has0 && m >= 8 * L && m < 8 * L + 8) { lp = m - 8 * L; lq = -1; sgn = 0.0; scale = 0.5; return; }
+    int j, k0;
+    if (m >= 8 * L) { const int d = m - 8 * L - (has0 ? 8 : 0); j = d / 8 + 1; k0 = d % 8; sgn = 1.0; }
+    else { const int d = 8 * L - 1 - m; j = d / 8 + 1; k0 = 7 - d % 8; sgn = -1.0; }
+    lp = b0 + 16 * (j - 1) + k0; lq = lp + 8; scale = 0.25;
+}
+// pairs per iteration and occupancy thresholds, measured on B200 (10 000 atoms; T pair.q/s, one pair per iteration -> two):
+// K = 104: 10.8 -> 11.6, 2 x K = 56: 7.75 -> 8.45, K = 128: 12.0 -> 13.1; K = 40 at 4 CTAs/SM 6.83, at 3 CTAs/SM 7.00;
+// K = 104 at 3 CTAs/SM (168 registers) 9.9 against 11.6 at 2
+#ifndef DEBYE_CENT_NP
+#define DEBYE_CENT_NP 2
+#endif
+#ifndef DEBYE_CK4
+#define DEBYE_CK4 24
+#endif
+#ifndef DEBYE_CK3
+#define DEBYE_CK3 88
+#endif
+__host__ __device__ constexpr int cent_min_ctas(int K) { return K <= DEBYE_CK4 ? 4 : (K <= DEBYE_CK3 ? 3 : 2); }
+// One tile, the same three-stage pipeline and masking as prod_tile.
+template <int K, bool W>
+__device__ __forceinline__ void cent_tile(u64 (&acc)[K / 2], const float4 *__restrict__ tile, const int jj0, const int cnt, const float4 pi,
+                                          const bool ivalid, const bool diag, const int i_local, const int jl0, const CentConst &cc, const int jfree)
+{
+    constexpr int NP = DEBYE_CENT_NP, LW = K / 16 + 1;
+    if (jj0 >= cnt) return;
+    const int jmin = ivalid ? (diag ? max(0, i_local + 1 - jl0) : 0) : 0x7fffffff;
+    auto geom_masked = [&](const int jbase, CentGeom (&g)[NP]) {
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            const int j = jbase + p;
+            cent_geom<W>(tile[min(j, cnt - 1)], pi, j >= jmin && j < cnt, cc, g[p]);
+        }
+    };
+    auto geom_free = [&](const int jbase, CentGeom (&g)[NP]) {
+#pragma unroll
+        for (int p = 0; p < NP; ++p) cent_geom<W>(tile[jbase + p], pi, true, cc, g[p]);
+    };
+    u64 Us[NP][4], Uc[NP][4];
+    float Cw[NP][LW], Sw[NP][LW];
+    CentGeom gn[NP];
+    geom_masked(jj0, gn);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) cent_vals<K>(gn[p], Us[p], Uc[p], Cw[p], Sw[p]);
+    geom_masked(jj0 + NP, gn);
+#define DEBYE_CENT_ITER(GEOM)                                                                                   \
+    {                                                                                                           \
+        u64 Usn[NP][4], Ucn[NP][4];                                                                             \
+        float Cwn[NP][LW], Swn[NP][LW];                                                                         \
+        _Pragma("unroll") for (int p = 0; p < NP; ++p) cent_vals<K>(gn[p], Usn[p], Ucn[p], Cwn[p], Swn[p]);     \
+        GEOM(jj + 2 * NP, gn);                                                                                  \
+        _Pragma("unroll") for (int p = 0; p < NP; ++p) cent_hot<K>(acc, Us[p], Uc[p], Cw[p], Sw[p]);            \
+        _Pragma("unroll") for (int p = 0; p < NP; ++p) {                                                        \
+            _Pragma("unroll") for (int a = 0; a < 4; ++a) { Us[p][a] = Usn[p][a]; Uc[p][a] = Ucn[p][a]; }       \
+            _Pragma("unroll") for (int j = 0; j < LW; ++j) { Cw[p][j] = Cwn[p][j]; Sw[p][j] = Swn[p][j]; }      \
+        }                                                                                                       \
+    }
+    int jj = jj0;
+#pragma unroll 1
+    for (int phase = 0; phase < 2; ++phase) {
+        const int stop = (phase == 0) ? ((jfree > cnt) ? cnt : min(cnt, max(jj0, jfree - 2 * NP))) : cnt;
+#pragma unroll 1
+        for (; jj < stop; jj += NP) DEBYE_CENT_ITER(geom_masked)
+        if (phase == 0) {
+            for (; jj + 3 * NP <= cnt; jj += NP) DEBYE_CENT_ITER(geom_free)
+        }
+    }
+#undef DEBYE_CENT_ITER
+}
+
 // ---- chain form (RM_G) ----------------------------------------------------------------------------------------------
 // Stage B (values): Bv = w_0 (the 8 residues), A = w_{-1}, cS = 2 cos(S theta).
 // General start (q_0 not a small multiple of dq, or more than 2 chunks): 8 accurate sines at k' = base .. base+7
@@ -550,7 +716,7 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
 __device__ unsigned long long debye_trace[3 * 4096];
 #endif
 template <int K, int VAR, bool W, bool SH = false>
-__global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR ? recur_min_ctas(K) : (K <= 64 ? 4 : (K <= 112 ? 3 : 2)))) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
+__global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR ? recur_min_ctas(K) : (VAR == V_CENT ? cent_min_ctas(K) : (K <= 64 ? 4 : (K <= 112 ? 3 : 2))))) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
                                                                double *__restrict__ records, int n_chunks, int is_auto, float theta_min, int alt_gate)
 {
     pdl_wait();      // programmatic dependent launch: everything before us in the call has completed (debye_plan.cuh)
@@ -569,7 +735,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
     __shared__ __align__(8) u64 mbar[2];
     __shared__ float tbuf[F64 ? 1 : NW][F64 ? 1 : 32][F64 ? 1 : 33];
     __shared__ double wsum[NW][K];
-    __shared__ float qs[(VAR == V_RECUR) ? 1 : K];
+    __shared__ float qs[(VAR == V_RECUR || VAR == V_CENT) ? 1 : K];
     __shared__ float wtab[16];                        // recurrence, general start: start frequencies (hi[8], lo[8])    // direct variants: q of each local slot (0 for padding)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -615,6 +781,9 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
     float cut2 = 0.f;
     int mode = RM_G, ch_cur = 0;
     (void)mode; (void)dq_d; (void)q0_d; (void)koff; (void)cut2;
+    CentConst cc;
+    cc.wc = cc.wc_lo = cc.w1 = cc.w1_lo = 0.f; cc.smult = 8.0f;
+    (void)cc;
 
     float wi = 1.0f;                  // weighted instantiations: weight of this thread's i atom (accumulators are flushed per row)
     (void)wi;
@@ -722,6 +891,14 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                     rc.w4 = (float)w4_d; rc.w4_lo = (float)(w4_d - (double)rc.w4);
                     const float rcut = theta_min / fabsf((float)dq_d);
                     rc.cut2 = rcut * rcut;
+                } else if constexpr (VAR == V_CENT) {
+                    // piece ch of the grid: q = q0 + m dq; seed k0 = 0 sits at local index mc (cent_slot_of)
+                    constexpr int mc = (K % 16 == 8) ? 8 * (K / 16) : 8 * (K / 16) - 4;
+                    const double pdq = plan->pieces.dq[ch];
+                    const double wc_d = fma((double)mc, pdq, plan->pieces.q0[ch]) * 0.15915494309189535, w1_d = pdq * 0.15915494309189535;
+                    cc.wc = (float)wc_d; cc.wc_lo = (float)(wc_d - (double)cc.wc);
+                    cc.w1 = (float)w1_d; cc.w1_lo = (float)(w1_d - (double)cc.w1);
+                    cc.smult = (K % 16 == 8) ? 8.0f : 4.0f;
                 } else {
                     __syncthreads();
                     if (tid < K) { int k = ch * K + tid; qs[tid] = (k < M) ? qv[k] : 0.0f; }
@@ -760,7 +937,11 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
             // on the diagonal, a warp whose every i is >= j has nothing to do for that j: start later
             int jj0 = 0;
             if (diag) { int first_i = row * DEBYE_IB + warp * 32; jj0 = max(0, first_i + 1 - jl0); }
-            if constexpr (VAR == V_RECUR) {
+            if constexpr (VAR == V_CENT) {
+                const int w_last_i = row * DEBYE_IB + warp * 32 + 31;
+                const int jfree = (w_last_i >= n_i) ? 0x7fffffff : (diag ? max(0, w_last_i + 1 - jl0) : 0);
+                if (row * DEBYE_IB + warp * 32 < n_i) cent_tile<K, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, cc, jfree);
+            } else if constexpr (VAR == V_RECUR) {
                 // first tile index from which every lane of this warp pairs with every j: 0 off the diagonal, behind the
                 // warp's last i atom on it; never if some lane has no i atom (ragged last row)
                 const int w_last_i = row * DEBYE_IB + warp * 32 + 31;

@@ -8,6 +8,7 @@
 //   contiguous ranges, so the assignment is static (bitwise reproducible) and balanced to one j atom.
 #pragma once
 #include <cstdint>
+#include <cmath>
 
 #define DEBYE_MAX_TYPES_I 32
 #define DEBYE_MAX_TP (DEBYE_MAX_TYPES_I * (DEBYE_MAX_TYPES_I + 1) / 2)
@@ -15,7 +16,17 @@
 #define DEBYE_JT 512          // j atoms per shared-memory tile (8 KB, one cp.async.bulk); 2 buffers per CTA
 #define DEBYE_TILE_PAD 8      // readable (finite) entries behind each buffer: the recurrence reads two groups ahead
 
-enum DebyeVariant : int32_t { V_NONE = 0, V_F64 = 1, V_MUFU = 2, V_RECUR = 3, V_ACCURATE = 4 };
+enum DebyeVariant : int32_t { V_NONE = 0, V_F64 = 1, V_MUFU = 2, V_RECUR = 3, V_ACCURATE = 4, V_CENT = 5 };
+
+// Piecewise-uniform grids (V_CENT, the centred product form of debye_pairs.cuh): q is a sequence of at most DEBYE_MAX_PIECES
+// pieces, piece p = the points off[p] .. off[p] + cnt[p] - 1 with q = q0[p] + m dq[p] (m the local index), cnt[p] <= K <= 128.
+#define DEBYE_MAX_PIECES 16
+#define DEBYE_PIECE_KCAP 128
+struct DebyePieces {
+    int32_t n, K;                 // number of pieces; accumulators per thread (a multiple of 8 >= the longest piece)
+    int32_t off[DEBYE_MAX_PIECES], cnt[DEBYE_MAX_PIECES];
+    double q0[DEBYE_MAX_PIECES], dq[DEBYE_MAX_PIECES];
+};
 
 struct DevPlan {
     int32_t N, T, M, B;
@@ -31,6 +42,7 @@ struct DevPlan {
     int32_t shard_rank, shard_world;   // tile split of ONE structure over GPUs (debye_partials_shard): pairs CTA c works iff
                                   // c % shard_world == shard_rank; the other CTAs leave their (zeroed) records alone
     int64_t U1;                   // units per conformer and per q-chunk
+    DebyePieces pieces;           // piecewise-uniform grid (only filled in when the caller's hint promised one)
     double sw[DEBYE_MAX_TYPES_I];             // weighted calls: sum of w_j over the atoms of each type ...
     double sw2[DEBYE_MAX_TYPES_I];            // ... and of w_j^2 (self terms; q = 0 pair sums)
     int32_t seg_off[DEBYE_MAX_TYPES_I + 1];   // sorted-array offset of each type segment
@@ -62,6 +74,45 @@ __host__ __device__ inline int debye_grid_class(double q0, double dq, float dev,
     if (q0 == 0.0) return 0;
     if (fabs(q0 / dq - 1.0) <= 1e-6) return 1;
     return -1;
+}
+
+// Piecewise-uniform grids: greedy maximal runs of equal steps (a loose test on the step finds the run, the 1.5-ulp criterion of
+// debye_grid_class with the step refitted through the run's end points then has to hold for every point of it), runs longer
+// than DEBYE_PIECE_KCAP cut into equal pieces.  Double arithmetic with fma and IEEE division only: the host (debye_q_hint)
+// and the device (debye_setup_kernel) get the same pieces from the same floats.  false: not piecewise uniform, or too many pieces.
+__host__ __device__ inline bool debye_find_pieces(const float *q, int M, DebyePieces &P)
+{
+    P.n = 0; P.K = 8;
+    int maxcnt = 0, s = 0;
+    while (s < M) {
+        int e = s + 1;
+        double dq = 0.0;
+        if (e < M) {
+            const double d0 = (double)q[s + 1] - (double)q[s];
+            const double a0 = fmax(fmax(fabs((double)q[s]), fabs((double)q[s + 1])), fabs(d0));   // d0 carries the rounding of the run's first two points
+            e = s + 2;
+            while (e < M) {
+                const double a = fmax(fmax(fabs((double)q[e]), fabs((double)q[e - 1])), a0);
+                if (fabs(((double)q[e] - (double)q[e - 1]) - d0) > 4.8e-7 * a) break;      // 4 float ulps: each difference carries up to 2
+                ++e;
+            }
+            dq = ((double)q[e - 1] - (double)q[s]) / (double)(e - 1 - s);
+            for (int k = s; k < e; ++k)
+                if (debye_grid_dev((double)q[k], k - s, (double)q[s], dq) > 1.8e-7f) return false;
+        }
+        const int n = e - s, np = (n + DEBYE_PIECE_KCAP - 1) / DEBYE_PIECE_KCAP, per = (n + np - 1) / np;
+        for (int x = 0; x < np; ++x) {
+            if (P.n == DEBYE_MAX_PIECES) return false;
+            const int o = x * per, c = (per < n - o) ? per : n - o;
+            P.off[P.n] = s + o; P.cnt[P.n] = c; P.q0[P.n] = fma((double)o, dq, (double)q[s]); P.dq[P.n] = dq;
+            ++P.n;
+            if (c > maxcnt) maxcnt = c;
+        }
+        s = e;
+    }
+    P.K = (maxcnt + 7) / 8 * 8;
+    if (P.K < 8) P.K = 8;
+    return true;
 }
 
 // ---- programmatic dependent launch (PDL) ------------------------------------------------------------------------

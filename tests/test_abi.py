@@ -55,6 +55,14 @@ def test_argument_validation_happens_before_cuda():
     assert L.debye_profile(p, p, 10, p, 2, p, 5, p, 1 << 9, None) == EINVAL                   # hint sub-bit without DEBYE_QHINT
     assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 8) | (1 << 10), None) == EINVAL     # start bit without uniform
     assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 8) | (1 << 9) | (1 << 10) | (1 << 11), None) == EINVAL
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, 1 << 12, None) == EINVAL                  # pieces hint without DEBYE_QHINT
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 8) | (1 << 12) | (1 << 9), None) == EINVAL   # pieces and uniform
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 8) | (3 << 16), None) == EINVAL     # piece count without the pieces bit
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 8) | (1 << 12) | (16 << 16), None) == EINVAL  # more than 16 pieces
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 8) | (1 << 12) | (16 << 21), None) == EINVAL  # more than 128 accumulators
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 5) | (1 << 3), None) == EINVAL      # centred and recurrence
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, 1 << 5, None) == EUNSUP                   # centred form without the pieces hint
+    assert L.debye_profile(p, p, 10, p, 2, p, 5, p, (1 << 5) | (1 << 8) | (1 << 9), None) == EUNSUP
     assert L.debye_profile(p, p, (1 << 24) + 1, p, 2, p, 5, p, 0, None) == EUNSUP
     assert L.debye_profile_batch(p, p, 10, 0, p, 2, p, 5, p, 0, None) == EINVAL
     assert L.debye_profile_host(None, p, 10, p, 2, p, 5, p, 0, None) == EINVAL
@@ -111,22 +119,41 @@ def test_q_hint_classifies_grids_on_the_host():
     H, U, Z, D = 1 << 8, 1 << 9, 1 << 10, 1 << 11
     assert binding.q_hint(wl.q_grid(0.5, 101)) == H | U | Z                    # starts at 0
     assert binding.q_hint(wl.q_grid(1.0, 50, 0.02)) == H | U | D               # the paper's grid k/50, k = 1..50
-    assert binding.q_hint(wl.q_grid(0.9, 64, 0.3)) == H | U                    # uniform, general start
-    assert binding.q_hint(wl.q_grid(0.3, 31)[::-1].copy()) == H | U            # descending
-    assert binding.q_hint(np.array([0.0, 0.1, 0.25], np.float32)) == H         # not uniform
+    P = 1 << 12
+
+    def pieces(n, K):
+        return H | P | ((n - 1) << 16) | ((K // 8 - 1) << 21)
+    # uniform with a general start, descending, or a few uniform pieces: the piecewise-uniform hint (centred product form) with
+    # the number of pieces and the accumulators per thread the launch is sized for
+    assert binding.q_hint(wl.q_grid(0.9, 64, 0.3)) == pieces(1, 64)
+    assert binding.q_hint(wl.q_grid(0.3, 31)[::-1].copy()) == pieces(1, 32)
+    assert binding.q_hint(wl.q_grid(0.9, 200, 0.3)) == pieces(2, 104)          # more than 128 points: equal pieces
+    assert binding.q_hint(np.array([0.0, 0.1, 0.25], np.float32)) == pieces(2, 8)
+    saxs_waxs = np.concatenate([np.arange(51) * 0.005, 0.25 + 0.01 * np.arange(1, 51)]).astype(np.float32)
+    assert binding.q_hint(saxs_waxs) == pieces(2, 56) and binding.pieces_of(binding.q_hint(saxs_waxs)) == (2, 56)
+    assert binding.q_hint(np.delete(wl.q_grid(0.5, 101), 37)) == pieces(2, 64)  # a dropped point: 37 + 63
+    assert binding.q_hint_pieces(wl.q_grid(0.5, 101)) == pieces(1, 104)        # any uniform grid can be forced into the centred form ...
+    assert binding.q_hint(wl.q_grid(0.5, 101)) == H | U | Z                    # ... but from 0 or dq the telescoped form is preferred
+    rng = np.random.default_rng(5)
+    assert binding.q_hint(np.sort(rng.uniform(0, 0.7, 40)).astype(np.float32)) == H      # no structure: the MUFU kernel
+    assert binding.q_hint_pieces(np.sort(rng.uniform(0, 0.7, 40)).astype(np.float32)) == 0
+    assert binding.pieces_of(H | U) == (0, 0)
     assert binding.q_hint(np.array([0.0], np.float32)) == H | U | Z
+    assert binding.q_hint(np.array([0.3], np.float32)) in (H | U | D, pieces(1, 8))
     # a grid is uniform if every q[k] is within 1.5 float ulps of ITSELF of the line through the end points: grids rounded once
     # from the exact line pass at every size and range, a jitter of 2 ulps of q_max at low k does not
     for qmax, M, qmin in ((0.5, 101, 0.0), (1.0, 50, 0.02), (0.3, 128, 0.0), (1.7, 4096, 0.0), (0.9, 64, 0.3), (25.0, 999, 0.0)):
-        assert binding.q_hint(wl.q_grid(qmax, M, qmin)) & U, (qmax, M, qmin)
-        assert binding.q_hint(np.linspace(qmin, qmax, M, dtype=np.float32)) & U
-        assert binding.q_hint((np.arange(M) * np.float32((qmax - qmin) / (M - 1)) + np.float32(qmin)).astype(np.float32)) & U or M > 500
+        assert binding.q_hint(wl.q_grid(qmax, M, qmin)) & (U | P), (qmax, M, qmin)
+        assert binding.q_hint(np.linspace(qmin, qmax, M, dtype=np.float32)) & (U | P)
+        assert binding.q_hint((np.arange(M) * np.float32((qmax - qmin) / (M - 1)) + np.float32(qmin)).astype(np.float32)) & (U | P) or M > 500
     g = wl.q_grid(0.5, 101)
     j = g.copy(); j[3] = np.nextafter(np.nextafter(j[3], np.float32(1)), np.float32(1)); j[7] += 2 * np.spacing(np.float32(0.5))
-    assert binding.q_hint(j) == H                                             # not uniform: the MUFU kernel takes q as it is
+    assert not binding.q_hint(j) & U                                          # not uniform as a whole ...
+    assert binding.q_hint(j) == pieces(3, 96)                                 # ... but three uniform pieces (7 + the lone jittered point + 93)
     L = binding.lib()
     assert L.debye_q_hint(None, 5) == 0
     # with a hint exactly one pairs instantiation is launched
     assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H | U | Z) == {"n_launches": 4, "q_chunk": 100, "n_chunks": 1}
     assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H | U | D) == {"n_launches": 4, "q_chunk": 104, "n_chunks": 1}
     assert binding.launch_info(10000, 1, 5, 101, "auto", hint=H)["n_launches"] == 4
+    assert binding.launch_info(10000, 1, 5, 101, "auto", hint=pieces(2, 56)) == {"n_launches": 4, "q_chunk": 56, "n_chunks": 2}

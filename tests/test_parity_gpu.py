@@ -335,6 +335,8 @@ def test_grid_hints_select_one_launch_and_are_checked(db):
         if db.launch_info(base.N, 1, 3, len(qg), "auto", hint=hints[name])["n_launches"] == 1:      # the fused small-structure launch
             assert name in ("zero", "dq", "zero_129") and rel(hinted, plain) <= 2e-6 and rel(hinted, ref) <= TOL32
             assert hinted.tobytes() == db.debye_profile(x, t, fd, qd, hint=hints[name]).cpu().numpy().tobytes()
+        elif db.pieces_of(hints[name])[0]:      # general start: the hint selects the centred product form, the unhinted call runs the chain
+            assert name == "offset" and rel(hinted, plain) <= 2e-6 and rel(hinted, ref) <= TOL32
         else:
             assert hinted.tobytes() == plain.tobytes(), name
         for other, h in hints.items():
@@ -407,7 +409,9 @@ def test_plan_execute_equals_the_plain_calls_bit_for_bit(db):
     with weights, and for a batch."""
     import torch
     rng = np.random.default_rng(21)
-    grids = [wl.q_grid(0.5, 101), wl.q_grid(1.0, 50, 0.02), np.sort(rng.uniform(0.01, 0.7, 33)).astype(np.float32)]
+    grids = [wl.q_grid(0.5, 101), wl.q_grid(1.0, 50, 0.02), np.sort(rng.uniform(0.01, 0.7, 33)).astype(np.float32),
+             np.concatenate([np.arange(41) * 0.005, 0.2 + 0.02 * np.arange(1, 31)]).astype(np.float32),      # two uniform pieces
+             wl.q_grid(0.9, 150, 0.3)]                                                                       # general start, two pieces
     for qg in grids:
         base = wl.small_random(60, 900, 4, 8)
         f = wl.gaussian_form_factors(5, 4, qg)
@@ -485,6 +489,124 @@ def test_grid_jittered_by_two_ulps_is_taken_as_it_is(db):
     assert rel(gpu_profile(db, wj), ref) <= 1e-5
     assert gpu_profile(db, wj).tobytes() == gpu_profile(db, wj, "mufu").tobytes()
     assert np.isnan(gpu_profile(db, wj, "recur")).all()                      # forced recurrence on a non-uniform grid: NaN
+
+
+def _regrid(w, q, seed=77):
+    q = np.ascontiguousarray(q, dtype=np.float32)
+    return wl.Workload(w.name + "_regrid", w.xyz, w.type, wl.gaussian_form_factors(seed, w.T, q), q)
+
+
+PIECE_GRIDS = [
+    # name, grid, (pieces, accumulators per thread) the hint must carry
+    ("saxs_waxs", np.concatenate([np.arange(51) * 0.005, 0.25 + 0.01 * np.arange(1, 51)]), (2, 56)),
+    ("dropped_point", np.delete(wl.q_grid(0.5, 101), 37), (2, 64)),
+    ("three_ranges", np.concatenate([np.arange(1, 41) * 0.002, 0.08 + 0.005 * np.arange(1, 41), 0.28 + 0.02 * np.arange(1, 30)]), (3, 40)),
+    ("general_start", wl.q_grid(0.9, 64, 0.3), (1, 64)),
+    ("general_start_200", 0.0123 + np.arange(200) * 0.004, (2, 104)),
+    ("descending", wl.q_grid(0.3, 31)[::-1].copy(), (1, 32)),
+    ("through_zero", np.linspace(-0.3, 0.3, 31), (1, 32)),
+    ("lone_points", np.array([0.0, 0.1, 0.25]), (2, 8)),
+    ("repeated_q", np.array([0.1, 0.1, 0.1, 0.2, 0.3, 0.4]), (2, 8)),
+    ("one_point", np.array([0.37]), None),
+]
+
+
+def test_piecewise_uniform_grids_run_the_centred_product_form(db):
+    """DEBYE_QHINT_PIECES / DEBYE_SINC_CENTRED (include/debye.h): a grid made of a few uniform
+    pieces -- SAXS + WAXS ranges, a dropped point, a general start -- runs the centred product form (debye_pairs.cuh), one
+    launch, against the oracle and against the MUFU kernel, which takes any grid."""
+    import torch
+    base = wl.small_random(50, 1500, 4, 8)
+    for name, qg, want in PIECE_GRIDS:
+        w = _regrid(base, qg)
+        h = db.q_hint(w.q)
+        if want is not None:
+            assert db.pieces_of(h) == want, (name, hex(h), db.pieces_of(h))
+        ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)
+        x, t, f, q = to_dev(w)
+        hp = db.q_hint_pieces(w.q)
+        assert hp != 0
+        I = db.debye_profile(x, t, f, q, variant="centred", hint=hp).cpu().numpy()
+        assert rel(I, ref) <= TOL32, (name, rel(I, ref))
+        assert I.tobytes() == db.debye_profile(x, t, f, q, variant="centred", hint=hp).cpu().numpy().tobytes()     # bitwise reproducible
+        if db.pieces_of(h)[0]:
+            assert h == hp
+            assert db.debye_profile(x, t, f, q, hint=h).cpu().numpy().tobytes() == I.tobytes()      # automatic mode takes it from the hint
+            assert db.launch_info(w.N, 1, w.T, w.M, "auto", hint=h)["n_launches"] == 4            # setup (+ pack), ONE pairs launch, reduce, epilogue
+        assert rel(db.debye_profile(x, t, f, q, variant="mufu").cpu().numpy(), I) <= 1e-5
+        assert rel(db.debye_profile(x, t, f, q).cpu().numpy(), ref) <= TOL32                        # no hint: whatever the device chooses
+    # every accumulator count (both layouts: K = 16 L + 8 with the seeds as level 0, K = 16 L without), general start
+    for K in range(8, 129, 8):
+        for M in (K, K - 7 if K > 8 else 1):
+            w = _regrid(wl.small_random(51, 600, 3, 8), 0.0371 + (0.55 / 128) * np.arange(M))
+            hp = db.q_hint_pieces(w.q)
+            assert db.pieces_of(hp) == (1, K)
+            x, t, f, q = to_dev(w)
+            I = db.debye_profile(x, t, f, q, variant="centred", hint=hp).cpu().numpy()
+            assert rel(I, orc.debye_sym(w.xyz, w.type, w.fftab, w.q)) <= TOL32, (K, M)
+    # weights, a batch, the host entry
+    rng = np.random.default_rng(3)
+    qg = PIECE_GRIDS[0][1]
+    w = _regrid(wl.small_random(52, 900, 4, 8), qg)
+    h = db.q_hint(w.q)
+    x, t, f, q = to_dev(w)
+    wt = (rng.uniform(0.3, 2.0, w.N) * np.where(rng.uniform(size=w.N) < 0.2, -1, 1)).astype(np.float32)
+    refw, A = orc.debye_sym(w.xyz, w.type, w.fftab, w.q, weight=wt, return_abs=True)
+    Iw = db.debye_profile_weighted(x, t, torch.from_numpy(wt).cuda(), f, q, hint=h).cpu().numpy()
+    assert float(np.max(np.abs(Iw - refw) / np.maximum(np.abs(refw), 1e-2 * A))) <= TOL32
+    wb = wl.cfg4(B=4, N=500)
+    wb = wl.Workload("batch_regrid", wb.xyz, wb.type, wl.gaussian_form_factors(9, wb.T, qg.astype(np.float32)), qg.astype(np.float32))
+    xb, t, f, q = to_dev(wb)
+    Ib = db.debye_profile_batch(xb, t, f, q, hint=h).cpu().numpy()
+    assert rel(Ib, orc.debye_batch(wb.xyz, wb.type, wb.fftab, wb.q)) <= TOL32
+    for b in range(4):       # same terms, other CTA ranges than in the batch: equal to rounding
+        one = db.debye_profile(xb[b].contiguous(), t, f, q, hint=h).cpu().numpy()
+        assert rel(Ib[b], one) <= 1e-6
+    Ih = db.debye_profile_host(wb.xyz[0], wb.type, wb.fftab, wb.q, hint=h)
+    assert Ih.tobytes() == db.debye_profile(xb[0].contiguous(), t, f, q, hint=h).cpu().numpy().tobytes()
+
+
+def test_piecewise_hint_is_checked_on_the_device_and_degenerate_pairs_keep_their_limits(db):
+    import torch
+    base = wl.small_random(53, 500, 3, 8)
+    grids = {n: np.ascontiguousarray(g, dtype=np.float32) for n, g, _ in PIECE_GRIDS[:5]}
+    hints = {n: db.q_hint(g) for n, g in grids.items()}
+    assert len(set(hints.values())) == len(hints)
+    for n, g in grids.items():
+        w = _regrid(base, g)
+        x, t, f, q = to_dev(w)
+        for other, h in hints.items():
+            I = db.debye_profile(x, t, f, q, hint=h).cpu().numpy()
+            assert np.isnan(I).all() == (other != n), (n, other)            # a hint sized for another grid: NaN, never a wrong number
+    # a grid with the promised piece count and size but other break points is still right: the device cuts q itself
+    ga = np.concatenate([np.arange(51) * 0.005, 0.25 + 0.01 * np.arange(1, 51)]).astype(np.float32)
+    gb = np.concatenate([np.arange(50) * 0.005, 0.245 + 0.01 * np.arange(1, 52)]).astype(np.float32)
+    assert db.q_hint(ga) == db.q_hint(gb)
+    w = _regrid(base, gb)
+    x, t, f, q = to_dev(w)
+    assert rel(db.debye_profile(x, t, f, q, hint=db.q_hint(ga)).cpu().numpy(), orc.debye_sym(w.xyz, w.type, w.fftab, w.q)) <= TOL32
+    # all atoms coincident: I = (sum f)^2 at every q (r = 0: every seed and weight takes its limit).  The centred form gets a term
+    # below the piece's centre q_c as a difference (P - Q)/4 of sums of size ~q_c, so a term at q carries ~1e-7 q_c/q relative
+    # error: random over pairs in a real structure, coherent here where all pairs are the same pair (q_c/q = 24 at the first
+    # non-zero q of this grid; the telescoped form and the MUFU kernel hold 1e-6, test_degenerate_inputs)
+    qg = grids["saxs_waxs"]
+    f = wl.gaussian_form_factors(1, 3, qg)
+    typ = np.array([0, 1, 2, 2, 1, 0, 0], np.int32)
+    wc = wl.Workload("coin", np.tile(np.array([[1.5, -2.0, 0.25]], np.float32), (7, 1)), typ, f, qg)
+    x, t, fd, q = to_dev(wc)
+    assert rel(db.debye_profile(x, t, fd, q, hint=hints["saxs_waxs"]).cpu().numpy(), f.astype(np.float64)[typ].sum(0) ** 2) <= 5e-6
+    # two atoms, closed form I = f1^2 + f2^2 + 2 f1 f2 sin(qd)/(qd), distances from far below one grid step to 3000 A
+    f2 = np.stack([np.linspace(6, 2, len(qg)), np.linspace(8, 1, len(qg))]).astype(np.float32)
+    worst = 0.0
+    for d in [0.0, 1e-3, 0.05, 0.3, 0.81, 1.37, 3.7, 9.9, 31.4159, 78.54, 400.3, 1234.5, 3000.0]:
+        xyz = np.array([[0.5, 0.25, -1.0], [0.5, 0.25, -1.0 + d]], np.float32)
+        dd = float(np.float64(xyz[1, 2]) - np.float64(xyz[0, 2]))
+        qq = qg.astype(np.float64)
+        sinc = np.where(qq * dd == 0, 1.0, np.sin(qq * dd) / np.where(qq * dd == 0, 1.0, qq * dd))
+        want = f2[0].astype(np.float64) ** 2 + f2[1].astype(np.float64) ** 2 + 2 * f2[0].astype(np.float64) * f2[1] * sinc
+        x, t, fd, q = to_dev(wl.Workload("two", xyz, np.array([0, 1], np.int32), f2, qg))
+        worst = max(worst, rel(db.debye_profile(x, t, fd, q, hint=hints["saxs_waxs"]).cpu().numpy(), want))
+    assert worst <= TOL32, worst
 
 
 def test_non_finite_input_propagates_and_does_not_poison_later_calls(db):

@@ -39,12 +39,16 @@ NCU_TRAFFIC_SOURCE = "profiles/r02_ncu_full_pairs_cfg{2,4,5}.txt (ncu --set full
 TABLE1 = {f"table1_{n}": n for n in (1000, 2000, 4000, 10000, 20000, 40000, 100000)}       # the paper's Table I rows
 
 
-def make_workload(name: str, rank: int = 0):
+def make_workload(name: str, rank: int = 0, grid: str = "config"):
     if name in TABLE1:
-        return wl.table1(TABLE1[name])
-    if name == "cfg2" and rank:
-        return wl.cfg2(seed_off=2 + 1000 * rank, tag=f"cfg2_globular_10k_rank{rank}")
-    return wl.CONFIGS[name]()
+        w = wl.table1(TABLE1[name])
+    elif name == "cfg2" and rank:
+        w = wl.cfg2(seed_off=2 + 1000 * rank, tag=f"cfg2_globular_10k_rank{rank}")
+    else:
+        w = wl.CONFIGS[name]()
+    if grid != "config":                  # the same structure on a grid that is not uniform from 0 or dq (workloads.GRIDS)
+        w = wl.with_grid(w, wl.GRIDS[grid](w), grid)
+    return w
 
 
 def measured_peaks():
@@ -218,7 +222,7 @@ def roofline_of(w, variant_ran, pairs_ms, fmax_ghz):
     uniform grid: one recurrence FMA + one accumulate = 2 FP32-pipe lane-operations (4 FMA-equivalent flop)."""
     nz = int(np.count_nonzero(w.q))                                             # q = 0 is answered in closed form by the epilogue
     pq_all, pq_nz = float(w.pair_q), float(w.pair_q) / w.M * nz
-    if variant_ran == "recur":
+    if variant_ran in ("recur", "centred"):
         peak = SM_COUNT * FP32_LANES * 2 * fmax_ghz / 1e3                       # TFLOP/s, FMA = 2 flop
         achieved = 4.0 * pq_nz / (pairs_ms * 1e-3) / 1e12
         return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
@@ -250,6 +254,10 @@ def measure(db, w, dev, variant, use_hint, steps, warmup, world=1, e2e=True):
     # the q grid exists on the host (it was generated there), so the caller can tell the library its shape: one pairs launch
     # instead of up to three (include/debye.h, DEBYE_QHINT_*); the device verifies the hint
     hint = db.q_hint(w.q) if use_hint else 0
+    if variant == "centred":              # forced centred product form: needs the pieces of the grid whatever its class
+        hint = db.q_hint_pieces(w.q)
+        if not hint:
+            raise SystemExit("bench.py: --variant centred needs a piecewise-uniform grid")
     info = db.launch_info(w.N, w.B, w.T, w.M, variant, with_grid=True, hint=hint)
 
     def barrier():
@@ -318,8 +326,15 @@ def measure(db, w, dev, variant, use_hint, steps, warmup, world=1, e2e=True):
     return res
 
 
-def variant_that_ran(variant, w):
-    return variant if variant != "auto" else ("recur" if _is_uniform(w.q) else "mufu")
+def variant_that_ran(variant, w, use_hint=True):
+    """the pairs kernel an automatic call runs: the library's own classification of the grid (debye_q_hint, host copy of q)"""
+    if variant != "auto":
+        return variant
+    from paper_1306_2258_b200 import binding as db
+    h = db.q_hint(w.q)
+    if use_hint and db.pieces_of(h)[0]:
+        return "centred"                  # piecewise uniform / general start, hinted: the centred product form
+    return "recur" if (h & (1 << 9)) or db.pieces_of(h)[0] == 1 else "mufu"
 
 
 def kernel_shape(db, w, res, variant_ran):
@@ -342,7 +357,7 @@ def config_summary(db, name, dev, variant, use_hint, fmax_ghz):
     w = make_workload(name)
     steps = {"cfg1": 50, "cfg2": 30, "cfg3": 8, "cfg4": 8, "cfg5": 4}.get(name, 10)
     res = measure(db, w, dev, variant, use_hint, steps, 3, e2e=False)
-    vr = variant_that_ran(variant, w)
+    vr = variant_that_ran(variant, w, use_hint)
     k_ran, chunks_ran = kernel_shape(db, w, res, vr)
     roof = roofline_of(w, vr, res["pairs_ms"], fmax_ghz)
     rows = stored_oracle(name)
@@ -368,7 +383,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", default="cfg2", choices=sorted(wl.CONFIGS) + list(TABLE1),
                     help="cfg1..cfg5: BASELINE.json's configs; table1_N: the shape of the paper's Table I rows (N atoms, 50 q on (0, 1])")
-    ap.add_argument("--variant", default="auto", choices=["auto", "recur", "mufu", "accurate", "fp64"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "recur", "mufu", "accurate", "fp64", "centred"])
+    ap.add_argument("--grid", default="config", choices=["config"] + sorted(wl.GRIDS),
+                    help="q grid: the config's own (uniform from 0), or the same number of points as a uniform grid with a general "
+                         "start / as two uniform pieces (workloads.GRIDS): these run the centred product form when hinted")
     ap.add_argument("--impl", default="libdebye", choices=["libdebye", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config summary (`configs` object) of the default 1-GPU run")
@@ -410,7 +428,7 @@ def main():
 
     if args.peaks:
         return run_peaks(dev) if rank == 0 else None
-    w = make_workload(args.config, rank)
+    w = make_workload(args.config, rank, args.grid)
     if args.path == "peratom":
         return run_peratom(args, w, rank, world, dev)
     if args.split == "tiles":
@@ -435,7 +453,7 @@ def main():
 
     peaks = measured_peaks()
     fmax_ghz = float(peaks.get("sm_max_mhz", 1965.0)) / 1e3
-    variant_ran = variant_that_ran(args.variant, w)
+    variant_ran = variant_that_ran(args.variant, w, not args.no_hint)
     pairs_ms, total_ms, info = res["pairs_ms"], res["total_ms"], res["info"]
     roof = roofline_of(w, variant_ran, pairs_ms, fmax_ghz)
     # dram__bytes_read.sum + dram__bytes_write.sum of the pairs kernel from a committed ncu --set full capture of this command
@@ -444,6 +462,10 @@ def main():
     roof["traffic_source"] = NCU_TRAFFIC_SOURCE if roof["traffic"] is not None else None
     k_ran, chunks_ran = kernel_shape(db, w, res, variant_ran)
     roof["kernel"] = f"debye_small_kernel<{k_ran}>" if info["n_launches"] == 1 else f"debye_pairs_kernel<{k_ran}, {variant_ran}>"
+    if variant_ran == "centred":
+        roof["note"] = ("FP32-pipe roofline with SURVEY 8(d)'s algorithmic count: 2 lane-ops (4 FMA-equivalent flop) per pair.q with q != 0; the "
+                        "centred product form (DESIGN.md section 5.5) executes 1 lane-op per pair.q plus a per-pair, per-piece start-up")
+        roof.pop("frac_product_form_1_lane_op", None)
     roof["kernel_ms"] = pairs_ms
     roof["pair_q_per_clk_per_sm"] = float(w.pair_q) / (pairs_ms * 1e-3) / (SM_COUNT * fmax_ghz * 1e9)
     roof["share_of_step"] = pairs_ms / (total_ms / args.steps)
@@ -452,7 +474,7 @@ def main():
         "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if variant_ran == "fp64" else "f32", "data": "synthetic",
-        "config": {"workload": w.name, "N": w.N, "T": w.T, "M": w.M, "B": w.B, "variant": variant_ran,
+        "config": {"workload": w.name, "N": w.N, "T": w.T, "M": w.M, "B": w.B, "variant": variant_ran, "grid": args.grid,
                    "pairs_grid": info["pairs_grid"], "q_chunk": k_ran, "n_chunks": chunks_ran,
                    "q_hint": "passed (grid classified from the host copy of q, verified on the device)" if res["hint"] else "none",
                    "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
@@ -714,12 +736,6 @@ def run_peratom(args, w, rank, world, dev):
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
-
-
-def _is_uniform(q):
-    """the library's own classification of the grid (debye_q_hint: host copy of q, DEBYE_QHINT_UNIFORM bit)"""
-    from paper_1306_2258_b200 import binding as db
-    return bool(db.q_hint(q) & (1 << 9))
 
 
 if __name__ == "__main__":

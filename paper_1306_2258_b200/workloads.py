@@ -256,6 +256,29 @@ def cubic_lattice(nx: int, ny: int, nz: int, a: float, M: int, q_max: float, T: 
     return Workload(f"lattice_{nx}x{ny}x{nz}", (g * a).astype(np.float32), typ, f, q, {"n": (nx, ny, nz), "a": a})
 
 
+def with_grid(w: Workload, q, tag: str, seed: int = 4242) -> Workload:
+    """The same structure on another q grid (form factors of the same 4-Gaussian family, re-drawn for that grid)."""
+    q = np.ascontiguousarray(q, dtype=np.float32)
+    return Workload(f"{w.name}_{tag}", w.xyz, w.type, gaussian_form_factors(BASE_SEED + seed, w.T, q), q, dict(w.meta))
+
+
+def grid_general_start(w: Workload) -> np.ndarray:
+    """Uniform, M points, same range, but starting 2.46 steps above 0 (neither 0 nor dq): a detector edge."""
+    dq = float(w.q[-1] - w.q[0]) / max(1, w.M - 1)
+    return ((2.46 + np.arange(w.M, dtype=np.float64)) * dq).astype(np.float32)
+
+
+def grid_two_pieces(w: Workload) -> np.ndarray:
+    """M points in two uniform pieces: the lower half of the config's range at its own step, then a coarser range (twice the
+    step) up to 1.5 x q_max -- a SAXS range followed by a WAXS range."""
+    dq = float(w.q[-1] - w.q[0]) / max(1, w.M - 1)
+    n1 = (w.M + 1) // 2
+    lo = np.arange(n1, dtype=np.float64) * dq
+    hi = lo[-1] + 2.0 * dq * np.arange(1, w.M - n1 + 1, dtype=np.float64)
+    return np.concatenate([lo, hi]).astype(np.float32)
+
+
+GRIDS = {"general_start": grid_general_start, "two_pieces": grid_two_pieces}
 CONFIGS = {"cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4, "cfg5": cfg5}
 
 

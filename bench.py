@@ -334,13 +334,18 @@ def variant_that_ran(variant, w, use_hint=True):
     h = db.q_hint(w.q)
     if use_hint and db.pieces_of(h)[0]:
         return "centred"                  # piecewise uniform / general start, hinted: the centred product form
-    return "recur" if (h & (1 << 9)) or db.pieces_of(h)[0] == 1 else "mufu"
+    if db.pieces_of(h)[0] == 1:           # uniform with a general start, no hint: the device picks the centred launch if one was offered
+        return "centred" if w.M <= 16 * 128 else "recur"
+    return "recur" if h & (1 << 9) else "mufu"
 
 
 def kernel_shape(db, w, res, variant_ran):
     """(K, n_chunks) of the pairs launch that did the work."""
     info, hint = res["info"], res["hint"]
     k_ran, chunks_ran = info["q_chunk"], info["n_chunks"]
+    if variant_ran == "centred":
+        chunks_ran, k_ran = db.pieces_of(db.q_hint_pieces(w.q))
+        return k_ran, chunks_ran
     if hint == 0 and variant_ran == "recur" and w.M >= 2 and float(w.q[0]) == 0.0:
         # grid starts at q = 0: the device runs the recurrence launch sized for M - 1 chain indices when the library
         # offered one (it does when that saves accumulators or a chunk; DESIGN.md section 5.1)

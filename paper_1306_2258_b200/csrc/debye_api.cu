@@ -149,7 +149,7 @@ Layout layout(int N, int B, int T, int M, int G_max, const Choice *ch, int nch)
     return L;
 }
 
-constexpr int MAX_CHOICES = 3;
+constexpr int MAX_CHOICES = 4;
 // grid class promised by the caller's hint flags (debye_grid_class), -3 without a hint, -4 for a piecewise-uniform grid
 int hint_class_of(uint32_t flags)
 {
@@ -181,6 +181,16 @@ int recur_choice_hinted(Choice *out, int M, int cls)
     out[0].alt_gate = -1;
     return 1;
 }
+// centred form for ONE uniform run of M points (a uniform grid with a general start): its pieces follow from M alone
+// (debye_find_pieces: equal pieces of at most DEBYE_PIECE_KCAP points); false if that needs more than DEBYE_MAX_PIECES
+bool cent_choice_uniform(Choice *out, int M)
+{
+    const int np = (M + DEBYE_PIECE_KCAP - 1) / DEBYE_PIECE_KCAP, per = (M + np - 1) / np;
+    if (np > DEBYE_MAX_PIECES) return false;
+    out->variant = V_CENT; out->K = (per + 7) / 8 * 8; out->n_chunks = np; out->alt_gate = -1;
+    if (out->K < 8) out->K = 8;
+    return true;
+}
 int variants_for(uint32_t flags, Choice *out, int M, int *is_auto)
 {
     *is_auto = 0;
@@ -194,7 +204,10 @@ int variants_for(uint32_t flags, Choice *out, int M, int *is_auto)
     if (cls == -4) { out[0] = cent_choice(flags); return 1; }         // hinted: piecewise uniform, the centred product form
     if (cls == -2) { out[0] = choose(V_MUFU, M); return 1; }          // hinted: not uniform
     if (cls >= -1) return recur_choice_hinted(out, M, cls);           // hinted: uniform
+    // no hint: every instantiation the grid could need is launched and the device runs one of them -- the recurrence (grids
+    // from 0 or dq: product form), the centred form (uniform with a general start), the MUFU kernel (anything else)
     int n = recur_choices(out, M);
+    if (cent_choice_uniform(&out[n], M)) ++n;
     out[n++] = choose(V_MUFU, M);
     return n;
 }
@@ -385,11 +398,6 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
 {
     int st = validate(xyz, type, N, B, mode == 0 ? (const void *)fftab : (const void *)q, T, q, M, out, flags);
     if (st) return st;
-    // the tile split has no centred-form instantiation: a pieces hint is dropped there (the device then finds the grid's class itself)
-    if (shard_world > 1 && (flags & DEBYE_QHINT_PIECES)) {
-        if (flags & DEBYE_SINC_CENTRED) return DEBYE_EUNSUPPORTED;
-        flags &= ~(uint32_t)(DEBYE_QHINT | DEBYE_QHINT_PIECES | (31u << DEBYE_QHINT_NPIECES_SHIFT) | (31u << DEBYE_QHINT_PIECEK_SHIFT));
-    }
     std::unique_lock<std::mutex> lock(g_mu);
     DevState *ds;
     if ((st = dev_state(&ds))) return st;
@@ -397,7 +405,7 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
         return run_small(ds, xyz, pre ? pre->type : type, N, fftab, T, q, M, out, n_out, flags, stream, mode, pre, lock);
     Choice ch[MAX_CHOICES]; int is_auto = 0;
     const int nch = variants_for(flags, ch, M, &is_auto);
-    int G[MAX_CHOICES] = {0, 0, 0}, Gmax = 0;
+    int G[MAX_CHOICES] = {0, 0, 0, 0}, Gmax = 0;
     for (int i = 0; i < nch; ++i) { if ((st = grid_for(ds, ch[i], N, B, &G[i]))) return st; if (G[i] > Gmax) Gmax = G[i]; }
     const Layout L = layout(N, B, T, M, Gmax, ch, nch);
     char *ws;
@@ -417,7 +425,11 @@ int run(const float *xyz, const int32_t *type, int N, int B, const float *fftab,
 
     int alt_offered = 0;
     for (int i = 0; i < nch; ++i) if (ch[i].alt_gate == 1) alt_offered = 1;
-    const int hint_class = hint_class_of(flags), hint_pieces = hint_pieces_of(flags);
+    const int hint_class = hint_class_of(flags);
+    int hint_pieces = hint_pieces_of(flags);
+    // no hint, automatic: tell the setup kernel which centred-form launch is on offer for a uniform grid with a general start
+    if (hint_class == -3 && is_auto)
+        for (int i = 0; i < nch; ++i) if (ch[i].variant == V_CENT) hint_pieces = (ch[i].n_chunks << 8) | (ch[i].K / 8);
     if (hint_class == 0 && nch == 1 && ch[0].variant == V_RECUR) {
         // hinted q[0] == 0 and a single recurrence launch: it is the one sized for M - 1 indices exactly when that pays
         Choice c2[2];

@@ -21,7 +21,8 @@ namespace debye {
 __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPlan *plan, const int32_t *__restrict__ type, const float *__restrict__ q,
                                                                             int32_t *__restrict__ perm, int N, int T, int M, int B, int alt_offered /* a recurrence launch sized for M - 1 indices exists */,
                                                                             int hint_class /* -3: no hint; -4: piecewise uniform (hint_pieces); else the grid class the caller promised (debye_grid_class) */,
-                                                                            int hint_pieces /* hint_class == -4: (number of pieces << 8) | K / 8 as debye_find_pieces gives them */,
+                                                                            int hint_pieces /* hint_class == -4: (number of pieces << 8) | K / 8 as debye_find_pieces gives them; hint_class == -3:
+                                                                                               the centred-form launch on offer for a uniform grid with a general start, 0 if none */,
                                                                             const float *__restrict__ xyz, float4 *__restrict__ sorted, int pack_here, const float *__restrict__ weight,
                                                                             int shard_rank, int shard_world)
 {
@@ -101,7 +102,14 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
         plan->q0 = q0;
         plan->dq = dq;
         plan->q_small = (s < 3.0e38f) ? s : 0.f;
-        plan->variant_auto = (hint_class == -4) ? V_CENT : (uni ? V_RECUR : V_MUFU);
+        int va = (hint_class == -4) ? V_CENT : (uni ? V_RECUR : V_MUFU);
+        if (hint_class == -3 && hint_pieces != 0 && cls == -1) {
+            // no hint, uniform grid with a general start: the centred product form if the launch on offer fits its pieces
+            // (it does: one run of M points is cut into equal pieces, which the host derived from M), else the chain form
+            if (debye_find_pieces(q, M, plan->pieces) && plan->pieces.n == (hint_pieces >> 8) && plan->pieces.K == 8 * (hint_pieces & 255)) va = V_CENT;
+            else plan->pieces.n = 0;
+        }
+        plan->variant_auto = va;
     }
     __syncthreads();
     // ---- unit prefix per type pair (thread 0, n_tp <= 528 steps) while the other warps sort -----------------------------
@@ -213,7 +221,7 @@ __device__ __forceinline__ double pair_count(int na, int nb, bool diag) { return
 #define DEBYE_FINAL_G 32
 #define DEBYE_FINAL_THREADS (DEBYE_FINAL_Q * DEBYE_FINAL_G)
 struct FinalSet { int variant, K, n_chunks, G, alt_gate; };   // parameters of one pairs launch (alt_gate as in the pairs kernel)
-struct FinalSets { FinalSet s[3]; int n; };                    // up to: recurrence (M - 1 indices), recurrence, MUFU
+struct FinalSets { FinalSet s[4]; int n; };                    // up to: recurrence (M - 1 indices), recurrence, centred, MUFU
 // which pairs launch did the work: the same device-side decisions the pairs kernels took
 __device__ __forceinline__ int final_pick(const DevPlan *plan, const FinalSets &sets, int is_auto)
 {

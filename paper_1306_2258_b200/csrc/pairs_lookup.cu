@@ -30,6 +30,10 @@ debye_pairs_fn debye_get_cent_w0(int K);
 debye_pairs_fn debye_get_cent_w1(int K);
 debye_pairs_fn debye_get_cent_w2(int K);
 debye_pairs_fn debye_get_cent_w3(int K);
+debye_pairs_fn debye_get_cent_s0(int K);
+debye_pairs_fn debye_get_cent_s1(int K);
+debye_pairs_fn debye_get_cent_s2(int K);
+debye_pairs_fn debye_get_cent_s3(int K);
 static debye_pairs_fn first_of(debye_pairs_fn (*const *fns)(int), int n, int K)
 {
     for (int i = 0; i < n; ++i) { debye_pairs_fn f = fns[i](K); if (f) return f; }
@@ -42,7 +46,7 @@ debye_pairs_fn debye_get_pairs_kernel(int variant, int K, bool weighted, bool sh
         if (variant == V_RECUR) { static debye_pairs_fn (*const f[])(int) = {debye_get_recur_s0, debye_get_recur_s1, debye_get_recur_s2, debye_get_recur_s3}; return first_of(f, 4, K); }
         if (variant == V_MUFU) { static debye_pairs_fn (*const f[])(int) = {debye_get_mufu_s0, debye_get_mufu_s1}; return first_of(f, 2, K); }
         if (variant == V_ACCURATE) return nullptr;      // the libdevice-sinf reference variant exists for the plain calls only
-        if (variant == V_CENT) return nullptr;          // the centred product form: not in the tile split
+        if (variant == V_CENT) { static debye_pairs_fn (*const f[])(int) = {debye_get_cent_s0, debye_get_cent_s1, debye_get_cent_s2, debye_get_cent_s3}; return first_of(f, 4, K); }
         if (variant == V_F64) { static debye_pairs_fn (*const f[])(int) = {debye_get_f64_s0}; return first_of(f, 1, K); }
         return nullptr;
     }

@@ -94,8 +94,9 @@ def test_workspace_and_launch_info_are_host_side():
     a, b = L.debye_workspace_bytes(100000, 1, 5, 64, 0), L.debye_workspace_bytes(200000, 1, 5, 64, 0)
     assert 15 * 100000 < b - a < 25 * 100000
     info = binding.launch_info(10000, 1, 5, 101, "auto")
-    # setup(+pack: N*B <= 16384), recurrence sized for 100 and for 101 chain indices, MUFU, reduce, epilogue
-    assert info == {"n_launches": 6, "q_chunk": 104, "n_chunks": 1}
+    # no hint: setup(+pack: N*B <= 16384), recurrence sized for 100 and for 101 chain indices, centred form (general start), MUFU,
+    # reduce, epilogue -- the device runs one of the four pairs launches, the others return at once
+    assert info == {"n_launches": 7, "q_chunk": 104, "n_chunks": 1}
     assert binding.launch_info(50000, 1, 4, 200, "recur") == {"n_launches": 5, "q_chunk": 104, "n_chunks": 2}
     assert binding.launch_info(1000, 1, 5, 51, "fp64")["n_chunks"] == 2
     assert binding.launch_info(1000, 1, 5, 300, "mufu") == {"n_launches": 4, "q_chunk": 104, "n_chunks": 3}

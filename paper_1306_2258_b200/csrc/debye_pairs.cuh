@@ -735,7 +735,7 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
     __shared__ __align__(8) u64 mbar[2];
     __shared__ float tbuf[F64 ? 1 : NW][F64 ? 1 : 32][F64 ? 1 : 33];
     __shared__ double wsum[NW][K];
-    __shared__ float qs[(VAR == V_RECUR || VAR == V_CENT) ? 1 : K];
+    __shared__ __align__(16) float qs[(VAR == V_RECUR || VAR == V_CENT) ? 4 : K];
     __shared__ float wtab[16];                        // recurrence, general start: start frequencies (hi[8], lo[8])    // direct variants: q of each local slot (0 for padding)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -995,10 +995,16 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                     }
                     if constexpr (VAR == V_MUFU) {
                         const float rt = r * 0.15915494309189535f;            // r / 2 pi: turns = q_k * rt
+                        // The XU pipe takes one MUFU.SIN per 8 cycles and scheduler (16 lanes per clock and SM), so the loop must
+                        // issue fewer than 8 instructions per term to be bound by it: four q per LDS.128 (was one LDS per
+                        // term) and the scaling by 1/r folded into the accumulation (one packed FMA per two terms instead of
+                        // two FMUL and a packed add)
+                        const u64 rinv2 = pk2(rinv, rinv);
 #pragma unroll
-                        for (int l = 0; l < K; l += 2) {
-                            float s0 = sin_turns_fma(rt, qs[l]) * rinv, s1 = sin_turns_fma(rt, qs[l + 1]) * rinv;
-                            acc.v[l / 2] = add2(acc.v[l / 2], pk2(s0, s1));
+                        for (int l = 0; l < K; l += 4) {
+                            const float4 q4 = *reinterpret_cast<const float4 *>(&qs[l]);
+                            acc.v[l / 2] = fma2(pk2(sin_turns_fma(rt, q4.x), sin_turns_fma(rt, q4.y)), rinv2, acc.v[l / 2]);
+                            acc.v[l / 2 + 1] = fma2(pk2(sin_turns_fma(rt, q4.z), sin_turns_fma(rt, q4.w)), rinv2, acc.v[l / 2 + 1]);
                         }
                     } else {   // V_ACCURATE
 #pragma unroll

@@ -53,7 +53,9 @@ enum {
 #define DEBYE_MAX_Q 4096
 
 /* flags (bitwise or).  At most one of the DEBYE_SINC_* bits; none = automatic choice (made on the device,
- * no host sync): the recurrence kernel when q is a uniform grid, else the MUFU kernel. */
+ * no host sync): the recurrence kernel when q is a uniform grid from 0 or dq (telescoped product form), the centred
+ * product form when it is uniform with another start or -- with the hint of debye_q_hint -- a few uniform pieces, else
+ * the MUFU kernel. */
 enum {
     DEBYE_FP64 = 1u << 0,         /* double-precision pair arithmetic (libdevice sin), tolerance 1e-10 mode     */
     DEBYE_SINC_MUFU = 1u << 2,    /* FP32, one range-reduced MUFU.SIN per term; any q grid                      */

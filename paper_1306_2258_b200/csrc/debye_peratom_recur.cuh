@@ -24,7 +24,11 @@
 
 namespace debye {
 
-#define DEBYE_PAR_JT 32          // j atoms per tile: 32 x (16 + 4 K) bytes, two buffers
+#define DEBYE_PAR_JT 64          // largest tile (the workspace is padded by one)
+// j atoms per tile: JT x (16 + 4 K) bytes, two buffers, within the 48 KB of static shared memory
+#ifndef DEBYE_PAR_JT_OF
+#define DEBYE_PAR_JT_OF(K) ((K) <= 64 ? 64 : ((K) <= 104 ? 48 : 40))
+#endif
 #define DEBYE_PAR_FLUSH 512
 
 struct PeratomPlan { int32_t bad, koff; double dq; };
@@ -137,12 +141,66 @@ __device__ __forceinline__ void chain_hot(u64 (&acc)[K / 2], u64 (&A)[4], u64 (&
     }
 }
 
+// One tile of j atoms against this thread's i atom: the three-stage pipeline of recur_tile (stage B of pair jj + NP, stage A
+// of pair jj + 2 NP, chains of pair jj), NP pairs per iteration, ONE copy of the loop per chunk mode (the mode is a template
+// parameter: a run-time branch between the three start-ups inside the loop splits its basic block, and the scheduler can
+// then no longer hide the start-up's dependency chains under the packed chain instructions).  Returns whether some pair of
+// this thread took the small-theta mask (contributed zero; the caller rescans the tile).
+// measured on B200 (T pair.q/s, cfg2 / cfg3): mode as a run-time branch inside the loop, 1 pair per iteration, 32-atom tiles
+// 5.08 / 6.66; one loop per mode 5.69 / 7.62; two pairs per iteration 5.93 / 8.04; 48-atom tiles (K = 104) 6.01 / 8.17;
+// 3 CTAs per SM at K = 104 (168 registers, 1 pair per iteration) 5.73 / 7.79
+#ifndef DEBYE_PAR_NP
+#define DEBYE_PAR_NP 2
+#endif
+#ifndef DEBYE_PAR_K3
+#define DEBYE_PAR_K3 64          // up to this K: 3 CTAs per SM (168 registers)
+#endif
+template <int K, int MODE>
+__device__ __forceinline__ bool peratom_tile(u64 (&acc)[K / 2], const float4 *__restrict__ tile, const float *__restrict__ tf, const int jj0, const int cnt,
+                                             const float4 pi, const int jmin, const RecurConst &rc)
+{
+    constexpr int NP = DEBYE_PAR_NP;
+    bool had_slow = false;
+    auto geom = [&](const int jbase, RecurGeom (&g)[NP]) {
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            const int j = jbase + p;
+            recur_geom<RM_G, false>(tile[min(j, cnt - 1)], pi, j >= jmin && j < cnt, rc, g[p]);     // RM_G: with the small-theta mask
+            had_slow = had_slow || g[p].slow;
+        }
+    };
+    u64 A[NP][4], Bv[NP][4];
+    float cS[NP];
+    RecurGeom gn[NP];
+    geom(jj0, gn);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) chain_vals<MODE>(gn[p], A[p], Bv[p], cS[p]);
+    geom(jj0 + NP, gn);
+    for (int jj = jj0; jj < cnt; jj += NP) {
+        u64 An[NP][4], Bn[NP][4];
+        float cSn[NP];
+#pragma unroll
+        for (int p = 0; p < NP; ++p) chain_vals<MODE>(gn[p], An[p], Bn[p], cSn[p]);
+        geom(jj + 2 * NP, gn);
+#pragma unroll
+        for (int p = 0; p < NP; ++p) chain_hot<K>(acc, A[p], Bv[p], cS[p], tf + (size_t)min(jj + p, cnt - 1) * K);   // a masked pair has zero start values
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+#pragma unroll
+            for (int a = 0; a < 4; ++a) { A[p][a] = An[p][a]; Bv[p][a] = Bn[p][a]; }
+            cS[p] = cSn[p];
+        }
+    }
+    return had_slow;
+}
+
 template <int K>
-__global__ void __launch_bounds__(DEBYE_IB, K <= 64 ? 3 : 2) debye_peratom_recur_kernel(const float4 *__restrict__ pos4, const float *__restrict__ ffp, const float *__restrict__ qv,
+__global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_peratom_recur_kernel(const float4 *__restrict__ pos4, const float *__restrict__ ffp, const float *__restrict__ qv,
                                                                                          const PeratomPlan *__restrict__ plan, int N, int M, int n_chunks, float theta_min,
                                                                                          double *__restrict__ records)
 {
-    constexpr int JT = DEBYE_PAR_JT, NW = DEBYE_IB / 32;
+    constexpr int JT = DEBYE_PAR_JT_OF(K), NW = DEBYE_IB / 32;
+    static_assert(JT <= DEBYE_PAR_JT && JT % 2 == 0, "tile size");
     __shared__ __align__(128) float4 tpos[2][JT + DEBYE_TILE_PAD];
     __shared__ __align__(128) float tff[2][JT][K];
     __shared__ __align__(8) u64 mbar[2];
@@ -224,31 +282,12 @@ __global__ void __launch_bounds__(DEBYE_IB, K <= 64 ? 3 : 2) debye_peratom_recur
             const int jj0 = max(0, row * DEBYE_IB + warp * 32 + 1 - jl0);
             if (jj0 < cnt && row * DEBYE_IB + warp * 32 < N) {
                 const int jmin = ivalid ? max(0, i + 1 - jl0) : 0x7fffffff;
-                bool had_slow = false;
-                auto geom = [&](const int j, RecurGeom &g) {
-                    recur_geom<RM_G, false>(tile[min(j, cnt - 1)], pi, j >= jmin && j < cnt, rc, g);     // RM_G: with the small-theta mask
-                    had_slow = had_slow || g.slow;
-                };
-                auto vals = [&](const RecurGeom &g, u64 (&A)[4], u64 (&Bv)[4], float &cS) {
-                    if (mode == PM_C1) chain_vals<PM_C1>(g, A, Bv, cS);
-                    else if (mode == PM_C2A) chain_vals<PM_C2A>(g, A, Bv, cS);
-                    else chain_vals<PM_C2B>(g, A, Bv, cS);
-                };
-                u64 A[4], Bv[4];
-                float cS;
-                RecurGeom gn;
-                geom(jj0, gn);
-                vals(gn, A, Bv, cS);
-                geom(jj0 + 1, gn);
-                for (int jj = jj0; jj < cnt; ++jj) {       // stage B of pair jj + 1, stage A of pair jj + 2, chains of pair jj
-                    u64 An[4], Bn[4];
-                    float cSn;
-                    vals(gn, An, Bn, cSn);
-                    geom(jj + 2, gn);
-                    chain_hot<K>(acc, A, Bv, cS, &tff[buf][jj][0]);
-#pragma unroll
-                    for (int a = 0; a < 4; ++a) { A[a] = An[a]; Bv[a] = Bn[a]; }
-                    cS = cSn;
+                bool had_slow;
+                const float *tf = &tff[buf][0][0];
+                switch (mode) {      // warp-uniform; one copy of the pipelined loop per mode
+                    case PM_C1: had_slow = peratom_tile<K, PM_C1>(acc, tile, tf, jj0, cnt, pi, jmin, rc); break;
+                    case PM_C2A: had_slow = peratom_tile<K, PM_C2A>(acc, tile, tf, jj0, cnt, pi, jmin, rc); break;
+                    default: had_slow = peratom_tile<K, PM_C2B>(acc, tile, tf, jj0, cnt, pi, jmin, rc); break;
                 }
                 // pairs with theta at or below theta_min (the chain would lose their frequency) and coincident atoms contributed
                 // zero above; they are rare: the tile is rescanned only if some lane of the warp met one, term by term

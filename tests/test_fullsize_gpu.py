@@ -82,6 +82,33 @@ def test_single_structure_configs_against_stored_oracle(db, name):
     assert run(db, w, "auto", hint=db.q_hint(w.q)).tobytes() == run(db, w, "auto").tobytes()
 
 
+@pytest.mark.parametrize("name", ["cfg3", "cfg5"])
+def test_centred_product_form_against_stored_oracle(db, name):
+    """The centred product form forced onto the configs' own uniform grids -- cfg3: 200 q in two pieces of
+    100, cfg5: one piece of 128 -- against the oracle's whole stored profiles: every accumulator level, every q."""
+    w = wl.CONFIGS[name]()
+    rows = golden()[name]
+    hp = db.q_hint_pieces(w.q)
+    assert db.pieces_of(hp) == {"cfg3": (2, 104), "cfg5": (1, 128)}[name]
+    worst = check(run(db, w, "centred", hint=hp), rows, w, TOL32, f"{name} centred")
+    assert worst <= 3e-5, (name, worst)
+
+
+@pytest.mark.parametrize("grid", sorted(wl.GRIDS))
+def test_cfg2_on_general_start_and_two_piece_grids_live_oracle(db, grid):
+    """What `bench.py --grid ...` times: cfg2's structure on a uniform grid that starts at 2.46 dq, and on two uniform pieces;
+    the hinted automatic call (centred product form), the unhinted one and the MUFU kernel against the oracle, every q."""
+    w0 = wl.cfg2()
+    w = wl.with_grid(w0, wl.GRIDS[grid](w0), grid)
+    ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)
+    h = db.q_hint(w.q)
+    assert db.pieces_of(h) == {"general_start": (1, 104), "two_pieces": (2, 56)}[grid]
+    for label, I in (("hinted", run(db, w, hint=h)), ("no hint", run(db, w)), ("mufu", run(db, w, "mufu"))):
+        e = float(np.max(np.abs(I - ref) / np.abs(ref)))
+        print(f"cfg2 {grid} {label}: max rel err {e:.3e}")
+        assert e <= 3e-5, (grid, label, e)
+
+
 def test_cfg2_full_profile_live_oracle_and_fp64(db):
     w = wl.cfg2()
     ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)          # ~3-20 s on the host cores

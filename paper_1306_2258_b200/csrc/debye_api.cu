@@ -56,6 +56,9 @@ cudaError_t scratch_release(ScratchOrder &o, cudaStream_t stream)
 #ifndef DEBYE_CENT_FOR_GENERAL_START
 #define DEBYE_CENT_FOR_GENERAL_START 1
 #endif
+#ifndef DEBYE_MUFU_KMAX
+#define DEBYE_MUFU_KMAX 112      // largest q-chunk of the MUFU kernel (choose())
+#endif
 constexpr int MAX_DEV = 64;
 constexpr int64_t DEBYE_PACK_IN_SETUP = 16384;   // N x B up to which debye_setup_kernel also packs the coordinates
 struct DevState {
@@ -104,7 +107,9 @@ Choice choose(int variant, int M)
         while (debye::recur_slots(M, nc) > DEBYE_KMAX_F32) nc *= 2;
         c.n_chunks = nc; c.K = debye::recur_slots(M, nc);
     } else {
-        int kmax = (variant == V_F64) ? DEBYE_KMAX_F64 : DEBYE_KMAX_F32;
+        // MUFU: the pipelined loop needs K + ~75 registers and spills inside the loop above K = 112 (measured: M = 128 as one
+        // chunk of 128 runs at 2.28 T pair.q/s on cfg5; two chunks repeat only the distance)
+        int kmax = (variant == V_F64) ? DEBYE_KMAX_F64 : (variant == V_MUFU ? DEBYE_MUFU_KMAX : DEBYE_KMAX_F32);
         int nc = (M + kmax - 1) / kmax;
         int per = (M + nc - 1) / nc;
         c.n_chunks = nc; c.K = (per + 7) / 8 * 8;

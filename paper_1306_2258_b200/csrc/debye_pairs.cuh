@@ -708,6 +708,77 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
     }
 }
 
+// ---- MUFU variant (any grid): one tile, software pipelined ---------------------------------------------------------------
+// One MUFU.SIN per term.  The XU pipe takes one per 8 cycles and scheduler, so the loop is bound by it as long as a MUFU.SIN is
+// always ready to issue: the geometry of pair jj + 1 (tile load, distance, MUFU.RSQ) is computed in the same basic block as the
+// K terms of pair jj, and pairs below the accuracy cut (theta small: MUFU's absolute error matters; coincident atoms) contribute
+// exactly zero here (1/r := 0) and are redone term by term in a rescan of the tile that runs only if some lane met one -- a vote
+// and a branch per pair would end the basic block at every pair.
+template <int K, bool W>
+__device__ __forceinline__ void mufu_tile(u64 (&acc)[K / 2], const float4 *__restrict__ tile, const float *__restrict__ qs, const int jj0, const int cnt,
+                                          const float4 pi, const bool ivalid, const bool diag, const int i_local, const int jl0, const float cut2)
+{
+    if (jj0 >= cnt) return;
+    const int jmin = ivalid ? (diag ? max(0, i_local + 1 - jl0) : 0) : 0x7fffffff;
+    bool had_slow = false;
+    auto geom = [&](const int j, float &rt, float &rinv) {
+        const float4 pj = tile[min(j, cnt - 1)];
+        const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+        const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+        const bool small = !(r2 > cut2), ok = j >= jmin && j < cnt;
+        const float r2c = fmaxf(r2, 1e-30f);
+        const float ri = rsqrt_mufu(r2c);
+        rt = (r2c * ri) * 0.15915494309189535f;                 // r / 2 pi: turns = q_k * rt
+        rinv = (ok && !small) ? (W ? ri * pj.w : ri) : 0.0f;
+        had_slow = had_slow || (small && ok);
+    };
+    float rt, rinv;
+    geom(jj0, rt, rinv);
+    for (int jj = jj0; jj < cnt; ++jj) {
+        float rtn, rinvn;
+        geom(jj + 1, rtn, rinvn);
+        const u64 rinv2 = pk2(rinv, rinv);
+#pragma unroll
+        for (int l = 0; l < K; l += 4) {
+            const float4 q4 = *reinterpret_cast<const float4 *>(&qs[l]);
+            acc[l / 2] = fma2(pk2(sin_turns_fma(rt, q4.x), sin_turns_fma(rt, q4.y)), rinv2, acc[l / 2]);
+            acc[l / 2 + 1] = fma2(pk2(sin_turns_fma(rt, q4.z), sin_turns_fma(rt, q4.w)), rinv2, acc[l / 2 + 1]);
+        }
+        rt = rtn; rinv = rinvn;
+    }
+    if (__any_sync(0xffffffffu, had_slow)) {
+        if (had_slow) {
+            for (int j = max(jj0, jmin); j < cnt; ++j) {
+                const float4 pj = tile[j];
+                const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+                const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                if (!(r2 > cut2)) {
+                    const float rs = sqrtf(r2);
+#pragma unroll
+                    for (int l = 0; l < K; ++l) {
+                        const float qk = qs[l];
+                        float tv = (rs == 0.0f) ? qk : term_accurate(qk, rs);
+                        if constexpr (W) tv *= pj.w;
+                        float lo_, hi_;
+                        upk2(acc[l / 2], lo_, hi_);
+                        if (l & 1) hi_ += tv; else lo_ += tv;
+                        acc[l / 2] = pk2(lo_, hi_);
+                    }
+                }
+            }
+        }
+    }
+}
+
+// direct variants (MUFU, accurate): CTAs per SM by accumulator count.  The pipelined MUFU loop needs K + ~75 registers: with
+// more CTAs per SM than these it spills inside the loop (K = 104 at 3 CTAs/SM, 168 registers: 1.3 KB of spills, 1.36 T
+// pair.q/s on cfg2 against 3.22 T at 2 CTAs/SM)
+#ifndef DEBYE_MK4
+#define DEBYE_MK4 48
+#endif
+#ifndef DEBYE_MK3
+#define DEBYE_MK3 72
+#endif
 #ifndef DEBYE_FLUSH_J
 #define DEBYE_FLUSH_J 512
 #endif
@@ -716,7 +787,7 @@ __device__ __forceinline__ void recur_tile(u64 (&acc)[K / 2], const float4 *__re
 __device__ unsigned long long debye_trace[3 * 4096];
 #endif
 template <int K, int VAR, bool W, bool SH = false>
-__global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR ? recur_min_ctas(K) : (VAR == V_CENT ? cent_min_ctas(K) : (K <= 64 ? 4 : (K <= 112 ? 3 : 2))))) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
+__global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR ? recur_min_ctas(K) : (VAR == V_CENT ? cent_min_ctas(K) : (K <= DEBYE_MK4 ? 4 : (K <= DEBYE_MK3 ? 3 : 2))))) debye_pairs_kernel(const DevPlan *__restrict__ plan, const float4 *__restrict__ sorted, const float *__restrict__ qv,
                                                                double *__restrict__ records, int n_chunks, int is_auto, float theta_min, int alt_gate)
 {
     pdl_wait();      // programmatic dependent launch: everything before us in the call has completed (debye_plan.cuh)
@@ -954,6 +1025,8 @@ __global__ void __launch_bounds__(DEBYE_IB, (VAR == V_F64) ? 1 : (VAR == V_RECUR
                     case RM_P2B: prod_tile<K, RM_P2B, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, jfree); break;
                     default: recur_tile<K, W>(acc.v, tile[buf], jj0, cnt, pi, ivalid, diag, i_local, jl0, rc, wtab); break;
                 }
+            } else if constexpr (VAR == V_MUFU) {
+                if (row * DEBYE_IB + warp * 32 < n_i) mufu_tile<K, W>(acc.v, tile[buf], qs, jj0, cnt, pi, ivalid, diag, i_local, jl0, cut2);
             } else {
             for (int jj = jj0; jj < cnt; ++jj) {
                 const float4 pj = tile[buf][jj];

@@ -355,17 +355,17 @@ def kernel_shape(db, w, res, variant_ran):
     return k_ran, chunks_ran
 
 
-def config_summary(db, name, dev, variant, use_hint, fmax_ghz):
+def config_summary(db, name, dev, variant, use_hint, fmax_ghz, grid="config"):
     """One entry of the `configs` object: a full-size BASELINE config measured like the headline (fewer steps) and checked
     against the oracle's stored whole profile (cfg1 / cfg2: the oracle runs live)."""
     from oracle import oracle as orc
-    w = make_workload(name)
+    w = make_workload(name, 0, grid)
     steps = {"cfg1": 50, "cfg2": 30, "cfg3": 8, "cfg4": 8, "cfg5": 4}.get(name, 10)
     res = measure(db, w, dev, variant, use_hint, steps, 3, e2e=False)
     vr = variant_that_ran(variant, w, use_hint)
     k_ran, chunks_ran = kernel_shape(db, w, res, vr)
     roof = roofline_of(w, vr, res["pairs_ms"], fmax_ghz)
-    rows = stored_oracle(name)
+    rows = stored_oracle(name) if grid == "config" else None
     I = res["result"]
     if rows is None:
         ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)
@@ -502,6 +502,8 @@ def main():
     if world == 1 and args.config == "cfg2" and args.variant == "auto" and not args.no_configs and not args.no_cpu_baseline:
         # the other BASELINE configs, same launch configuration, fewer steps; each checked against the oracle's whole profile
         line["configs"] = {name: config_summary(db, name, dev, args.variant, not args.no_hint, fmax_ghz) for name in sorted(wl.CONFIGS)}
+        # cfg2's structure on grids that are not uniform from 0 (workloads.GRIDS): the centred product form
+        line["grids"] = {g: config_summary(db, "cfg2", dev, args.variant, not args.no_hint, fmax_ghz, g) for g in sorted(wl.GRIDS)}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

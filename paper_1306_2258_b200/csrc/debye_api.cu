@@ -676,7 +676,7 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
     // resident CTAs x up to 8 waves, at least ~192 units (j atoms x 128 i atoms x 32 q) per CTA
     // whole waves of resident CTAs (a grid slightly above one wave runs its last CTAs alone: N = 4 000 took 0.25 ms with
     // 594 CTAs, 0.20 ms with 589); small structures: one full wave of short ranges (at least 24 units each)
-    const int64_t one_wave = (int64_t)ds->sms * (f64 ? 2 : 4);
+    const int64_t one_wave = (int64_t)ds->sms * (f64 ? 2 : DEBYE_PA_CTAS);
     const int64_t Gmax = one_wave * 8;
     int64_t G = U / (192 * DEBYE_PA_KQ / KQ);
     if (G < one_wave) { G = U / 24; if (G > one_wave) G = one_wave; }

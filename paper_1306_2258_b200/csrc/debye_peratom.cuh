@@ -24,6 +24,9 @@ namespace debye {
 
 #define DEBYE_PA_KQ 32           // largest q-chunk (accumulators per thread); the kernel is instantiated for 16, 20, ... 32
 #define DEBYE_PA_JT 64
+#ifndef DEBYE_PA_CTAS
+#define DEBYE_PA_CTAS 4          // FP32 kernel: CTAs per SM
+#endif
 #define DEBYE_PA_FLUSH 2048
 #define DEBYE_PA_SLICES 64       // self-term kernel: atom slices (grid.y)
 
@@ -63,7 +66,7 @@ __host__ __device__ inline int debye_peratom_kq(int M)
 }
 
 template <bool F64, int KQ>
-__global__ void __launch_bounds__(DEBYE_IB, F64 ? 2 : 4) debye_peratom_pairs_kernel(const float *__restrict__ xyz, const float *__restrict__ ff,
+__global__ void __launch_bounds__(DEBYE_IB, F64 ? 2 : DEBYE_PA_CTAS) debye_peratom_pairs_kernel(const float *__restrict__ xyz, const float *__restrict__ ff,
                                                                                       const float *__restrict__ qv, int N, int M, int n_chunks,
                                                                                       double *__restrict__ records)
 {
@@ -139,6 +142,59 @@ __global__ void __launch_bounds__(DEBYE_IB, F64 ? 2 : 4) debye_peratom_pairs_ker
             __syncthreads();
             // rows are diagonal blocks of the j > i triangle: a warp whose every i is >= j has nothing to do for that j
             const int jj0 = max(0, row * DEBYE_IB + warp * 32 + 1 - jg0);
+            if constexpr (!F64) {
+                // Software pipeline as mufu_tile (debye_pairs.cuh): the geometry of pair jj + 1 (tile load, distance, MUFU.RSQ) sits
+                // in the basic block of the KQ terms of pair jj, so a MUFU.SIN is always ready to issue; pairs below the accuracy
+                // cut contribute zero here (1/r := 0) and are redone term by term in a rescan of the tile that runs only if
+                // some lane met one (a vote and a branch per pair would end the block at every pair).
+                if (jj0 < cnt) {
+                    bool had_slow = false;
+                    auto geom = [&](const int jj, float &rt, float &rinv) {
+                        const float4 pj = pos[min(jj, cnt - 1)];
+                        const float dx = pj.x - pix, dy = pj.y - piy, dz = pj.z - piz;
+                        const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                        const bool small = !(r2 > cut2), ok = ivalid && (jg0 + jj > i) && jj < cnt;
+                        const float r2c = fmaxf(r2, 1e-30f);
+                        const float ri = rsqrt_mufu(r2c);
+                        rt = (r2c * ri) * 0.15915494309189535f;                       // r / 2 pi: turns = q_k * rt
+                        rinv = (ok && !small) ? ri : 0.0f;
+                        had_slow = had_slow || (small && ok);
+                    };
+                    float rt, rinv;
+                    geom(jj0, rt, rinv);
+                    for (int jj = jj0; jj < cnt; ++jj) {
+                        float rtn, rinvn;
+                        geom(jj + 1, rtn, rinvn);
+#pragma unroll
+                        for (int l = 0; l < KQ; l += 4) {
+                            const float4 f4 = *reinterpret_cast<const float4 *>(&fj[jj][l]);
+                            acc[l + 0] = fmaf(sin_turns_fma(rt, qr[l + 0]) * rinv, f4.x, acc[l + 0]);
+                            acc[l + 1] = fmaf(sin_turns_fma(rt, qr[l + 1]) * rinv, f4.y, acc[l + 1]);
+                            acc[l + 2] = fmaf(sin_turns_fma(rt, qr[l + 2]) * rinv, f4.z, acc[l + 2]);
+                            acc[l + 3] = fmaf(sin_turns_fma(rt, qr[l + 3]) * rinv, f4.w, acc[l + 3]);
+                        }
+                        rt = rtn; rinv = rinvn;
+                    }
+                    if (__any_sync(0xffffffffu, had_slow)) {
+                        if (had_slow) {
+                            for (int jj = jj0; jj < cnt; ++jj) {
+                                const float4 pj = pos[jj];
+                                const float dx = pj.x - pix, dy = pj.y - piy, dz = pj.z - piz;
+                                const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+                                if (ivalid && (jg0 + jj > i) && !(r2 > cut2)) {
+                                    const float rs = sqrtf(r2);
+#pragma unroll
+                                    for (int l = 0; l < KQ; ++l) {
+                                        const float qk = qr[l];
+                                        const float tv = (rs == 0.0f) ? qk : term_accurate(qk, rs);
+                                        acc[l] = fmaf(fj[jj][l], tv, acc[l]);
+                                    }
+                                }
+                            }
+                        }
+                    }
+                }
+            } else
             for (int jj = jj0; jj < cnt; ++jj) {
                 const float4 pj = pos[jj];
                 const bool ok = ivalid && (jg0 + jj > i);
@@ -152,34 +208,6 @@ __global__ void __launch_bounds__(DEBYE_IB, F64 ? 2 : 4) debye_peratom_pairs_ker
                             const double tv = (x == 0.0) ? qk : sin(x) / r;          // sin(q r)/r -> q as r -> 0
                             acc[l] += (double)fj[jj][l] * tv;
                         }
-                    }
-                } else {
-                    const float dx = pj.x - pix, dy = pj.y - piy, dz = pj.z - piz;
-                    const float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-                    const bool small = !(r2 > cut2);
-                    const float r2c = fmaxf(r2, 1e-30f);
-                    float rinv = rsqrt_mufu(r2c);
-                    const float r = r2c * rinv;
-                    rinv = (ok && !small) ? rinv : 0.0f;
-                    if (__any_sync(0xffffffffu, small && ok)) {
-                        if (small && ok) {
-                            const float rs = sqrtf(r2);
-#pragma unroll
-                            for (int l = 0; l < KQ; ++l) {
-                                const float qk = qr[l];
-                                const float tv = (rs == 0.0f) ? qk : term_accurate(qk, rs);
-                                acc[l] = fmaf(fj[jj][l], tv, acc[l]);
-                            }
-                        }
-                    }
-                    const float rt = r * 0.15915494309189535f;                        // r / 2 pi: turns = q_k * rt
-#pragma unroll
-                    for (int l = 0; l < KQ; l += 4) {
-                        const float4 f4 = *reinterpret_cast<const float4 *>(&fj[jj][l]);
-                        acc[l + 0] = fmaf(sin_turns_fma(rt, qr[l + 0]) * rinv, f4.x, acc[l + 0]);
-                        acc[l + 1] = fmaf(sin_turns_fma(rt, qr[l + 1]) * rinv, f4.y, acc[l + 1]);
-                        acc[l + 2] = fmaf(sin_turns_fma(rt, qr[l + 2]) * rinv, f4.z, acc[l + 2]);
-                        acc[l + 3] = fmaf(sin_turns_fma(rt, qr[l + 3]) * rinv, f4.w, acc[l + 3]);
                     }
                 }
             }

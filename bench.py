@@ -634,8 +634,7 @@ def run_peratom(args, w, rank, world, dev):
     import torch
     import torch.distributed as dist
     from paper_1306_2258_b200 import binding as db, sharding
-    if w.xyz.ndim == 3:
-        raise SystemExit("--path peratom takes single-structure configs")
+    batch = w.xyz.ndim == 3            # cfg4: B conformers sharing the table, debye_profile_peratom_batch
     variant = args.variant if args.variant in ("auto", "mufu", "fp64", "recur") else "auto"
     ff = wl.peratom_table(w, rank)
     # with the grid hint (q was generated on the host) a grid q_k = (k + koff) dq runs the recurrence (debye_peratom_recur.cuh)
@@ -643,8 +642,9 @@ def run_peratom(args, w, rank, world, dev):
     H, U, Z, D = 1 << 8, 1 << 9, 1 << 10, 1 << 11
     recur = bool(hint & U) and bool(hint & (Z | D)) and (w.M - (1 if hint & Z else 0)) <= 256
     x, f, q = (torch.from_numpy(a).to(dev) for a in (w.xyz, ff, w.q))
-    out = torch.empty(w.M, dtype=torch.float64, device=dev)
+    out = torch.empty((w.B, w.M) if batch else w.M, dtype=torch.float64, device=dev)
     flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    entry = db.debye_profile_peratom_batch if batch else db.debye_profile_peratom
 
     def barrier():
         if world > 1:
@@ -652,7 +652,7 @@ def run_peratom(args, w, rank, world, dev):
         torch.cuda.synchronize()
 
     for _ in range(args.warmup):
-        db.debye_profile_peratom(x, f, q, out, variant=variant, hint=hint)
+        entry(x, f, q, out, variant=variant, hint=hint)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
     sampler = ClockSampler(dev.index or 0)
@@ -661,7 +661,7 @@ def run_peratom(args, w, rank, world, dev):
     for a, b in ev:
         flush.fill_(1)
         a.record()
-        db.debye_profile_peratom(x, f, q, out, variant=variant, hint=hint)
+        entry(x, f, q, out, variant=variant, hint=hint)
         b.record()
     barrier()
     wall = time.perf_counter() - wall0
@@ -675,20 +675,31 @@ def run_peratom(args, w, rank, world, dev):
     pk = []
     for _ in range(min(args.steps, 30)):
         flush.fill_(1)
-        db.debye_profile_peratom(x, f, q, out, variant=variant, hint=hint)
+        entry(x, f, q, out, variant=variant, hint=hint)
         torch.cuda.synchronize()
         pk.append(e0.elapsed_time(e1))
     db.set_pairs_events(None, None)
     pairs_ms = float(np.mean(pk))
     hx, hf, hq = (torch.from_numpy(a).pin_memory().numpy() for a in (w.xyz, ff, w.q))
-    hout = torch.empty(w.M, dtype=torch.float64).pin_memory().numpy()
+    hout = torch.empty((w.B, w.M) if batch else w.M, dtype=torch.float64).pin_memory().numpy()
+    if batch:       # no host-buffer C entry for batches: pinned host tensors copied in, the device entry, the result copied back
+        tx, tf, tq, tout = (torch.from_numpy(a) for a in (hx, hf, hq, hout))
+
+        def host_call():
+            x.copy_(tx, non_blocking=True); f.copy_(tf, non_blocking=True); q.copy_(tq, non_blocking=True)
+            entry(x, f, q, out, variant=variant, hint=hint)
+            tout.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+    else:
+        def host_call():
+            db.debye_profile_peratom_host(hx, hf, hq, hout, variant=variant, hint=hint)
     for _ in range(3):
-        db.debye_profile_peratom_host(hx, hf, hq, hout, variant=variant, hint=hint)
+        host_call()
     barrier()
     n_e2e = max(5, min(args.steps, 50))
     t0 = time.perf_counter()
     for _ in range(n_e2e):
-        db.debye_profile_peratom_host(hx, hf, hq, hout, variant=variant, hint=hint)
+        host_call()
     barrier()
     e2e_s = sharding.max_over_ranks(time.perf_counter() - t0, dev)
     result_dev = out.cpu().numpy()
@@ -710,7 +721,7 @@ def run_peratom(args, w, rank, world, dev):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if variant == "fp64" else "f32", "data": "synthetic",
-        "config": {"workload": w.name + "+peratom_table", "path": "peratom", "N": w.N, "M": w.M, "B": 1,
+        "config": {"workload": w.name + "+peratom_table", "path": "peratom", "N": w.N, "M": w.M, "B": w.B,
                    "variant": "fp64" if variant == "fp64" else ("recur" if recur else "mufu"), "q_chunk": kq, "n_chunks": (w.M + kq - 1) // kq,
                    "q_hint": "passed" if hint else "none",
                    "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
@@ -718,7 +729,7 @@ def run_peratom(args, w, rank, world, dev):
         "clocks": clocks,
         "e2e": {"value": units * n_e2e / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(hx.nbytes + hf.nbytes + hq.nbytes),
                 "d2h_bytes_per_step": int(hout.nbytes), "ms_per_step": e2e_s / n_e2e * 1e3, "steps": n_e2e},
-        "gpu_launches": (4 if recur else 3) * args.steps,
+        "gpu_launches": (4 if recur else 3 * w.B) * args.steps,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s" if recur else "T sin/s", "frac": achieved / peak,
                      # dram__bytes_read.sum + write.sum of the pairs kernel from the full ncu capture (profiles/r01_v6.md)
                      "traffic": 4248064 if (args.config == "cfg2" and variant != "fp64" and not recur) else None,
@@ -732,11 +743,19 @@ def run_peratom(args, w, rank, world, dev):
     if world == 1 and not args.no_cpu_baseline:
         from oracle import oracle as orc
         ks = list(range(0, w.M, max(1, w.M // 8)))
-        ref = orc.debye_peratom(w.xyz, ff[:, ks].copy(), w.q[ks].copy())
-        line["parity_max_rel_err"] = float(np.max(np.abs(result_dev[ks] - ref) / np.abs(ref)))
+        if batch:       # first and last conformer
+            errs = []
+            for bb in (0, w.B - 1):
+                ref = orc.debye_peratom(w.xyz[bb], ff[:, ks].copy(), w.q[ks].copy())
+                errs.append(float(np.max(np.abs(result_dev[bb][ks] - ref) / np.abs(ref))))
+            line["parity_max_rel_err"] = max(errs)
+        else:
+            ref = orc.debye_peratom(w.xyz, ff[:, ks].copy(), w.q[ks].copy())
+            line["parity_max_rel_err"] = float(np.max(np.abs(result_dev[ks] - ref) / np.abs(ref)))
         ns = min(w.N, 6000)
+        x0 = w.xyz[0] if batch else w.xyz
         t0 = time.perf_counter()
-        orc.debye_peratom(w.xyz[:ns], ff[:ns], w.q)
+        orc.debye_peratom(x0[:ns], ff[:ns], w.q)
         dt = time.perf_counter() - t0
         line["cpu_baseline"] = {"value": ns * (ns - 1) / 2 * w.M / dt / 1e9, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
                                 "sample": f"oracle_debye_peratom on the first {ns} atoms, all {w.M} q ({dt:.2f} s)", "seconds": dt}

@@ -154,6 +154,14 @@ int debye_profile_weighted_host(const float *xyz, const int32_t *type, const flo
  *   the result equals debye_profile's to rounding -- and debye_profile is several times faster. */
 int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, double *I_out,
                           uint32_t flags, debye_stream_t stream);
+/* B conformers of one molecule with per-atom form factors (ensembles, refinement: PAPER.md:25, 46): xyz dev [B][N][3], the table
+ * ff dev [N][M] is shared, I_out dev [B][M].  With a grid hint q_k = (k + koff) dq (at most 2 x 128 chain indices; automatic mode
+ * or DEBYE_SINC_RECUR) all conformers run as ONE launch sequence -- the table is re-laid once, the unit line is conformer ->
+ * chunk -> row -> j, which keeps the GPU full for small molecules; any other grid or variant runs the single-structure
+ * sequence once per conformer on `stream`.  Every conformer's profile is what debye_profile_peratom gives for it to rounding
+ * (the CTA ranges differ).  Errors as debye_profile_peratom; B outside [1, 65535] is DEBYE_EINVAL. */
+int debye_profile_peratom_batch(const float *xyz, const float *ff, int32_t N, int32_t B, const float *q, int32_t M,
+                                double *I_out, uint32_t flags, debye_stream_t stream);
 /* The same through HOST buffers (copies in, runs the device path, copies I_out back, synchronises `stream`). */
 int debye_profile_peratom_host(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, double *I_out,
                                uint32_t flags, debye_stream_t stream);

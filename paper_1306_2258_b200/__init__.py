@@ -5,7 +5,7 @@ include/debye.h); they are re-exported lazily so that importing `workloads` neve
 no CPU fallback: a missing libdebye.so raises."""
 
 _API = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_profile_batch_host",
-        "debye_profile_weighted", "debye_profile_weighted_host", "debye_partials", "debye_partials_shard", "debye_profile_peratom", "debye_profile_peratom_host", "debye_profile_from_partials", "debye_profile_static", "static_limits", "q_hint", "q_hint_pieces", "pieces_of", "Plan", "lib", "LibdebyeError", "FLAGS")
+        "debye_profile_weighted", "debye_profile_weighted_host", "debye_partials", "debye_partials_shard", "debye_profile_peratom", "debye_profile_peratom_host", "debye_profile_peratom_batch", "debye_profile_from_partials", "debye_profile_static", "static_limits", "q_hint", "q_hint_pieces", "pieces_of", "Plan", "lib", "LibdebyeError", "FLAGS")
 
 
 def __getattr__(name):

@@ -23,7 +23,7 @@ EXPORTS = ("debye_profile", "debye_profile_batch", "debye_profile_host", "debye_
            "debye_launch_info", "debye_set_pairs_events", "debye_q_hint", "debye_plan_create", "debye_plan_execute",
            "debye_plan_destroy", "debye_strerror", "debye_last_cuda_error", "debye_version", "debye_pipe_bench_count",
            "debye_pipe_bench_name", "debye_pipe_bench", "debye_mufu_sin_error", "debye_mufu_rsq_error",
-           "debye_profile_static", "debye_profile_static_error", "debye_profile_static_limits", "debye_q_hint_pieces")
+           "debye_profile_static", "debye_profile_static_error", "debye_profile_static_limits", "debye_q_hint_pieces", "debye_profile_peratom_batch")
 
 
 # status codes of include/debye.h (debye_status)
@@ -61,6 +61,8 @@ def lib():
     L.debye_profile_peratom.argtypes = [vp, vp, i32, vp, i32, vp, u32, vp]
     L.debye_profile_peratom.restype = C.c_int
     L.debye_profile_peratom_host.argtypes = L.debye_profile_peratom.argtypes
+    L.debye_profile_peratom_batch.argtypes = [vp, vp, i32, i32, vp, i32, vp, u32, vp]
+    L.debye_profile_peratom_batch.restype = C.c_int
     L.debye_profile_peratom_host.restype = C.c_int
     L.debye_profile_weighted.argtypes = [vp, vp, vp, i32, vp, i32, vp, i32, vp, u32, vp]
     L.debye_profile_weighted_host.argtypes = L.debye_profile_weighted.argtypes
@@ -308,6 +310,19 @@ def debye_profile_peratom(xyz, ff, q, I_out=None, variant="auto", stream=None, h
     _check(lib().debye_profile_peratom(_dev(xyz, torch.float32, "xyz", (N, 3)), _dev(ff, torch.float32, "ff", (N, M)), N,
                                        _dev(q, torch.float32, "q", (M,)), M, _dev(I_out, torch.float64, "I_out", (M,)),
                                        _flags(variant, hint), _stream_ptr(stream)))
+    return I_out
+
+
+def debye_profile_peratom_batch(xyz, ff, q, I_out=None, variant="auto", stream=None, hint=0):
+    """I_out[B,M] for B conformers xyz[B,N,3] sharing the per-atom table ff[N,M]; with the hint of a grid q_k = (k + koff) dq all
+    conformers run in one launch sequence."""
+    import torch
+    B, N, M = xyz.shape[0], xyz.shape[1], q.shape[0]
+    if I_out is None:
+        I_out = torch.empty((B, M), dtype=torch.float64, device=xyz.device)
+    _check(lib().debye_profile_peratom_batch(_dev(xyz, torch.float32, "xyz", (B, N, 3)), _dev(ff, torch.float32, "ff", (N, M)), N, B,
+                                             _dev(q, torch.float32, "q", (M,)), M, _dev(I_out, torch.float64, "I_out", (B, M)),
+                                             _flags(variant, hint), _stream_ptr(stream)))
     return I_out
 
 

@@ -14,6 +14,7 @@
 #include <cstddef>
 #include <cmath>
 #include <mutex>
+#include <algorithm>
 #include <vector>
 #include "../../include/debye.h"
 #include "debye_aux.cuh"
@@ -594,13 +595,15 @@ int debye_profile_from_partials(const double *S_parts, int32_t n_parts, const in
 
 namespace {
 // per-atom form factors, recurrence (debye_peratom_recur.cuh): pack (+ grid check) | self terms | pairs | final.  Called with g_mu held.
-int run_peratom_recur(DevState *ds, const float *xyz, const float *ff, int N, const float *q, int M, double *I_out, int cls, int n_chunks, int K, cudaStream_t stream)
+// B conformers (xyz[B][N][3], I_out[B][M]) share the table: one unit line conformer -> chunk -> row -> j.
+int run_peratom_recur(DevState *ds, const float *xyz, const float *ff, int N, const float *q, int M, double *I_out, int cls, int n_chunks, int K, cudaStream_t stream,
+                      int B = 1)
 {
     debye_peratom_recur_fn fn = debye_get_peratom_recur_kernel(K);
     if (!fn) return DEBYE_EUNSUPPORTED;
     int st;
     const int rows = debye_diag_rows(N);
-    const int64_t U = (rows > 0 ? debye_diag_row_prefix(N, rows) : 0) * n_chunks;
+    const int64_t U = (rows > 0 ? debye_diag_row_prefix(N, rows) : 0) * n_chunks * B;
     const int64_t one_wave = (int64_t)ds->sms * (K <= 64 ? 3 : 2);
     int64_t G = U / 150 / one_wave * one_wave;                 // whole waves, at least ~150 units (j atoms x 128 i atoms) per CTA
     if (G > one_wave * 16) G = one_wave * 16;
@@ -608,9 +611,9 @@ int run_peratom_recur(DevState *ds, const float *xyz, const float *ff, int N, co
     if (G < 1) G = 1;
     size_t o = 0;
     const size_t o_plan = o; o += align_up(sizeof(debye::PeratomPlan));
-    const size_t o_pos = o; o += align_up((size_t)N * 16 + 16 * DEBYE_PAR_JT);
+    const size_t o_pos = o; o += align_up((size_t)N * B * 16 + 16 * DEBYE_PAR_JT);
     const size_t o_ffp = o; o += align_up((size_t)n_chunks * N * K * 4 + (size_t)DEBYE_PAR_JT * K * 4);
-    const size_t o_rec = o; o += align_up((size_t)(G + n_chunks) * K * 8);
+    const size_t o_rec = o; o += align_up((size_t)(G + (int64_t)n_chunks * B) * K * 8);
     const size_t o_self = o; o += align_up((size_t)DEBYE_PA_SLICES * 2 * M * 8);
     char *ws;
     if (ds->user_ws) { if (ds->user_bytes < o) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
@@ -620,15 +623,15 @@ int run_peratom_recur(DevState *ds, const float *xyz, const float *ff, int N, co
     float *ffp = (float *)(ws + o_ffp);
     double *records = (double *)(ws + o_rec), *selfbuf = (double *)(ws + o_self);
     CU(scratch_acquire(ds->order, stream));
-    int pb = (int)(((int64_t)N * K + 255) / 256);
+    int pb = (int)((std::max((int64_t)N * K, (int64_t)N * B) + 255) / 256);
     if (pb > ds->sms * 8) pb = ds->sms * 8;
     if (pb < 1) pb = 1;
-    debye::debye_peratom_pack_kernel<<<dim3(pb, n_chunks + 1), 256, 0, stream>>>(xyz, ff, q, N, M, K, n_chunks, cls, pos4, ffp, plan);
+    debye::debye_peratom_pack_kernel<<<dim3(pb, n_chunks + 1), 256, 0, stream>>>(xyz, ff, q, N, M, K, n_chunks, cls, pos4, ffp, plan, B);
     debye::debye_peratom_self_kernel<<<dim3((M + 31) / 32, DEBYE_PA_SLICES), 256, 0, stream>>>(ff, N, M, selfbuf);
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
-    if (U > 0) fn<<<(int)G, DEBYE_IB, 0, stream>>>(pos4, ffp, q, plan, N, M, n_chunks, 0.002f, records);
+    if (U > 0) fn<<<(int)G, DEBYE_IB, 0, stream>>>(pos4, ffp, q, plan, N, M, n_chunks, 0.002f, records, B);
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
-    debye::debye_peratom_final_kernel<<<(M + 31) / 32, 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, K, I_out, (const int32_t *)plan);
+    debye::debye_peratom_final_kernel<<<dim3((M + 31) / 32, B), 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, K, I_out, (const int32_t *)plan);
     CU(scratch_release(ds->order, stream));
     CU(cudaGetLastError());
     return DEBYE_OK;
@@ -706,6 +709,37 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
     debye::debye_peratom_final_kernel<<<(M + 31) / 32, 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, KQ, I_out, nullptr);
     CU(scratch_release(ds->order, stream));
     CU(cudaGetLastError());
+    return DEBYE_OK;
+}
+
+int debye_profile_peratom_batch(const float *xyz, const float *ff, int32_t N, int32_t B, const float *q, int32_t M, double *I_out, uint32_t flags, debye_stream_t stream_)
+{
+    if (B < 1 || B > 65535) return DEBYE_EINVAL;                      // the final kernel puts the conformer on blockIdx.y
+    if (B == 1) return debye_profile_peratom(xyz, ff, N, q, M, I_out, flags, stream_);
+    if (!xyz || !ff || !q || !I_out || N < 1 || M < 1 || M > DEBYE_MAX_Q) return DEBYE_EINVAL;
+    if ((int64_t)N * B > ((int64_t)1 << 31)) return DEBYE_EUNSUPPORTED;
+    // hinted grid q_k = (k + koff) dq: ONE launch sequence for all conformers (the recurrence; the table is packed once)
+    const int cls = hint_class_of(flags);
+    const int n_idx = M - (cls == 0 ? 1 : 0);
+    const bool other = (flags & (DEBYE_FP64 | DEBYE_SINC_MUFU)) != 0;
+    if (!other && (cls == 0 || cls == 1) && n_idx >= 1 && choose(V_RECUR, n_idx).n_chunks <= 2) {
+        // argument checks of the single-structure entry (flags, sizes) on the first conformer's terms
+        const uint32_t hint_bits = DEBYE_QHINT | DEBYE_QHINT_UNIFORM | DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ;
+        if (flags & ~(uint32_t)(DEBYE_SINC_RECUR | hint_bits)) return DEBYE_EINVAL;
+        if ((flags & DEBYE_QHINT_START0) && (flags & DEBYE_QHINT_STARTDQ)) return DEBYE_EINVAL;
+        if (N > (1 << 24)) return DEBYE_EUNSUPPORTED;
+        std::lock_guard<std::mutex> lock(g_mu);
+        DevState *ds; int st;
+        if ((st = dev_state(&ds))) return st;
+        const Choice c = choose(V_RECUR, n_idx);
+        return run_peratom_recur(ds, xyz, ff, N, q, M, I_out, cls, c.n_chunks, (c.K + 7) / 8 * 8, (cudaStream_t)stream_, B);
+    }
+    // any other grid or variant: the single-structure sequence per conformer on the same stream (stream order serialises the
+    // shared scratch)
+    for (int b = 0; b < B; ++b) {
+        const int st = debye_profile_peratom(xyz + (size_t)b * N * 3, ff, N, q, M, I_out + (size_t)b * M, flags, stream_);
+        if (st) return st;
+    }
     return DEBYE_OK;
 }
 

@@ -241,6 +241,7 @@ __global__ void __launch_bounds__(DEBYE_IB, F64 ? 2 : DEBYE_PA_CTAS) debye_perat
 // that touched q index k (8 record loads in flight, added in CTA order); the parts are then added in slice order, so the
 // order is a fixed function of (N, M, G) and the result is bitwise reproducible.
 #define DEBYE_PA_FS 8
+// Batches (debye_profile_peratom_batch): blockIdx.y is the conformer; the unit line is conformer -> chunk -> row -> j.
 // rplan != nullptr: the records come from debye_peratom_recur_kernel (debye_peratom_recur.cuh): chain slots (slot_of) holding
 // sums of 2 sin(q r)/r; a wrong grid hint (rplan->bad) gives NaN.
 struct PeratomPlan;
@@ -252,6 +253,8 @@ __global__ void __launch_bounds__(32 * DEBYE_PA_FS) debye_peratom_final_kernel(c
     pdl_wait();
     const int kk = threadIdx.x & 31, sl = threadIdx.x >> 5;
     const int k = blockIdx.x * 32 + kk;
+    const int b = blockIdx.y, Bn = gridDim.y;
+    out += (int64_t)b * M;
     const int rows = debye_diag_rows(N);
     const int64_t U1 = rows > 0 ? debye_diag_row_prefix(N, rows) : 0;
     const bool recur = rplan != nullptr;
@@ -260,13 +263,14 @@ __global__ void __launch_bounds__(32 * DEBYE_PA_FS) debye_peratom_final_kernel(c
     if (k < M && U1 > 0 && qv[k] != 0.0f && !bad) {
         int ch = k / KQ, l = k % KQ;
         if (recur) slot_of(V_RECUR, KQ, n_chunks, k + rplan[1] - 1, ch, l);
-        const int64_t U = U1 * n_chunks, ub = (int64_t)ch * U1, ue = ub + U1 - 1;
+        const int64_t X = (int64_t)b * n_chunks + ch;          // record slot of (conformer, chunk)
+        const int64_t U = U1 * n_chunks * Bn, ub = X * U1, ue = ub + U1 - 1;
         const DebyeRanges ranges(U, G);
         if (U >= G) {           // every CTA owns at least one unit: all CTAs between the owners took part
             const int c_lo = ranges.owner(ub), c_hi = ranges.owner(ue);
             const int n = c_hi - c_lo + 1, per = (n + DEBYE_PA_FS - 1) / DEBYE_PA_FS;
             const int cb = c_lo + sl * per, ce = min(c_hi + 1, cb + per);
-            const double *rp = records + ((int64_t)cb + ch) * KQ + l;
+            const double *rp = records + ((int64_t)cb + X) * KQ + l;
             int c = cb;
             for (; c + 8 <= ce; c += 8, rp += 8 * (int64_t)KQ) {
                 double r[8];
@@ -277,7 +281,7 @@ __global__ void __launch_bounds__(32 * DEBYE_PA_FS) debye_peratom_final_kernel(c
             }
             for (; c < ce; ++c, rp += KQ) s += rp[0];
         } else if (sl == 0) {   // fewer units than CTAs: each unit has its own CTA
-            for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)ranges.owner(u) + ch) * KQ + l];
+            for (int64_t u = ub; u <= ue; ++u) s += records[((int64_t)ranges.owner(u) + X) * KQ + l];
         }
     }
     part[sl][kk] = s;

@@ -37,11 +37,12 @@ struct PeratomPlan { int32_t bad, koff; double dq; };
 // (0, n_chunks) classifies the grid).  K slots per chunk.
 static __global__ void __launch_bounds__(256) debye_peratom_pack_kernel(const float *__restrict__ xyz, const float *__restrict__ ff, const float *__restrict__ q, int N, int M,
                                                                    int K, int n_chunks, int hint_class, float4 *__restrict__ pos4, float *__restrict__ ffp,
-                                                                   PeratomPlan *__restrict__ plan)
+                                                                   PeratomPlan *__restrict__ plan, int B)
 {
     const int y = blockIdx.y;
     if (y == n_chunks) {
-        for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+        const int64_t NB = (int64_t)N * B;                  // positions of all conformers, [B][N]
+        for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < NB; i += (int64_t)gridDim.x * blockDim.x) {
             const float *s = xyz + (size_t)i * 3;
             pos4[i] = make_float4(s[0], s[1], s[2], 0.f);
         }
@@ -197,7 +198,7 @@ __device__ __forceinline__ bool peratom_tile(u64 (&acc)[K / 2], const float4 *__
 template <int K>
 __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_peratom_recur_kernel(const float4 *__restrict__ pos4, const float *__restrict__ ffp, const float *__restrict__ qv,
                                                                                          const PeratomPlan *__restrict__ plan, int N, int M, int n_chunks, float theta_min,
-                                                                                         double *__restrict__ records)
+                                                                                         double *__restrict__ records, int B)
 {
     constexpr int JT = DEBYE_PAR_JT_OF(K), NW = DEBYE_IB / 32;
     static_assert(JT <= DEBYE_PAR_JT && JT % 2 == 0, "tile size");
@@ -211,7 +212,7 @@ __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_per
     const int G = gridDim.x, c = blockIdx.x;
     const int rows = debye_diag_rows(N);
     const int64_t U1 = rows > 0 ? debye_diag_row_prefix(N, rows) : 0;
-    const int64_t U = U1 * n_chunks;
+    const int64_t U = U1 * n_chunks * B;                    // unit line: conformer -> chunk -> row -> j
     if (U == 0) return;
     const int64_t u0 = debye_range_begin(U, c, G);
     const int64_t u1 = (c + 1 == G) ? U : debye_range_begin(U, c + 1, G);
@@ -239,27 +240,29 @@ __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_per
 #pragma unroll
     for (int i = 0; i < K / 2; ++i) acc[i] = 0;
     double run = 0.0;                  // thread l < K: FP64 running sum of slot l of the current chunk
-    int ch_cur = -1;
+    int64_t X_cur = -1;                // record slot (conformer, chunk) the running sums belong to
 
     int64_t u = u0;
     while (u < u1) {
-        // ---- decode unit u -> (q-chunk, row, first j) ------------------------------------------------------------------
-        const int ch = (int)(u / U1);
-        const int64_t v = u - (int64_t)ch * U1;
+        // ---- decode unit u -> (conformer, q-chunk, row, first j) ---------------------------------------------------------
+        const int64_t X = u / U1;
+        const int b = (int)(X / n_chunks), ch = (int)(X - (int64_t)b * n_chunks);
+        const int64_t v = u - X * U1;
+        const float4 *pos4b = pos4 + (int64_t)b * N;
         int rl = 0, rh = rows;
         while (rh - rl > 1) { const int mid = (rl + rh) >> 1; if (debye_diag_row_prefix(N, mid) <= v) rl = mid; else rh = mid; }
         const int row = rl;
         const int64_t jo = v - debye_diag_row_prefix(N, row);
         const int64_t row_units = (int64_t)N - 1 - (int64_t)row * DEBYE_IB;
         const int len = (int)min(min((int64_t)(u1 - u), row_units - jo), (int64_t)DEBYE_PAR_FLUSH);
-        if (ch != ch_cur) {
-            if (ch_cur >= 0 && tid < K) { records[((int64_t)c + ch_cur) * K + tid] = run; run = 0.0; }
-            ch_cur = ch;
+        if (X != X_cur) {
+            if (X_cur >= 0 && tid < K) { records[((int64_t)c + X_cur) * K + tid] = run; run = 0.0; }
+            X_cur = X;
         }
         const int mode = (n_chunks == 1) ? PM_C1 : (ch == 0 ? PM_C2A : PM_C2B);
         const int i = row * DEBYE_IB + tid;
         const bool ivalid = i < N;
-        const float4 pi = pos4[ivalid ? i : 0];
+        const float4 pi = pos4b[ivalid ? i : 0];
         const int j_first = row * DEBYE_IB + 1 + (int)jo;
         const float *ffc = ffp + (size_t)ch * N * K;
         const int ntile = (len + JT - 1) / JT;
@@ -268,7 +271,7 @@ __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_per
             const int cnt = min(len - t * JT, JT);
             const uint32_t pb = (uint32_t)cnt * 16u, fb = (uint32_t)cnt * (uint32_t)K * 4u;
             mbar_expect_tx(&mbar[buf], pb + fb);
-            bulk_g2s(&tpos[buf][0], pos4 + j_first + t * JT, pb, &mbar[buf]);
+            bulk_g2s(&tpos[buf][0], pos4b + j_first + t * JT, pb, &mbar[buf]);
             bulk_g2s(&tff[buf][0][0], ffc + (size_t)(j_first + t * JT) * K, fb, &mbar[buf]);
         };
         if (tid == 0) issue(0, 0);
@@ -343,7 +346,7 @@ __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_per
         }
         u += len;
     }
-    if (ch_cur >= 0 && tid < K) records[((int64_t)c + ch_cur) * K + tid] = run;
+    if (X_cur >= 0 && tid < K) records[((int64_t)c + X_cur) * K + tid] = run;
 }
 
 }  // namespace debye

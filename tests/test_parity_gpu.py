@@ -812,6 +812,38 @@ def test_peratom_recurrence_on_hinted_uniform_grids(db):
     assert rel(db.debye_profile_peratom(x, f, q, hint=db.q_hint(w.q)).cpu().numpy(), orc.debye_peratom(w.xyz, ff, w.q)) <= TOL32
 
 
+def test_peratom_batch_of_conformers_shares_the_table(db):
+    """debye_profile_peratom_batch (include/debye.h): B conformers, one per-atom table.  Hinted grids from 0 and from dq run one
+    fused launch sequence (unit line conformer -> chunk -> row -> j), one and two chunks, a wave of CTAs that spans several
+    conformers and conformers that span several CTAs; other grids / variants run conformer by conformer.  Against the
+    per-atom oracle on every conformer and against the single-structure entry."""
+    import torch
+    rng = np.random.default_rng(17)
+    for si, (B, N, M, q_min) in enumerate([(5, 300, 64, 0.0), (3, 900, 101, 0.0), (7, 130, 50, 0.02), (2, 1100, 200, 0.0), (33, 40, 17, 0.0)]):
+        w = wl.small_random(500 + si, N, 3, M, q_min=q_min, q_max=q_min * M if q_min else 0.6, box=10.0 + N ** (1 / 3) * 3)
+        ff = _peratom_ff(w, 600 + si)
+        xyz = (w.xyz[None] + rng.normal(0, 0.7, (B,) + w.xyz.shape)).astype(np.float32)
+        hint = db.q_hint(w.q)
+        x, f, q = (torch.from_numpy(a_).cuda() for a_ in (xyz, ff, w.q))
+        Ib = db.debye_profile_peratom_batch(x, f, q, hint=hint).cpu().numpy()
+        assert Ib.shape == (B, M)
+        assert Ib.tobytes() == db.debye_profile_peratom_batch(x, f, q, hint=hint).cpu().numpy().tobytes()          # run to run
+        for b in range(B):
+            ref = orc.debye_peratom(xyz[b], ff, w.q)
+            assert rel(Ib[b], ref) <= TOL32, (B, N, M, b, rel(Ib[b], ref))
+            one = db.debye_profile_peratom(x[b].contiguous(), f, q, hint=hint).cpu().numpy()
+            assert rel(Ib[b], one) <= 1e-6                                                                        # same terms, other CTA ranges
+        if si == 0:      # no hint, MUFU and FP64: conformer by conformer, bit for bit the single-structure call
+            for kw in (dict(), dict(variant="mufu"), dict(variant="fp64")):
+                I2 = db.debye_profile_peratom_batch(x, f, q, **kw).cpu().numpy()
+                for b in range(B):
+                    assert I2[b].tobytes() == db.debye_profile_peratom(x[b].contiguous(), f, q, **kw).cpu().numpy().tobytes()
+            wrong = (1 << 8) | (1 << 9) | (1 << 11)          # "q_k = (k + 1) dq" promised for a grid that starts at 0
+            assert np.isnan(db.debye_profile_peratom_batch(x, f, q, hint=wrong).cpu().numpy()).all()
+    with pytest.raises(db.LibdebyeError):
+        db.debye_profile_peratom_batch(x[:0], f, q)
+
+
 def test_peratom_degenerate_inputs(db):
     import torch
     q = np.array([0.0, 0.05, 0.4, 1.3], dtype=np.float32)

@@ -362,6 +362,7 @@ int small_grid(DevState *ds, int N, int T, int K, int *G)
     // with 296, 33.3 / 42.9 with 592: every CTA pays the sort, and the final stage grows with the number of records)
     int64_t g = units / 6;
     if (g > (int64_t)ds->sms) g = (int64_t)ds->sms;
+    if (g > DEBYE_SMALL_GMAX) g = DEBYE_SMALL_GMAX;            // what the kernel's shared-memory layout of the final stage holds
     if (g < 1) g = 1;
     *G = (int)g;
     return DEBYE_OK;

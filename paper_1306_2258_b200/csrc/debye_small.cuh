@@ -29,6 +29,16 @@ namespace debye {
 #define DEBYE_SMALL_TMAX 8
 #define DEBYE_SMALL_TP (DEBYE_SMALL_TMAX * (DEBYE_SMALL_TMAX + 1) / 2)
 #define DEBYE_KMAX_LEVELS 17      // chain elements of one output: at most ceil(129 / 8)
+#define DEBYE_SMALL_GMAX 256      // largest grid (one CTA per SM at most; the hosts cap it)
+// Cost balance of the unit line: starting a row segment (pipeline fill, masked head, its share of a flush) costs about as much as
+// DEBYE_SMALL_WROW units (one j atom x 128 i atoms), measured on B200 with 1000 atoms / 5 types: 26 units in one segment 6.1 us,
+// in five segments 12.0 us.  Every row therefore counts DEBYE_SMALL_WROW virtual units in front of its real ones when the line
+// is cut into equal ranges, so a CTA whose range crosses many short rows gets fewer real units.  0: plain unit count.
+#ifndef DEBYE_SMALL_WROW
+#define DEBYE_SMALL_WROW 16
+#endif
+// diagonal type pair with n atoms: weighted units before row r
+__host__ __device__ inline int debye_small_diag_prefix(int n, int r) { return (int)debye_diag_row_prefix(n, r) + DEBYE_SMALL_WROW * r; }
 
 struct SmallPlan {
     int32_t n_a[DEBYE_SMALL_TMAX], seg_off[DEBYE_SMALL_TMAX + 1];
@@ -41,7 +51,9 @@ struct SmallPlan {
 __host__ __device__ inline size_t debye_small_dyn_smem(int N, int T, int K)
 {
     (void)K;
-    const size_t a = (size_t)((N + 7) / 8 * 8 + 8) * 16, s = (size_t)(T * (T + 1) / 2) * (DEBYE_KMAX_LEVELS + 1) * 8;
+    // final phase: part[n_tp][levels] + S[n_tp], then the slice sums [levels][slices], slices <= grid / 8 + n_tp, grid <= 256
+    const size_t a = (size_t)((N + 7) / 8 * 8 + 8) * 16,
+                 s = (size_t)(T * (T + 1) / 2) * (DEBYE_KMAX_LEVELS + 1) * 8 + (size_t)(DEBYE_SMALL_GMAX / 8 + T * (T + 1) / 2) * DEBYE_KMAX_LEVELS * 8;
     return a > s ? a : s;
 }
 
@@ -137,11 +149,11 @@ __global__ void __launch_bounds__(DEBYE_IB, recur_min_ctas(K)) debye_small_kerne
                 int units, ti = a, tj = b2;
                 if (a == b2) {
                     const int rows = debye_diag_rows(na);
-                    units = rows > 0 ? (int)debye_diag_row_prefix(na, rows) : 0;
+                    units = rows > 0 ? debye_small_diag_prefix(na, rows) : 0;
                 } else {
                     const int ra = (na + DEBYE_IB - 1) / DEBYE_IB, rb = (nb + DEBYE_IB - 1) / DEBYE_IB;
-                    const int ua = ra * nb, ub = rb * na;
-                    if (ub < ua) { ti = b2; tj = a; units = ub; } else units = ua;
+                    const int ua = ra * nb, ub = rb * na;                  // the side with less padding becomes the row side ...
+                    if (ub < ua) { ti = b2; tj = a; units = rb * (na + DEBYE_SMALL_WROW); } else units = ra * (nb + DEBYE_SMALL_WROW);   // ... weighted
                     if (na == 0 || nb == 0) units = 0;
                 }
                 sp.tp_ti[tp] = ti; sp.tp_tj[tp] = tj; sp.tp_prefix[tp] = upre;
@@ -229,18 +241,24 @@ __global__ void __launch_bounds__(DEBYE_IB, recur_min_ctas(K)) debye_small_kerne
             const int ti = sp.tp_ti[tp], tj = sp.tp_tj[tp];
             const bool diag = (ti == tj);
             const int n_i = sp.n_a[ti], n_j = sp.n_a[tj];
-            int row, jo, row_units;
-            if (!diag) { row = v / n_j; jo = v % n_j; row_units = n_j; }
+            int row, jo, row_units;          // jo < 0: inside the row's virtual units (DEBYE_SMALL_WROW)
+            if (!diag) { row = v / (n_j + DEBYE_SMALL_WROW); jo = v % (n_j + DEBYE_SMALL_WROW) - DEBYE_SMALL_WROW; row_units = n_j; }
             else {
                 int rl = 0, rh = debye_diag_rows(n_i);
-                while (rh - rl > 1) { const int mid = (rl + rh) >> 1; if ((int)debye_diag_row_prefix(n_i, mid) <= v) rl = mid; else rh = mid; }
-                row = rl; jo = v - (int)debye_diag_row_prefix(n_i, row); row_units = n_i - 1 - row * DEBYE_IB;
+                while (rh - rl > 1) { const int mid = (rl + rh) >> 1; if (debye_small_diag_prefix(n_i, mid) <= v) rl = mid; else rh = mid; }
+                row = rl; jo = v - debye_small_diag_prefix(n_i, row) - DEBYE_SMALL_WROW; row_units = n_i - 1 - row * DEBYE_IB;
             }
-            const int len = min(u1 - u, row_units - jo);
+            // every CTA whose range touches the type pair -- even in virtual units only -- owns a record of it (the final stage
+            // reads the records of all CTAs between the owners of the type pair's first and last unit)
             if (tp != curX) {
                 if (curX >= 0) { if (pending) flush(); pending = 0; if (tid < K) { records[((int64_t)c + curX) * K + tid] = run; run = 0.0; } }
                 curX = tp;
             }
+            if (jo < 0) {                    // skip the virtual units; the range may end inside them
+                u += -jo; jo = 0;
+                if (u >= u1) break;
+            }
+            const int len = min(u1 - u, row_units - jo);
             const int i_local = row * DEBYE_IB + tid;
             const bool ivalid = i_local < n_i;
             const float4 pi = atoms[sp.seg_off[ti] + (ivalid ? i_local : 0)];
@@ -277,17 +295,27 @@ __global__ void __launch_bounds__(DEBYE_IB, recur_min_ctas(K)) debye_small_kerne
         }
         s_clo[tid] = lo_c; s_chi[tid] = hi_c;
     }
-    TR(2);
-    __threadfence();
-    cooperative_groups::this_grid().sync();
-    TR(3);
+    // slices of 8 CTAs per type pair (final stage): s_soff[tp] = slices before type pair tp
+    __shared__ int s_soff[DEBYE_SMALL_TP + 1], s_maxg;
+    __syncthreads();
+    if (tid == 0) {
+        int pre = 0, mg = 1;
+        for (int tp = 0; tp < n_tp; ++tp) {
+            const int g8 = (s_chi[tp] >= s_clo[tp]) ? (s_chi[tp] - s_clo[tp]) / 8 + 1 : 0;
+            s_soff[tp] = pre; pre += g8;
+            if (g8 > mg) mg = g8;
+        }
+        s_soff[n_tp] = pre; s_maxg = mg;                    // most slices of one type pair
+    }
+    // What output k needs beyond the records -- q_k, the table column F[.][k], the slots of its telescoped chain -- does not
+    // depend on the pairs phase: it is fetched BEFORE the grid barrier for the CTA's first output (two global-memory latencies
+    // off the critical path of the final stage, which every CTA with an output runs after the slowest CTA's arrival).
     __shared__ int s_slot[DEBYE_KMAX_LEVELS], s_nlev;
-    double *part = reinterpret_cast<double *>(dyn);       // the atoms are no longer needed: part[n_tp][nlev], Sq[n_tp]
-    const double nan = __longlong_as_double(0x7ff8000000000000LL);
-    for (int k = c; k < M; k += G) {                      // one CTA per q index (both modes)
-        const double qk = (double)q[k];
-        __syncthreads();                                  // part / s_slot of the previous k are no longer read
-        if (tid == 0) {                                   // the telescoped chain  B_kappa = Out[slot(kappa)] + B_{8 j - kres}  (debye_pairs.cuh)
+    __shared__ float s_F[DEBYE_SMALL_TMAX], s_qk;
+    auto prep = [&](const int k) {
+        if (tid < DEBYE_SMALL_TMAX) s_F[tid] = (tid < T && mode == 0) ? fftab[tid * M + k] : 0.f;
+        if (tid == 32) s_qk = q[k];
+        if (tid == 64) {                                  // the telescoped chain  B_kappa = Out[slot(kappa)] + B_{8 j - kres}  (debye_pairs.cuh)
             int n = 0;
             for (int kap = k + koff; kap > 0;) {
                 const int j = (kap - 1) >> 3, kres = kap - 8 * j;
@@ -296,25 +324,70 @@ __global__ void __launch_bounds__(DEBYE_IB, recur_min_ctas(K)) debye_small_kerne
             }
             s_nlev = n;
         }
-        __syncthreads();
+    };
+    if (c < M) prep(c);
+    TR(2);
+    __threadfence();
+    cooperative_groups::this_grid().sync();
+    TR(3);
+    double *part = reinterpret_cast<double *>(dyn);       // the atoms are no longer needed: part[n_tp][nlev], Sq[n_tp]
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
+    for (int k = c; k < M; k += G) {                      // one CTA per q index (both modes)
+        if (k != c) {
+            __syncthreads();                              // part / s_slot / s_F of the previous k are no longer read
+            prep(k);
+            __syncthreads();
+        }
+        const double qk = (double)s_qk;
         const int nlev = s_nlev;
-        // one thread per (type pair, chain element): the records of the type pair's CTAs in CTA order, eight loads in flight
-        for (int task = tid; task < n_tp * nlev; task += DEBYE_IB) {
+        // The records of a type pair's CTAs are added in CTA order in slices of 8 (one thread per (chain element, slice): eight
+        // loads in flight, the records sit in L2), then the slices in slice order (one thread per (type pair, chain element)).
+        // One thread per (type pair, chain element) walking the whole CTA range took 5 us for the outputs with five chain
+        // elements (measured, 1000 atoms) -- and the slowest CTA of the final stage ends the kernel.
+        const int ntask = n_tp * nlev;
+        double *Sq = part + ntask;
+        double *ssum = Sq + n_tp;                                   // [nlev][slices]
+        const int nsl = s_soff[n_tp];
+        // ... unless the (type pair, chain element) tasks already fill the CTA and no type pair spans many CTAs (many types): in
+        // global-memory latencies, passes x slices of the longest walk against passes over the slices + 1
+        const bool by_slices = (nsl * nlev + DEBYE_IB - 1) / DEBYE_IB + 1 < (ntask + DEBYE_IB - 1) / DEBYE_IB * s_maxg;
+        if (!bad && U >= G && by_slices) {
+            for (int item = tid; item < nsl * nlev; item += DEBYE_IB) {
+                const int e = item / nsl, sidx = item - e * nsl, l = s_slot[e];
+                int tp = 0;
+                while (s_soff[tp + 1] <= sidx) ++tp;                // <= 36 steps
+                int cc = s_clo[tp] + 8 * (sidx - s_soff[tp]);
+                const int ce = min(s_chi[tp] + 1, cc + 8);
+                const double *rp = records + ((int64_t)cc + tp) * K + l;
+                double r[8];
+#pragma unroll
+                for (int x = 0; x < 8; ++x) r[x] = (cc + x < ce) ? __ldcg(rp + x * K) : 0.0;
+                double sum = 0.0;
+#pragma unroll
+                for (int x = 0; x < 8; ++x) sum += r[x];
+                ssum[item] = sum;
+            }
+        }
+        __syncthreads();
+        for (int task = tid; task < ntask; task += DEBYE_IB) {
             const int tp = task / nlev, e = task - tp * nlev, l = s_slot[e];
             double sum = 0.0;
             if (!bad && U > 0) {
-                if (U >= G) {
-                    const int c_lo = s_clo[tp], c_hi = s_chi[tp];
-                    const double *rp = records + ((int64_t)c_lo + tp) * K + l;
-                    int cc = c_lo;
-                    for (; cc + 8 <= c_hi + 1; cc += 8, rp += 8 * K) {
+                if (U >= G && by_slices) {
+                    for (int x = s_soff[tp]; x < s_soff[tp + 1]; ++x) sum += ssum[e * nsl + x];
+                } else if (U >= G) {                      // this thread walks the type pair's CTA range: slices of 8 in CTA order
+                    int cc = s_clo[tp];
+                    const int c_hi = s_chi[tp];
+                    const double *rp = records + ((int64_t)cc + tp) * K + l;
+                    for (; cc <= c_hi; cc += 8, rp += 8 * K) {
                         double r[8];
 #pragma unroll
-                        for (int x = 0; x < 8; ++x) r[x] = __ldcg(rp + x * K);
+                        for (int x = 0; x < 8; ++x) r[x] = (cc + x <= c_hi) ? __ldcg(rp + x * K) : 0.0;
+                        double s8 = 0.0;
 #pragma unroll
-                        for (int x = 0; x < 8; ++x) sum += r[x];
+                        for (int x = 0; x < 8; ++x) s8 += r[x];
+                        sum += s8;
                     }
-                    for (; cc <= c_hi; ++cc, rp += K) sum += __ldcg(rp);
                 } else {                                  // fewer units than CTAs: each unit has its own CTA
                     const DebyeRanges ranges(U, G);
                     for (int uu = sp.tp_prefix[tp]; uu < sp.tp_prefix[tp + 1]; ++uu) sum += __ldcg(records + ((int64_t)ranges.owner(uu) + tp) * K + l);
@@ -323,7 +396,6 @@ __global__ void __launch_bounds__(DEBYE_IB, recur_min_ctas(K)) debye_small_kerne
             part[task] = sum;
         }
         __syncthreads();
-        double *Sq = part + n_tp * nlev;
         if (tid < n_tp) {
             const int tp = tid;
             const int a = min(sp.tp_ti[tp], sp.tp_tj[tp]), b2 = max(sp.tp_ti[tp], sp.tp_tj[tp]);
@@ -336,23 +408,20 @@ __global__ void __launch_bounds__(DEBYE_IB, recur_min_ctas(K)) debye_small_kerne
                 for (int e = 0; e < nlev; ++e) sum += part[tp * nlev + e];
                 S = 0.5 * sum / qk;
             }
-            if (mode == 0) Sq[tp] = S; else out[tp * M + k] = S;
+            // mode 0: the type pair's term of I(q_k) (one thread per type pair: a single thread multiplying all of them out ran a
+            // dependent FP64 chain of 1.8 us, measured with 15 type pairs)
+            if (mode == 0) Sq[tp] = 2.0 * (double)s_F[a] * (double)s_F[b2] * S; else out[tp * M + k] = S;
         }
         if (mode == 0) {
             __syncthreads();
             if (tid == 0) {
                 double F[DEBYE_SMALL_TMAX];                 // the table column of this q: all loads in flight together
 #pragma unroll
-                for (int a = 0; a < DEBYE_SMALL_TMAX; ++a) F[a] = (a < T) ? (double)fftab[a * M + k] : 0.0;
+                for (int a = 0; a < DEBYE_SMALL_TMAX; ++a) F[a] = (double)s_F[a];               // 0 beyond T
                 double tot = 0.0;
 #pragma unroll
                 for (int a = 0; a < DEBYE_SMALL_TMAX; ++a) tot += (double)sp.n_a[a] * F[a] * F[a];        // n_a = 0 beyond T
-                int tp = 0;
-#pragma unroll
-                for (int a = 0; a < DEBYE_SMALL_TMAX; ++a)
-#pragma unroll
-                    for (int b2 = a; b2 < DEBYE_SMALL_TMAX; ++b2)
-                        if (b2 < T) { tot += 2.0 * F[a] * F[b2] * Sq[tp]; ++tp; }      // type pairs in increasing order
+                for (int tp = 0; tp < n_tp; ++tp) tot += Sq[tp];                                         // type pairs in increasing order
                 out[k] = tot;
             }
         }

@@ -333,12 +333,16 @@ __device__ __forceinline__ void prod_hot(u64 (&acc)[K / 2], const u64 (&U)[4], c
 #else
 #define DEBYE_PROD_UNROLL_PRAGMA
 #endif
-// pairs per iteration: two (amortises the loop overhead and gives the scheduler two independent start-up chains; measured
-// on B200 against one pair per iteration: +4 % cfg2, +9 % cfg3, +4 % cfg4, +6 % cfg5)
-#ifndef DEBYE_NPP
-#define DEBYE_NPP 2
-#endif
+// pairs per iteration: two or three (amortises the loop overhead and gives the scheduler independent start-up chains).  Measured
+// on B200: two against one +4 % cfg2, +9 % cfg3, +4 % cfg4, +6 % cfg5; three against two on a 10 000-atom structure, T pair.q/s by
+// K: 24 6.79/6.83, 32 8.61/8.18, 40 9.45/9.59, 48 10.32/10.42, 56 11.63/11.52, 64 12.67/12.05, 72 12.96/12.72, 80 14.13/13.90,
+// 88 14.66/14.54, 96 14.31/14.62, 100 13.54/15.18, 104 13.49/15.09 (2.4 KB of spills at 168 registers), 112 15.55/14.70,
+// 120 16.00/15.82, 128 16.84/16.02; cfg4 (K = 64) 0.710 -> 0.757, cfg5 (K = 128) 1.014 -> 1.076 of the 2-lane-op roofline
+#ifdef DEBYE_NPP
 __host__ __device__ constexpr int prod_np(int K) { return DEBYE_NPP; }
+#else
+__host__ __device__ constexpr int prod_np(int K) { return ((K >= 56 && K <= 88) || K >= 112 || K == 32) ? 3 : 2; }
+#endif
 template <int K, int MODE, bool W>
 __device__ __forceinline__ void prod_tile(u64 (&acc)[K / 2], const float4 *__restrict__ tile, const int jj0, const int cnt, const float4 pi,
                                           const bool ivalid, const bool diag, const int i_local, const int jl0, const RecurConst &rc,

@@ -51,9 +51,11 @@ struct SmallPlan {
 __host__ __device__ inline size_t debye_small_dyn_smem(int N, int T, int K)
 {
     (void)K;
-    // final phase: part[n_tp][levels] + S[n_tp], then the slice sums [levels][slices], slices <= grid / 8 + n_tp, grid <= 256
+    // final phase: part[n_tp][levels] + S[n_tp], then the slice sums [levels][slices]; the CTA ranges of the n_tp type pairs cover
+    // at most grid + n_tp CTAs (neighbours share a CTA), so slices <= (grid + n_tp) / 8 + n_tp, grid <= DEBYE_SMALL_GMAX
+    const size_t n_tp = (size_t)(T * (T + 1) / 2);
     const size_t a = (size_t)((N + 7) / 8 * 8 + 8) * 16,
-                 s = (size_t)(T * (T + 1) / 2) * (DEBYE_KMAX_LEVELS + 1) * 8 + (size_t)(DEBYE_SMALL_GMAX / 8 + T * (T + 1) / 2) * DEBYE_KMAX_LEVELS * 8;
+                 s = n_tp * (DEBYE_KMAX_LEVELS + 1) * 8 + ((DEBYE_SMALL_GMAX + n_tp) / 8 + n_tp + 1) * DEBYE_KMAX_LEVELS * 8;
     return a > s ? a : s;
 }
 

@@ -66,6 +66,7 @@ struct DevState {
     void *ws = nullptr; size_t ws_bytes = 0;          // library-owned scratch
     void *user_ws = nullptr; size_t user_bytes = 0;   // caller-owned scratch (debye_set_workspace)
     void *stage = nullptr; size_t stage_bytes = 0;    // device staging for the *_host entry points
+    void *hstage = nullptr; size_t hstage_bytes = 0;  // pinned host staging: small inputs of the *_host entries travel as ONE copy
     int sms = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;         // optional: recorded around the pairs launches
     // cross-stream ordering of the shared scratch (workspace, staging buffer): every call records ws_done behind its last
@@ -77,7 +78,9 @@ struct DevState {
 };
 DevState g_dev[MAX_DEV];
 std::mutex g_mu;
+std::mutex g_hstage_mu;                               // one *_host call at a time fills and drains the pinned staging buffer
 bool g_atexit = false;
+constexpr size_t HOST_ONE_COPY_MAX = 256 * 1024;      // inputs up to this size are gathered on the host and copied once
 
 size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
@@ -294,13 +297,14 @@ int grid_for(DevState *s, const Choice &c, int N, int B, int *G, bool weighted =
 void shutdown_all()
 {
     for (int d = 0; d < MAX_DEV; ++d) {
-        if (g_dev[d].ws || g_dev[d].stage) {
+        if (g_dev[d].ws || g_dev[d].stage || g_dev[d].hstage) {
             int cur = 0;
             if (cudaGetDevice(&cur) != cudaSuccess) return;
             if (cudaSetDevice(d) != cudaSuccess) continue;
             if (g_dev[d].ws) cudaFree(g_dev[d].ws);
             if (g_dev[d].stage) cudaFree(g_dev[d].stage);
-            g_dev[d].ws = g_dev[d].stage = nullptr; g_dev[d].ws_bytes = g_dev[d].stage_bytes = 0;
+            if (g_dev[d].hstage) cudaFreeHost(g_dev[d].hstage);
+            g_dev[d].ws = g_dev[d].stage = g_dev[d].hstage = nullptr; g_dev[d].ws_bytes = g_dev[d].stage_bytes = g_dev[d].hstage_bytes = 0;
             cudaSetDevice(cur);
         }
     }
@@ -492,31 +496,59 @@ int run_host(const float *xyz, const int32_t *type, int N, int B, const float *f
     int st = validate(xyz, type, N, B, fftab, T, q, M, out, flags);
     if (st) return st;
     DevState *ds;
-    char *base;
-    size_t o_xyz, o_type, o_tab, o_q, o_out, o_w, total;
+    char *base, *hbase = nullptr;
+    size_t o_xyz, o_type, o_tab, o_q, o_out, o_w, o_in, total;
     {
-        std::lock_guard<std::mutex> lock(g_mu);
-        if ((st = dev_state(&ds))) return st;
-        size_t o = 0;
+        size_t o = 0;                              // the inputs first, contiguous, so that they can travel as one copy
         o_xyz = o; o += align_up((size_t)N * B * 12);
         o_type = o; o += align_up((size_t)N * 4);
         o_tab = o; o += align_up((size_t)T * M * 4);
         o_q = o; o += align_up((size_t)M * 4);
-        o_out = o; o += align_up((size_t)B * M * 8);
         o_w = o; o += align_up((size_t)N * 4);
+        o_in = o;
+        o_out = o; o += align_up((size_t)B * M * 8);
         total = o;
+    }
+    // Small inputs (for small proteins the transfers, not the pairs, dominate): gathered into a pinned staging buffer
+    // on the host and copied ONCE instead of four or five copies of a few KB each.  One such call at a time per process: the
+    // buffer is refilled by the next call, so the lock is held until this call's copy has been consumed (the final synchronise).
+    const bool one_copy = o_in <= HOST_ONE_COPY_MAX;
+    std::unique_lock<std::mutex> hlock(g_hstage_mu, std::defer_lock);
+    if (one_copy) hlock.lock();
+    {
+        std::lock_guard<std::mutex> lock(g_mu);
+        if ((st = dev_state(&ds))) return st;
         if ((st = ensure(&ds->stage, &ds->stage_bytes, total))) return st;
         base = (char *)ds->stage;
+        if (one_copy) {
+            if (ds->hstage_bytes < o_in) {
+                if (ds->hstage) { CU(cudaFreeHost(ds->hstage)); ds->hstage = nullptr; ds->hstage_bytes = 0; }
+                cudaError_t e = cudaHostAlloc(&ds->hstage, HOST_ONE_COPY_MAX, cudaHostAllocDefault);
+                if (e != cudaSuccess) { (void)cudaGetLastError(); g_last_cuda = (int)e; ds->hstage = nullptr; return DEBYE_ENOMEM; }
+                ds->hstage_bytes = HOST_ONE_COPY_MAX;
+                if (!g_atexit) { g_atexit = true; atexit(shutdown_all); }
+            }
+            hbase = (char *)ds->hstage;
+        }
         CU(scratch_acquire(ds->order, stream));    // the staging buffer is shared scratch too; run() releases behind the last kernel
     }
-    CU(cudaMemcpyAsync(base + o_xyz, xyz, (size_t)N * B * 12, cudaMemcpyHostToDevice, stream));
-    CU(cudaMemcpyAsync(base + o_type, type, (size_t)N * 4, cudaMemcpyHostToDevice, stream));
-    CU(cudaMemcpyAsync(base + o_tab, fftab, (size_t)T * M * 4, cudaMemcpyHostToDevice, stream));
-    CU(cudaMemcpyAsync(base + o_q, q, (size_t)M * 4, cudaMemcpyHostToDevice, stream));
-    if (weight) CU(cudaMemcpyAsync(base + o_w, weight, (size_t)N * 4, cudaMemcpyHostToDevice, stream));
+    if (one_copy) {
+        memcpy(hbase + o_xyz, xyz, (size_t)N * B * 12);
+        memcpy(hbase + o_type, type, (size_t)N * 4);
+        memcpy(hbase + o_tab, fftab, (size_t)T * M * 4);
+        memcpy(hbase + o_q, q, (size_t)M * 4);
+        if (weight) memcpy(hbase + o_w, weight, (size_t)N * 4);
+        CU(cudaMemcpyAsync(base, hbase, weight ? o_in : o_w, cudaMemcpyHostToDevice, stream));
+    } else {
+        CU(cudaMemcpyAsync(base + o_xyz, xyz, (size_t)N * B * 12, cudaMemcpyHostToDevice, stream));
+        CU(cudaMemcpyAsync(base + o_type, type, (size_t)N * 4, cudaMemcpyHostToDevice, stream));
+        CU(cudaMemcpyAsync(base + o_tab, fftab, (size_t)T * M * 4, cudaMemcpyHostToDevice, stream));
+        CU(cudaMemcpyAsync(base + o_q, q, (size_t)M * 4, cudaMemcpyHostToDevice, stream));
+        if (weight) CU(cudaMemcpyAsync(base + o_w, weight, (size_t)N * 4, cudaMemcpyHostToDevice, stream));
+    }
     st = run((const float *)(base + o_xyz), (const int32_t *)(base + o_type), N, B, (const float *)(base + o_tab), T, (const float *)(base + o_q), M,
              (double *)(base + o_out), nullptr, flags, stream, 0, weight ? (const float *)(base + o_w) : nullptr);
-    if (st) return st;
+    if (st) { if (one_copy) (void)cudaStreamSynchronize(stream); return st; }      // the pinned staging buffer must be drained before it is released
     CU(cudaMemcpyAsync(out, base + o_out, (size_t)B * M * 8, cudaMemcpyDeviceToHost, stream));
     CU(cudaStreamSynchronize(stream));             // the staging buffer is free again when this returns
     return DEBYE_OK;

@@ -609,6 +609,44 @@ def test_piecewise_hint_is_checked_on_the_device_and_degenerate_pairs_keep_their
     assert worst <= TOL32, worst
 
 
+def test_c_abi_from_plain_c(db, tmp_path):
+    """The boundary is a C ABI: tests/c_abi_client.c -- plain C, include/debye.h and the CUDA runtime only, no Python and no torch
+    in the process -- is compiled with gcc, linked against libdebye.so and run on cfg1 and on a 2000-atom case; its profiles
+    (host-buffer entry, device-buffer entry, the no-allocation entry) are compared with the oracle here.  Prints the latencies
+    the client measured (host entry: one H2D copy of the gathered inputs, the kernel, one D2H copy, synchronise)."""
+    import shutil
+    import subprocess
+    import sys
+    from paper_1306_2258_b200 import binding
+    gcc, cuda = shutil.which("gcc"), os.environ.get("CUDA_HOME", "/usr/local/cuda")
+    if gcc is None or not os.path.exists(os.path.join(cuda, "include", "cuda_runtime.h")):
+        pytest.skip("needs gcc and the CUDA runtime headers")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    libdir = os.path.dirname(binding.LIB_PATH)
+    exe = str(tmp_path / "c_abi_client")
+    subprocess.check_call([gcc, "-O2", "-std=c11", "-D_POSIX_C_SOURCE=200809L", "-o", exe, os.path.join(root, "tests", "c_abi_client.c"),
+                           "-I", os.path.join(root, "include"), "-I", os.path.join(cuda, "include"), "-L", libdir, "-L", os.path.join(cuda, "lib64"),
+                           "-l:" + os.path.basename(binding.LIB_PATH), "-lcudart", "-lm",
+                           "-Wl,-rpath," + libdir, "-Wl,-rpath," + os.path.join(cuda, "lib64")])
+    for w in (wl.cfg1(), wl.small_random(71, 2000, 5, 50, q_min=0.02, q_max=1.0)):
+        fin, fout = str(tmp_path / "in.bin"), str(tmp_path / "out.bin")
+        with open(fin, "wb") as fh:
+            np.array([w.N, w.T, w.M], np.int32).tofile(fh)
+            for a in (w.xyz, w.type, w.fftab, w.q):
+                np.ascontiguousarray(a).tofile(fh)
+        r = subprocess.run([exe, fin, fout, "300"], capture_output=True, text=True, timeout=300)
+        assert r.returncode == 0, (r.stdout, r.stderr)
+        sys.stdout.write("c_abi_client: " + r.stdout)
+        res = np.fromfile(fout, np.float64)
+        assert res.shape == (3 * w.M + 3,)
+        I_host, I_dev, I_static, lat = res[:w.M], res[w.M:2 * w.M], res[2 * w.M:3 * w.M], res[3 * w.M:]
+        ref = orc.debye_sym(w.xyz, w.type, w.fftab, w.q)
+        assert rel(I_host, ref) <= TOL32 and I_host.tobytes() == I_dev.tobytes() == I_static.tobytes()
+        x, t, f, q = to_dev(w)
+        assert I_dev.tobytes() == db.debye_profile(x, t, f, q, hint=db.q_hint(w.q)).cpu().numpy().tobytes()      # the binding adds nothing
+        assert (lat > 0).all() and lat[0] < 5e3
+
+
 def test_non_finite_input_propagates_and_does_not_poison_later_calls(db):
     """include/debye.h: NaN / Inf in the inputs propagate to I_out (no hang, no crash); the next call is unaffected."""
     w = wl.small_random(70, 500, 3, 40)

@@ -60,6 +60,7 @@ cudaError_t scratch_release(ScratchOrder &o, cudaStream_t stream)
 #ifndef DEBYE_MUFU_KMAX
 #define DEBYE_MUFU_KMAX 112      // largest q-chunk of the MUFU kernel (choose())
 #endif
+static_assert(DEBYE_SETUP_MAXQ == DEBYE_MAX_Q, "the setup kernel stages the whole q grid in shared memory");
 constexpr int MAX_DEV = 64;
 constexpr int64_t DEBYE_PACK_IN_SETUP = 16384;   // N x B up to which debye_setup_kernel also packs the coordinates
 struct DevState {

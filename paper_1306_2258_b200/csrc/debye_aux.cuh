@@ -9,6 +9,7 @@
 namespace debye {
 
 #define DEBYE_SETUP_THREADS 1024
+#define DEBYE_SETUP_MAXQ 4096
 
 // S0 + S1.  One CTA: type histogram, segment offsets, stable counting-sort permutation, q-grid analysis and the
 // unit prefix per type pair.  Stable = atoms of one type keep their input order, so the sorted layout (and with
@@ -32,7 +33,9 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
     __shared__ int wcnt[NWARP][DEBYE_MAX_TYPES_I];      // pass 1: atoms of type t in warp w's chunk; pass 2: running output slot
     __shared__ int seg[DEBYE_MAX_TYPES_I + 1];
     __shared__ float red[NWARP], red2[NWARP], qmax_s[NWARP];
-    __shared__ int hint_bad_s;
+    __shared__ int hint_bad_s, s_cls, s_runs_ok, s_nruns;
+    __shared__ int32_t s_run_start[DEBYE_MAX_PIECES + 1];
+    __shared__ float q_sh[DEBYE_SETUP_MAXQ];            // q, for the piece finding (DEBYE_MAX_Q of include/debye.h)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int chunk = ((N + NWARP - 1) / NWARP + 31) / 32 * 32;
     const int c0 = warp * chunk, c1 = min(N, c0 + chunk);
@@ -77,21 +80,45 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
         plan->n_a[lane] = tot;
         if (lane == 31) plan->seg_off[32] = incl;
     }
+    float d = 0.f, s = 3.0e38f, mx = 0.f;          // thread 32: the grid's deviation from the line, smallest non-zero |q|, largest |q|
+    int cls = -2;
     if (tid == 32) {
-        float d = 0.f, s = 3.0e38f, mx = 0.f;
         for (int w = 0; w < NWARP; ++w) { d = fmaxf(d, red[w]); s = fminf(s, red2[w]); mx = fmaxf(mx, qmax_s[w]); }
-        const int cls = debye_grid_class(q0, dq, d, mx);
+        cls = debye_grid_class(q0, dq, d, mx);
+        s_cls = cls;
+    }
+    __syncthreads();
+    // Piecewise-uniform grid (the centred product form, V_CENT): promised by the hint, or -- no hint -- a uniform grid with a general
+    // start for which a centred launch is on offer.  The same segmentation as the host's (debye_plan.cuh), from a copy of q in
+    // shared memory: runs by one thread, the 1.5-ulp test of every point by all threads, pieces by one thread; it has to give the
+    // piece count and accumulator count the launch was sized for.  (A serial scan of global memory took 0.5 ms for 2000 points.)
+    const bool need_pieces = hint_class == -4 || (hint_class == -3 && hint_pieces != 0 && s_cls == -1);
+    bool pieces_ok = false;
+    if (need_pieces) {
+        for (int k = tid; k < M; k += blockDim.x) q_sh[k] = q[k];
+        __syncthreads();
+        if (tid == 32) s_runs_ok = debye_find_runs(q_sh, M, s_run_start, s_nruns) ? 1 : 0;
+        __syncthreads();
+        int ok = s_runs_ok;
+        if (ok) {
+            for (int k = tid; k < M; k += blockDim.x) {
+                int r = 0;
+                while (s_run_start[r + 1] <= k) ++r;
+                if (!debye_run_point_ok(q_sh, s_run_start[r], s_run_start[r + 1], k)) ok = 0;
+            }
+        }
+        ok = __syncthreads_and(ok);
+        if (tid == 32)
+            pieces_ok = ok && debye_pieces_from_runs(q_sh, s_run_start, s_nruns, plan->pieces) && plan->pieces.n == (hint_pieces >> 8) &&
+                        plan->pieces.K == 8 * (hint_pieces & 255);
+    }
+    if (tid == 32) {
         const int uni = cls != -2;
         // zero start: q0 == 0 exactly (koff = 0) or q0 == dq to 1e-6 (koff = 1, the paper's own grid q_k = k dq, k >= 1)
         const int koff = cls >= 0 ? cls : -1;
         hint_bad_s = (hint_class != -3 && hint_class != cls) ? 1 : 0;
-        plan->pieces.n = 0;
-        if (hint_class == -4) {
-            // piecewise-uniform grid promised (the centred product form, V_CENT): the same segmentation as the host's, and it
-            // has to give the piece count and accumulator count the launch was sized for.  Serial, O(M): hinted calls only.
-            const bool ok = debye_find_pieces(q, M, plan->pieces) && plan->pieces.n == (hint_pieces >> 8) && plan->pieces.K == 8 * (hint_pieces & 255);
-            hint_bad_s = ok ? 0 : 1;
-        }
+        if (!pieces_ok) plan->pieces.n = 0;
+        if (hint_class == -4) hint_bad_s = pieces_ok ? 0 : 1;
         plan->hint_bad = hint_bad_s;
         plan->recur_alt = (koff == 0 && alt_offered) ? 1 : 0;
         plan->N = N; plan->T = T; plan->M = M; plan->B = B; plan->n_tp = T * (T + 1) / 2;
@@ -103,12 +130,9 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
         plan->dq = dq;
         plan->q_small = (s < 3.0e38f) ? s : 0.f;
         int va = (hint_class == -4) ? V_CENT : (uni ? V_RECUR : V_MUFU);
-        if (hint_class == -3 && hint_pieces != 0 && cls == -1) {
-            // no hint, uniform grid with a general start: the centred product form if the launch on offer fits its pieces
-            // (it does: one run of M points is cut into equal pieces, which the host derived from M), else the chain form
-            if (debye_find_pieces(q, M, plan->pieces) && plan->pieces.n == (hint_pieces >> 8) && plan->pieces.K == 8 * (hint_pieces & 255)) va = V_CENT;
-            else plan->pieces.n = 0;
-        }
+        // no hint, uniform grid with a general start: the centred product form if the launch on offer fits its pieces (it does:
+        // one run of M points is cut into equal pieces, which the host derived from M), else the chain form
+        if (hint_class == -3 && pieces_ok) va = V_CENT;
         plan->variant_auto = va;
     }
     __syncthreads();

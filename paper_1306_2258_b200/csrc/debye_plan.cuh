@@ -76,30 +76,53 @@ __host__ __device__ inline int debye_grid_class(double q0, double dq, float dev,
     return -1;
 }
 
-// Piecewise-uniform grids: greedy maximal runs of equal steps (a loose test on the step finds the run, the 1.5-ulp criterion of
-// debye_grid_class with the step refitted through the run's end points then has to hold for every point of it), runs longer
-// than DEBYE_PIECE_KCAP cut into equal pieces.  Double arithmetic with fma and IEEE division only: the host (debye_q_hint)
-// and the device (debye_setup_kernel) get the same pieces from the same floats.  false: not piecewise uniform, or too many pieces.
-__host__ __device__ inline bool debye_find_pieces(const float *q, int M, DebyePieces &P)
+// Piecewise-uniform grids in three steps, the same arithmetic on the host (debye_q_hint: all three serially) and on the device
+// (debye_setup_kernel: q staged in shared memory, step 2 by all threads), double arithmetic with fma and IEEE division only, so
+// both get the same pieces from the same floats:
+//   1. debye_find_runs: greedy maximal runs of equal steps (a loose test: the step into q[e] within 4 float ulps of the run's
+//      first step, each difference carrying up to 2);
+//   2. debye_run_point_ok for every point: the 1.5-ulp criterion of debye_grid_class against the line through the end points
+//      of the point's run;
+//   3. debye_pieces_from_runs: runs longer than DEBYE_PIECE_KCAP cut into equal pieces.
+// false anywhere: not piecewise uniform, or more than DEBYE_MAX_PIECES pieces.
+__host__ __device__ inline bool debye_find_runs(const float *q, int M, int32_t *run_start /* [DEBYE_MAX_PIECES + 1] */, int &n_runs)
 {
-    P.n = 0; P.K = 8;
-    int maxcnt = 0, s = 0;
+    n_runs = 0;
+    int s = 0;
     while (s < M) {
+        if (n_runs == DEBYE_MAX_PIECES) return false;
+        run_start[n_runs++] = s;
         int e = s + 1;
-        double dq = 0.0;
         if (e < M) {
             const double d0 = (double)q[s + 1] - (double)q[s];
             const double a0 = fmax(fmax(fabs((double)q[s]), fabs((double)q[s + 1])), fabs(d0));   // d0 carries the rounding of the run's first two points
             e = s + 2;
             while (e < M) {
                 const double a = fmax(fmax(fabs((double)q[e]), fabs((double)q[e - 1])), a0);
-                if (fabs(((double)q[e] - (double)q[e - 1]) - d0) > 4.8e-7 * a) break;      // 4 float ulps: each difference carries up to 2
+                if (fabs(((double)q[e] - (double)q[e - 1]) - d0) > 4.8e-7 * a) break;
                 ++e;
             }
-            dq = ((double)q[e - 1] - (double)q[s]) / (double)(e - 1 - s);
-            for (int k = s; k < e; ++k)
-                if (debye_grid_dev((double)q[k], k - s, (double)q[s], dq) > 1.8e-7f) return false;
         }
+        s = e;
+    }
+    run_start[n_runs] = M;
+    return true;
+}
+__host__ __device__ inline double debye_run_dq(const float *q, int s, int e) { return (e - s > 1) ? ((double)q[e - 1] - (double)q[s]) / (double)(e - 1 - s) : 0.0; }
+// point k of the run [s, e): within 1.5 float ulps (1.8e-7 of max(|q_k|, |dq|)) of q[s] + (k - s) dq; no division per point
+__host__ __device__ inline bool debye_run_point_ok(const float *q, int s, int e, int k)
+{
+    const double dq = debye_run_dq(q, s, e), qk = (double)q[k];
+    const double scale = fmax(fabs(qk), fabs(dq));
+    return fabs(qk - fma((double)(k - s), dq, (double)q[s])) <= 1.8e-7 * scale;
+}
+__host__ __device__ inline bool debye_pieces_from_runs(const float *q, const int32_t *run_start, int n_runs, DebyePieces &P)
+{
+    P.n = 0; P.K = 8;
+    int maxcnt = 0;
+    for (int r = 0; r < n_runs; ++r) {
+        const int s = run_start[r], e = run_start[r + 1];
+        const double dq = debye_run_dq(q, s, e);
         const int n = e - s, np = (n + DEBYE_PIECE_KCAP - 1) / DEBYE_PIECE_KCAP, per = (n + np - 1) / np;
         for (int x = 0; x < np; ++x) {
             if (P.n == DEBYE_MAX_PIECES) return false;
@@ -108,11 +131,22 @@ __host__ __device__ inline bool debye_find_pieces(const float *q, int M, DebyePi
             ++P.n;
             if (c > maxcnt) maxcnt = c;
         }
-        s = e;
     }
     P.K = (maxcnt + 7) / 8 * 8;
     if (P.K < 8) P.K = 8;
     return true;
+}
+// all three steps serially (the host's debye_q_hint)
+__host__ __device__ inline bool debye_find_pieces(const float *q, int M, DebyePieces &P)
+{
+    int32_t run_start[DEBYE_MAX_PIECES + 1];
+    int n_runs = 0;
+    P.n = 0; P.K = 8;
+    if (!debye_find_runs(q, M, run_start, n_runs)) return false;
+    for (int r = 0; r < n_runs; ++r)
+        for (int k = run_start[r]; k < run_start[r + 1]; ++k)
+            if (!debye_run_point_ok(q, run_start[r], run_start[r + 1], k)) return false;
+    return debye_pieces_from_runs(q, run_start, n_runs, P);
 }
 
 // ---- programmatic dependent launch (PDL) ------------------------------------------------------------------------

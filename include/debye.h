@@ -54,8 +54,8 @@ enum {
 
 /* flags (bitwise or).  At most one of the DEBYE_SINC_* bits; none = automatic choice (made on the device,
  * no host sync): the recurrence kernel when q is a uniform grid from 0 or dq (telescoped product form), the centred
- * product form when it is uniform with another start or -- with the hint of debye_q_hint -- a few uniform pieces, else
- * the MUFU kernel. */
+ * product form when it is uniform with another start, has more than 256 non-zero points or -- with the hint of debye_q_hint --
+ * is a sequence of a few uniform pieces, else the MUFU kernel. */
 enum {
     DEBYE_FP64 = 1u << 0,         /* double-precision pair arithmetic (libdevice sin), tolerance 1e-10 mode     */
     DEBYE_SINC_MUFU = 1u << 2,    /* FP32, one range-reduced MUFU.SIN per term; any q grid                      */

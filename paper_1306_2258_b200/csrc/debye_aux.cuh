@@ -92,7 +92,8 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
     // start for which a centred launch is on offer.  The same segmentation as the host's (debye_plan.cuh), from a copy of q in
     // shared memory: runs by one thread, the 1.5-ulp test of every point by all threads, pieces by one thread; it has to give the
     // piece count and accumulator count the launch was sized for.  (A serial scan of global memory took 0.5 ms for 2000 points.)
-    const bool need_pieces = hint_class == -4 || (hint_class == -3 && hint_pieces != 0 && s_cls == -1);
+    // ... or a grid from 0 or dq with more than 256 chain indices (more than two chunks: the recurrence would run its chain form).
+    const bool need_pieces = hint_class == -4 || (hint_class == -3 && hint_pieces != 0 && (s_cls == -1 || (s_cls >= 0 && M - (s_cls == 0 ? 1 : 0) > 256)));
     bool pieces_ok = false;
     if (need_pieces) {
         for (int k = tid; k < M; k += blockDim.x) q_sh[k] = q[k];

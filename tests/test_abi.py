@@ -133,6 +133,9 @@ def test_q_hint_classifies_grids_on_the_host():
     saxs_waxs = np.concatenate([np.arange(51) * 0.005, 0.25 + 0.01 * np.arange(1, 51)]).astype(np.float32)
     assert binding.q_hint(saxs_waxs) == pieces(2, 56) and binding.pieces_of(binding.q_hint(saxs_waxs)) == (2, 56)
     assert binding.q_hint(np.delete(wl.q_grid(0.5, 101), 37)) == pieces(2, 64)  # a dropped point: 37 + 63
+    # a grid from 0 or dq with more than 256 chain indices would need more than two recurrence chunks (chain form): pieces instead
+    assert binding.q_hint(wl.q_grid(1.7, 1000)) == pieces(8, 128) and binding.q_hint(wl.q_grid(1.7, 257)) == H | U | Z
+    assert binding.q_hint(wl.q_grid(2.57, 257, 0.01)) == pieces(3, 88) and binding.q_hint(wl.q_grid(2.56, 256, 0.01)) == H | U | D
     assert binding.q_hint_pieces(wl.q_grid(0.5, 101)) == pieces(1, 104)        # any uniform grid can be forced into the centred form ...
     assert binding.q_hint(wl.q_grid(0.5, 101)) == H | U | Z                    # ... but from 0 or dq the telescoped form is preferred
     rng = np.random.default_rng(5)

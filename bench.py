@@ -38,11 +38,15 @@ NCU_TRAFFIC_SOURCE = ("profiles/r02_ncu_full_pairs_cfg2.txt, r02_ncu_full_pairs_
 
 
 TABLE1 = {f"table1_{n}": n for n in (1000, 2000, 4000, 10000, 20000, 40000, 100000)}       # the paper's Table I rows
+# wide grids (more than 256 non-zero q from 0: more than two recurrence chunks, run as contiguous pieces of the centred form)
+WIDE = {"wide_1000q": lambda: wl.small_random(5, 30000, 4, 1000, q_max=2.0, box=150.0), "wide_512q": lambda: wl.small_random(4, 3000, 5, 512, q_max=1.5, box=60.0)}
 
 
 def make_workload(name: str, rank: int = 0, grid: str = "config"):
     if name in TABLE1:
         w = wl.table1(TABLE1[name])
+    elif name in WIDE:
+        w = WIDE[name]()
     elif name == "cfg2" and rank:
         w = wl.cfg2(seed_off=2 + 1000 * rank, tag=f"cfg2_globular_10k_rank{rank}")
     else:
@@ -387,7 +391,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", default="cfg2", choices=sorted(wl.CONFIGS) + list(TABLE1),
+    ap.add_argument("--config", default="cfg2", choices=sorted(wl.CONFIGS) + list(TABLE1) + list(WIDE),
                     help="cfg1..cfg5: BASELINE.json's configs; table1_N: the shape of the paper's Table I rows (N atoms, 50 q on (0, 1])")
     ap.add_argument("--variant", default="auto", choices=["auto", "recur", "mufu", "accurate", "fp64", "centred"])
     ap.add_argument("--grid", default="config", choices=["config"] + sorted(wl.GRIDS),

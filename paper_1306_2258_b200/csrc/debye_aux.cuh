@@ -45,11 +45,14 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
         int tt[SORT_UNROLL];
 #pragma unroll
         for (int x = 0; x < SORT_UNROLL; ++x) { const int i = s0 + 32 * x + lane; tt[x] = (i < c1) ? type[i] : -1; }   // loads in flight together
+        // the SORT_UNROLL rankings first (independent of one another: pipelined), then the dependent counter updates
+        unsigned pm[SORT_UNROLL];
+#pragma unroll
+        for (int x = 0; x < SORT_UNROLL; ++x) pm[x] = __match_any_sync(0xffffffffu, tt[x]);
 #pragma unroll
         for (int x = 0; x < SORT_UNROLL; ++x) {
             const int t = tt[x];
-            const unsigned peers = __match_any_sync(0xffffffffu, t);
-            if (t >= 0 && (peers & ((1u << lane) - 1)) == 0) wcnt[warp][t] += __popc(peers);
+            if (t >= 0 && (pm[x] & ((1u << lane) - 1)) == 0) wcnt[warp][t] += __popc(pm[x]);
             __syncwarp();
         }
     }
@@ -169,22 +172,42 @@ __global__ void __launch_bounds__(DEBYE_SETUP_THREADS) debye_setup_kernel(DevPla
     __syncthreads();
     wcnt[warp][lane] = first;
     __syncwarp();
+    // One structure packed here: the thread that places atom i also moves its coordinates (loaded together with the type labels,
+    // coalesced in i, their latency under the ranking) -- no second pass through perm (the gather took 4 of the kernel's ~13 us
+    // at 10 000 atoms: three batches of two dependent global loads).
+    const bool fuse_pack = pack_here && B == 1;
     for (int s0 = c0; s0 < c1; s0 += 32 * SORT_UNROLL) {
         int tt[SORT_UNROLL];
+        float cx[SORT_UNROLL][4];
 #pragma unroll
         for (int x = 0; x < SORT_UNROLL; ++x) { const int i = s0 + 32 * x + lane; tt[x] = (i < c1) ? type[i] : -1; }
+        if (fuse_pack) {
+#pragma unroll
+            for (int x = 0; x < SORT_UNROLL; ++x) {
+                const int i = s0 + 32 * x + lane;
+                if (i < c1) { const float *sx = xyz + (int64_t)i * 3; cx[x][0] = sx[0]; cx[x][1] = sx[1]; cx[x][2] = sx[2]; cx[x][3] = weight ? weight[i] : 1.0f; }
+                else { cx[x][0] = cx[x][1] = cx[x][2] = cx[x][3] = 0.f; }
+            }
+        }
+        unsigned pm[SORT_UNROLL];
+#pragma unroll
+        for (int x = 0; x < SORT_UNROLL; ++x) pm[x] = __match_any_sync(0xffffffffu, tt[x]);
 #pragma unroll
         for (int x = 0; x < SORT_UNROLL; ++x) {
             const int t = tt[x];
-            const unsigned peers = __match_any_sync(0xffffffffu, t);
+            const unsigned peers = pm[x];
             const int rank = __popc(peers & ((1u << lane) - 1));
-            if (t >= 0) perm[wcnt[warp][t] + rank] = s0 + 32 * x + lane;
+            if (t >= 0) {
+                const int slot = wcnt[warp][t] + rank;
+                perm[slot] = s0 + 32 * x + lane;
+                if (fuse_pack) sorted[slot] = make_float4(cx[x][0], cx[x][1], cx[x][2], cx[x][3]);
+            }
             __syncwarp();
             if (t >= 0 && rank == 0) wcnt[warp][t] += __popc(peers);
             __syncwarp();
         }
     }
-    if (pack_here) {
+    if (pack_here && !fuse_pack) {
         __syncthreads();                       // perm was written by this CTA: visible after the barrier
         const int total = N * B;                 // <= DEBYE_PACK_IN_SETUP
 #pragma unroll 4

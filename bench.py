@@ -257,7 +257,7 @@ def measure(db, w, dev, variant, use_hint, steps, warmup, world=1, e2e=True):
     out = torch.empty((w.B, w.M) if batch else (w.M,), dtype=torch.float64, device=dev)
     flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device=dev)        # > 126 MB L2
     # the q grid exists on the host (it was generated there), so the caller can tell the library its shape: one pairs launch
-    # instead of up to three (include/debye.h, DEBYE_QHINT_*); the device verifies the hint
+    # instead of up to four (include/debye.h, DEBYE_QHINT_*); the device verifies the hint
     hint = db.q_hint(w.q) if use_hint else 0
     if variant == "centred":              # forced centred product form: needs the pieces of the grid whatever its class
         hint = db.q_hint_pieces(w.q)

@@ -66,8 +66,8 @@ enum {
                                    * plain calls only: DEBYE_EUNSUPPORTED with weights or in a tile split      */
     /* Optional grid hint, as returned by debye_q_hint() from a HOST copy of q.  Without it the library cannot know the
      * shape of the grid when it launches (q is device memory and calls never synchronise), so it launches every pairs
-     * instantiation that could be needed and the device runs exactly one; with it, only that one is launched (two to
-     * three launches fewer: ~8 us per call).  The device checks the hint against q; if it is wrong nothing is computed
+     * instantiation that could be needed and the device runs exactly one; with it, only that one is launched (two or
+     * three launches fewer: ~12 us per call).  The device checks the hint against q; if it is wrong nothing is computed
      * and the output is filled with NaN. */
     DEBYE_QHINT = 1u << 8,          /* a hint is present                                                        */
     DEBYE_QHINT_UNIFORM = 1u << 9,  /* q[k] = q[0] + k dq, dq = (q[M-1] - q[0])/(M-1): every q[k] within 1.5 float

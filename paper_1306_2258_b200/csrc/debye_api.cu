@@ -633,7 +633,7 @@ namespace {
 int run_peratom_recur(DevState *ds, const float *xyz, const float *ff, int N, const float *q, int M, double *I_out, int cls, int n_chunks, int K, cudaStream_t stream,
                       int B = 1)
 {
-    debye_peratom_recur_fn fn = debye_get_peratom_recur_kernel(K);
+    debye_peratom_recur_fn fn = debye_get_peratom_recur_kernel(K, B > 1);
     if (!fn) return DEBYE_EUNSUPPORTED;
     int st;
     const int rows = debye_diag_rows(N);
@@ -661,11 +661,22 @@ int run_peratom_recur(DevState *ds, const float *xyz, const float *ff, int N, co
     if (pb > ds->sms * 8) pb = ds->sms * 8;
     if (pb < 1) pb = 1;
     debye::debye_peratom_pack_kernel<<<dim3(pb, n_chunks + 1), 256, 0, stream>>>(xyz, ff, q, N, M, K, n_chunks, cls, pos4, ffp, plan, B);
-    debye::debye_peratom_self_kernel<<<dim3((M + 31) / 32, DEBYE_PA_SLICES), 256, 0, stream>>>(ff, N, M, selfbuf);
+    // Small problems (at most one wave of pairs CTAs): the rest of the chain with programmatic stream serialisation -- every
+    // kernel starts with pdl_wait() (debye_plan.cuh) -- which hides the launch gaps (1000 atoms: 48 -> 42 us per call).  Larger
+    // ones: ordinary launches (measured on B200: the pairs kernel itself runs 6 % slower when launched that way, cfg2 0.79 ->
+    // 0.84 ms, cfg3 30.5 -> 32.6 ms).
+    const bool chain_pdl = G <= one_wave;
+    if (chain_pdl) CU(launch_pdl(debye::debye_peratom_self_kernel, dim3((M + 31) / 32, DEBYE_PA_SLICES), dim3(256), stream, ff, N, M, selfbuf));
+    else debye::debye_peratom_self_kernel<<<dim3((M + 31) / 32, DEBYE_PA_SLICES), 256, 0, stream>>>(ff, N, M, selfbuf);
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
-    if (U > 0) fn<<<(int)G, DEBYE_IB, 0, stream>>>(pos4, ffp, q, plan, N, M, n_chunks, 0.002f, records, B);
+    if (U > 0) {
+        if (chain_pdl) CU(launch_pdl(fn, dim3((unsigned)G), dim3(DEBYE_IB), stream, (const float4 *)pos4, (const float *)ffp, q, (const debye::PeratomPlan *)plan, N, M, n_chunks, 0.002f, records, B));
+        else fn<<<(int)G, DEBYE_IB, 0, stream>>>(pos4, ffp, q, plan, N, M, n_chunks, 0.002f, records, B);
+    }
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
-    debye::debye_peratom_final_kernel<<<dim3((M + 31) / 32, B), 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, K, I_out, (const int32_t *)plan);
+    if (chain_pdl) CU(launch_pdl(debye::debye_peratom_final_kernel, dim3((M + 31) / 32, B), dim3(32 * DEBYE_PA_FS), stream, (const double *)records, (const double *)selfbuf, q, N, M, n_chunks,
+                                 (int)G, K, I_out, (const int32_t *)plan));
+    else debye::debye_peratom_final_kernel<<<dim3((M + 31) / 32, B), 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, K, I_out, (const int32_t *)plan);
     CU(scratch_release(ds->order, stream));
     CU(cudaGetLastError());
     return DEBYE_OK;
@@ -728,19 +739,24 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
     else { if ((st = ensure(&ds->ws, &ds->ws_bytes, o))) return st; ws = (char *)ds->ws; }
     double *records = (double *)(ws + o_rec), *selfbuf = (double *)(ws + o_self);
     CU(scratch_acquire(ds->order, stream));
+    const bool chain_pdl = G <= one_wave;      // small problems: programmatic stream serialisation along the chain (as run_peratom_recur)
     debye::debye_peratom_self_kernel<<<dim3((M + 31) / 32, DEBYE_PA_SLICES), 256, 0, stream>>>(ff, N, M, selfbuf);
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
     if (U > 0) {
 #define DEBYE_PA_LAUNCH(KQ_)                                                                                                              \
     case KQ_:                                                                                                                           \
-        if (f64) debye::debye_peratom_pairs_kernel<true, KQ_><<<(int)G, DEBYE_IB, 0, stream>>>(xyz, ff, q, N, M, n_chunks, records);    \
-        else debye::debye_peratom_pairs_kernel<false, KQ_><<<(int)G, DEBYE_IB, 0, stream>>>(xyz, ff, q, N, M, n_chunks, records);      \
+        if (f64) { if (chain_pdl) CU(launch_pdl(debye::debye_peratom_pairs_kernel<true, KQ_>, dim3((unsigned)G), dim3(DEBYE_IB), stream, xyz, ff, q, N, M, n_chunks, records));    \
+                   else debye::debye_peratom_pairs_kernel<true, KQ_><<<(int)G, DEBYE_IB, 0, stream>>>(xyz, ff, q, N, M, n_chunks, records); }                                 \
+        else { if (chain_pdl) CU(launch_pdl(debye::debye_peratom_pairs_kernel<false, KQ_>, dim3((unsigned)G), dim3(DEBYE_IB), stream, xyz, ff, q, N, M, n_chunks, records));      \
+               else debye::debye_peratom_pairs_kernel<false, KQ_><<<(int)G, DEBYE_IB, 0, stream>>>(xyz, ff, q, N, M, n_chunks, records); }                                   \
         break;
         switch (KQ) { DEBYE_PA_LAUNCH(16) DEBYE_PA_LAUNCH(20) DEBYE_PA_LAUNCH(24) DEBYE_PA_LAUNCH(28) DEBYE_PA_LAUNCH(32) default: return DEBYE_EUNSUPPORTED; }
 #undef DEBYE_PA_LAUNCH
     }
     if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
-    debye::debye_peratom_final_kernel<<<(M + 31) / 32, 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, KQ, I_out, nullptr);
+    if (chain_pdl) CU(launch_pdl(debye::debye_peratom_final_kernel, dim3((M + 31) / 32), dim3(32 * DEBYE_PA_FS), stream, (const double *)records, (const double *)selfbuf, q, N, M, n_chunks,
+                                 (int)G, KQ, I_out, (const int32_t *)nullptr));
+    else debye::debye_peratom_final_kernel<<<(M + 31) / 32, 32 * DEBYE_PA_FS, 0, stream>>>(records, selfbuf, q, N, M, n_chunks, (int)G, KQ, I_out, nullptr);
     CU(scratch_release(ds->order, stream));
     CU(cudaGetLastError());
     return DEBYE_OK;

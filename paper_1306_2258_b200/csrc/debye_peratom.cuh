@@ -34,6 +34,8 @@ namespace debye {
 // interleaved sub-slices that are added in order.  selfbuf[s][0][m] = sum f, selfbuf[s][1][m] = sum f^2.
 __global__ void __launch_bounds__(256) debye_peratom_self_kernel(const float *__restrict__ ff, int N, int M, double *__restrict__ selfbuf)
 {
+    pdl_wait();                            // launched with programmatic stream serialisation behind the pack kernel (debye_plan.cuh)
+    pdl_trigger();
     __shared__ double p1[8][32], p2[8][32];
     const int kk = threadIdx.x & 31, sub = threadIdx.x >> 5;
     const int k = blockIdx.x * 32 + kk, s = blockIdx.y;
@@ -70,6 +72,7 @@ __global__ void __launch_bounds__(DEBYE_IB, F64 ? 2 : DEBYE_PA_CTAS) debye_perat
                                                                                       const float *__restrict__ qv, int N, int M, int n_chunks,
                                                                                       double *__restrict__ records)
 {
+    pdl_wait();
     typedef typename std::conditional<F64, double, float>::type acc_t;
     constexpr int JT = DEBYE_PA_JT, NW = DEBYE_IB / 32;
     __shared__ __align__(16) float4 pos[JT];

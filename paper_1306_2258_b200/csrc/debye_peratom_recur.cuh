@@ -39,6 +39,7 @@ static __global__ void __launch_bounds__(256) debye_peratom_pack_kernel(const fl
                                                                    int K, int n_chunks, int hint_class, float4 *__restrict__ pos4, float *__restrict__ ffp,
                                                                    PeratomPlan *__restrict__ plan, int B)
 {
+    pdl_trigger();                         // first kernel of the call: the next grids are staged while this one runs
     const int y = blockIdx.y;
     if (y == n_chunks) {
         const int64_t NB = (int64_t)N * B;                  // positions of all conformers, [B][N]
@@ -195,7 +196,9 @@ __device__ __forceinline__ bool peratom_tile(u64 (&acc)[K / 2], const float4 *__
     return had_slow;
 }
 
-template <int K>
+// BATCH: several conformers on the unit line (debye_profile_peratom_batch).  A template parameter: the kernel uses all 255
+// registers at K >= 96, and the conformer's state as run-time values cost the single-structure call 4 % (spills).
+template <int K, bool BATCH>
 __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_peratom_recur_kernel(const float4 *__restrict__ pos4, const float *__restrict__ ffp, const float *__restrict__ qv,
                                                                                          const PeratomPlan *__restrict__ plan, int N, int M, int n_chunks, float theta_min,
                                                                                          double *__restrict__ records, int B)
@@ -212,7 +215,7 @@ __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_per
     const int G = gridDim.x, c = blockIdx.x;
     const int rows = debye_diag_rows(N);
     const int64_t U1 = rows > 0 ? debye_diag_row_prefix(N, rows) : 0;
-    const int64_t U = U1 * n_chunks * B;                    // unit line: conformer -> chunk -> row -> j
+    const int64_t U = U1 * n_chunks * (BATCH ? B : 1);      // unit line: conformer -> chunk -> row -> j
     if (U == 0) return;
     const int64_t u0 = debye_range_begin(U, c, G);
     const int64_t u1 = (c + 1 == G) ? U : debye_range_begin(U, c + 1, G);
@@ -240,15 +243,15 @@ __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_per
 #pragma unroll
     for (int i = 0; i < K / 2; ++i) acc[i] = 0;
     double run = 0.0;                  // thread l < K: FP64 running sum of slot l of the current chunk
-    int64_t X_cur = -1;                // record slot (conformer, chunk) the running sums belong to
+    int X_cur = -1;                    // record slot (conformer, chunk) the running sums belong to (< 65535 x 2)
 
     int64_t u = u0;
     while (u < u1) {
         // ---- decode unit u -> (conformer, q-chunk, row, first j) ---------------------------------------------------------
-        const int64_t X = u / U1;
-        const int b = (int)(X / n_chunks), ch = (int)(X - (int64_t)b * n_chunks);
-        const int64_t v = u - X * U1;
-        const float4 *pos4b = pos4 + (int64_t)b * N;
+        const int X = (int)(u / U1);
+        const int b = BATCH ? X / n_chunks : 0, ch = X - b * n_chunks;
+        const int64_t v = u - (int64_t)X * U1;
+        const int64_t boff = BATCH ? (int64_t)b * N : 0;       // this conformer's positions
         int rl = 0, rh = rows;
         while (rh - rl > 1) { const int mid = (rl + rh) >> 1; if (debye_diag_row_prefix(N, mid) <= v) rl = mid; else rh = mid; }
         const int row = rl;
@@ -262,7 +265,7 @@ __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_per
         const int mode = (n_chunks == 1) ? PM_C1 : (ch == 0 ? PM_C2A : PM_C2B);
         const int i = row * DEBYE_IB + tid;
         const bool ivalid = i < N;
-        const float4 pi = pos4b[ivalid ? i : 0];
+        const float4 pi = pos4[boff + (ivalid ? i : 0)];
         const int j_first = row * DEBYE_IB + 1 + (int)jo;
         const float *ffc = ffp + (size_t)ch * N * K;
         const int ntile = (len + JT - 1) / JT;
@@ -271,7 +274,7 @@ __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_per
             const int cnt = min(len - t * JT, JT);
             const uint32_t pb = (uint32_t)cnt * 16u, fb = (uint32_t)cnt * (uint32_t)K * 4u;
             mbar_expect_tx(&mbar[buf], pb + fb);
-            bulk_g2s(&tpos[buf][0], pos4b + j_first + t * JT, pb, &mbar[buf]);
+            bulk_g2s(&tpos[buf][0], pos4 + boff + j_first + t * JT, pb, &mbar[buf]);
             bulk_g2s(&tff[buf][0][0], ffc + (size_t)(j_first + t * JT) * K, fb, &mbar[buf]);
         };
         if (tid == 0) issue(0, 0);

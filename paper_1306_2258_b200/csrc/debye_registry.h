@@ -19,4 +19,4 @@ debye_small_fn debye_get_small_kernel(int K);
 // per-atom form factors on a uniform grid (debye_peratom_recur.cuh): K a multiple of 8 in [8, 128]; nullptr otherwise
 namespace debye { struct PeratomPlan; }
 typedef void (*debye_peratom_recur_fn)(const float4 *, const float *, const float *, const debye::PeratomPlan *, int, int, int, float, double *, int);
-debye_peratom_recur_fn debye_get_peratom_recur_kernel(int K);
+debye_peratom_recur_fn debye_get_peratom_recur_kernel(int K, bool batch);     // batch: several conformers on the unit line

@@ -61,6 +61,9 @@ cudaError_t scratch_release(ScratchOrder &o, cudaStream_t stream)
 #define DEBYE_MUFU_KMAX 112      // largest q-chunk of the MUFU kernel (choose())
 #endif
 static_assert(DEBYE_SETUP_MAXQ == DEBYE_MAX_Q, "the setup kernel stages the whole q grid in shared memory");
+#ifndef DEBYE_PA_PDL
+#define DEBYE_PA_PDL 1           // per-atom launch chains with programmatic dependent launch (0: ordinary launches, for measurement)
+#endif
 constexpr int MAX_DEV = 64;
 constexpr int64_t DEBYE_PACK_IN_SETUP = 16384;   // N x B up to which debye_setup_kernel also packs the coordinates
 struct DevState {
@@ -661,11 +664,9 @@ int run_peratom_recur(DevState *ds, const float *xyz, const float *ff, int N, co
     if (pb > ds->sms * 8) pb = ds->sms * 8;
     if (pb < 1) pb = 1;
     debye::debye_peratom_pack_kernel<<<dim3(pb, n_chunks + 1), 256, 0, stream>>>(xyz, ff, q, N, M, K, n_chunks, cls, pos4, ffp, plan, B);
-    // Small problems (at most one wave of pairs CTAs): the rest of the chain with programmatic stream serialisation -- every
-    // kernel starts with pdl_wait() (debye_plan.cuh) -- which hides the launch gaps (1000 atoms: 48 -> 42 us per call).  Larger
-    // ones: ordinary launches (measured on B200: the pairs kernel itself runs 6 % slower when launched that way, cfg2 0.79 ->
-    // 0.84 ms, cfg3 30.5 -> 32.6 ms).
-    const bool chain_pdl = G <= one_wave;
+    // The rest of the chain with programmatic stream serialisation -- every kernel starts with pdl_wait() (debye_plan.cuh) --
+    // which hides the launch gaps: 1000 atoms 48 -> 42 us per call, cfg2 0.827 -> 0.819 ms, cfg3 unchanged (measured on B200).
+    const bool chain_pdl = DEBYE_PA_PDL != 0;
     if (chain_pdl) CU(launch_pdl(debye::debye_peratom_self_kernel, dim3((M + 31) / 32, DEBYE_PA_SLICES), dim3(256), stream, ff, N, M, selfbuf));
     else debye::debye_peratom_self_kernel<<<dim3((M + 31) / 32, DEBYE_PA_SLICES), 256, 0, stream>>>(ff, N, M, selfbuf);
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
@@ -739,7 +740,7 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
     else { if ((st = ensure(&ds->ws, &ds->ws_bytes, o))) return st; ws = (char *)ds->ws; }
     double *records = (double *)(ws + o_rec), *selfbuf = (double *)(ws + o_self);
     CU(scratch_acquire(ds->order, stream));
-    const bool chain_pdl = G <= one_wave;      // small problems: programmatic stream serialisation along the chain (as run_peratom_recur)
+    const bool chain_pdl = DEBYE_PA_PDL != 0;  // programmatic stream serialisation along the chain (as run_peratom_recur)
     debye::debye_peratom_self_kernel<<<dim3((M + 31) / 32, DEBYE_PA_SLICES), 256, 0, stream>>>(ff, N, M, selfbuf);
     if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
     if (U > 0) {

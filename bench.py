@@ -340,7 +340,7 @@ def variant_that_ran(variant, w, use_hint=True):
     if use_hint and db.pieces_of(h)[0]:
         return "centred"                  # piecewise uniform / general start, hinted: the centred product form
     if db.pieces_of(h)[0] == 1:           # uniform with a general start, no hint: the device picks the centred launch if one was offered
-        return "centred" if w.M <= 16 * 128 else "recur"
+        return "centred" if w.M <= 32 * 128 else "recur"
     return "recur" if h & (1 << 9) else "mufu"
 
 

@@ -74,11 +74,11 @@ enum {
                                      * ulps (1.8e-7 relative to max(|q[k]|, |dq|)) of that line                  */
     DEBYE_QHINT_START0 = 1u << 10,  /* ... and q[0] == 0                                                        */
     DEBYE_QHINT_STARTDQ = 1u << 11, /* ... and q[0] == dq (the paper's grid q_k = k dq, k >= 1)   */
-    /* Piecewise-uniform grid: q is a sequence of at most 16 uniform pieces (a SAXS range followed by a coarser WAXS range, a
+    /* Piecewise-uniform grid: q is a sequence of at most 32 uniform pieces (a SAXS range followed by a coarser WAXS range, a
      * grid with a dropped point, a uniform grid with a general start cut into pieces of at most 128 points).  Such grids run
      * the CENTRED PRODUCT FORM (one FP32 lane-operation per term) instead of one MUFU.SIN per term.
      * The host sizes the launch from the pieces, so this hint carries their number and the accumulators per thread in bits
-     * 16-20 (pieces - 1) and 21-25 (K / 8 - 1): take it from debye_q_hint / debye_q_hint_pieces, never build it by hand.
+     * 16-20 (pieces - 1, at most 32 pieces) and 21-25 (K / 8 - 1): take it from debye_q_hint / debye_q_hint_pieces, never build it by hand.
      * Excludes DEBYE_QHINT_UNIFORM / _START*.  The device repeats the segmentation and fills the output with NaN if the
      * hint does not match q. */
     DEBYE_QHINT_PIECES = 1u << 12,
@@ -214,7 +214,7 @@ int debye_profile_from_partials(const double *S_parts, int32_t n_parts, const in
  * Returns 0 (no hint) for q_host == NULL or M < 1. */
 uint32_t debye_q_hint(const float *q_host, int32_t M);
 /* The piecewise-uniform hint (DEBYE_QHINT | DEBYE_QHINT_PIECES | piece count | accumulator count) for ANY grid made of at most
- * 16 uniform pieces -- also a plain uniform grid, for which debye_q_hint prefers the telescoped product form or the chain --
+ * 32 uniform pieces -- also a plain uniform grid, for which debye_q_hint prefers the telescoped product form or the chain --
  * or 0 if q is not such a grid.  debye_q_hint returns this hint by itself for grids that are not uniform as a whole. */
 uint32_t debye_q_hint_pieces(const float *q_host, int32_t M);
 

@@ -135,7 +135,7 @@ def q_hint(q_host) -> int:
 
 
 def q_hint_pieces(q_host) -> int:
-    """The piecewise-uniform hint (centred product form) for ANY grid made of at most 16 uniform pieces, 0 if q is not one;
+    """The piecewise-uniform hint (centred product form) for ANY grid made of at most 32 uniform pieces, 0 if q is not one;
     q_hint() returns it by itself for grids that are not uniform as a whole.  (pieces, K) = pieces_of(hint)."""
     q_host = np.ascontiguousarray(q_host, dtype=np.float32)
     return int(lib().debye_q_hint_pieces(C.c_void_p(q_host.ctypes.data), q_host.shape[0]))

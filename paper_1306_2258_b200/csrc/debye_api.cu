@@ -242,7 +242,7 @@ int validate(const void *xyz, const void *type, int N, int B, const void *tab, i
         if (sub && !(flags & DEBYE_QHINT)) return DEBYE_EINVAL;
         if (st2 && !(flags & DEBYE_QHINT_UNIFORM)) return DEBYE_EINVAL;
         if (st2 == (DEBYE_QHINT_START0 | DEBYE_QHINT_STARTDQ)) return DEBYE_EINVAL;
-        // piecewise-uniform hint: excludes the uniform bits; its fields (pieces - 1, K / 8 - 1) only with it, at most 16 each
+        // piecewise-uniform hint: excludes the uniform bits; its fields (pieces - 1, K / 8 - 1) only with it, at most 32 pieces and K <= 128
         if ((flags & DEBYE_QHINT_PIECES) && (!(flags & DEBYE_QHINT) || sub)) return DEBYE_EINVAL;
         if (!(flags & DEBYE_QHINT_PIECES) && (flags & piece_fields)) return DEBYE_EINVAL;
         if ((flags & DEBYE_QHINT_PIECES) && ((((flags >> DEBYE_QHINT_NPIECES_SHIFT) & 31u) >= DEBYE_MAX_PIECES) || (((flags >> DEBYE_QHINT_PIECEK_SHIFT) & 31u) >= 16u)))
@@ -924,8 +924,13 @@ uint32_t debye_q_hint(const float *q_host, int32_t M)
     const bool many_chunks = cls >= 0 && M - (cls == 0 ? 1 : 0) > 2 * DEBYE_KMAX_F32;
     if (cls == -2 || (cls == -1 && DEBYE_CENT_FOR_GENERAL_START) || many_chunks) {
         // not one uniform grid from 0 or dq: a few uniform pieces (the centred product form) if the grid has that shape
+        // ... and if it pays: a piece costs its start-up (~110 issue cycles per pair) plus one packed lane per accumulator, the MUFU
+        // kernel 8 cycles per q -- a grid of many short pieces (any 40 random points are 20 "uniform" pieces of two) stays there
         const uint32_t fp = debye_q_hint_pieces(q_host, M);
-        if (fp) return fp;
+        if (fp) {
+            const int64_t np = ((fp >> DEBYE_QHINT_NPIECES_SHIFT) & 31u) + 1, Kp = 8 * (((fp >> DEBYE_QHINT_PIECEK_SHIFT) & 31u) + 1);
+            if (np == 1 || np * (110 + Kp) < 8 * (int64_t)M) return fp;
+        }
     }
     uint32_t f = DEBYE_QHINT;
     if (cls != -2) f |= DEBYE_QHINT_UNIFORM;

@@ -20,7 +20,7 @@ enum DebyeVariant : int32_t { V_NONE = 0, V_F64 = 1, V_MUFU = 2, V_RECUR = 3, V_
 
 // Piecewise-uniform grids (V_CENT, the centred product form of debye_pairs.cuh): q is a sequence of at most DEBYE_MAX_PIECES
 // pieces, piece p = the points off[p] .. off[p] + cnt[p] - 1 with q = q0[p] + m dq[p] (m the local index), cnt[p] <= K <= 128.
-#define DEBYE_MAX_PIECES 16
+#define DEBYE_MAX_PIECES 32
 #define DEBYE_PIECE_KCAP 128
 struct DebyePieces {
     int32_t n, K;                 // number of pieces; accumulators per thread (a multiple of 8 >= the longest piece)

@@ -24,6 +24,7 @@
 #include "debye_peratom.cuh"
 #include "debye_small.cuh"
 #include "debye_peratom_recur.cuh"
+#include "debye_peratom_small.cuh"
 
 namespace {
 
@@ -61,6 +62,12 @@ cudaError_t scratch_release(ScratchOrder &o, cudaStream_t stream)
 #define DEBYE_MUFU_KMAX 112      // largest q-chunk of the MUFU kernel (choose())
 #endif
 static_assert(DEBYE_SETUP_MAXQ == DEBYE_MAX_Q, "the setup kernel stages the whole q grid in shared memory");
+#ifndef DEBYE_PAS_CTAS_PER_SM
+#define DEBYE_PAS_CTAS_PER_SM 1  // fused per-atom kernel for small structures: CTAs per SM of its cooperative grid
+#endif
+#ifndef DEBYE_PAS_UNITS
+#define DEBYE_PAS_UNITS 6
+#endif
 #ifndef DEBYE_PA_PDL
 #define DEBYE_PA_PDL 1           // per-atom launch chains with programmatic dependent launch (0: ordinary launches, for measurement)
 #endif
@@ -684,6 +691,48 @@ int run_peratom_recur(DevState *ds, const float *xyz, const float *ff, int N, co
 }
 }  // namespace
 
+namespace {
+// per-atom form factors, one small structure, hinted one-chunk grid: ONE cooperative launch (debye_peratom_small.cuh).  Called with g_mu held.
+int run_peratom_small(DevState *ds, const float *xyz, const float *ff, int N, const float *q, int M, double *I_out, int cls, int K, cudaStream_t stream)
+{
+    debye_peratom_small_fn fn = debye_get_peratom_small_kernel(K);
+    if (!fn) return DEBYE_EUNSUPPORTED;
+    int st;
+    static bool attr_set[MAX_DEV][DEBYE_KMAX_F32 / 8 + 1];
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    if (!attr_set[dev][K / 8]) {
+        CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)debye::debye_peratom_small_dyn_smem(DEBYE_PAS_NMAX, DEBYE_KMAX_F32)));
+        attr_set[dev][K / 8] = true;
+    }
+    // cooperative launch: the grid is one resident wave, DEBYE_PAS_CTAS_PER_SM CTAs per SM at most (if that many fit); at least
+    // ~DEBYE_PAS_UNITS units (j atom x 128 i atoms) per CTA
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, DEBYE_IB, debye::debye_peratom_small_dyn_smem(N, K)));
+    if (occ < 1) occ = 1;
+    if (occ > DEBYE_PAS_CTAS_PER_SM) occ = DEBYE_PAS_CTAS_PER_SM;
+    int64_t g = ((int64_t)N * N / (2 * DEBYE_IB) + 1) / DEBYE_PAS_UNITS;
+    if (g > (int64_t)ds->sms * occ) g = (int64_t)ds->sms * occ;
+    if (g > DEBYE_PAS_GMAX) g = DEBYE_PAS_GMAX;
+    if (g < 1) g = 1;
+    const int G = (int)g;
+    const size_t need = align_up((size_t)G * K * 8);
+    char *ws;
+    if (ds->user_ws) { if (ds->user_bytes < need) return DEBYE_ENOMEM; ws = (char *)ds->user_ws; }
+    else { if ((st = ensure(&ds->ws, &ds->ws_bytes, need))) return st; ws = (char *)ds->ws; }
+    double *records = (double *)ws;
+    CU(scratch_acquire(ds->order, stream));
+    if (ds->ev0) CU(cudaEventRecord(ds->ev0, stream));
+    int hc = cls;
+    void *args[] = {(void *)&xyz, (void *)&ff, (void *)&q, (void *)&N, (void *)&M, (void *)&hc, (void *)&records, (void *)&I_out};
+    CU(cudaLaunchCooperativeKernel((const void *)fn, dim3(G), dim3(DEBYE_IB), args, debye::debye_peratom_small_dyn_smem(N, K), stream));
+    if (ds->ev1) CU(cudaEventRecord(ds->ev1, stream));
+    CU(scratch_release(ds->order, stream));
+    CU(cudaGetLastError());
+    return DEBYE_OK;
+}
+}  // namespace
+
 int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const float *q, int32_t M, double *I_out, uint32_t flags, debye_stream_t stream_)
 {
     cudaStream_t stream = (cudaStream_t)stream_;
@@ -715,6 +764,8 @@ int debye_profile_peratom(const float *xyz, const float *ff, int32_t N, const fl
         const int n_idx = M - (cls == 0 ? 1 : 0);
         if (!f64 && !(flags & DEBYE_SINC_MUFU) && (cls == 0 || cls == 1) && n_idx >= 1) {
             const Choice c = choose(V_RECUR, n_idx);
+            // one small structure on a one-chunk grid: a single fused launch (debye_peratom_small.cuh)
+            if (c.n_chunks == 1 && N <= DEBYE_PAS_NMAX) return run_peratom_small(ds, xyz, ff, N, q, M, I_out, cls, (c.K + 7) / 8 * 8, stream);
             if (c.n_chunks <= 2) return run_peratom_recur(ds, xyz, ff, N, q, M, I_out, cls, c.n_chunks, (c.K + 7) / 8 * 8, stream);
         }
     }

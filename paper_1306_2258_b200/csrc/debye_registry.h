@@ -20,3 +20,7 @@ debye_small_fn debye_get_small_kernel(int K);
 namespace debye { struct PeratomPlan; }
 typedef void (*debye_peratom_recur_fn)(const float4 *, const float *, const float *, const debye::PeratomPlan *, int, int, int, float, double *, int);
 debye_peratom_recur_fn debye_get_peratom_recur_kernel(int K, bool batch);     // batch: several conformers on the unit line
+
+// per-atom form factors, one launch for one small structure (debye_peratom_small.cuh): K a multiple of 8 in [8, 128]; nullptr otherwise
+typedef void (*debye_peratom_small_fn)(const float *, const float *, const float *, int, int, int, double *, double *);
+debye_peratom_small_fn debye_get_peratom_small_kernel(int K);

@@ -821,8 +821,9 @@ def test_peratom_recurrence_on_hinted_uniform_grids(db):
     element and against the direct kernel; one and two chunks, K % 8 == 4, grids from 0 and from dq, ragged rows, close and
     coincident atoms (the small-theta path), a wrong hint, a grid it does not take."""
     import torch
+    # up to 2048 atoms on a one-chunk grid: the single fused launch (debye_peratom_small.cuh); beyond, or two chunks: four launches
     shapes = [(2, 9, 0.0), (3, 17, 0.0), (130, 33, 0.0), (777, 101, 0.0), (1500, 129, 0.0), (700, 128, 0.004), (1100, 200, 0.0),
-              (400, 257, 0.0), (515, 52, 0.01), (900, 64, 0.0)]
+              (400, 257, 0.0), (515, 52, 0.01), (900, 64, 0.0), (2048, 128, 0.004), (2049, 64, 0.0), (2600, 101, 0.0)]
     for si, (N, M, q_min) in enumerate(shapes):
         w = wl.small_random(300 + si, N, 3, M, q_min=q_min, q_max=q_min * M if q_min else 0.7, box=12.0 + N ** (1 / 3) * 3)
         ff = _peratom_ff(w, 400 + si)

@@ -148,7 +148,7 @@ int debye_profile_weighted_host(const float *xyz, const int32_t *type, const flo
  *   2 sin(q_k r)/r across the grid and each value is accumulated with one packed FMA against ff[j][k] from shared memory: 2 FP32
  *   lane-operations per term instead of ~9 instructions and a MUFU.SIN, four launches (re-layout of ff + grid check, self
  *   terms, pairs, final), scratch N x (16 + 4 K n_chunks) bytes more -- or, for at most 2048 atoms and at most 128 such q, ONE
- *   fused cooperative launch (debye_peratom_small.cuh: 31 us per 1000-atom profile).  The device checks the hint; a wrong one
+ *   fused cooperative launch (debye_peratom_small.cuh: 27 us per 1000-atom profile).  The device checks the hint; a wrong one
  *   gives NaN.
  *   DEBYE_SINC_RECUR demands the recurrence: DEBYE_EUNSUPPORTED if the hinted grid is not one it takes.  Asynchronous on
  *   `stream`, same workspace rules and error codes as debye_profile (direct path scratch: at most 1.3 MB + 1 KB x M; a

@@ -57,6 +57,7 @@ __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_per
     float4 *pos = reinterpret_cast<float4 *>(dyn);
     float *tf = reinterpret_cast<float *>(dyn + (size_t)npad * 16);          // [JT][K], pre-signed rows of the tile's j atoms
     __shared__ double wsum[NW][K];
+    __shared__ float tbuf[NW][32][33];
     __shared__ double red[DEBYE_IB];
     __shared__ int s_dev, s_qmax, s_bad, s_koff;
     __shared__ double s_dq;
@@ -162,28 +163,42 @@ __global__ void __launch_bounds__(DEBYE_IB, K <= DEBYE_PAR_K3 ? 3 : 2) debye_per
                     }
                 }
             }
-            // ---- flush: times f_i (sigma^2 = 1: the raw row), FP64, fixed order (xor tree over the lanes, then the warps in order) ----
+            // ---- flush: times f_i (sigma^2 = 1: the raw row), then FP64 in a fixed order: per warp the products are transposed
+            // through shared memory, lane l adds slot 32 s + l over the 32 i atoms (four interleaved partial sums), then the warps in
+            // order.  (An xor-shuffle tree over the lanes in FP64, as in the large kernel, took 4 us per flush here: 10 64-bit
+            // shuffles per slot pair; the kernel flushes once per row segment, and the slowest CTA holds the grid barrier.)
             {
                 const float *fi = ff + (size_t)(ivalid ? i : 0) * M;
 #pragma unroll
-                for (int l = 0; l < K; l += 2) {
-                    float lo, hi;
-                    upk2(acc[l / 2], lo, hi);
-                    acc[l / 2] = 0;
-                    const int k0 = l + 1 - koff, k1 = l + 2 - koff;
-                    double v0 = (ivalid && k0 >= 0 && k0 < M) ? (double)lo * (double)fi[k0] : 0.0;
-                    double v1 = (ivalid && k1 >= 0 && k1 < M) ? (double)hi * (double)fi[k1] : 0.0;
+                for (int s = 0; s < (K + 31) / 32; ++s) {
 #pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) { v0 += __shfl_xor_sync(0xffffffffu, v0, o); v1 += __shfl_xor_sync(0xffffffffu, v1, o); }
-                    if (lane == 0) { wsum[warp][l] = v0; wsum[warp][l + 1] = v1; }
+                    for (int t = 0; t < 32; t += 2) {
+                        const int l = 32 * s + t;
+                        if (l < K) {
+                            float lo, hi;
+                            upk2(acc[l / 2], lo, hi);
+                            acc[l / 2] = 0;
+                            const int k0 = l + 1 - koff, k1 = l + 2 - koff;
+                            const float f0 = (ivalid && k0 >= 0 && k0 < M) ? fi[k0] : 0.f, f1 = (ivalid && k1 >= 0 && k1 < M) ? fi[k1] : 0.f;
+                            tbuf[warp][t][lane] = lo * f0;
+                            tbuf[warp][t + 1][lane] = hi * f1;
+                        }
+                    }
+                    __syncwarp();
+                    if (32 * s + lane < K) {
+                        double p0 = 0.0, p1 = 0.0, p2 = 0.0, p3 = 0.0;
+#pragma unroll
+                        for (int x = 0; x < 32; x += 4) {
+                            p0 += (double)tbuf[warp][lane][x]; p1 += (double)tbuf[warp][lane][x + 1];
+                            p2 += (double)tbuf[warp][lane][x + 2]; p3 += (double)tbuf[warp][lane][x + 3];
+                        }
+                        wsum[warp][32 * s + lane] = (p0 + p1) + (p2 + p3);
+                    }
+                    __syncwarp();
                 }
                 __syncthreads();
-                if (tid < K) {
-                    double s = 0.0;
-#pragma unroll
-                    for (int w = 0; w < NW; ++w) s += wsum[w][tid];
-                    run += s;
-                }
+                if (tid < K) run += (wsum[0][tid] + wsum[1][tid]) + (wsum[2][tid] + wsum[3][tid]);
+                __syncthreads();
             }
             u += len;
         }

@@ -646,6 +646,8 @@ def run_peratom(args, w, rank, world, dev):
     hint = 0 if (args.no_hint or variant in ("mufu", "fp64")) else db.q_hint(w.q)
     H, U, Z, D = 1 << 8, 1 << 9, 1 << 10, 1 << 11
     recur = bool(hint & U) and bool(hint & (Z | D)) and (w.M - (1 if hint & Z else 0)) <= 256
+    # one small structure on a one-chunk grid: the single fused launch (debye_peratom_small.cuh)
+    fused = recur and not batch and w.N <= 2048 and (w.M - (1 if hint & Z else 0)) <= 128
     x, f, q = (torch.from_numpy(a).to(dev) for a in (w.xyz, ff, w.q))
     out = torch.empty((w.B, w.M) if batch else w.M, dtype=torch.float64, device=dev)
     flush = torch.empty(192 * 1024 * 1024, dtype=torch.uint8, device=dev)
@@ -734,7 +736,7 @@ def run_peratom(args, w, rank, world, dev):
         "clocks": clocks,
         "e2e": {"value": units * n_e2e / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(hx.nbytes + hf.nbytes + hq.nbytes),
                 "d2h_bytes_per_step": int(hout.nbytes), "ms_per_step": e2e_s / n_e2e * 1e3, "steps": n_e2e},
-        "gpu_launches": (4 if recur else 3 * w.B) * args.steps,
+        "gpu_launches": (1 if fused else (4 if recur else 3 * w.B)) * args.steps,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s" if recur else "T sin/s", "frac": achieved / peak,
                      # dram__bytes_read.sum + write.sum of the pairs kernel from the full ncu capture (profiles/r01_v6.md)
                      "traffic": 4248064 if (args.config == "cfg2" and variant != "fp64" and not recur) else None,
@@ -742,7 +744,7 @@ def run_peratom(args, w, rank, world, dev):
                               "with q != 0; peak = 148 SM x 128 lanes x 2 x sm_max_mhz") if recur else
                              ("XU (MUFU) roofline: one MUFU.SIN per pair.q, 16 lanes/clk/SM x 148 SM x sm_max_mhz; the q-chunks "
                               "are padded (M = 101 runs 4 x 28 = 112 slots), which the algorithmic count does not credit"),
-                     "kernel": "debye_peratom_recur_kernel" if recur else f"debye_peratom_pairs_kernel<{'fp64' if variant == 'fp64' else 'fp32'}>", "kernel_ms": pairs_ms,
+                     "kernel": "debye_peratom_small_kernel (one fused launch)" if fused else "debye_peratom_recur_kernel" if recur else f"debye_peratom_pairs_kernel<{'fp64' if variant == 'fp64' else 'fp32'}>", "kernel_ms": pairs_ms,
                      "share_of_step": pairs_ms / (total_ms / args.steps)},
     }
     if world == 1 and not args.no_cpu_baseline:

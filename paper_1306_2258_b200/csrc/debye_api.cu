@@ -68,6 +68,11 @@ static_assert(DEBYE_SETUP_MAXQ == DEBYE_MAX_Q, "the setup kernel stages the whol
 #ifndef DEBYE_PAS_UNITS
 #define DEBYE_PAS_UNITS 6
 #endif
+#ifndef DEBYE_UNITS_PER_CTA
+// grid_for: at least this many units (one j atom x 128 i atoms) per pairs CTA.  Measured on B200 with the product form, cfg2
+// (G pair.q/s by units per CTA): 75 14 334, 100 14 631, 150 15 040, 250 15 160, 400 15 152, 800 14 854 (a single wave)
+#define DEBYE_UNITS_PER_CTA 250.0
+#endif
 #ifndef DEBYE_PA_PDL
 #define DEBYE_PA_PDL 1           // per-atom launch chains with programmatic dependent launch (0: ordinary launches, for measurement)
 #endif
@@ -283,8 +288,8 @@ int dev_state(DevState **st)
 // the CTAs that share an SM, so with exactly one wave the favoured CTA finishes ~30 % early and its partner runs the tail
 // alone (measured); more waves let the hardware block scheduler refill the SM.  Each extra CTA costs
 // one prologue, one FP64 flush and one more record for the final kernel, so the count is bounded by the work available
-// (estimated from N alone: the host never sees the type histogram): at least ~150 units (one j atom x 128 i atoms) per
-// CTA, at most 16 waves -- the measured optimum on cfg2 (8 waves) and flat beyond 4 waves on the large configs.
+// (estimated from N alone: the host never sees the type histogram): at least DEBYE_UNITS_PER_CTA units (one j atom x 128 i
+// atoms) per CTA, at most 16 waves -- cfg2 with the product form: 3 waves of 3 CTAs per SM; flat beyond 4 waves on the large configs.
 int grid_for(DevState *s, const Choice &c, int N, int B, int *G, bool weighted = false)
 {
     int &o = s->occ[c.variant][c.K / 4];
@@ -298,7 +303,7 @@ int grid_for(DevState *s, const Choice &c, int N, int B, int *G, bool weighted =
     }
     const int resident = s->sms * o;
     const double units = (double)B * c.n_chunks * ((double)N * (double)N / (2.0 * DEBYE_IB));   // j atoms x rows, all type pairs
-    int waves = (int)(units / ((double)resident * 150.0));
+    int waves = (int)(units / ((double)resident * DEBYE_UNITS_PER_CTA));
     if (waves < 1) waves = 1;
     if (waves > 16) waves = 16;
     *G = resident * waves;

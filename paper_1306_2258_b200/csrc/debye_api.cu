@@ -73,6 +73,9 @@ static_assert(DEBYE_SETUP_MAXQ == DEBYE_MAX_Q, "the setup kernel stages the whol
 // (G pair.q/s by units per CTA): 75 14 334, 100 14 631, 150 15 040, 250 15 160, 400 15 152, 800 14 854 (a single wave)
 #define DEBYE_UNITS_PER_CTA 250.0
 #endif
+#ifndef DEBYE_PAR_UNITS_PER_CTA
+#define DEBYE_PAR_UNITS_PER_CTA 250  // per-atom recurrence: units per pairs CTA (cfg2: 150 6 189, 250 6 270, 400 5 857 G pair.q/s)
+#endif
 #ifndef DEBYE_PA_PDL
 #define DEBYE_PA_PDL 1           // per-atom launch chains with programmatic dependent launch (0: ordinary launches, for measurement)
 #endif
@@ -303,7 +306,10 @@ int grid_for(DevState *s, const Choice &c, int N, int B, int *G, bool weighted =
     }
     const int resident = s->sms * o;
     const double units = (double)B * c.n_chunks * ((double)N * (double)N / (2.0 * DEBYE_IB));   // j atoms x rows, all type pairs
-    int waves = (int)(units / ((double)resident * DEBYE_UNITS_PER_CTA));
+    // the direct variants (one MUFU.SIN / sinf / double sin per term) keep 150: their units take 5 to 50 times longer, and the MUFU
+    // kernel measured 3 237 G pair.q/s on cfg2 with 150 units per CTA against 3 120 G with 250
+    const double units_per_cta = (c.variant == V_RECUR || c.variant == V_CENT) ? DEBYE_UNITS_PER_CTA : 150.0;
+    int waves = (int)(units / ((double)resident * units_per_cta));
     if (waves < 1) waves = 1;
     if (waves > 16) waves = 16;
     *G = resident * waves;
@@ -654,7 +660,7 @@ int run_peratom_recur(DevState *ds, const float *xyz, const float *ff, int N, co
     const int rows = debye_diag_rows(N);
     const int64_t U = (rows > 0 ? debye_diag_row_prefix(N, rows) : 0) * n_chunks * B;
     const int64_t one_wave = (int64_t)ds->sms * (K <= 64 ? 3 : 2);
-    int64_t G = U / 150 / one_wave * one_wave;                 // whole waves, at least ~150 units (j atoms x 128 i atoms) per CTA
+    int64_t G = U / DEBYE_PAR_UNITS_PER_CTA / one_wave * one_wave;                 // whole waves, at least ~150 units (j atoms x 128 i atoms) per CTA
     if (G > one_wave * 16) G = one_wave * 16;
     if (G < one_wave) { G = U / 8; if (G > one_wave) G = one_wave; }
     if (G < 1) G = 1;

@@ -33,7 +33,7 @@ SM_COUNT, FP32_LANES, MUFU_LANES = 148, 128, 16           # per B200 / per SM pe
 # dram__bytes_read.sum + dram__bytes_write.sum of the pairs kernel, per launch, from the committed ncu --set full captures
 # (profiles/r02_ncu_full_pairs_cfg{2,4,5}.txt); None where no capture exists
 NCU_TRAFFIC = {("cfg2", "recur"): 239104, ("cfg4", "recur"): 32863232 + 145920, ("cfg5", "recur"): 3322624, ("cfg2", "mufu"): 366336}
-NCU_TRAFFIC_SOURCE = ("profiles/r02_ncu_full_pairs_cfg2.txt, r02_ncu_full_pairs_cfg{4,5}_v2.txt, r02_ncu_full_pairs_mufu_cfg2.txt (ncu --set full captures of "
+NCU_TRAFFIC_SOURCE = ("profiles/r02_ncu_full_pairs_cfg2_v2.txt, r02_ncu_full_pairs_cfg{4,5}_v2.txt, r02_ncu_full_pairs_mufu_cfg2.txt (ncu --set full captures of "
                       "this kernel, commands in profiles/r02_product_form.md and r02_centred_form.md); not measured by this run")
 
 

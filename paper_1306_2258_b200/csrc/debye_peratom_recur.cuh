@@ -151,6 +151,8 @@ __device__ __forceinline__ void chain_hot(u64 (&acc)[K / 2], u64 (&A)[4], u64 (&
 // measured on B200 (T pair.q/s, cfg2 / cfg3): mode as a run-time branch inside the loop, 1 pair per iteration, 32-atom tiles
 // 5.08 / 6.66; one loop per mode 5.69 / 7.62; two pairs per iteration 5.93 / 8.04; 48-atom tiles (K = 104) 6.01 / 8.17;
 // 3 CTAs per SM at K = 104 (168 registers, 1 pair per iteration) 5.73 / 7.79
+// two copies of the body with the roles of (A, Bv) and (An, Bn) exchanged (no register moves at the loop's tail: 55 of its 452
+// instructions are MOVs): 6.00 / 7.98 against 6.19 / 8.18 (K = 104 spills 108 bytes instead of 44) -- not kept
 #ifndef DEBYE_PAR_NP
 #define DEBYE_PAR_NP 2
 #endif

@@ -726,6 +726,12 @@ def run_peratom(args, w, rank, world, dev):
         peak = SM_COUNT * FP32_LANES * 2 * fmax_ghz / 1e3                       # TFLOP/s, FMA = 2 flop
     # the library's q-chunk (debye_peratom_kq): the multiple of 4 in [16, 32] with the fewest padded slots, larger on ties
     kq = min(range(32, 12, -4), key=lambda c: ((w.M + c - 1) // c * c, -c))
+    n_chunks_label = (w.M + kq - 1) // kq
+    if recur:       # the recurrence keeps every chain index of a chunk in registers: K accumulators (a multiple of 8), 1 or 2 chunks
+        n_idx = w.M - (1 if float(w.q[0]) == 0.0 else 0)
+        n_chunks_label = 1 if n_idx <= 128 else 2
+        last = max(n_idx - 1, 0)
+        kq = max(8, (8 * (last // (8 * n_chunks_label)) + min(last % (8 * n_chunks_label), 7) + 1 + 7) // 8 * 8)
     achieved = float(w.pair_q) / (pairs_ms * 1e-3) / 1e12
     if recur:       # 2 FP32-pipe lane-operations (chain FFMA + weighted-accumulate FFMA = 4 flop) per pair.q with q != 0
         achieved = 4.0 * float(w.pair_q) / w.M * int(np.count_nonzero(w.q)) / (pairs_ms * 1e-3) / 1e12
@@ -734,7 +740,7 @@ def run_peratom(args, w, rank, world, dev):
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if variant == "fp64" else "f32", "data": "synthetic",
         "config": {"workload": w.name + "+peratom_table", "path": "peratom", "N": w.N, "M": w.M, "B": w.B,
-                   "variant": "fp64" if variant == "fp64" else ("recur" if recur else "mufu"), "q_chunk": kq, "n_chunks": (w.M + kq - 1) // kq,
+                   "variant": "fp64" if variant == "fp64" else ("recur" if recur else "mufu"), "q_chunk": kq, "n_chunks": n_chunks_label,
                    "q_hint": "passed" if hint else "none",
                    "l2": "flushed between steps (192 MiB fill, outside the per-step events)",
                    "parallelism": f"{world} independent structure(s), one per GPU", "wall_s_timed_loop": wall},

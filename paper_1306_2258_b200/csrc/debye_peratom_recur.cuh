@@ -153,6 +153,7 @@ __device__ __forceinline__ void chain_hot(u64 (&acc)[K / 2], u64 (&A)[4], u64 (&
 // 3 CTAs per SM at K = 104 (168 registers, 1 pair per iteration) 5.73 / 7.79
 // two copies of the body with the roles of (A, Bv) and (An, Bn) exchanged (no register moves at the loop's tail: 55 of its 452
 // instructions are MOVs): 6.00 / 7.98 against 6.19 / 8.18 (K = 104 spills 108 bytes instead of 44) -- not kept
+// three pairs per iteration for K <= 64: cfg4 as a batch (K = 64) 6.58 against 6.59, 4000 atoms x 50 q (K = 56) 3.57 / 3.65 -- not kept
 #ifndef DEBYE_PAR_NP
 #define DEBYE_PAR_NP 2
 #endif
